@@ -1,0 +1,120 @@
+/* tfs.h -- C ABI of libtfs: batch evaluation of the semi-coherent time-frequency detection
+ * statistic Upsilon_Nseg on one NVIDIA B200 (sm_100a).
+ *
+ * Method: arXiv 2510.19047, "Global time-frequency search for stellar-mass binary black holes
+ * in LISA".  Citations "P:<n>" are line numbers of the paper text with the equation
+ * they fall in; "C<n>" are the readings listed in DESIGN.md section 3.
+ *
+ * What one call of tfs_eval computes, for every template theta_i of a batch:
+ *   track   f_m, fdot_m, phi_m, A_m at each tranche start t_m = m*DT        (Eqs. 12-15)
+ *   pixels  h~_m(f_k)/DT in the window k_lo..k_hi around f_m, Fresnel kernel (Eqs. 16-22)
+ *   sums    z_n  = sum_alpha T_alpha sum_{m in seg n} sum_k g[m] W conj(D) h~  (Eq. 31, Eq. 30)
+ *           hh_n = sum_alpha |T_alpha|^2 sum_m sum_k g[m] W |h~|^2
+ *   result  P_n = |z_n|^2 / hh_n (0 if hh_n = 0),  Upsilon = sum_n P_n         (Eq. 8, Eq. 9)
+ * with n(m) = floor(m*N_seg/Nt) (C9) and W = 4 df / S in the data's units so that noise has
+ * E|D|^2 = 2/W (absorbs the 4 and delta-f of Eqs. 1 and 7).
+ *
+ * Geometry (C1): Nt tranches of length DT = 2*Nf*dt; Nf frequency bins of width df = 1/DT;
+ * bin k sits at f_k = k*df.  All arrays are C-contiguous, frequency fastest.
+ *
+ * Every step runs in CUDA kernels of this library; there is no CPU fallback.  All functions
+ * return 0 on success or a negative TFS_E* code; nothing throws or aborts across the ABI.
+ * Pointers marked "host or device" are classified with cudaPointerGetAttributes; the caller
+ * owns every array it passes and the library never keeps a caller pointer after the call
+ * returns (device-pointer work is only ENQUEUED on `stream`: the caller must keep those
+ * arrays alive and unchanged until it has synchronised that stream).  Host outputs imply a
+ * stream synchronisation inside the call.  A context must not be used from two threads at once.
+ */
+#ifndef TFS_H
+#define TFS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define TFS_API __attribute__((visibility("default")))
+#else
+#define TFS_API
+#endif
+
+#define TFS_OK       0
+#define TFS_EINVAL  -1   /* bad shape / N_seg<1 / N_seg>Nt / k<1 / k>n / NULL required pointer / unsupported option */
+#define TFS_ESTATE  -2   /* tfs_eval or tfs_count_pixels before tfs_upload_data */
+#define TFS_ENOMEM  -3   /* host or device allocation failed */
+#define TFS_ECUDA   -4   /* CUDA runtime error; text in tfs_last_error */
+
+#define TFS_PARAM_COLS 8 /* doubles per template row, see tfs_eval */
+
+typedef struct tfs_ctx tfs_ctx;   /* opaque; owns every device buffer it allocates */
+
+/* Options; pass NULL to tfs_create for the defaults.  A zero-initialised struct is NOT the
+ * default set: fill it with tfs_default_opts first. */
+typedef struct {
+  int    half_width;     /* H: window reaches H bins below ceil(f_m/df); default 10 -> N_F = 21 (C3)   */
+  int    adaptive_width; /* 1 (default): k_hi = ceil((f_m + fdot_m DT)/df) + H (C4); 0: paper-strict ceil(f_m/df)+H */
+  double c_max;          /* tranches with fdot_m*DT^2 > c_max are skipped; default 300 (C4)              */
+  double f_lo, f_hi;     /* band [Hz]: tranche active iff f_lo <= f_m and f_m + fdot_m DT <= f_hi;
+                            <= 0 means the default [1*df, (Nf-1)*df]                                           */
+  int    fresnel_mode;   /* 0 (default): Fresnel auxiliary functions accurate to ~1e-7;
+                            1: the paper's approximants Eqs. 23-28 verbatim (C8)                    */
+} tfs_opts;
+
+TFS_API void tfs_default_opts(tfs_opts* opts);
+
+/* Create a context for an Nt x Nf grid sampled at dt seconds with n_channels TDI channels
+ * (this build supports n_channels == 2, the A and E channels).  Uses the current CUDA
+ * device.  *out is set to NULL on failure (the reason is then in tfs_last_error(NULL)). */
+TFS_API int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const tfs_opts* opts);
+
+/* Upload (copy + repack) the TF data product.
+ *   coeff    [C][Nt][Nf][2] float, (re, im) of D[alpha, m, k]          host or device, required
+ *   weight   [C][Nt][Nf]    float, W >= 0 per pixel (C11)               host or device, NULL => 1
+ *   gap_mask [Nt]           uint8, 1 = valid, 0 = tranche overlaps a gap (C10); NULL => all valid
+ * The library stores Y = W*D interleaved by channel and W, frequency-contiguous.  May be called
+ * again to replace the data.  Returns after the copy out of host memory is complete. */
+TFS_API int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight,
+                    const uint8_t* gap_mask, void* stream);
+
+/* Evaluate Upsilon_{N_seg} for n templates.
+ *   params  [n][8] double: Mc [Msun], tc [s after data start], phic [rad],
+ *                          T_A.re, T_A.im, T_E.re, T_E.im (Eq. 29, constant per template, C5),
+ *                          amp (A_m = amp * f_m^(2/3))                   host or device, required
+ *   template model: 0PN chirp (C5): M = Mc*GMsun/c^3, tau = tc - t_m (> DT), X = tau/(5M),
+ *     f = X^(-3/8)/(8 pi M), phi = phic - 2 X^(5/8), fdot = 3 f/(8 tau).
+ *   upsilon   [n]           float   required      host or device
+ *   seg_power [n][N_seg]    float   nullable      P_n
+ *   seg_dh    [n][N_seg][2] float   nullable      (re, im) of z_n
+ *   seg_hh    [n][N_seg]    float   nullable      hh_n
+ * 1 <= N_seg <= Nt.  Rows containing NaN/Inf or Mc <= 0 yield zeros and are counted
+ * (tfs_bad_param_count), not fatal.  n == 0 is a no-op.  Arithmetic: fp64 track, fp32 pixels,
+ * fp32 partial sums promoted to fp64 per 32-tranche chunk, fp64 combine, fp32 stores. */
+TFS_API int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg,
+             float* upsilon, float* seg_power, float* seg_dh, float* seg_hh, void* stream);
+
+/* Indices and values of the k largest entries of upsilon[0..n), descending; equal values are
+ * ordered by lower index first; NaN sorts below everything.  1 <= k <= n.
+ *   upsilon host or device;  idx [k] int64 and val [k] float, host or device, required. */
+TFS_API int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k,
+             long long* idx, float* val, void* stream);
+
+/* Number of window pixels (k_hi-k_lo+1 summed over active tranches) of each template:
+ * pixel_evals = n_channels * counts[i].  counts [n] int64, host or device.  Used by the
+ * benchmark for the pixel-evals/s metric and by tests for the window logic. */
+TFS_API int tfs_count_pixels(tfs_ctx* ctx, const double* params, long long n, long long* counts, void* stream);
+
+/* Templates rejected (NaN/Inf/Mc<=0) by the most recent tfs_eval on this context. */
+TFS_API long long tfs_bad_param_count(const tfs_ctx* ctx);
+
+TFS_API void tfs_destroy(tfs_ctx* ctx);
+
+/* Message of the last failure on this context (or of the last failed tfs_create when ctx is
+ * NULL); never NULL; valid until the next failing call. */
+TFS_API const char* tfs_last_error(const tfs_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TFS_H */

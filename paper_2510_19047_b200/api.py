@@ -1,0 +1,183 @@
+"""Thin Python binding of libtfs (include/tfs.h): same names, argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  PyTorch is used here only to own
+device memory and to name the current stream.  There is no fallback: if ``libtfs.so`` is
+missing or no CUDA device is present these calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtfs.so")
+
+TFS_OK, TFS_EINVAL, TFS_ESTATE, TFS_ENOMEM, TFS_ECUDA = 0, -1, -2, -3, -4
+PARAM_COLS = 8
+
+
+class tfs_opts(C.Structure):
+    _fields_ = [("half_width", C.c_int), ("adaptive_width", C.c_int), ("c_max", C.c_double),
+                ("f_lo", C.c_double), ("f_hi", C.c_double), ("fresnel_mode", C.c_int)]
+
+
+class TfsError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libtfs error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libtfs.so (built in-tree by ``python -m paper_2510_19047_b200.build``)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} not found: build it with `python -m paper_2510_19047_b200.build` "
+                           "(libtfs has no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, ip, dp, ll = C.c_void_p, C.c_int, C.c_double, C.c_longlong
+    lib.tfs_default_opts.argtypes = [C.POINTER(tfs_opts)]
+    lib.tfs_default_opts.restype = None
+    lib.tfs_create.argtypes = [C.POINTER(vp), ip, ip, dp, ip, C.POINTER(tfs_opts)]
+    lib.tfs_create.restype = ip
+    lib.tfs_upload_data.argtypes = [vp, vp, vp, vp, vp]
+    lib.tfs_upload_data.restype = ip
+    lib.tfs_eval.argtypes = [vp, vp, ll, ip, vp, vp, vp, vp, vp]
+    lib.tfs_eval.restype = ip
+    lib.tfs_topk.argtypes = [vp, vp, ll, ip, vp, vp, vp]
+    lib.tfs_topk.restype = ip
+    lib.tfs_count_pixels.argtypes = [vp, vp, ll, vp, vp]
+    lib.tfs_count_pixels.restype = ip
+    lib.tfs_bad_param_count.argtypes = [vp]
+    lib.tfs_bad_param_count.restype = ll
+    lib.tfs_destroy.argtypes = [vp]
+    lib.tfs_destroy.restype = None
+    lib.tfs_last_error.argtypes = [vp]
+    lib.tfs_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _ptr(x, dtype, nelem=None):
+    """Raw address of a contiguous numpy array or torch tensor of the given dtype (or None)."""
+    if x is None:
+        return None
+    if isinstance(x, np.ndarray):
+        if x.dtype != np.dtype(dtype) or not x.flags["C_CONTIGUOUS"]:
+            raise TypeError(f"expected C-contiguous {np.dtype(dtype)} array, got {x.dtype}")
+        if nelem is not None and x.size < nelem:
+            raise ValueError(f"array too small: {x.size} < {nelem}")
+        return x.ctypes.data
+    import torch
+    if isinstance(x, torch.Tensor):
+        want = {np.float32: torch.float32, np.float64: torch.float64, np.int64: torch.int64,
+                np.uint8: torch.uint8}[dtype]
+        if x.dtype != want or not x.is_contiguous():
+            raise TypeError(f"expected contiguous {want} tensor, got {x.dtype}")
+        if nelem is not None and x.numel() < nelem:
+            raise ValueError(f"tensor too small: {x.numel()} < {nelem}")
+        return x.data_ptr()
+    raise TypeError(f"unsupported buffer type {type(x)}")
+
+
+def _stream(stream):
+    if stream is not None:
+        return int(stream)
+    import torch
+    return torch.cuda.current_stream().cuda_stream
+
+
+class Tfs:
+    """One libtfs context (``tfs_ctx``).  Methods carry the C names without the prefix."""
+
+    def __init__(self, Nt, Nf, dt, n_channels=2, **opts):
+        self._lib = load_library()
+        o = tfs_opts()
+        self._lib.tfs_default_opts(C.byref(o))
+        for k, v in opts.items():
+            if not hasattr(o, k):
+                raise TypeError(f"unknown option {k}")
+            setattr(o, k, v)
+        h = C.c_void_p()
+        rc = self._lib.tfs_create(C.byref(h), Nt, Nf, dt, n_channels, C.byref(o))
+        if rc != TFS_OK:
+            raise TfsError(rc, self._lib.tfs_last_error(None).decode())
+        self._h = h
+        self.Nt, self.Nf, self.dt, self.C = Nt, Nf, dt, n_channels
+
+    def _check(self, rc):
+        if rc != TFS_OK:
+            raise TfsError(rc, self._lib.tfs_last_error(self._h).decode())
+
+    def upload_data(self, coeff, weight=None, gap_mask=None, stream=None):
+        npix = self.C * self.Nt * self.Nf
+        self._check(self._lib.tfs_upload_data(self._h, _ptr(coeff, np.float32, 2 * npix),
+                                              _ptr(weight, np.float32, npix),
+                                              _ptr(gap_mask, np.uint8, self.Nt), _stream(stream)))
+
+    def eval(self, params, N_seg, upsilon, seg_power=None, seg_dh=None, seg_hh=None, n=None, stream=None):
+        if n is None:
+            n = (params.size if isinstance(params, np.ndarray) else params.numel()) // PARAM_COLS
+        self._check(self._lib.tfs_eval(self._h, _ptr(params, np.float64, n * PARAM_COLS), n, N_seg,
+                                       _ptr(upsilon, np.float32, n), _ptr(seg_power, np.float32, n * N_seg),
+                                       _ptr(seg_dh, np.float32, 2 * n * N_seg),
+                                       _ptr(seg_hh, np.float32, n * N_seg), _stream(stream)))
+
+    def topk(self, upsilon, k, idx, val, n=None, stream=None):
+        if n is None:
+            n = upsilon.size if isinstance(upsilon, np.ndarray) else upsilon.numel()
+        self._check(self._lib.tfs_topk(self._h, _ptr(upsilon, np.float32, n), n, k,
+                                       _ptr(idx, np.int64, k), _ptr(val, np.float32, k), _stream(stream)))
+
+    def count_pixels(self, params, counts, n=None, stream=None):
+        if n is None:
+            n = (params.size if isinstance(params, np.ndarray) else params.numel()) // PARAM_COLS
+        self._check(self._lib.tfs_count_pixels(self._h, _ptr(params, np.float64, n * PARAM_COLS), n,
+                                               _ptr(counts, np.int64, n), _stream(stream)))
+
+    def bad_param_count(self):
+        return int(self._lib.tfs_bad_param_count(self._h))
+
+    def last_error(self):
+        return self._lib.tfs_last_error(self._h).decode()
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._lib.tfs_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+# ---- convenience wrappers on host numpy buffers (used by tests, smoke and the e2e bench leg) ----
+def eval_host(ctx: Tfs, params: np.ndarray, N_seg: int, segments: bool = True):
+    """tfs_eval with HOST buffers in and out (the library does the copies)."""
+    params = np.ascontiguousarray(params, dtype=np.float64)
+    n = params.shape[0]
+    ups = np.empty(n, dtype=np.float32)
+    if not segments:
+        ctx.eval(params, N_seg, ups)
+        return dict(upsilon=ups)
+    P = np.empty((n, N_seg), dtype=np.float32)
+    z = np.empty((n, N_seg, 2), dtype=np.float32)
+    hh = np.empty((n, N_seg), dtype=np.float32)
+    ctx.eval(params, N_seg, ups, P, z, hh)
+    return dict(upsilon=ups, seg_power=P, seg_dh=z[..., 0] + 1j * z[..., 1], seg_hh=hh)
+
+
+def topk_host(ctx: Tfs, upsilon: np.ndarray, k: int):
+    upsilon = np.ascontiguousarray(upsilon, dtype=np.float32)
+    idx = np.empty(k, dtype=np.int64)
+    val = np.empty(k, dtype=np.float32)
+    ctx.topk(upsilon, k, idx, val)
+    return idx, val

@@ -1,0 +1,507 @@
+// tfs.cu -- host side of libtfs: C ABI (include/tfs.h), context, launches.
+// No torch, no third-party libraries: CUDA runtime only.
+#include "../../include/tfs.h"
+#include "tfs_kernels.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace tfs;
+
+namespace {
+
+thread_local char g_create_err[512] = "";
+
+constexpr int kTileMax = 256;                 // tranches per time tile (upper bound)
+constexpr size_t kScratchBytes = 1ull << 30;  // cap for the tile-partials buffer per sub-batch
+
+}  // namespace
+
+struct tfs_ctx {
+  int Nt = 0, Nf = 0, C = 0;
+  double dt = 0, DT = 0, df = 0;
+  tfs_opts opts{};
+  double f_lo = 0, f_hi = 0;
+  int device = 0, sm_count = 0;
+  bool uploaded = false;
+
+  float4* grid = nullptr;
+  float2* wgt = nullptr;
+  uint8_t* gap = nullptr;
+  float4* lut = nullptr;
+  unsigned long long* bad = nullptr;       // device counter
+  long long bad_host = 0;
+
+  // growable device scratch
+  void* buf_params = nullptr;   size_t cap_params = 0;
+  void* buf_partials = nullptr; size_t cap_partials = 0;
+  void* buf_out[4] = {nullptr, nullptr, nullptr, nullptr}; size_t cap_out[4] = {0, 0, 0, 0};
+  void* buf_keys = nullptr;     size_t cap_keys = 0;
+  void* buf_tk_in = nullptr;    size_t cap_tk_in = 0;
+  void* buf_tk_idx = nullptr;   size_t cap_tk_idx = 0;
+  void* buf_tk_val = nullptr;   size_t cap_tk_val = 0;
+  void* buf_counts = nullptr;   size_t cap_counts = 0;
+  SelectState* sel = nullptr;
+
+  char err[512] = "";
+};
+
+namespace {
+
+int fail(tfs_ctx* ctx, int code, const char* fmt, ...) {
+  char* dst = ctx ? ctx->err : g_create_err;
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(dst, 512, fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define TFS_CUDA(ctx, expr)                                                              \
+  do {                                                                                   \
+    cudaError_t e_ = (expr);                                                             \
+    if (e_ != cudaSuccess) {                                                             \
+      const int code_ = (e_ == cudaErrorMemoryAllocation) ? TFS_ENOMEM : TFS_ECUDA;      \
+      return fail(ctx, code_, "%s failed: %s", #expr, cudaGetErrorString(e_));           \
+    }                                                                                    \
+  } while (0)
+
+// true if p is device-accessible memory (device or managed); host (pageable/pinned) otherwise
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes at;
+  cudaError_t e = cudaPointerGetAttributes(&at, p);
+  if (e != cudaSuccess) { cudaGetLastError(); return false; }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+int ensure(tfs_ctx* ctx, void** buf, size_t* cap, size_t bytes) {
+  if (*cap >= bytes) return TFS_OK;
+  if (*buf) { cudaFree(*buf); *buf = nullptr; *cap = 0; }
+  const size_t want = bytes + bytes / 8;
+  cudaError_t e = cudaMalloc(buf, want);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    e = cudaMalloc(buf, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(ctx, TFS_ENOMEM, "cudaMalloc(%zu bytes) failed", bytes); }
+    *cap = bytes;
+    return TFS_OK;
+  }
+  *cap = want;
+  return TFS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Host-side Fresnel auxiliary functions f(v), g(v) (A&S 7.3.5-6; ref [52] of the paper) for the LUT.
+//   v <= 5.5 : C(v), S(v) by composite Gauss-Legendre quadrature of the defining integrals
+//   v  > 5.5 : asymptotic series (DLMF 7.12.2-3; ref [53] of the paper)
+// ---------------------------------------------------------------------------------------------
+struct GaussLegendre {
+  static constexpr int N = 16;
+  double x[N], w[N];
+  GaussLegendre() {
+    for (int i = 0; i < N; ++i) {
+      double z = std::cos(kPi * (i + 0.75) / (N + 0.5));
+      double pp = 1.0;
+      for (int it = 0; it < 100; ++it) {
+        double p1 = 1.0, p2 = 0.0;
+        for (int j = 1; j <= N; ++j) { double p3 = p2; p2 = p1; p1 = ((2.0 * j - 1.0) * z * p2 - (j - 1.0) * p3) / j; }
+        pp = N * (z * p1 - p2) / (z * z - 1.0);
+        const double dz = p1 / pp;
+        z -= dz;
+        if (std::fabs(dz) < 1e-16) break;
+      }
+      x[i] = z;
+      w[i] = 2.0 / ((1.0 - z * z) * pp * pp);
+    }
+  }
+};
+
+void fresnel_cs_quadrature(double v, double& C, double& S) {
+  static const GaussLegendre gl;
+  C = 0.0; S = 0.0;
+  const int panels = std::max(1, (int)std::ceil(v / 0.125));
+  const double h = v / panels;
+  for (int p = 0; p < panels; ++p) {
+    const double a = p * h, mid = a + 0.5 * h;
+    for (int i = 0; i < GaussLegendre::N; ++i) {
+      const double t = mid + 0.5 * h * gl.x[i];
+      const double ph = 0.5 * kPi * t * t;
+      C += 0.5 * h * gl.w[i] * std::cos(ph);
+      S += 0.5 * h * gl.w[i] * std::sin(ph);
+    }
+  }
+}
+
+void fresnel_aux_host(double v, double& f, double& g) {
+  if (v <= 5.5) {
+    double C, S;
+    fresnel_cs_quadrature(v, C, S);
+    const double a = 0.5 * kPi * std::fmod(v * v, 4.0);
+    f = (0.5 - S) * std::cos(a) - (0.5 - C) * std::sin(a);
+    g = (0.5 - C) * std::cos(a) + (0.5 - S) * std::sin(a);
+    return;
+  }
+  const double w = 0.5 * kPi * v * v;
+  double sf = 0.0, sg = 0.0, poch = 1.0, wp = 1.0, last = 1e300, sign = 1.0;   // poch = (1/2)_{2m}, wp = w^{2m}
+  for (int m = 0; m < 200; ++m) {
+    const double tf = poch / wp;
+    if (tf > last || tf < 1e-20) break;
+    last = tf;
+    const double tg = poch * (0.5 + 2 * m) / (wp * w);
+    sf += sign * tf;
+    sg += sign * tg;
+    poch *= (0.5 + 2 * m) * (1.5 + 2 * m);
+    wp *= w * w;
+    sign = -sign;
+  }
+  f = sf / (kPi * v);
+  g = sg / (kPi * v);
+}
+
+void build_lut(std::vector<float4>& lut) {
+  std::vector<double> F(kLutN + 1), G(kLutN + 1);
+  F[0] = 1.0 / kPi;       // t -> 0: f/t = f (1+v) -> 1/pi ; g -> 0
+  G[0] = 0.0;
+  for (int i = 1; i <= kLutN; ++i) {
+    const double t = (double)i / kLutN;
+    const double v = 1.0 / t - 1.0;
+    double f, g;
+    fresnel_aux_host(v, f, g);
+    F[i] = f / t;
+    G[i] = g;
+  }
+  lut.resize(kLutN + 1);
+  for (int i = 0; i <= kLutN; ++i) {
+    const int j = std::min(i + 1, kLutN);
+    lut[i] = make_float4((float)F[i], (float)(F[j] - F[i]), (float)G[i], (float)(G[j] - G[i]));
+  }
+}
+
+EvalArgs base_args(const tfs_ctx* ctx) {
+  EvalArgs a{};
+  a.grid = ctx->grid; a.wgt = ctx->wgt; a.gap = ctx->gap; a.lut = ctx->lut;
+  a.bad_count = ctx->bad;
+  a.Nt = ctx->Nt; a.Nf = ctx->Nf;
+  a.H = ctx->opts.half_width; a.adaptive = ctx->opts.adaptive_width;
+  a.DT = ctx->DT;
+  a.x_lo = ctx->f_lo * ctx->DT; a.x_hi = ctx->f_hi * ctx->DT;
+  a.c_max = ctx->opts.c_max;
+  a.N_seg = 1; a.tiles_per_seg = 1; a.n_tiles = 1;
+  return a;
+}
+
+// params on host -> staged copy in ctx scratch; on device -> used in place
+int stage_params(tfs_ctx* ctx, const double* params, long long n, cudaStream_t st, const double** d_params) {
+  if (is_device_ptr(params)) { *d_params = params; return TFS_OK; }
+  const size_t bytes = (size_t)n * TFS_PARAM_COLS * sizeof(double);
+  int rc = ensure(ctx, &ctx->buf_params, &ctx->cap_params, bytes);
+  if (rc) return rc;
+  TFS_CUDA(ctx, cudaMemcpyAsync(ctx->buf_params, params, bytes, cudaMemcpyHostToDevice, st));
+  *d_params = (const double*)ctx->buf_params;
+  return TFS_OK;
+}
+
+}  // namespace
+
+// =============================================================================================
+extern "C" {
+
+void tfs_default_opts(tfs_opts* o) {
+  if (!o) return;
+  o->half_width = 10;
+  o->adaptive_width = 1;
+  o->c_max = 300.0;
+  o->f_lo = 0.0;
+  o->f_hi = 0.0;
+  o->fresnel_mode = 0;
+}
+
+const char* tfs_last_error(const tfs_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
+
+long long tfs_bad_param_count(const tfs_ctx* ctx) {
+  if (!ctx) return 0;
+  if (ctx->bad_host < 0) {
+    // the last tfs_eval wrote only device outputs and did not synchronise: read the counter now
+    unsigned long long bad = 0;
+    if (cudaDeviceSynchronize() != cudaSuccess ||
+        cudaMemcpy(&bad, ctx->bad, sizeof(bad), cudaMemcpyDeviceToHost) != cudaSuccess) {
+      cudaGetLastError();
+      return -1;
+    }
+    const_cast<tfs_ctx*>(ctx)->bad_host = (long long)bad;
+  }
+  return ctx->bad_host;
+}
+
+int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const tfs_opts* opts) {
+  if (!out) return fail(nullptr, TFS_EINVAL, "tfs_create: out is NULL");
+  *out = nullptr;
+  if (Nt < 1 || Nf < 2 || !(dt > 0.0) || !std::isfinite(dt))
+    return fail(nullptr, TFS_EINVAL, "tfs_create: need Nt >= 1, Nf >= 2, dt > 0 (got %d, %d, %g)", Nt, Nf, dt);
+  if ((long long)Nt * Nf >= (1ll << 31))
+    return fail(nullptr, TFS_EINVAL, "tfs_create: Nt*Nf must be < 2^31");
+  if (n_channels != 2)
+    return fail(nullptr, TFS_EINVAL, "tfs_create: this build supports n_channels == 2 (A, E); got %d", n_channels);
+  tfs_opts o;
+  tfs_default_opts(&o);
+  if (opts) o = *opts;
+  if (o.half_width < 0 || o.half_width > 4096 || !(o.c_max >= 0.0) || o.c_max > 1e6 ||
+      (o.fresnel_mode != 0 && o.fresnel_mode != 1))
+    return fail(nullptr, TFS_EINVAL, "tfs_create: bad options (half_width %d, c_max %g, fresnel_mode %d)",
+                o.half_width, o.c_max, o.fresnel_mode);
+  tfs_ctx* ctx = new (std::nothrow) tfs_ctx();
+  if (!ctx) return fail(nullptr, TFS_ENOMEM, "tfs_create: host allocation failed");
+  ctx->Nt = Nt; ctx->Nf = Nf; ctx->C = n_channels; ctx->dt = dt;
+  ctx->DT = 2.0 * Nf * dt;
+  ctx->df = 1.0 / ctx->DT;
+  ctx->opts = o;
+  ctx->f_lo = o.f_lo > 0.0 ? o.f_lo : ctx->df;
+  ctx->f_hi = o.f_hi > 0.0 ? o.f_hi : (Nf - 1) * ctx->df;
+
+  auto bail = [&](int code, const char* what, cudaError_t e) {
+    fail(nullptr, code, "tfs_create: %s: %s", what, cudaGetErrorString(e));
+    tfs_destroy(ctx);
+    return code;
+  };
+  cudaError_t e = cudaGetDevice(&ctx->device);
+  if (e != cudaSuccess) return bail(TFS_ECUDA, "cudaGetDevice (no CUDA device: libtfs has no CPU fallback)", e);
+  e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
+  if (e != cudaSuccess) return bail(TFS_ECUDA, "cudaDeviceGetAttribute", e);
+  const size_t npix = (size_t)Nt * Nf;
+  if ((e = cudaMalloc((void**)&ctx->grid, npix * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc grid", e);
+  if ((e = cudaMalloc((void**)&ctx->wgt, npix * sizeof(float2))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc weights", e);
+  if ((e = cudaMalloc((void**)&ctx->gap, (size_t)Nt)) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc gap", e);
+  if ((e = cudaMalloc((void**)&ctx->lut, (kLutN + 1) * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc lut", e);
+  if ((e = cudaMalloc((void**)&ctx->bad, sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
+  if ((e = cudaMalloc((void**)&ctx->sel, sizeof(SelectState))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc select state", e);
+  std::vector<float4> lut;
+  build_lut(lut);
+  if ((e = cudaMemcpy(ctx->lut, lut.data(), lut.size() * sizeof(float4), cudaMemcpyHostToDevice)) != cudaSuccess)
+    return bail(TFS_ECUDA, "cudaMemcpy lut", e);
+  *out = ctx;
+  return TFS_OK;
+}
+
+void tfs_destroy(tfs_ctx* ctx) {
+  if (!ctx) return;
+  void* bufs[] = {ctx->grid, ctx->wgt, ctx->gap, ctx->lut, ctx->bad, ctx->sel, ctx->buf_params, ctx->buf_partials,
+                  ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
+                  ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts};
+  for (void* b : bufs) if (b) cudaFree(b);
+  delete ctx;
+}
+
+int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const uint8_t* gap_mask, void* stream) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_upload_data: ctx is NULL");
+  if (!coeff) return fail(ctx, TFS_EINVAL, "tfs_upload_data: coeff is NULL");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t npix = (size_t)ctx->Nt * ctx->Nf;
+  const float* d_coeff = coeff;
+  const float* d_weight = weight;
+  void* tmp_c = nullptr;
+  void* tmp_w = nullptr;
+  int rc = TFS_OK;
+  auto cleanup = [&]() { if (tmp_c) cudaFree(tmp_c); if (tmp_w) cudaFree(tmp_w); };
+#define UP_CUDA(expr)                                                                      \
+  do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { cleanup();                       \
+       return fail(ctx, e_ == cudaErrorMemoryAllocation ? TFS_ENOMEM : TFS_ECUDA,          \
+                   "%s failed: %s", #expr, cudaGetErrorString(e_)); } } while (0)
+  if (!is_device_ptr(coeff)) {
+    UP_CUDA(cudaMalloc(&tmp_c, npix * 2 * 2 * sizeof(float)));
+    UP_CUDA(cudaMemcpyAsync(tmp_c, coeff, npix * 2 * 2 * sizeof(float), cudaMemcpyHostToDevice, st));
+    d_coeff = (const float*)tmp_c;
+  }
+  if (weight && !is_device_ptr(weight)) {
+    UP_CUDA(cudaMalloc(&tmp_w, npix * 2 * sizeof(float)));
+    UP_CUDA(cudaMemcpyAsync(tmp_w, weight, npix * 2 * sizeof(float), cudaMemcpyHostToDevice, st));
+    d_weight = (const float*)tmp_w;
+  }
+  if (gap_mask) {
+    UP_CUDA(cudaMemcpyAsync(ctx->gap, gap_mask, (size_t)ctx->Nt,
+                            is_device_ptr(gap_mask) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+  } else {
+    UP_CUDA(cudaMemsetAsync(ctx->gap, 1, (size_t)ctx->Nt, st));
+  }
+  const int threads = 256;
+  const unsigned blocks = (unsigned)((npix + threads - 1) / threads);
+  pack_kernel<<<blocks, threads, 0, st>>>((const float2*)d_coeff, d_weight, (long long)npix, ctx->grid, ctx->wgt);
+  UP_CUDA(cudaGetLastError());
+  if (tmp_c || tmp_w || (gap_mask && !is_device_ptr(gap_mask))) UP_CUDA(cudaStreamSynchronize(st));
+  cleanup();
+#undef UP_CUDA
+  ctx->uploaded = true;
+  return rc;
+}
+
+int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* upsilon, float* seg_power,
+             float* seg_dh, float* seg_hh, void* stream) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_eval: ctx is NULL");
+  if (n < 0) return fail(ctx, TFS_EINVAL, "tfs_eval: n < 0");
+  if (N_seg < 1 || N_seg > ctx->Nt) return fail(ctx, TFS_EINVAL, "tfs_eval: need 1 <= N_seg <= Nt (got %d, Nt %d)", N_seg, ctx->Nt);
+  if (!ctx->uploaded) return fail(ctx, TFS_ESTATE, "tfs_eval: no data uploaded (call tfs_upload_data first)");
+  if (n == 0) { ctx->bad_host = 0; return TFS_OK; }
+  if (!params || !upsilon) return fail(ctx, TFS_EINVAL, "tfs_eval: params and upsilon are required");
+  if (n >= (1ll << 32)) return fail(ctx, TFS_EINVAL, "tfs_eval: n must be < 2^32");
+  cudaStream_t st = (cudaStream_t)stream;
+
+  const double* d_params = nullptr;
+  int rc = stage_params(ctx, params, n, st, &d_params);
+  if (rc) return rc;
+
+  // outputs: device pointers are written in place, host pointers via ctx scratch + D2H
+  float* user[4] = {upsilon, seg_power, seg_dh, seg_hh};
+  const size_t per[4] = {1, (size_t)N_seg, (size_t)N_seg * 2, (size_t)N_seg};
+  float* dev[4] = {nullptr, nullptr, nullptr, nullptr};
+  bool host_out[4] = {false, false, false, false};
+  bool any_host = false;
+  for (int i = 0; i < 4; ++i) {
+    if (!user[i]) continue;
+    if (is_device_ptr(user[i])) { dev[i] = user[i]; continue; }
+    host_out[i] = true; any_host = true;
+    rc = ensure(ctx, &ctx->buf_out[i], &ctx->cap_out[i], (size_t)n * per[i] * sizeof(float));
+    if (rc) return rc;
+    dev[i] = (float*)ctx->buf_out[i];
+  }
+
+  // tiling: each segment is cut into tiles_per_seg tiles of <= kTileMax tranches
+  const int max_seg_len = (ctx->Nt + N_seg - 1) / N_seg;
+  const int tps = (max_seg_len + kTileMax - 1) / kTileMax;
+  const int n_tiles = N_seg * tps;
+  long long sub = (long long)(kScratchBytes / ((size_t)n_tiles * sizeof(float4)));
+  sub = std::max<long long>(sub, 1024);
+  sub = std::min<long long>(sub, n);
+  rc = ensure(ctx, &ctx->buf_partials, &ctx->cap_partials, (size_t)sub * n_tiles * sizeof(float4));
+  if (rc) return rc;
+
+  TFS_CUDA(ctx, cudaMemsetAsync(ctx->bad, 0, sizeof(unsigned long long), st));
+  EvalArgs a = base_args(ctx);
+  a.N_seg = N_seg; a.tiles_per_seg = tps; a.n_tiles = n_tiles;
+  a.partials = (float4*)ctx->buf_partials;
+  for (long long off = 0; off < n; off += sub) {
+    const long long nb = std::min(sub, n - off);
+    a.params = d_params + off * TFS_PARAM_COLS;
+    a.n = nb;
+    const long long n_work = nb * n_tiles;
+    const long long want = (n_work + kWarpsPerCta - 1) / kWarpsPerCta;
+    const unsigned blocks = (unsigned)std::min<long long>(want, (long long)ctx->sm_count * 16);
+    if (ctx->opts.fresnel_mode == 0)
+      eval_tiles_kernel<0><<<blocks, kWarpsPerCta * 32, 0, st>>>(a);
+    else
+      eval_tiles_kernel<1><<<blocks, kWarpsPerCta * 32, 0, st>>>(a);
+    TFS_CUDA(ctx, cudaGetLastError());
+    const int threads = 128;
+    combine_kernel<<<(unsigned)((nb + threads - 1) / threads), threads, 0, st>>>(
+        a.partials, nb, N_seg, tps, dev[0] + off, dev[1] ? dev[1] + off * per[1] : nullptr,
+        dev[2] ? dev[2] + off * per[2] : nullptr, dev[3] ? dev[3] + off * per[3] : nullptr);
+    TFS_CUDA(ctx, cudaGetLastError());
+  }
+  if (any_host) {
+    for (int i = 0; i < 4; ++i)
+      if (host_out[i])
+        TFS_CUDA(ctx, cudaMemcpyAsync(user[i], dev[i], (size_t)n * per[i] * sizeof(float), cudaMemcpyDeviceToHost, st));
+    unsigned long long bad = 0;
+    TFS_CUDA(ctx, cudaMemcpyAsync(&bad, ctx->bad, sizeof(bad), cudaMemcpyDeviceToHost, st));
+    TFS_CUDA(ctx, cudaStreamSynchronize(st));
+    ctx->bad_host = (long long)bad;
+  } else {
+    ctx->bad_host = -1;     // not known yet: tfs_bad_param_count synchronises and reads it on demand
+    if (!is_device_ptr(params)) TFS_CUDA(ctx, cudaStreamSynchronize(st));   // host params buffer may be reused
+  }
+  return TFS_OK;
+}
+
+int tfs_count_pixels(tfs_ctx* ctx, const double* params, long long n, long long* counts, void* stream) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_count_pixels: ctx is NULL");
+  if (n < 0) return fail(ctx, TFS_EINVAL, "tfs_count_pixels: n < 0");
+  if (!ctx->uploaded) return fail(ctx, TFS_ESTATE, "tfs_count_pixels: no data uploaded (the gap mask is part of the data)");
+  if (n == 0) return TFS_OK;
+  if (!params || !counts) return fail(ctx, TFS_EINVAL, "tfs_count_pixels: params and counts are required");
+  cudaStream_t st = (cudaStream_t)stream;
+  const double* d_params = nullptr;
+  int rc = stage_params(ctx, params, n, st, &d_params);
+  if (rc) return rc;
+  long long* d_counts = counts;
+  const bool host = !is_device_ptr(counts);
+  if (host) {
+    rc = ensure(ctx, &ctx->buf_counts, &ctx->cap_counts, (size_t)n * sizeof(long long));
+    if (rc) return rc;
+    d_counts = (long long*)ctx->buf_counts;
+  }
+  EvalArgs a = base_args(ctx);
+  a.params = d_params;
+  a.n = n;
+  const int threads = 256;
+  const long long blocks = (n * 32 + threads - 1) / threads;
+  count_pixels_kernel<<<(unsigned)blocks, threads, 0, st>>>(a, d_counts);
+  TFS_CUDA(ctx, cudaGetLastError());
+  if (host) {
+    TFS_CUDA(ctx, cudaMemcpyAsync(counts, d_counts, (size_t)n * sizeof(long long), cudaMemcpyDeviceToHost, st));
+    TFS_CUDA(ctx, cudaStreamSynchronize(st));
+  } else if (!is_device_ptr(params)) {
+    TFS_CUDA(ctx, cudaStreamSynchronize(st));
+  }
+  return TFS_OK;
+}
+
+int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k, long long* idx, float* val, void* stream) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_topk: ctx is NULL");
+  if (!upsilon || !idx || !val) return fail(ctx, TFS_EINVAL, "tfs_topk: upsilon, idx and val are required");
+  if (n < 1 || n >= (1ll << 32)) return fail(ctx, TFS_EINVAL, "tfs_topk: need 1 <= n < 2^32");
+  if (k < 1 || k > n) return fail(ctx, TFS_EINVAL, "tfs_topk: need 1 <= k <= n (got k %d, n %lld)", k, n);
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc;
+  const float* d_in = upsilon;
+  if (!is_device_ptr(upsilon)) {
+    rc = ensure(ctx, &ctx->buf_tk_in, &ctx->cap_tk_in, (size_t)n * sizeof(float));
+    if (rc) return rc;
+    TFS_CUDA(ctx, cudaMemcpyAsync(ctx->buf_tk_in, upsilon, (size_t)n * sizeof(float), cudaMemcpyHostToDevice, st));
+    d_in = (const float*)ctx->buf_tk_in;
+  }
+  unsigned P = 1;
+  while (P < (unsigned)k) P <<= 1;
+  rc = ensure(ctx, &ctx->buf_keys, &ctx->cap_keys, (size_t)P * sizeof(unsigned long long));
+  if (rc) return rc;
+  unsigned long long* keys = (unsigned long long*)ctx->buf_keys;
+  long long* d_idx = idx;
+  float* d_val = val;
+  const bool host_idx = !is_device_ptr(idx), host_val = !is_device_ptr(val);
+  if (host_idx) {
+    rc = ensure(ctx, &ctx->buf_tk_idx, &ctx->cap_tk_idx, (size_t)k * sizeof(long long));
+    if (rc) return rc;
+    d_idx = (long long*)ctx->buf_tk_idx;
+  }
+  if (host_val) {
+    rc = ensure(ctx, &ctx->buf_tk_val, &ctx->cap_tk_val, (size_t)k * sizeof(float));
+    if (rc) return rc;
+    d_val = (float*)ctx->buf_tk_val;
+  }
+  const int threads = 256;
+  const unsigned blocks = (unsigned)std::min<long long>((n + threads - 1) / threads, (long long)ctx->sm_count * 8);
+  topk_init_kernel<<<1, 256, 0, st>>>(ctx->sel, (unsigned long long)k);
+  for (int pass = 0; pass < 8; ++pass) {
+    topk_hist_kernel<<<blocks, threads, 0, st>>>(d_in, n, pass, ctx->sel);
+    topk_pick_kernel<<<1, 256, 0, st>>>(pass, ctx->sel);
+  }
+  topk_gather_kernel<<<blocks, threads, 0, st>>>(d_in, n, ctx->sel, keys, (unsigned)k);
+  if (P > (unsigned)k) topk_pad_kernel<<<(P - k + threads - 1) / threads, threads, 0, st>>>(keys, (unsigned)k, P);
+  if (P <= 4096) {
+    bitonic_small_kernel<<<1, 1024, P * sizeof(unsigned long long), st>>>(keys, P);
+  } else {
+    for (unsigned size = 2; size <= P; size <<= 1)
+      for (unsigned stride = size >> 1; stride > 0; stride >>= 1)
+        bitonic_step_kernel<<<(P / 2 + threads - 1) / threads, threads, 0, st>>>(keys, P, size, stride);
+  }
+  topk_emit_kernel<<<(k + threads - 1) / threads, threads, 0, st>>>(keys, d_in, k, d_idx, d_val);
+  TFS_CUDA(ctx, cudaGetLastError());
+  if (host_idx) TFS_CUDA(ctx, cudaMemcpyAsync(idx, d_idx, (size_t)k * sizeof(long long), cudaMemcpyDeviceToHost, st));
+  if (host_val) TFS_CUDA(ctx, cudaMemcpyAsync(val, d_val, (size_t)k * sizeof(float), cudaMemcpyDeviceToHost, st));
+  if (host_idx || host_val || !is_device_ptr(upsilon)) TFS_CUDA(ctx, cudaStreamSynchronize(st));
+  return TFS_OK;
+}
+
+}  // extern "C"
