@@ -108,6 +108,15 @@ TFS_API int tfs_count_pixels(tfs_ctx* ctx, const double* params, long long n, lo
 /* Templates rejected (NaN/Inf/Mc<=0) by the most recent tfs_eval on this context. */
 TFS_API long long tfs_bad_param_count(const tfs_ctx* ctx);
 
+/* Measurement hooks (bench.py).  With profiling on, every launch of the main kernel (track +
+ * gather + tile sums) inside tfs_eval is bracketed by CUDA events on the caller's stream.
+ * tfs_get_profile synchronises those events and returns, since the last call of
+ * tfs_set_profiling: the summed duration [ms] and number of main-kernel launches, and the number
+ * of kernels of this library launched in total (all entry points).  Any output may be NULL. */
+TFS_API int tfs_set_profiling(tfs_ctx* ctx, int on);
+TFS_API int tfs_get_profile(tfs_ctx* ctx, double* main_kernel_ms, long long* main_kernel_launches,
+                            long long* kernel_launches);
+
 TFS_API void tfs_destroy(tfs_ctx* ctx);
 
 /* Message of the last failure on this context (or of the last failed tfs_create when ctx is

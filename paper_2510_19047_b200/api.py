@@ -56,6 +56,10 @@ def load_library():
     lib.tfs_count_pixels.restype = ip
     lib.tfs_bad_param_count.argtypes = [vp]
     lib.tfs_bad_param_count.restype = ll
+    lib.tfs_set_profiling.argtypes = [vp, ip]
+    lib.tfs_set_profiling.restype = ip
+    lib.tfs_get_profile.argtypes = [vp, C.POINTER(dp), C.POINTER(ll), C.POINTER(ll)]
+    lib.tfs_get_profile.restype = ip
     lib.tfs_destroy.argtypes = [vp]
     lib.tfs_destroy.restype = None
     lib.tfs_last_error.argtypes = [vp]
@@ -143,6 +147,14 @@ class Tfs:
 
     def bad_param_count(self):
         return int(self._lib.tfs_bad_param_count(self._h))
+
+    def set_profiling(self, on=True):
+        self._check(self._lib.tfs_set_profiling(self._h, int(bool(on))))
+
+    def get_profile(self):
+        ms, nk, nl = C.c_double(), C.c_longlong(), C.c_longlong()
+        self._check(self._lib.tfs_get_profile(self._h, C.byref(ms), C.byref(nk), C.byref(nl)))
+        return dict(main_kernel_ms=ms.value, main_kernel_launches=nk.value, kernel_launches=nl.value)
 
     def last_error(self):
         return self._lib.tfs_last_error(self._h).decode()

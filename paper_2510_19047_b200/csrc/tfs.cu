@@ -48,6 +48,12 @@ struct tfs_ctx {
   void* buf_counts = nullptr;   size_t cap_counts = 0;
   SelectState* sel = nullptr;
 
+  // measurement hooks
+  bool profiling = false;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pool;   // reused event pairs
+  size_t ev_used = 0;
+  long long launches = 0;
+
   char err[512] = "";
 };
 
@@ -287,8 +293,32 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   return TFS_OK;
 }
 
+int tfs_set_profiling(tfs_ctx* ctx, int on) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_set_profiling: ctx is NULL");
+  ctx->profiling = (on != 0);
+  ctx->ev_used = 0;
+  ctx->launches = 0;
+  return TFS_OK;
+}
+
+int tfs_get_profile(tfs_ctx* ctx, double* main_kernel_ms, long long* main_kernel_launches, long long* kernel_launches) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_get_profile: ctx is NULL");
+  double ms = 0.0;
+  for (size_t i = 0; i < ctx->ev_used; ++i) {
+    float t = 0.f;
+    TFS_CUDA(ctx, cudaEventSynchronize(ctx->ev_pool[i].second));
+    TFS_CUDA(ctx, cudaEventElapsedTime(&t, ctx->ev_pool[i].first, ctx->ev_pool[i].second));
+    ms += t;
+  }
+  if (main_kernel_ms) *main_kernel_ms = ms;
+  if (main_kernel_launches) *main_kernel_launches = (long long)ctx->ev_used;
+  if (kernel_launches) *kernel_launches = ctx->launches;
+  return TFS_OK;
+}
+
 void tfs_destroy(tfs_ctx* ctx) {
   if (!ctx) return;
+  for (auto& p : ctx->ev_pool) { cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
   void* bufs[] = {ctx->grid, ctx->wgt, ctx->gap, ctx->lut, ctx->bad, ctx->sel, ctx->buf_params, ctx->buf_partials,
                   ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
                   ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts};
@@ -331,6 +361,7 @@ int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const
   const unsigned blocks = (unsigned)((npix + threads - 1) / threads);
   pack_kernel<<<blocks, threads, 0, st>>>((const float2*)d_coeff, d_weight, (long long)npix, ctx->grid, ctx->wgt);
   UP_CUDA(cudaGetLastError());
+  ctx->launches += 1;
   if (tmp_c || tmp_w || (gap_mask && !is_device_ptr(gap_mask))) UP_CUDA(cudaStreamSynchronize(st));
   cleanup();
 #undef UP_CUDA
@@ -389,11 +420,26 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
     const long long n_work = nb * n_tiles;
     const long long want = (n_work + kWarpsPerCta - 1) / kWarpsPerCta;
     const unsigned blocks = (unsigned)std::min<long long>(want, (long long)ctx->sm_count * 16);
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    if (ctx->profiling) {
+      if (ctx->ev_used == ctx->ev_pool.size()) {
+        cudaEvent_t e0, e1;
+        TFS_CUDA(ctx, cudaEventCreate(&e0));
+        TFS_CUDA(ctx, cudaEventCreate(&e1));
+        ctx->ev_pool.emplace_back(e0, e1);
+      }
+      ev0 = ctx->ev_pool[ctx->ev_used].first;
+      ev1 = ctx->ev_pool[ctx->ev_used].second;
+      ++ctx->ev_used;
+      TFS_CUDA(ctx, cudaEventRecord(ev0, st));
+    }
     if (ctx->opts.fresnel_mode == 0)
       eval_tiles_kernel<0><<<blocks, kWarpsPerCta * 32, 0, st>>>(a);
     else
       eval_tiles_kernel<1><<<blocks, kWarpsPerCta * 32, 0, st>>>(a);
     TFS_CUDA(ctx, cudaGetLastError());
+    if (ev1) TFS_CUDA(ctx, cudaEventRecord(ev1, st));
+    ctx->launches += 2;     // main kernel + combine
     const int threads = 128;
     combine_kernel<<<(unsigned)((nb + threads - 1) / threads), threads, 0, st>>>(
         a.partials, nb, N_seg, tps, dev[0] + off, dev[1] ? dev[1] + off * per[1] : nullptr,
@@ -439,6 +485,7 @@ int tfs_count_pixels(tfs_ctx* ctx, const double* params, long long n, long long*
   const long long blocks = (n * 32 + threads - 1) / threads;
   count_pixels_kernel<<<(unsigned)blocks, threads, 0, st>>>(a, d_counts);
   TFS_CUDA(ctx, cudaGetLastError());
+  ctx->launches += 1;
   if (host) {
     TFS_CUDA(ctx, cudaMemcpyAsync(counts, d_counts, (size_t)n * sizeof(long long), cudaMemcpyDeviceToHost, st));
     TFS_CUDA(ctx, cudaStreamSynchronize(st));
@@ -483,18 +530,25 @@ int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k, long long* 
   const int threads = 256;
   const unsigned blocks = (unsigned)std::min<long long>((n + threads - 1) / threads, (long long)ctx->sm_count * 8);
   topk_init_kernel<<<1, 256, 0, st>>>(ctx->sel, (unsigned long long)k);
+  ctx->launches += 1 + 16 + 1 + 1;   // init, 8 x (hist, pick), gather, emit
   for (int pass = 0; pass < 8; ++pass) {
     topk_hist_kernel<<<blocks, threads, 0, st>>>(d_in, n, pass, ctx->sel);
     topk_pick_kernel<<<1, 256, 0, st>>>(pass, ctx->sel);
   }
   topk_gather_kernel<<<blocks, threads, 0, st>>>(d_in, n, ctx->sel, keys, (unsigned)k);
-  if (P > (unsigned)k) topk_pad_kernel<<<(P - k + threads - 1) / threads, threads, 0, st>>>(keys, (unsigned)k, P);
+  if (P > (unsigned)k) {
+    topk_pad_kernel<<<(P - k + threads - 1) / threads, threads, 0, st>>>(keys, (unsigned)k, P);
+    ctx->launches += 1;
+  }
   if (P <= 4096) {
     bitonic_small_kernel<<<1, 1024, P * sizeof(unsigned long long), st>>>(keys, P);
+    ctx->launches += 1;
   } else {
     for (unsigned size = 2; size <= P; size <<= 1)
-      for (unsigned stride = size >> 1; stride > 0; stride >>= 1)
+      for (unsigned stride = size >> 1; stride > 0; stride >>= 1) {
         bitonic_step_kernel<<<(P / 2 + threads - 1) / threads, threads, 0, st>>>(keys, P, size, stride);
+        ctx->launches += 1;
+      }
   }
   topk_emit_kernel<<<(k + threads - 1) / threads, threads, 0, st>>>(keys, d_in, k, d_idx, d_val);
   TFS_CUDA(ctx, cudaGetLastError());
