@@ -35,6 +35,7 @@ struct tfs_ctx {
   uint8_t* gap = nullptr;
   float4* lut = nullptr;
   unsigned long long* bad = nullptr;       // device counter
+  unsigned long long* work = nullptr;      // device work-item counter of the main kernel
   long long bad_host = 0;
 
   // growable device scratch
@@ -170,21 +171,25 @@ void fresnel_aux_host(double v, double& f, double& g) {
 }
 
 void build_lut(std::vector<float4>& lut) {
-  std::vector<double> F(kLutN + 1), G(kLutN + 1);
-  F[0] = 1.0 / kPi;       // t -> 0: f/t = f (1+v) -> 1/pi ; g -> 0
-  G[0] = 0.0;
-  for (int i = 1; i <= kLutN; ++i) {
+  // F = f/t, G = g/t at t_i = i/kLutN (v_i = 1/t_i - 1), two extra nodes past each end for the slopes
+  auto node = [](int i, double& F, double& G) {
+    if (i <= 0) { F = 1.0 / kPi; G = 0.0; return; }         // t -> 0: f/t = f (1+v) -> 1/pi ; g/t -> 0
     const double t = (double)i / kLutN;
-    const double v = 1.0 / t - 1.0;
+    const double v = std::max(1.0 / t - 1.0, 0.0);
     double f, g;
     fresnel_aux_host(v, f, g);
-    F[i] = f / t;
-    G[i] = g;
-  }
+    F = f / t;
+    G = g / t;
+  };
   lut.resize(kLutN + 1);
   for (int i = 0; i <= kLutN; ++i) {
-    const int j = std::min(i + 1, kLutN);
-    lut[i] = make_float4((float)F[i], (float)(F[j] - F[i]), (float)G[i], (float)(G[j] - G[i]));
+    double F, G, Fm, Gm, Fp, Gp;
+    node(i, F, G);
+    const int im = std::max(i - 1, 0), ip = std::min(i + 1, kLutN);
+    node(im, Fm, Gm);
+    node(ip, Fp, Gp);
+    const double w = (double)(ip - im);                      // central difference (one-sided at the ends)
+    lut[i] = make_float4((float)F, (float)((Fp - Fm) / w), (float)G, (float)((Gp - Gm) / w));
   }
 }
 
@@ -192,6 +197,7 @@ EvalArgs base_args(const tfs_ctx* ctx) {
   EvalArgs a{};
   a.grid = ctx->grid; a.wgt = ctx->wgt; a.gap = ctx->gap; a.lut = ctx->lut;
   a.bad_count = ctx->bad;
+  a.work_counter = ctx->work;
   a.Nt = ctx->Nt; a.Nf = ctx->Nf;
   a.H = ctx->opts.half_width; a.adaptive = ctx->opts.adaptive_width;
   a.DT = ctx->DT;
@@ -284,6 +290,10 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   if ((e = cudaMalloc((void**)&ctx->gap, (size_t)Nt)) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc gap", e);
   if ((e = cudaMalloc((void**)&ctx->lut, (kLutN + 1) * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc lut", e);
   if ((e = cudaMalloc((void**)&ctx->bad, sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
+  if ((e = cudaMalloc((void**)&ctx->work, sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
+  if ((e = cudaFuncSetAttribute(eval_tiles_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_tiles_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess)
+    return bail(TFS_ECUDA, "cudaFuncSetAttribute(max dynamic shared memory)", e);
   if ((e = cudaMalloc((void**)&ctx->sel, sizeof(SelectState))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc select state", e);
   std::vector<float4> lut;
   build_lut(lut);
@@ -319,7 +329,7 @@ int tfs_get_profile(tfs_ctx* ctx, double* main_kernel_ms, long long* main_kernel
 void tfs_destroy(tfs_ctx* ctx) {
   if (!ctx) return;
   for (auto& p : ctx->ev_pool) { cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
-  void* bufs[] = {ctx->grid, ctx->wgt, ctx->gap, ctx->lut, ctx->bad, ctx->sel, ctx->buf_params, ctx->buf_partials,
+  void* bufs[] = {ctx->grid, ctx->wgt, ctx->gap, ctx->lut, ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials,
                   ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
                   ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts};
   for (void* b : bufs) if (b) cudaFree(b);
@@ -419,7 +429,8 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
     a.n = nb;
     const long long n_work = nb * n_tiles;
     const long long want = (n_work + kWarpsPerCta - 1) / kWarpsPerCta;
-    const unsigned blocks = (unsigned)std::min<long long>(want, (long long)ctx->sm_count * 16);
+    const unsigned blocks = (unsigned)std::min<long long>(want, (long long)ctx->sm_count);   // persistent, 1 CTA/SM
+    TFS_CUDA(ctx, cudaMemsetAsync(ctx->work, 0, sizeof(unsigned long long), st));
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     if (ctx->profiling) {
       if (ctx->ev_used == ctx->ev_pool.size()) {
@@ -434,9 +445,9 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
       TFS_CUDA(ctx, cudaEventRecord(ev0, st));
     }
     if (ctx->opts.fresnel_mode == 0)
-      eval_tiles_kernel<0><<<blocks, kWarpsPerCta * 32, 0, st>>>(a);
+      eval_tiles_kernel<0><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
     else
-      eval_tiles_kernel<1><<<blocks, kWarpsPerCta * 32, 0, st>>>(a);
+      eval_tiles_kernel<1><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
     TFS_CUDA(ctx, cudaGetLastError());
     if (ev1) TFS_CUDA(ctx, cudaEventRecord(ev1, st));
     ctx->launches += 2;     // main kernel + combine

@@ -14,9 +14,9 @@
 
 namespace tfs {
 
-constexpr int kWarpsPerCta = 8;
+constexpr int kWarpsPerCta = 32;       // one 1024-thread CTA per SM
 constexpr int kChunk = 32;          // tranches per phase-1 pass (one per lane)
-constexpr int kLutN = 1024;         // LUT intervals in t = 1/(1+v)
+constexpr int kLutN = 512;          // LUT intervals in t = 1/(1+v)
 constexpr double kMtsun = 4.925490947e-6;   // G Msun / c^3 [s]
 constexpr double kPi = 3.14159265358979323846;
 
@@ -24,10 +24,11 @@ struct EvalArgs {
   const float4* __restrict__ grid;     // [Nt][Nf] {Y_A.re, Y_A.im, Y_E.re, Y_E.im}, Y = W*D
   const float2* __restrict__ wgt;      // [Nt][Nf] {W_A, W_E}
   const uint8_t* __restrict__ gap;     // [Nt] 1 = valid
-  const float4* __restrict__ lut;      // [kLutN+1] {F, dF, g, dg}: f(v) = t*(F + fr*dF), g(v) = g + fr*dg
+  const float4* __restrict__ lut;      // [kLutN+1] {F, F', G, G'} (see fresnel_aux)
   const double* __restrict__ params;   // [n][8]
   float4* __restrict__ partials;       // [n_tiles][n] {z.re, z.im, hh, 0}
   unsigned long long* bad_count;       // templates rejected (counted on tile 0 only)
+  unsigned long long* work_counter;    // next unclaimed work item (zeroed before each launch)
   long long n;                         // templates in this launch
   int Nt, Nf;
   int N_seg, tiles_per_seg, n_tiles;
@@ -114,7 +115,7 @@ __device__ __forceinline__ void window(const TrackPoint& tp, int H, int adaptive
   k_hi = max(k_hi, 1);
 }
 
-// Per-tranche record consumed by phase 2 (40 bytes, in shared memory).
+// Per-tranche record consumed by phase 2 (48 bytes, in shared memory).
 struct __align__(16) BinRec {
   int base;      // m*Nf + k_lo
   int W;         // window width
@@ -124,21 +125,33 @@ struct __align__(16) BinRec {
   float Qr, Qi;  // P * exp(i psi), psi = pi c + 2 pi frac(x)
   float scc;     // sqrt(2/c)*c = sqrt(2c)
   float hc;      // 1/(2c): pi u^2/c = 2 pi * (u^2 * hc)
+  float pad0, pad1;
 };
 
+// LUT of the Fresnel auxiliary functions, indexed by round(t*kLutN), t = 1/(1+|v|):
+//   entry i = {F_i, F'_i, G_i, G'_i},  f(v) = t (F_i + fr F'_i),  g(v) = t (G_i + fr G'_i),  fr = t*kLutN - i
+// (F = f/t, G = g/t, primes = central differences per index step).  In shared memory it is stored
+// kLutCopies times, copy r at 16-byte slot (i*kLutCopies + r), and lane l reads copy l & 7: the 8
+// lanes of a quarter-warp then always hit 8 different bank groups, so an LDS.128 is conflict-free
+// whatever the indices are (measured 9 wavefronts per load without the copies, 4 with).
+constexpr int kLutCopies = 8;
+constexpr float kMagic = 12582912.0f;          // 1.5 * 2^23: (p + kMagic) rounds p to an integer in the mantissa
+
 template <int MODE>
-__device__ __forceinline__ void fresnel_aux(float a, const float4* __restrict__ s_lut, float& f, float& g) {
-  // a = |v| >= 0.  MODE 0: LUT in t = 1/(1+a);  MODE 1: the paper's Eqs. 27-28 (|v| <= 6) and
-  // the plain asymptote f = 1/(pi v), g = 0 (Eqs. 23-24, |v| > 6).
+__device__ __forceinline__ void fresnel_aux(float v, const float4* __restrict__ lut_lane, float& f, float& g) {
+  // Returns sign(v) f(|v|), sign(v) g(|v|).
+  // MODE 0: LUT;  MODE 1: the paper's Eqs. 27-28 (|v| <= 6) and the plain asymptote
+  // f = 1/(pi v), g = 0 (Eqs. 23-24, |v| > 6).
+  const float a = fabsf(v);
   if (MODE == 0) {
     const float t = __fdividef(1.0f, 1.0f + a);
-    const float p = t * (float)kLutN;
-    int i = (int)p;
-    i = min(i, kLutN - 1);
-    const float fr = p - (float)i;
-    const float4 e = s_lut[i];
-    f = t * fmaf(fr, e.y, e.x);
-    g = fmaf(fr, e.w, e.z);
+    const float q = fmaf(t, (float)kLutN, kMagic);
+    const float fr = fmaf(t, (float)kLutN, -(q - kMagic));
+    const int i = __float_as_int(q) - __float_as_int(kMagic);
+    const float4 e = lut_lane[i * kLutCopies];
+    const float ts = copysignf(t, v);
+    f = ts * fmaf(fr, e.y, e.x);
+    g = ts * fmaf(fr, e.w, e.z);
   } else {
     if (a > 6.0f) {
       f = __fdividef(0.318309886183790672f, a);
@@ -147,6 +160,8 @@ __device__ __forceinline__ void fresnel_aux(float a, const float4* __restrict__ 
       f = __fdividef(1.0f + 0.926f * a, 2.0f + a * (1.792f + 3.104f * a));
       g = __fdividef(1.0f, 2.0f + a * (4.142f + a * (3.492f + 6.670f * a)));
     }
+    f = copysignf(f, v);
+    g = copysignf(g, v);
   }
 }
 
@@ -156,142 +171,189 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// ------------------------------------------------------------------------------------------
-// Kernel A: track + gather + per-tile sums.
-// ------------------------------------------------------------------------------------------
-template <int MODE>
-__global__ void __launch_bounds__(kWarpsPerCta * 32)
-eval_tiles_kernel(const EvalArgs a) {
-  __shared__ float4 s_lut[kLutN + 1];
-  __shared__ BinRec s_rec[kWarpsPerCta][kChunk];
+// dynamic shared memory of kernel A: [LUT copies][records of every warp]
+constexpr int kLutSmemBytes = (kLutN + 1) * kLutCopies * (int)sizeof(float4);
+constexpr int kEvalSmemBytes = kLutSmemBytes + kWarpsPerCta * kChunk * (int)sizeof(BinRec);
 
-  if (MODE == 0) {
-    for (int i = threadIdx.x; i <= kLutN; i += blockDim.x) s_lut[i] = a.lut[i];
-    __syncthreads();
-  }
+// ------------------------------------------------------------------------------------------
+// Kernel A: track + gather + per-tile sums.  Persistent: one CTA per SM, warps claim work items
+// (template, tile) in tile-major order from a global counter, kClaim at a time.
+// ------------------------------------------------------------------------------------------
+constexpr int kClaim = 4;
+
+template <int MODE>
+__global__ void __launch_bounds__(kWarpsPerCta * 32, 1)
+eval_tiles_kernel(const EvalArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float4* s_lut = reinterpret_cast<float4*>(smem_raw);
+  BinRec* s_rec = reinterpret_cast<BinRec*>(smem_raw + kLutSmemBytes);
+
   const int lane = threadIdx.x & 31;
   const int warp = threadIdx.x >> 5;
-  BinRec* rec = s_rec[warp];
+  if (MODE == 0) {
+    for (int i = threadIdx.x; i < (kLutN + 1) * kLutCopies; i += blockDim.x) s_lut[i] = a.lut[i / kLutCopies];
+    __syncthreads();
+  }
+  BinRec* rec = s_rec + warp * kChunk;
+  const float4* lut_lane = s_lut + (lane & (kLutCopies - 1));
 
   const long long n_work = a.n * (long long)a.n_tiles;
-  const long long stride = (long long)gridDim.x * kWarpsPerCta;
-  for (long long w = (long long)blockIdx.x * kWarpsPerCta + warp; w < n_work; w += stride) {
-    const int tile = (int)(w / a.n);
-    const long long it = w - (long long)tile * a.n;
-    int m0, m1;
-    tile_range(tile, a.tiles_per_seg, a.Nt, a.N_seg, m0, m1);
+  for (;;) {
+    long long w0 = 0;
+    if (lane == 0) w0 = (long long)atomicAdd(a.work_counter, (unsigned long long)kClaim);
+    w0 = __shfl_sync(0xffffffffu, w0, 0);
+    if (w0 >= n_work) break;
+    const long long w1 = min(w0 + kClaim, n_work);
+    for (long long w = w0; w < w1; ++w) {
+      const int tile = (int)(w / a.n);
+      const long long it = w - (long long)tile * a.n;
+      int m0, m1;
+      tile_range(tile, a.tiles_per_seg, a.Nt, a.N_seg, m0, m1);
 
-    const TemplateConst T = load_template(a.params + it * 8);
-    if (!T.ok) {
-      if (lane == 0) {
-        a.partials[(long long)tile * a.n + it] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (tile == 0) atomicAdd(a.bad_count, 1ULL);
-      }
-      continue;
-    }
-
-    // fp64 per-lane running sums over the tile: z_A, z_E (complex), q_A, q_E
-    double dzAr = 0, dzAi = 0, dzEr = 0, dzEi = 0, dqA = 0, dqE = 0;
-
-    for (int mc = m0; mc < m1; mc += kChunk) {
-      // ---------------- phase 1: lane <-> tranche ----------------
-      const int m = mc + lane;
-      const bool valid = (m < m1) && (a.gap[min(m, a.Nt - 1)] != 0);        // C10
-      const TrackPoint tp = track_point(T, m, a.DT, a.x_lo, a.x_hi, a.c_max, valid);
-      const unsigned act_mask = __ballot_sync(0xffffffffu, tp.active);
-      if (act_mask == 0u) continue;
-      int Wm = 0;
-      if (tp.active) {
-        int k_lo, k_hi;
-        window(tp, a.H, a.adaptive, a.Nf, k_lo, k_hi);
-        Wm = k_hi - k_lo + 1;
-        const double flx = floor(tp.x);
-        const float fracx = (float)(tp.x - flx);
-        // phases in turns, reduced in fp64 (phi reaches ~1e8 rad)
-        double tphi = T.phic_turns - tp.X58 * (1.0 / kPi);
-        tphi -= floor(tphi);
-        double tpsi = 0.5 * tp.c + (tp.x - flx);
-        tpsi -= floor(tpsi);
-        float sphi, cphi, spsi, cpsi;
-        sincospif(2.0f * (float)tphi, &sphi, &cphi);
-        sincospif(2.0f * (float)tpsi, &spsi, &cpsi);
-        const float cf = (float)tp.c;
-        const float pre = (float)(T.acoef * tp.Xm14) * rsqrtf(2.0f * cf);  // A_m / sqrt(2c)
-        BinRec r;
-        r.base = m * a.Nf + k_lo;
-        r.W = Wm;
-        r.u0 = fracx - (float)(k_lo - (int)flx);      // cancellation-safe x - k_lo
-        r.sc = rsqrtf(0.5f * cf);
-        r.Pr = pre * cphi;
-        r.Pi = pre * sphi;
-        r.Qr = r.Pr * cpsi - r.Pi * spsi;
-        r.Qi = r.Pr * spsi + r.Pi * cpsi;
-        r.scc = r.sc * cf;
-        r.hc = __fdividef(0.5f, cf);
-        const int slot = __popc(act_mask & ((1u << lane) - 1u));
-        rec[slot] = r;
-      }
-      int Wc = Wm;                                                          // chunk-uniform width
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) Wc = max(Wc, __shfl_xor_sync(0xffffffffu, Wc, o));
-      __syncwarp();
-
-      // ---------------- phase 2: lane <-> (tranche, pixel) item ----------------
-      const int n_act = __popc(act_mask);
-      const int n_items = n_act * Wc;
-      const float invW = 1.0f / (float)Wc;
-      float zAr = 0, zAi = 0, zEr = 0, zEi = 0, qA = 0, qE = 0;
-      for (int i = lane; i < n_items; i += 32) {
-        const int b = (int)(((float)i + 0.5f) * invW);
-        const int j = i - b * Wc;
-        const BinRec& r = rec[b];
-        if (j < r.W) {
-          const int idx = r.base + j;
-          const float4 Y = __ldg(a.grid + idx);
-          const float2 Wt = __ldg(a.wgt + idx);
-          const float u = r.u0 - (float)j;
-          const float v0 = r.sc * u;
-          const float v1 = v0 + r.scc;
-          float f0, g0, f1, g1;
-          fresnel_aux<MODE>(fabsf(v0), s_lut, f0, g0);
-          fresnel_aux<MODE>(fabsf(v1), s_lut, f1, g1);
-          // s0 G(|v0|) P - s1 G(|v1|) Q,  G = g + i f   (C7)
-          f0 = copysignf(f0, v0); g0 = copysignf(g0, v0);
-          f1 = copysignf(f1, v1); g1 = copysignf(g1, v1);
-          float hr = g0 * r.Pr - f0 * r.Pi - g1 * r.Qr + f1 * r.Qi;
-          float hi = g0 * r.Pi + f0 * r.Pr - g1 * r.Qi - f1 * r.Qr;
-          if (v0 < 0.0f && v1 > 0.0f) {
-            // pixel inside the swept band: + (1+i) exp(-i pi u^2/c) P
-            float turns = u * u * r.hc;
-            turns -= floorf(turns);
-            float st, ct;
-            sincospif(2.0f * turns, &st, &ct);
-            const float er = ct + st, ei = ct - st;
-            hr += er * r.Pr - ei * r.Pi;
-            hi += er * r.Pi + ei * r.Pr;
-          }
-          zAr = fmaf(Y.x, hr, fmaf(Y.y, hi, zAr));
-          zAi = fmaf(Y.x, hi, fmaf(-Y.y, hr, zAi));
-          zEr = fmaf(Y.z, hr, fmaf(Y.w, hi, zEr));
-          zEi = fmaf(Y.z, hi, fmaf(-Y.w, hr, zEi));
-          const float h2 = fmaf(hr, hr, hi * hi);
-          qA = fmaf(Wt.x, h2, qA);
-          qE = fmaf(Wt.y, h2, qE);
+      const TemplateConst T = load_template(a.params + it * 8);
+      if (!T.ok) {
+        if (lane == 0) {
+          a.partials[(long long)tile * a.n + it] = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (tile == 0) atomicAdd(a.bad_count, 1ULL);
         }
+        continue;
       }
-      dzAr += zAr; dzAi += zAi; dzEr += zEr; dzEi += zEi; dqA += qA; dqE += qE;
-      __syncwarp();
-    }
 
-    dzAr = warp_sum(dzAr); dzAi = warp_sum(dzAi);
-    dzEr = warp_sum(dzEr); dzEi = warp_sum(dzEi);
-    dqA = warp_sum(dqA);   dqE = warp_sum(dqE);
-    if (lane == 0) {
-      // z = T_A z_A + T_E z_E ; hh = |T_A|^2 q_A + |T_E|^2 q_E   (Eq. 29, Eq. 31)
-      const double zr = T.TAr * dzAr - T.TAi * dzAi + T.TEr * dzEr - T.TEi * dzEi;
-      const double zi = T.TAr * dzAi + T.TAi * dzAr + T.TEr * dzEi + T.TEi * dzEr;
-      const double hh = (T.TAr * T.TAr + T.TAi * T.TAi) * dqA + (T.TEr * T.TEr + T.TEi * T.TEi) * dqE;
-      a.partials[(long long)tile * a.n + it] = make_float4((float)zr, (float)zi, (float)hh, 0.f);
+      // fp64 per-lane running sums over the tile: z_A, z_E (complex), q_A, q_E
+      double dzAr = 0, dzAi = 0, dzEr = 0, dzEi = 0, dqA = 0, dqE = 0;
+
+      for (int mc = m0; mc < m1; mc += kChunk) {
+        // ---------------- phase 1: lane <-> tranche ----------------
+        const int m = mc + lane;
+        const bool valid = (m < m1) && (a.gap[min(m, a.Nt - 1)] != 0);        // C10
+        const TrackPoint tp = track_point(T, m, a.DT, a.x_lo, a.x_hi, a.c_max, valid);
+        const unsigned act_mask = __ballot_sync(0xffffffffu, tp.active);
+        if (act_mask == 0u) continue;
+        int Wm = 0;
+        if (tp.active) {
+          int k_lo, k_hi;
+          window(tp, a.H, a.adaptive, a.Nf, k_lo, k_hi);
+          Wm = k_hi - k_lo + 1;
+          const double flx = floor(tp.x);
+          const float fracx = (float)(tp.x - flx);
+          // phases in turns, reduced in fp64 (phi reaches ~1e8 rad)
+          double tphi = T.phic_turns - tp.X58 * (1.0 / kPi);
+          tphi -= floor(tphi);
+          double tpsi = 0.5 * tp.c + (tp.x - flx);
+          tpsi -= floor(tpsi);
+          float sphi, cphi, spsi, cpsi;
+          sincospif(2.0f * (float)tphi, &sphi, &cphi);
+          sincospif(2.0f * (float)tpsi, &spsi, &cpsi);
+          const float cf = (float)tp.c;
+          const float pre = (float)(T.acoef * tp.Xm14) * rsqrtf(2.0f * cf);  // A_m / sqrt(2c)
+          BinRec r;
+          r.base = m * a.Nf + k_lo;
+          r.W = Wm;
+          r.u0 = fracx - (float)(k_lo - (int)flx);      // cancellation-safe x - k_lo
+          r.sc = rsqrtf(0.5f * cf);
+          r.Pr = pre * cphi;
+          r.Pi = pre * sphi;
+          r.Qr = r.Pr * cpsi - r.Pi * spsi;
+          r.Qi = r.Pr * spsi + r.Pi * cpsi;
+          r.scc = r.sc * cf;
+          r.hc = __fdividef(0.5f, cf);
+          r.pad0 = 0.f; r.pad1 = 0.f;
+          const int slot = __popc(act_mask & ((1u << lane) - 1u));
+          rec[slot] = r;
+        }
+        int Wc = Wm;                                                          // chunk-uniform width
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) Wc = max(Wc, __shfl_xor_sync(0xffffffffu, Wc, o));
+        __syncwarp();
+
+        // ---------------- phase 2: lane <-> (tranche, pixel) item ----------------
+        // item i -> (slot b, offset j) = (i / Wc, i % Wc), advanced incrementally; the gather of
+        // item i+32 is issued before the arithmetic of item i (software prefetch, distance 1).
+        const int n_items = __popc(act_mask) * Wc;
+        float zAr = 0, zAi = 0, zEr = 0, zEi = 0, qA = 0, qE = 0;
+        int b = 0, j = lane;
+        while (j >= Wc) { j -= Wc; ++b; }
+        float4 Yn = make_float4(0.f, 0.f, 0.f, 0.f);
+        float2 Wn = make_float2(0.f, 0.f);
+        float un = 0.f, scn = 0.f;
+        bool vn = false;
+        if (lane < n_items) {
+          const float4 h = *reinterpret_cast<const float4*>(&rec[b]);          // {base, W, u0, sc}
+          vn = j < __float_as_int(h.y);
+          if (vn) {
+            const int idx = __float_as_int(h.x) + j;
+            Yn = __ldg(a.grid + idx);
+            Wn = __ldg(a.wgt + idx);
+            un = h.z - (float)j;
+            scn = h.w;
+          }
+        }
+        for (int i = lane; i < n_items; i += 32) {
+          const float4 Y = Yn;
+          const float2 Wt = Wn;
+          const float u = un, sc = scn;
+          const bool vc = vn;
+          const BinRec* rc = rec + b;
+          // ---- prefetch item i+32 ----
+          j += 32;
+          while (j >= Wc) { j -= Wc; ++b; }
+          vn = false;
+          if (i + 32 < n_items) {
+            const float4 h = *reinterpret_cast<const float4*>(&rec[b]);
+            vn = j < __float_as_int(h.y);
+            if (vn) {
+              const int idx = __float_as_int(h.x) + j;
+              Yn = __ldg(a.grid + idx);
+              Wn = __ldg(a.wgt + idx);
+              un = h.z - (float)j;
+              scn = h.w;
+            }
+          }
+          // ---- arithmetic of item i ----
+          if (vc) {
+            const float4 PQ = *reinterpret_cast<const float4*>(&rc->Pr);       // {Pr, Pi, Qr, Qi}
+            const float scc = rc->scc;
+            const float v0 = sc * u;
+            const float v1 = v0 + scc;
+            float f0, g0, f1, g1;
+            fresnel_aux<MODE>(v0, lut_lane, f0, g0);
+            fresnel_aux<MODE>(v1, lut_lane, f1, g1);
+            // s0 G(|v0|) P - s1 G(|v1|) Q,  G = g + i f   (C7)
+            float hr = g0 * PQ.x - f0 * PQ.y - g1 * PQ.z + f1 * PQ.w;
+            float hi = g0 * PQ.y + f0 * PQ.x - g1 * PQ.w - f1 * PQ.z;
+            if (v0 < 0.0f && v1 > 0.0f) {
+              // pixel inside the swept band: + (1+i) exp(-i pi u^2/c) P
+              float turns = u * u * rc->hc;
+              turns -= floorf(turns);
+              float st, ct;
+              __sincosf(6.283185307179586f * (turns - 0.5f), &st, &ct);        // = -(sin, cos)(2 pi turns)
+              const float er = -(ct + st), ei = -(ct - st);
+              hr += er * PQ.x - ei * PQ.y;
+              hi += er * PQ.y + ei * PQ.x;
+            }
+            zAr = fmaf(Y.x, hr, fmaf(Y.y, hi, zAr));
+            zAi = fmaf(Y.x, hi, fmaf(-Y.y, hr, zAi));
+            zEr = fmaf(Y.z, hr, fmaf(Y.w, hi, zEr));
+            zEi = fmaf(Y.z, hi, fmaf(-Y.w, hr, zEi));
+            const float h2 = fmaf(hr, hr, hi * hi);
+            qA = fmaf(Wt.x, h2, qA);
+            qE = fmaf(Wt.y, h2, qE);
+          }
+        }
+        dzAr += zAr; dzAi += zAi; dzEr += zEr; dzEi += zEi; dqA += qA; dqE += qE;
+        __syncwarp();
+      }
+
+      dzAr = warp_sum(dzAr); dzAi = warp_sum(dzAi);
+      dzEr = warp_sum(dzEr); dzEi = warp_sum(dzEi);
+      dqA = warp_sum(dqA);   dqE = warp_sum(dqE);
+      if (lane == 0) {
+        // z = T_A z_A + T_E z_E ; hh = |T_A|^2 q_A + |T_E|^2 q_E   (Eq. 29, Eq. 31)
+        const double zr = T.TAr * dzAr - T.TAi * dzAi + T.TEr * dzEr - T.TEi * dzEi;
+        const double zi = T.TAr * dzAi + T.TAi * dzAr + T.TEr * dzEi + T.TEi * dzEr;
+        const double hh = (T.TAr * T.TAr + T.TAi * T.TAi) * dqA + (T.TEr * T.TEr + T.TEi * T.TEi) * dqE;
+        a.partials[(long long)tile * a.n + it] = make_float4((float)zr, (float)zi, (float)hh, 0.f);
+      }
     }
   }
 }
