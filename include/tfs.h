@@ -73,8 +73,9 @@ TFS_API int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels,
  *   coeff    [C][Nt][Nf][2] float, (re, im) of D[alpha, m, k]          host or device, required
  *   weight   [C][Nt][Nf]    float, W >= 0 per pixel (C11)               host or device, NULL => 1
  *   gap_mask [Nt]           uint8, 1 = valid, 0 = tranche overlaps a gap (C10); NULL => all valid
- * The library stores Y = W*D interleaved by channel and W, frequency-contiguous.  May be called
- * again to replace the data.  Returns after the copy out of host memory is complete. */
+ * The library keeps its own repacked copy (Y = W*D interleaved by channel, and W, both transposed
+ * to time-contiguous [k][m]) plus the compacted list of valid tranches.  May be called again to
+ * replace the data.  Returns after the copy out of host memory is complete. */
 TFS_API int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight,
                     const uint8_t* gap_mask, void* stream);
 

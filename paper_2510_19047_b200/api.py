@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libtfs.so")
+LIB_PATH = os.environ.get("TFS_LIB_PATH") or os.path.join(_HERE, "libtfs.so")   # override: A/B-testing builds
 
 TFS_OK, TFS_EINVAL, TFS_ESTATE, TFS_ENOMEM, TFS_ECUDA = 0, -1, -2, -3, -4
 PARAM_COLS = 8

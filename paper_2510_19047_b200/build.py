@@ -31,6 +31,8 @@ def up_to_date() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    if os.environ.get("TFS_LIB_PATH"):          # an explicitly chosen prebuilt library: nothing to do
+        return os.environ["TFS_LIB_PATH"]
     if not force and up_to_date():
         return LIB
     extra = ["-Xptxas", "-v"] if verbose else []

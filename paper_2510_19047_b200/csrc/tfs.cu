@@ -17,7 +17,6 @@ namespace {
 
 thread_local char g_create_err[512] = "";
 
-constexpr int kTileMax = 256;                 // tranches per time tile (upper bound)
 constexpr size_t kScratchBytes = 1ull << 30;  // cap for the tile-partials buffer per sub-batch
 
 }  // namespace
@@ -33,6 +32,8 @@ struct tfs_ctx {
   float4* grid = nullptr;
   float2* wgt = nullptr;
   uint8_t* gap = nullptr;
+  int* vprefix = nullptr;                  // [Nt+1] valid tranches before m
+  int* valid_m = nullptr;                  // [max(#valid,1)] valid tranche indices
   float4* lut = nullptr;
   unsigned long long* bad = nullptr;       // device counter
   unsigned long long* work = nullptr;      // device work-item counter of the main kernel
@@ -189,13 +190,16 @@ void build_lut(std::vector<float4>& lut) {
     node(im, Fm, Gm);
     node(ip, Fp, Gp);
     const double w = (double)(ip - im);                      // central difference (one-sided at the ends)
-    lut[i] = make_float4((float)F, (float)((Fp - Fm) / w), (float)G, (float)((Gp - Gm) / w));
+    // interpolant around node i as intercept + slope * t:  F(t) ~ F_i + (t kLutN - i) dF  (see fresnel_aux)
+    const double dF = (Fp - Fm) / w, dG = (Gp - Gm) / w;
+    lut[i] = make_float4((float)(F - i * dF), (float)(kLutN * dF), (float)(G - i * dG), (float)(kLutN * dG));
   }
 }
 
 EvalArgs base_args(const tfs_ctx* ctx) {
   EvalArgs a{};
   a.grid = ctx->grid; a.wgt = ctx->wgt; a.gap = ctx->gap; a.lut = ctx->lut;
+  a.vprefix = ctx->vprefix; a.valid_m = ctx->valid_m;
   a.bad_count = ctx->bad;
   a.work_counter = ctx->work;
   a.Nt = ctx->Nt; a.Nf = ctx->Nf;
@@ -288,6 +292,8 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   if ((e = cudaMalloc((void**)&ctx->grid, npix * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc grid", e);
   if ((e = cudaMalloc((void**)&ctx->wgt, npix * sizeof(float2))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc weights", e);
   if ((e = cudaMalloc((void**)&ctx->gap, (size_t)Nt)) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc gap", e);
+  if ((e = cudaMalloc((void**)&ctx->vprefix, ((size_t)Nt + 1) * sizeof(int))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc vprefix", e);
+  if ((e = cudaMalloc((void**)&ctx->valid_m, (size_t)Nt * sizeof(int))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc valid_m", e);
   if ((e = cudaMalloc((void**)&ctx->lut, (kLutN + 1) * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc lut", e);
   if ((e = cudaMalloc((void**)&ctx->bad, sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
   if ((e = cudaMalloc((void**)&ctx->work, sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
@@ -329,7 +335,7 @@ int tfs_get_profile(tfs_ctx* ctx, double* main_kernel_ms, long long* main_kernel
 void tfs_destroy(tfs_ctx* ctx) {
   if (!ctx) return;
   for (auto& p : ctx->ev_pool) { cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
-  void* bufs[] = {ctx->grid, ctx->wgt, ctx->gap, ctx->lut, ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials,
+  void* bufs[] = {ctx->grid, ctx->wgt, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut, ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials,
                   ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
                   ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts};
   for (void* b : bufs) if (b) cudaFree(b);
@@ -367,11 +373,12 @@ int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const
   } else {
     UP_CUDA(cudaMemsetAsync(ctx->gap, 1, (size_t)ctx->Nt, st));
   }
-  const int threads = 256;
-  const unsigned blocks = (unsigned)((npix + threads - 1) / threads);
-  pack_kernel<<<blocks, threads, 0, st>>>((const float2*)d_coeff, d_weight, (long long)npix, ctx->grid, ctx->wgt);
+  const dim3 blocks((unsigned)((ctx->Nf + 31) / 32), (unsigned)((ctx->Nt + 31) / 32));
+  pack_kernel<<<blocks, 256, 0, st>>>((const float2*)d_coeff, d_weight, ctx->Nt, ctx->Nf, ctx->grid, ctx->wgt);
   UP_CUDA(cudaGetLastError());
-  ctx->launches += 1;
+  valid_list_kernel<<<1, 1024, 0, st>>>(ctx->gap, ctx->Nt, ctx->vprefix, ctx->valid_m);
+  UP_CUDA(cudaGetLastError());
+  ctx->launches += 2;
   if (tmp_c || tmp_w || (gap_mask && !is_device_ptr(gap_mask))) UP_CUDA(cudaStreamSynchronize(st));
   cleanup();
 #undef UP_CUDA

@@ -2,29 +2,32 @@
 // DESIGN.md section 6 for the kernel design.  Citations: P:<line> of PAPER.md, C<n> = DESIGN.md.
 //
 // Work decomposition: one WARP evaluates one (template, time tile) pair.  A time tile is a run
-// of <= TILE_MAX consecutive tranches inside one segment; work items are ordered tile-major so
+// of <= kTileMax consecutive tranches inside one segment; work items are ordered tile-major so
 // that all templates sweep the same slab of the grid together and the slab stays L2-resident.
-// Inside a tile the warp alternates, per chunk of 32 tranches, between
-//   phase 1: lane <-> tranche: fp64 0PN track, window, phases  -> per-tranche record in smem
-//   phase 2: lane <-> (tranche, pixel) item of the flattened window list: Fresnel-kernel value
-//            from the auxiliary-function LUT, 16-byte gather of both channels, accumulate.
+// Inside a tile lanes are tranches (32 at a time): fp64 0PN track per lane, then each lane walks
+// its own window; the grid is stored time-contiguous so those loads coalesce across lanes.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace tfs {
 
-constexpr int kWarpsPerCta = 32;       // one 1024-thread CTA per SM
-constexpr int kChunk = 32;          // tranches per phase-1 pass (one per lane)
+#ifndef TFS_WARPS_PER_CTA
+#define TFS_WARPS_PER_CTA 24
+#endif
+constexpr int kWarpsPerCta = TFS_WARPS_PER_CTA;   // one persistent CTA per SM
+constexpr int kTileMax = 256;       // tranches per time tile (upper bound)
 constexpr int kLutN = 512;          // LUT intervals in t = 1/(1+v)
 constexpr double kMtsun = 4.925490947e-6;   // G Msun / c^3 [s]
 constexpr double kPi = 3.14159265358979323846;
 
 struct EvalArgs {
-  const float4* __restrict__ grid;     // [Nt][Nf] {Y_A.re, Y_A.im, Y_E.re, Y_E.im}, Y = W*D
-  const float2* __restrict__ wgt;      // [Nt][Nf] {W_A, W_E}
+  const float4* __restrict__ grid;     // [Nf][Nt] (time-contiguous) {Y_A.re, Y_A.im, Y_E.re, Y_E.im}, Y = W*D
+  const float2* __restrict__ wgt;      // [Nf][Nt] {W_A, W_E}
   const uint8_t* __restrict__ gap;     // [Nt] 1 = valid
-  const float4* __restrict__ lut;      // [kLutN+1] {F, F', G, G'} (see fresnel_aux)
+  const int* __restrict__ vprefix;     // [Nt+1] number of valid tranches before m
+  const int* __restrict__ valid_m;     // [vprefix[Nt]] the valid tranche indices, ascending (padded to >= 1 entry)
+  const float4* __restrict__ lut;      // [kLutN+1] {a_F, b_F, a_G, b_G} (see fresnel_aux)
   const double* __restrict__ params;   // [n][8]
   float4* __restrict__ partials;       // [n_tiles][n] {z.re, z.im, hh, 0}
   unsigned long long* bad_count;       // templates rejected (counted on tile 0 only)
@@ -115,44 +118,46 @@ __device__ __forceinline__ void window(const TrackPoint& tp, int H, int adaptive
   k_hi = max(k_hi, 1);
 }
 
-// Per-tranche record consumed by phase 2 (48 bytes, in shared memory).
-struct __align__(16) BinRec {
-  int base;      // m*Nf + k_lo
-  int W;         // window width
-  float u0;      // x - k_lo
-  float sc;      // sqrt(2/c)
-  float Pr, Pi;  // A/sqrt(2c) * exp(i phi_m)
-  float Qr, Qi;  // P * exp(i psi), psi = pi c + 2 pi frac(x)
-  float scc;     // sqrt(2/c)*c = sqrt(2c)
-  float hc;      // 1/(2c): pi u^2/c = 2 pi * (u^2 * hc)
-  float pad0, pad1;
-};
-
-// LUT of the Fresnel auxiliary functions, indexed by round(t*kLutN), t = 1/(1+|v|):
-//   entry i = {F_i, F'_i, G_i, G'_i},  f(v) = t (F_i + fr F'_i),  g(v) = t (G_i + fr G'_i),  fr = t*kLutN - i
-// (F = f/t, G = g/t, primes = central differences per index step).  In shared memory it is stored
-// kLutCopies times, copy r at 16-byte slot (i*kLutCopies + r), and lane l reads copy l & 7: the 8
-// lanes of a quarter-warp then always hit 8 different bank groups, so an LDS.128 is conflict-free
-// whatever the indices are (measured 9 wavefronts per load without the copies, 4 with).
+// LUT of the Fresnel auxiliary functions f(v), g(v) (P:184-207 defines them through Eqs. 25-26;
+// A&S 7.3.5-6), tabulated against t = 1/(1+|v|) in (0, 1] with kLutN intervals:
+//   entry i = {a_F, b_F, a_G, b_G}: for t within half a step of i/kLutN,
+//     f(v) = t (a_F + b_F t),  g(v) = t (a_G + b_G t)
+//   (the linear interpolant of F = f/t, G = g/t around node i with central-difference slope,
+//    rewritten as intercept + slope*t so the fractional index is never formed).
+// In shared memory it is stored kLutCopies times, copy r of entry i at 16-byte slot
+// (i*kLutCopies + r), and lane l reads copy l & 7: the 8 lanes of a quarter-warp always hit 8
+// different bank groups, so an LDS.128 is conflict-free whatever the indices are.
 constexpr int kLutCopies = 8;
 constexpr float kMagic = 12582912.0f;          // 1.5 * 2^23: (p + kMagic) rounds p to an integer in the mantissa
+constexpr unsigned kMagicBits = 0x4B400000u;
 
+__device__ __forceinline__ float rcp_approx(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
+__device__ __forceinline__ float4 lds128(unsigned addr) {
+  float4 r;
+  asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "r"(addr));
+  return r;
+}
+
+// Returns F = f(|v|)/t, G = g(|v|)/t and ts = sign(v) t, so that sign(v) f = ts F, sign(v) g = ts G.
+// lut_lane = shared address of this lane's LUT copy minus kMagicBits * (16 * kLutCopies)  (mod 2^32).
 template <int MODE>
-__device__ __forceinline__ void fresnel_aux(float v, const float4* __restrict__ lut_lane, float& f, float& g) {
-  // Returns sign(v) f(|v|), sign(v) g(|v|).
-  // MODE 0: LUT;  MODE 1: the paper's Eqs. 27-28 (|v| <= 6) and the plain asymptote
-  // f = 1/(pi v), g = 0 (Eqs. 23-24, |v| > 6).
+__device__ __forceinline__ void fresnel_aux(float v, unsigned lut_lane, float& F, float& G, float& ts) {
   const float a = fabsf(v);
   if (MODE == 0) {
-    const float t = __fdividef(1.0f, 1.0f + a);
+    const float t = rcp_approx(1.0f + a);         // MUFU.RCP
     const float q = fmaf(t, (float)kLutN, kMagic);
-    const float fr = fmaf(t, (float)kLutN, -(q - kMagic));
-    const int i = __float_as_int(q) - __float_as_int(kMagic);
-    const float4 e = lut_lane[i * kLutCopies];
-    const float ts = copysignf(t, v);
-    f = ts * fmaf(fr, e.y, e.x);
-    g = ts * fmaf(fr, e.w, e.z);
+    const float4 e = lds128(__float_as_uint(q) * (16u * kLutCopies) + lut_lane);
+    ts = copysignf(t, v);
+    F = fmaf(t, e.y, e.x);
+    G = fmaf(t, e.w, e.z);
   } else {
+    // the paper's Eqs. 27-28 (|v| <= 6) and the plain asymptote f = 1/(pi v), g = 0 (Eqs. 23-24, |v| > 6)
+    float f, g;
     if (a > 6.0f) {
       f = __fdividef(0.318309886183790672f, a);
       g = 0.0f;
@@ -160,8 +165,9 @@ __device__ __forceinline__ void fresnel_aux(float v, const float4* __restrict__ 
       f = __fdividef(1.0f + 0.926f * a, 2.0f + a * (1.792f + 3.104f * a));
       g = __fdividef(1.0f, 2.0f + a * (4.142f + a * (3.492f + 6.670f * a)));
     }
-    f = copysignf(f, v);
-    g = copysignf(g, v);
+    ts = copysignf(1.0f, v);
+    F = f;
+    G = g;
   }
 }
 
@@ -171,13 +177,63 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// dynamic shared memory of kernel A: [LUT copies][records of every warp]
+// dynamic shared memory of kernel A: [LUT copies][fp64 tile sums: 6 per thread, stored [6][threads]]
 constexpr int kLutSmemBytes = (kLutN + 1) * kLutCopies * (int)sizeof(float4);
-constexpr int kEvalSmemBytes = kLutSmemBytes + kWarpsPerCta * kChunk * (int)sizeof(BinRec);
+constexpr int kEvalSmemBytes = kLutSmemBytes + 6 * kWarpsPerCta * 32 * (int)sizeof(double);
+
+// One pixel of one tranche (a3-a5): template coefficient from the auxiliary-function form of Eq. 16
+// (DESIGN.md section 6.3), then z_alpha += Y_alpha^* h, q_alpha += W_alpha |h|^2 for both channels.
+struct LaneTrack {      // per-lane (= per-tranche) constants of the pixel loop
+  float sc;             // sqrt(2/c)
+  float scc;            // sqrt(2c) = v1 - v0
+  float hc;             // 1/(2c): pi u^2/c = 2 pi (u^2 hc)
+  float Pr, Pi;         // A/sqrt(2c) exp(i phi_m)
+  float Qr, Qi;         // P exp(i psi), psi = pi c + 2 pi frac(x)
+};
+
+struct LaneSums { float zAr, zAi, zEr, zEi, qA, qE; };
+
+template <int MODE>
+__device__ __forceinline__ void pixel(const LaneTrack& L, float u, const float4 Y, const float2 Wt,
+                                      unsigned lut_lane, LaneSums& s) {
+  const float v0 = L.sc * u;
+  const float v1 = v0 + L.scc;
+  float F0, G0, t0, F1, G1, t1;
+  fresnel_aux<MODE>(v0, lut_lane, F0, G0, t0);
+  fresnel_aux<MODE>(v1, lut_lane, F1, G1, t1);
+  // h = s0 G(|v0|) P - s1 G(|v1|) Q,  G = g + i f
+  const float w0r = G0 * L.Pr - F0 * L.Pi, w0i = G0 * L.Pi + F0 * L.Pr;
+  const float w1r = G1 * L.Qr - F1 * L.Qi, w1i = G1 * L.Qi + F1 * L.Qr;
+  float hr = fmaf(t0, w0r, -t1 * w1r);
+  float hi = fmaf(t0, w0i, -t1 * w1i);
+  if (v0 < 0.0f && v1 > 0.0f) {
+    // pixel inside the swept band: + (1+i) exp(-i pi u^2/c) P
+    float turns = u * u * L.hc;
+    turns -= floorf(turns);
+    float st, ct;
+    __sincosf(6.283185307179586f * (turns - 0.5f), &st, &ct);        // = -(sin, cos)(2 pi turns)
+    const float er = -(ct + st), ei = -(ct - st);
+    hr += er * L.Pr - ei * L.Pi;
+    hi += er * L.Pi + ei * L.Pr;
+  }
+  s.zAr = fmaf(Y.x, hr, fmaf(Y.y, hi, s.zAr));
+  s.zAi = fmaf(Y.x, hi, fmaf(-Y.y, hr, s.zAi));
+  s.zEr = fmaf(Y.z, hr, fmaf(Y.w, hi, s.zEr));
+  s.zEi = fmaf(Y.z, hi, fmaf(-Y.w, hr, s.zEi));
+  const float h2 = fmaf(hr, hr, hi * hi);
+  s.qA = fmaf(Wt.x, h2, s.qA);
+  s.qE = fmaf(Wt.y, h2, s.qE);
+}
 
 // ------------------------------------------------------------------------------------------
 // Kernel A: track + gather + per-tile sums.  Persistent: one CTA per SM, warps claim work items
 // (template, tile) in tile-major order from a global counter, kClaim at a time.
+// Inside a work item LANES ARE TRANCHES: lane l owns the l-th valid (non-gap) tranche of the
+// current chunk of 32, computes its track point in fp64 and then walks its own window pixel by
+// pixel.  The grid is stored time-contiguous ([k][m]), so the 32 lanes' loads of pixel offset j
+// fall on consecutive addresses wherever neighbouring tranches share k_lo (slow chirps: runs of
+// 1/c tranches).  Lanes past their window (or inactive) keep running with zeroed data: the loop has
+// no divergent branch except the rare in-band term.
 // ------------------------------------------------------------------------------------------
 constexpr int kClaim = 4;
 
@@ -186,16 +242,16 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 1)
 eval_tiles_kernel(const EvalArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* s_lut = reinterpret_cast<float4*>(smem_raw);
-  BinRec* s_rec = reinterpret_cast<BinRec*>(smem_raw + kLutSmemBytes);
+  double* s_acc = reinterpret_cast<double*>(smem_raw + kLutSmemBytes) + threadIdx.x;   // [6][blockDim]
+  constexpr int kAccStride = kWarpsPerCta * 32;
 
   const int lane = threadIdx.x & 31;
-  const int warp = threadIdx.x >> 5;
   if (MODE == 0) {
     for (int i = threadIdx.x; i < (kLutN + 1) * kLutCopies; i += blockDim.x) s_lut[i] = a.lut[i / kLutCopies];
     __syncthreads();
   }
-  BinRec* rec = s_rec + warp * kChunk;
-  const float4* lut_lane = s_lut + (lane & (kLutCopies - 1));
+  const unsigned lut_lane = (unsigned)__cvta_generic_to_shared(s_lut) + 16u * (unsigned)(lane & (kLutCopies - 1)) -
+                            kMagicBits * (16u * kLutCopies);
 
   const long long n_work = a.n * (long long)a.n_tiles;
   for (;;) {
@@ -209,6 +265,8 @@ eval_tiles_kernel(const EvalArgs a) {
       const long long it = w - (long long)tile * a.n;
       int m0, m1;
       tile_range(tile, a.tiles_per_seg, a.Nt, a.N_seg, m0, m1);
+      // valid (non-gap) tranches of the tile: entries [i0, i1) of the compacted list (C10)
+      const int i0 = a.vprefix[m0], i1 = a.vprefix[m1];
 
       const TemplateConst T = load_template(a.params + it * 8);
       if (!T.ok) {
@@ -219,23 +277,29 @@ eval_tiles_kernel(const EvalArgs a) {
         continue;
       }
 
-      // fp64 per-lane running sums over the tile: z_A, z_E (complex), q_A, q_E
-      double dzAr = 0, dzAi = 0, dzEr = 0, dzEi = 0, dqA = 0, dqE = 0;
+      // fp64 per-lane running sums over the tile (z_A, z_E complex, q_A, q_E) live in shared memory
+#pragma unroll
+      for (int v = 0; v < 6; ++v) s_acc[v * kAccStride] = 0.0;
 
-      for (int mc = m0; mc < m1; mc += kChunk) {
-        // ---------------- phase 1: lane <-> tranche ----------------
-        const int m = mc + lane;
-        const bool valid = (m < m1) && (a.gap[min(m, a.Nt - 1)] != 0);        // C10
+      for (int ic = i0; ic < i1; ic += 32) {
+        // ---------------- track point of this lane's tranche (a2) ----------------
+        const int i = ic + lane;
+        const bool valid = i < i1;
+        const int m = a.valid_m[valid ? i : i0];
         const TrackPoint tp = track_point(T, m, a.DT, a.x_lo, a.x_hi, a.c_max, valid);
-        const unsigned act_mask = __ballot_sync(0xffffffffu, tp.active);
-        if (act_mask == 0u) continue;
-        int Wm = 0;
+        if (__ballot_sync(0xffffffffu, tp.active) == 0u) continue;
+        int Wm = 0, idx = 0;
+        float u = 0.f;
+        LaneTrack L;
+        L.sc = 1.f; L.scc = 1.f; L.hc = 0.f; L.Pr = 0.f; L.Pi = 0.f; L.Qr = 0.f; L.Qi = 0.f;
         if (tp.active) {
           int k_lo, k_hi;
           window(tp, a.H, a.adaptive, a.Nf, k_lo, k_hi);
           Wm = k_hi - k_lo + 1;
+          idx = k_lo * a.Nt + m;
           const double flx = floor(tp.x);
           const float fracx = (float)(tp.x - flx);
+          u = fracx - (float)(k_lo - (int)flx);          // cancellation-safe x - k_lo
           // phases in turns, reduced in fp64 (phi reaches ~1e8 rad)
           double tphi = T.phic_turns - tp.X58 * (1.0 / kPi);
           tphi -= floor(tphi);
@@ -246,107 +310,43 @@ eval_tiles_kernel(const EvalArgs a) {
           sincospif(2.0f * (float)tpsi, &spsi, &cpsi);
           const float cf = (float)tp.c;
           const float pre = (float)(T.acoef * tp.Xm14) * rsqrtf(2.0f * cf);  // A_m / sqrt(2c)
-          BinRec r;
-          r.base = m * a.Nf + k_lo;
-          r.W = Wm;
-          r.u0 = fracx - (float)(k_lo - (int)flx);      // cancellation-safe x - k_lo
-          r.sc = rsqrtf(0.5f * cf);
-          r.Pr = pre * cphi;
-          r.Pi = pre * sphi;
-          r.Qr = r.Pr * cpsi - r.Pi * spsi;
-          r.Qi = r.Pr * spsi + r.Pi * cpsi;
-          r.scc = r.sc * cf;
-          r.hc = __fdividef(0.5f, cf);
-          r.pad0 = 0.f; r.pad1 = 0.f;
-          const int slot = __popc(act_mask & ((1u << lane) - 1u));
-          rec[slot] = r;
+          L.sc = rsqrtf(0.5f * cf);
+          L.scc = L.sc * cf;
+          L.hc = __fdividef(0.5f, cf);
+          L.Pr = pre * cphi;
+          L.Pi = pre * sphi;
+          L.Qr = L.Pr * cpsi - L.Pi * spsi;
+          L.Qi = L.Pr * spsi + L.Pi * cpsi;
         }
-        int Wc = Wm;                                                          // chunk-uniform width
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) Wc = max(Wc, __shfl_xor_sync(0xffffffffu, Wc, o));
-        __syncwarp();
+        const int Wmax = __reduce_max_sync(0xffffffffu, Wm);
 
-        // ---------------- phase 2: lane <-> (tranche, pixel) item ----------------
-        // item i -> (slot b, offset j) = (i / Wc, i % Wc), advanced incrementally; the gather of
-        // item i+32 is issued before the arithmetic of item i (software prefetch, distance 1).
-        const int n_items = __popc(act_mask) * Wc;
-        float zAr = 0, zAi = 0, zEr = 0, zEi = 0, qA = 0, qE = 0;
-        int b = 0, j = lane;
-        while (j >= Wc) { j -= Wc; ++b; }
-        float4 Yn = make_float4(0.f, 0.f, 0.f, 0.f);
-        float2 Wn = make_float2(0.f, 0.f);
-        float un = 0.f, scn = 0.f;
-        bool vn = false;
-        if (lane < n_items) {
-          const float4 h = *reinterpret_cast<const float4*>(&rec[b]);          // {base, W, u0, sc}
-          vn = j < __float_as_int(h.y);
-          if (vn) {
-            const int idx = __float_as_int(h.x) + j;
-            Yn = __ldg(a.grid + idx);
-            Wn = __ldg(a.wgt + idx);
-            un = h.z - (float)j;
-            scn = h.w;
-          }
+        // ---------------- pixel loop (a3-a5): lane walks its own window ----------------
+        // the gather of pixel j+1 is issued before the arithmetic of pixel j
+        LaneSums s;
+        s.zAr = 0.f; s.zAi = 0.f; s.zEr = 0.f; s.zEi = 0.f; s.qA = 0.f; s.qE = 0.f;
+        float4 Ya = make_float4(0.f, 0.f, 0.f, 0.f), Yb;
+        float2 Wa = make_float2(0.f, 0.f), Wb;
+        if (0 < Wm) { Ya = __ldg(a.grid + idx); Wa = __ldg(a.wgt + idx); }
+        for (int j = 0; j < Wmax; j += 2) {
+          Yb = make_float4(0.f, 0.f, 0.f, 0.f); Wb = make_float2(0.f, 0.f);
+          idx += a.Nt;
+          if (j + 1 < Wm) { Yb = __ldg(a.grid + idx); Wb = __ldg(a.wgt + idx); }
+          pixel<MODE>(L, u, Ya, Wa, lut_lane, s);
+          u -= 1.0f;
+          Ya = make_float4(0.f, 0.f, 0.f, 0.f); Wa = make_float2(0.f, 0.f);
+          idx += a.Nt;
+          if (j + 2 < Wm) { Ya = __ldg(a.grid + idx); Wa = __ldg(a.wgt + idx); }
+          pixel<MODE>(L, u, Yb, Wb, lut_lane, s);
+          u -= 1.0f;
         }
-        for (int i = lane; i < n_items; i += 32) {
-          const float4 Y = Yn;
-          const float2 Wt = Wn;
-          const float u = un, sc = scn;
-          const bool vc = vn;
-          const BinRec* rc = rec + b;
-          // ---- prefetch item i+32 ----
-          j += 32;
-          while (j >= Wc) { j -= Wc; ++b; }
-          vn = false;
-          if (i + 32 < n_items) {
-            const float4 h = *reinterpret_cast<const float4*>(&rec[b]);
-            vn = j < __float_as_int(h.y);
-            if (vn) {
-              const int idx = __float_as_int(h.x) + j;
-              Yn = __ldg(a.grid + idx);
-              Wn = __ldg(a.wgt + idx);
-              un = h.z - (float)j;
-              scn = h.w;
-            }
-          }
-          // ---- arithmetic of item i ----
-          if (vc) {
-            const float4 PQ = *reinterpret_cast<const float4*>(&rc->Pr);       // {Pr, Pi, Qr, Qi}
-            const float scc = rc->scc;
-            const float v0 = sc * u;
-            const float v1 = v0 + scc;
-            float f0, g0, f1, g1;
-            fresnel_aux<MODE>(v0, lut_lane, f0, g0);
-            fresnel_aux<MODE>(v1, lut_lane, f1, g1);
-            // s0 G(|v0|) P - s1 G(|v1|) Q,  G = g + i f   (C7)
-            float hr = g0 * PQ.x - f0 * PQ.y - g1 * PQ.z + f1 * PQ.w;
-            float hi = g0 * PQ.y + f0 * PQ.x - g1 * PQ.w - f1 * PQ.z;
-            if (v0 < 0.0f && v1 > 0.0f) {
-              // pixel inside the swept band: + (1+i) exp(-i pi u^2/c) P
-              float turns = u * u * rc->hc;
-              turns -= floorf(turns);
-              float st, ct;
-              __sincosf(6.283185307179586f * (turns - 0.5f), &st, &ct);        // = -(sin, cos)(2 pi turns)
-              const float er = -(ct + st), ei = -(ct - st);
-              hr += er * PQ.x - ei * PQ.y;
-              hi += er * PQ.y + ei * PQ.x;
-            }
-            zAr = fmaf(Y.x, hr, fmaf(Y.y, hi, zAr));
-            zAi = fmaf(Y.x, hi, fmaf(-Y.y, hr, zAi));
-            zEr = fmaf(Y.z, hr, fmaf(Y.w, hi, zEr));
-            zEi = fmaf(Y.z, hi, fmaf(-Y.w, hr, zEi));
-            const float h2 = fmaf(hr, hr, hi * hi);
-            qA = fmaf(Wt.x, h2, qA);
-            qE = fmaf(Wt.y, h2, qE);
-          }
-        }
-        dzAr += zAr; dzAi += zAi; dzEr += zEr; dzEi += zEi; dqA += qA; dqE += qE;
-        __syncwarp();
+        s_acc[0 * kAccStride] += s.zAr; s_acc[1 * kAccStride] += s.zAi;
+        s_acc[2 * kAccStride] += s.zEr; s_acc[3 * kAccStride] += s.zEi;
+        s_acc[4 * kAccStride] += s.qA;  s_acc[5 * kAccStride] += s.qE;
       }
 
-      dzAr = warp_sum(dzAr); dzAi = warp_sum(dzAi);
-      dzEr = warp_sum(dzEr); dzEi = warp_sum(dzEi);
-      dqA = warp_sum(dqA);   dqE = warp_sum(dqE);
+      const double dzAr = warp_sum(s_acc[0 * kAccStride]), dzAi = warp_sum(s_acc[1 * kAccStride]);
+      const double dzEr = warp_sum(s_acc[2 * kAccStride]), dzEi = warp_sum(s_acc[3 * kAccStride]);
+      const double dqA = warp_sum(s_acc[4 * kAccStride]),  dqE = warp_sum(s_acc[5 * kAccStride]);
       if (lane == 0) {
         // z = T_A z_A + T_E z_E ; hh = |T_A|^2 q_A + |T_E|^2 q_E   (Eq. 29, Eq. 31)
         const double zr = T.TAr * dzAr - T.TAi * dzAi + T.TEr * dzEr - T.TEi * dzEi;
@@ -407,17 +407,65 @@ __global__ void count_pixels_kernel(const EvalArgs a, long long* __restrict__ co
 }
 
 // ------------------------------------------------------------------------------------------
-// Upload: Y = W*D interleaved by channel, W interleaved.
+// Upload (a0): Y = W*D interleaved by channel and W interleaved, transposed to time-contiguous
+// [k][m] through a 32x32 shared-memory tile (reads coalesced along k, writes coalesced along m).
 // ------------------------------------------------------------------------------------------
-__global__ void pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight,
-                            long long npix, float4* __restrict__ grid, float2* __restrict__ wgt) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= npix) return;
-  const float2 dA = coeff[i], dE = coeff[npix + i];
-  const float wA = weight ? weight[i] : 1.0f;
-  const float wE = weight ? weight[npix + i] : 1.0f;
-  grid[i] = make_float4(wA * dA.x, wA * dA.y, wE * dE.x, wE * dE.y);
-  wgt[i] = make_float2(wA, wE);
+__global__ void __launch_bounds__(256)
+pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, int Nt, int Nf,
+            float4* __restrict__ grid, float2* __restrict__ wgt) {
+  __shared__ float4 sY[32][33];
+  __shared__ float2 sW[32][33];
+  const int k0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;        // 32 x 8
+  const long long npix = (long long)Nt * Nf;
+  for (int r = ty; r < 32; r += 8) {
+    const int m = m0 + r, k = k0 + tx;
+    if (m < Nt && k < Nf) {
+      const long long i = (long long)m * Nf + k;
+      const float2 dA = coeff[i], dE = coeff[npix + i];
+      const float wA = weight ? weight[i] : 1.0f;
+      const float wE = weight ? weight[npix + i] : 1.0f;
+      sY[r][tx] = make_float4(wA * dA.x, wA * dA.y, wE * dE.x, wE * dE.y);
+      sW[r][tx] = make_float2(wA, wE);
+    }
+  }
+  __syncthreads();
+  for (int r = ty; r < 32; r += 8) {
+    const int k = k0 + r, m = m0 + tx;
+    if (m < Nt && k < Nf) {
+      const long long o = (long long)k * Nt + m;
+      grid[o] = sY[tx][r];
+      wgt[o] = sW[tx][r];
+    }
+  }
+}
+
+// Compacted list of valid (non-gap) tranches and its prefix counts (C10).  One block.
+__global__ void __launch_bounds__(1024)
+valid_list_kernel(const uint8_t* __restrict__ gap, int Nt, int* __restrict__ vprefix, int* __restrict__ valid_m) {
+  __shared__ int s_cnt[1024];
+  const int t = threadIdx.x;
+  const int per = (Nt + 1023) / 1024;
+  const int b = min(t * per, Nt), e = min(b + per, Nt);
+  int c = 0;
+  for (int m = b; m < e; ++m) c += gap[m] != 0;
+  s_cnt[t] = c;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {                           // inclusive Hillis-Steele scan
+    const int v = t >= o ? s_cnt[t - o] : 0;
+    __syncthreads();
+    s_cnt[t] += v;
+    __syncthreads();
+  }
+  int pos = s_cnt[t] - c;
+  for (int m = b; m < e; ++m) {
+    vprefix[m] = pos;
+    if (gap[m] != 0) valid_m[pos++] = m;
+  }
+  if (t == 1023) {
+    vprefix[Nt] = s_cnt[1023];
+    if (s_cnt[1023] == 0) valid_m[0] = 0;                        // keep entry 0 readable when everything is masked
+  }
 }
 
 // ------------------------------------------------------------------------------------------
