@@ -101,6 +101,20 @@ TFS_API int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg,
 TFS_API int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k,
              long long* idx, float* val, void* stream);
 
+/* Ladder refinement (BASELINE.json configs[4]; the hierarchical N_seg reduction of P:104, P:347;
+ * reading C19 of DESIGN.md).  For each of the k survivors j (row idx[j] of params) write r*r
+ * children on a lattice r times denser per dimension that tiles the parent's (Mc, tc) cell of
+ * size (Mc*d_mc_rel) x d_tc:
+ *     o_i = (2 i + 1 - r) / (2 r),  i = 0..r-1            (r = 4: -3/8, -1/8, 1/8, 3/8)
+ *     child (a, b):  Mc' = Mc * (1 + o_a * d_mc_rel),  tc' = tc + o_b * d_tc,  other columns copied,
+ * stored at row j*r*r + a*r + b of children.  fp64, every product and sum rounded separately, so
+ * the result is bit-reproducible.  An idx[j] outside [0, n) yields a row of NaN (which tfs_eval
+ * scores 0 and counts as bad).
+ *   params   [n][8] double, host or device;  idx [k] int64, host or device (tfs_topk's output)
+ *   children [k*r*r][8] double, host or device, required;  1 <= r <= 64;  k == 0 is a no-op. */
+TFS_API int tfs_refine(tfs_ctx* ctx, const double* params, long long n, const long long* idx, long long k,
+               int r, double d_mc_rel, double d_tc, double* children, void* stream);
+
 /* Number of window pixels (k_hi-k_lo+1 summed over active tranches) of each template:
  * pixel_evals = n_channels * counts[i].  counts [n] int64, host or device.  Used by the
  * benchmark for the pixel-evals/s metric and by tests for the window logic. */

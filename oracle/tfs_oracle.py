@@ -338,3 +338,47 @@ def injection(p, rho: float, W, gap_mask, grid: Grid, opts: Opts = Opts(), trunc
     norm2 = float(np.sum(Wd * (S.real ** 2 + S.imag ** 2) * g[None, :, None]))
     S *= rho / math.sqrt(norm2)
     return S * g[None, :, None]
+
+
+# ----------------------------------------------------------------------------------------------
+# N_seg ladder (BASELINE.json configs[4]; hierarchical N_seg reduction; C19)
+# ----------------------------------------------------------------------------------------------
+def refine(params, idx, r: int, d_mc_rel: float, d_tc: float):
+    """r*r children per survivor on a lattice r times denser per dimension that tiles the parent's
+    (Mc, tc) cell of size (Mc d_mc_rel) x d_tc:  o_i = (2i+1-r)/(2r);  child (a, b) of parent j at
+    row j r^2 + a r + b:  Mc' = Mc (1 + o_a d_mc_rel),  tc' = tc + o_b d_tc,  rest copied."""
+    params = np.asarray(params, dtype=np.float64)
+    out = np.empty((len(idx) * r * r, PARAM_COLS), dtype=np.float64)
+    row = 0
+    for j in idx:
+        p = params[int(j)]
+        for a in range(r):
+            oa = np.float64(2 * a + 1 - r) / np.float64(2 * r)
+            for b in range(r):
+                ob = np.float64(2 * b + 1 - r) / np.float64(2 * r)
+                out[row] = p
+                out[row, 0] = p[0] * (1.0 + oa * d_mc_rel)
+                out[row, 1] = p[1] + ob * d_tc
+                row += 1
+    return out
+
+
+def ladder(params, D, W, gap_mask, grid: Grid, d_mc_rel: float, d_tc: float, stages=(64, 16, 4, 1),
+           keep_frac: float = 0.01, r: int = 4, keep_min: int = 1, opts: Opts = Opts()):
+    """Stage s: evaluate at N_seg = stages[s], keep the top ceil(keep_frac n) (at least keep_min),
+    refine each survivor r x r with the steps divided by r per stage.  Returns a list of dicts
+    (N_seg, params, upsilon, top_idx, top_val, d_mc_rel, d_tc), one per stage."""
+    out = []
+    cur = np.asarray(params, dtype=np.float64)
+    for s, N_seg in enumerate(stages):
+        ups = evaluate(cur, D, W, gap_mask, grid, N_seg, opts)["upsilon"]
+        n = len(cur)
+        k = min(n, max(keep_min, int(math.ceil(keep_frac * n))))
+        idx, val = topk(ups, k)
+        out.append(dict(N_seg=N_seg, params=cur, upsilon=ups, top_idx=idx, top_val=val,
+                        d_mc_rel=d_mc_rel, d_tc=d_tc))
+        if s + 1 < len(stages):
+            cur = refine(cur, idx, r, d_mc_rel, d_tc)
+            d_mc_rel /= r
+            d_tc /= r
+    return out

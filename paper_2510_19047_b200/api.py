@@ -52,6 +52,8 @@ def load_library():
     lib.tfs_eval.restype = ip
     lib.tfs_topk.argtypes = [vp, vp, ll, ip, vp, vp, vp]
     lib.tfs_topk.restype = ip
+    lib.tfs_refine.argtypes = [vp, vp, ll, vp, ll, ip, dp, dp, vp, vp]
+    lib.tfs_refine.restype = ip
     lib.tfs_count_pixels.argtypes = [vp, vp, ll, vp, vp]
     lib.tfs_count_pixels.restype = ip
     lib.tfs_bad_param_count.argtypes = [vp]
@@ -138,6 +140,15 @@ class Tfs:
             n = upsilon.size if isinstance(upsilon, np.ndarray) else upsilon.numel()
         self._check(self._lib.tfs_topk(self._h, _ptr(upsilon, np.float32, n), n, k,
                                        _ptr(idx, np.int64, k), _ptr(val, np.float32, k), _stream(stream)))
+
+    def refine(self, params, idx, r, d_mc_rel, d_tc, children, n=None, k=None, stream=None):
+        if n is None:
+            n = (params.size if isinstance(params, np.ndarray) else params.numel()) // PARAM_COLS
+        if k is None:
+            k = idx.size if isinstance(idx, np.ndarray) else idx.numel()
+        self._check(self._lib.tfs_refine(self._h, _ptr(params, np.float64, n * PARAM_COLS), n,
+                                         _ptr(idx, np.int64, k), k, r, d_mc_rel, d_tc,
+                                         _ptr(children, np.float64, k * r * r * PARAM_COLS), _stream(stream)))
 
     def count_pixels(self, params, counts, n=None, stream=None):
         if n is None:

@@ -48,6 +48,7 @@ struct tfs_ctx {
   void* buf_tk_idx = nullptr;   size_t cap_tk_idx = 0;
   void* buf_tk_val = nullptr;   size_t cap_tk_val = 0;
   void* buf_counts = nullptr;   size_t cap_counts = 0;
+  void* buf_children = nullptr; size_t cap_children = 0;
   SelectState* sel = nullptr;
 
   // measurement hooks
@@ -337,7 +338,7 @@ void tfs_destroy(tfs_ctx* ctx) {
   for (auto& p : ctx->ev_pool) { cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
   void* bufs[] = {ctx->grid, ctx->wgt, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut, ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials,
                   ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
-                  ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts};
+                  ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children};
   for (void* b : bufs) if (b) cudaFree(b);
   delete ctx;
 }
@@ -510,6 +511,44 @@ int tfs_count_pixels(tfs_ctx* ctx, const double* params, long long n, long long*
   } else if (!is_device_ptr(params)) {
     TFS_CUDA(ctx, cudaStreamSynchronize(st));
   }
+  return TFS_OK;
+}
+
+int tfs_refine(tfs_ctx* ctx, const double* params, long long n, const long long* idx, long long k, int r,
+               double d_mc_rel, double d_tc, double* children, void* stream) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_refine: ctx is NULL");
+  if (n < 0 || k < 0) return fail(ctx, TFS_EINVAL, "tfs_refine: n < 0 or k < 0");
+  if (r < 1 || r > 64) return fail(ctx, TFS_EINVAL, "tfs_refine: need 1 <= r <= 64 (got %d)", r);
+  if (!std::isfinite(d_mc_rel) || !std::isfinite(d_tc)) return fail(ctx, TFS_EINVAL, "tfs_refine: steps must be finite");
+  if (k == 0) return TFS_OK;
+  if (!params || !idx || !children) return fail(ctx, TFS_EINVAL, "tfs_refine: params, idx and children are required");
+  if (k * (long long)r * r >= (1ll << 32)) return fail(ctx, TFS_EINVAL, "tfs_refine: k*r*r must be < 2^32");
+  cudaStream_t st = (cudaStream_t)stream;
+  const long long nc = k * (long long)r * r;
+  const double* d_params = nullptr;
+  int rc = stage_params(ctx, params, n, st, &d_params);
+  if (rc) return rc;
+  const long long* d_idx = idx;
+  const bool host_idx = !is_device_ptr(idx), host_out = !is_device_ptr(children);
+  if (host_idx) {
+    rc = ensure(ctx, &ctx->buf_tk_idx, &ctx->cap_tk_idx, (size_t)k * sizeof(long long));
+    if (rc) return rc;
+    TFS_CUDA(ctx, cudaMemcpyAsync(ctx->buf_tk_idx, idx, (size_t)k * sizeof(long long), cudaMemcpyHostToDevice, st));
+    d_idx = (const long long*)ctx->buf_tk_idx;
+  }
+  double* d_out = children;
+  if (host_out) {
+    rc = ensure(ctx, &ctx->buf_children, &ctx->cap_children, (size_t)nc * TFS_PARAM_COLS * sizeof(double));
+    if (rc) return rc;
+    d_out = (double*)ctx->buf_children;
+  }
+  const int threads = 256;
+  refine_kernel<<<(unsigned)((nc + threads - 1) / threads), threads, 0, st>>>(d_params, n, d_idx, k, r, d_mc_rel, d_tc, d_out);
+  TFS_CUDA(ctx, cudaGetLastError());
+  ctx->launches += 1;
+  if (host_out)
+    TFS_CUDA(ctx, cudaMemcpyAsync(children, d_out, (size_t)nc * TFS_PARAM_COLS * sizeof(double), cudaMemcpyDeviceToHost, st));
+  if (host_out || host_idx || !is_device_ptr(params)) TFS_CUDA(ctx, cudaStreamSynchronize(st));
   return TFS_OK;
 }
 

@@ -469,6 +469,39 @@ valid_list_kernel(const uint8_t* __restrict__ gap, int Nt, int* __restrict__ vpr
 }
 
 // ------------------------------------------------------------------------------------------
+// Ladder refinement (a10; C19): child (a, b) of survivor j, a, b in [0, r), sits at
+//   Mc' = Mc (1 + o_a d_mc_rel),  tc' = tc + o_b d_tc,  o_i = (2i + 1 - r) / (2r)
+// (an r x r lattice, r times denser per dimension, that tiles the parent's cell); the other six
+// columns are copied.  One thread per child; products and sums are rounded separately (no FMA
+// contraction) so the rows are bit-identical to an IEEE fp64 evaluation in the stated order.
+// A parent index outside [0, n) gives a NaN row, which tfs_eval counts as a bad template.
+// ------------------------------------------------------------------------------------------
+__global__ void refine_kernel(const double* __restrict__ params, long long n, const long long* __restrict__ idx,
+                              long long k, int r, double d_mc_rel, double d_tc, double* __restrict__ out) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long rr = (long long)r * r;
+  if (t >= k * rr) return;
+  const long long j = t / rr;
+  const int ab = (int)(t - j * rr);
+  const int ia = ab / r, ib = ab - ia * r;
+  const long long src = idx[j];
+  double* o = out + t * 8;
+  if (src < 0 || src >= n) {
+    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+#pragma unroll
+    for (int c = 0; c < 8; ++c) o[c] = qnan;
+    return;
+  }
+  const double* p = params + src * 8;
+  const double oa = __ddiv_rn((double)(2 * ia + 1 - r), (double)(2 * r));
+  const double ob = __ddiv_rn((double)(2 * ib + 1 - r), (double)(2 * r));
+  o[0] = __dmul_rn(p[0], __dadd_rn(1.0, __dmul_rn(oa, d_mc_rel)));
+  o[1] = __dadd_rn(p[1], __dmul_rn(ob, d_tc));
+#pragma unroll
+  for (int c = 2; c < 8; ++c) o[c] = p[c];
+}
+
+// ------------------------------------------------------------------------------------------
 // Top-k: radix select on 64-bit composite keys (value order, then lower index), then bitonic sort.
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned long long topk_key(float v, unsigned idx) {

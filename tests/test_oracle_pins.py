@@ -460,3 +460,87 @@ def test_segments_and_topk():
     assert list(O.segment_of_bin(np.arange(7), 7, 3)) == [0, 0, 0, 1, 1, 2, 2]
     idx, val = O.topk(np.array([1.0, 5.0, 3.0, 5.0, 0.0]), 3)
     assert list(idx) == [1, 3, 2] and list(val) == [5.0, 5.0, 3.0]
+
+
+# ------------------------------------------------------------------------------------------
+# P13  ladder refinement lattice and ladder driver (BASELINE.json configs[4]; C19)
+# ------------------------------------------------------------------------------------------
+def test_p13_refine_offsets_written_out():
+    # r = 4: the offsets the header prints, -3/8, -1/8, 1/8, 3/8 of the parent's cell
+    p = np.array([[30.0, 1000.0, 0.1, 0.2, 0.3, 0.4, 0.5, 0.6], [7.0, 5.0e7, 1, 2, 3, 4, 5, 6]])
+    ch = O.refine(p, [1, 0], 4, 1e-3, 800.0)
+    assert ch.shape == (32, 8)
+    offs = [-0.375, -0.125, 0.125, 0.375]
+    for j, src in enumerate([1, 0]):
+        for a in range(4):
+            for b in range(4):
+                row = ch[j * 16 + a * 4 + b]
+                assert row[0] == p[src, 0] * (1.0 + offs[a] * 1e-3)
+                assert row[1] == p[src, 1] + offs[b] * 800.0
+                assert np.array_equal(row[2:], p[src, 2:])
+
+
+@pytest.mark.parametrize("r", [1, 2, 3, 4, 5])
+def test_p13_refine_tiles_the_parent_lattice(r):
+    # parents on a regular tc lattice of step d: the children of all parents form ONE regular lattice
+    # of step d/r (no hole, no overlap at cell borders); same in Mc to first order in d_mc_rel
+    d_tc, d_mc = 640.0, 1e-4
+    par = np.array([[50.0, 1e6 + i * d_tc, 0, 1, 0, 0, 0, 1] for i in range(5)])
+    ch = O.refine(par, range(5), r, d_mc, d_tc)
+    tcs = np.unique(ch[:, 1])
+    assert len(tcs) == 5 * r
+    assert np.allclose(np.diff(tcs), d_tc / r, rtol=0, atol=1e-6)
+    assert abs(tcs.mean() - par[:, 1].mean()) < 1e-6          # children are centred on the parents
+    parM = np.array([[50.0 * (1 + d_mc) ** i, 1e6, 0, 1, 0, 0, 0, 1] for i in range(5)])
+    chM = O.refine(parM, range(5), r, d_mc, d_tc)
+    lm = np.log(np.unique(chM[:, 0]))
+    assert len(lm) == 5 * r
+    assert np.allclose(np.diff(lm), d_mc / r, rtol=0, atol=2 * d_mc ** 2)
+    # r = 1 is the identity
+    if r == 1:
+        assert np.array_equal(ch, par)
+
+
+def test_p13_ladder_reduces_to_plain_evaluation():
+    # keep everything, r = 1: every stage is O.evaluate of the same bank at that stage's N_seg
+    g = SMALL
+    D = _noise(g, 5)
+    rng = np.random.default_rng(8)
+    P = np.array([[rng.uniform(25, 35), rng.uniform(0.3, 3) * O.YEAR_S, 0.0, 0.6, 0.1, -0.3, 0.5, 1.0] for _ in range(6)])
+    st = O.ladder(P, D, None, None, g, 1e-4, 100.0, stages=(8, 2, 1), keep_frac=1.0, r=1)
+    for s, N in zip(st, (8, 2, 1)):
+        u = O.evaluate(P, D, None, None, g, N)["upsilon"]
+        assert np.array_equal(np.sort(s["upsilon"]), np.sort(u))
+        assert list(s["top_idx"]) == list(O.topk(s["upsilon"], len(P))[0])
+
+
+def test_p13_ladder_recovers_a_noiseless_injection():
+    # a coarse lattice around (not on) the injection: each stage's survivors contain the cell that
+    # holds the truth, the final candidate is within half a final step of it, and the recovered
+    # coherent SNR^2 is most of rho^2 (hierarchical reduction of N_seg ends at the coherent limit)
+    g = O.Grid(256, 1024, 5.0)
+    inj = np.array([30.0, 1.0 * O.YEAR_S, 0.3, 0.7, 0.0, 0.5, 0.0, 1.0])
+    S = O.injection(inj, 20.0, None, None, g)
+    d_mc, d_tc, r = 4e-4, 2.0e4, 4
+    nodes = np.arange(-3, 4)
+    bank = []
+    for i in nodes:
+        for j in nodes:
+            p = inj.copy()
+            p[0] = inj[0] * (1.0 + (i + 0.31) * d_mc)
+            p[1] = inj[1] + (j - 0.27) * d_tc
+            p[2] = 0.0
+            bank.append(p)
+    bank = np.array(bank)
+    st = O.ladder(bank, S, None, None, g, d_mc, d_tc, stages=(64, 16, 4, 1), keep_frac=0.05, r=r, keep_min=2)
+    assert [len(s["params"]) for s in st] == [49, 48, 48, 48]
+    # (Mc, tc) are degenerate along a ridge (a lighter system merging later has the same in-grid track),
+    # so the best lattice point need not be in the truth's own cell; what the ladder must deliver is a
+    # candidate near the truth in units of the FINAL step whose coherent SNR^2 is most of rho^2
+    best = st[-1]["params"][st[-1]["top_idx"][0]]
+    assert abs(best[0] / inj[0] - 1) <= 1.5 * st[-1]["d_mc_rel"]
+    assert abs(best[1] - inj[1]) <= 1.5 * st[-1]["d_tc"]
+    assert all(s["top_val"][0] > 0.9 * 400.0 for s in st)
+    # without refinement the stage-0 lattice is far too coarse for the coherent statistic
+    u1 = O.evaluate(bank, S, None, None, g, 1)["upsilon"]
+    assert u1.max() < 0.5 * 400.0 < 0.9 * 400.0 < st[-1]["top_val"][0]
