@@ -49,6 +49,7 @@ struct tfs_ctx {
   void* buf_tk_val = nullptr;   size_t cap_tk_val = 0;
   void* buf_counts = nullptr;   size_t cap_counts = 0;
   void* buf_children = nullptr; size_t cap_children = 0;
+  void* buf_tiles = nullptr;    size_t cap_tiles = 0;
   SelectState* sel = nullptr;
 
   // measurement hooks
@@ -338,7 +339,7 @@ void tfs_destroy(tfs_ctx* ctx) {
   for (auto& p : ctx->ev_pool) { cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
   void* bufs[] = {ctx->grid, ctx->wgt, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut, ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials,
                   ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
-                  ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children};
+                  ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children, ctx->buf_tiles};
   for (void* b : bufs) if (b) cudaFree(b);
   delete ctx;
 }
@@ -427,9 +428,17 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
   rc = ensure(ctx, &ctx->buf_partials, &ctx->cap_partials, (size_t)sub * n_tiles * sizeof(float4));
   if (rc) return rc;
 
+  rc = ensure(ctx, &ctx->buf_tiles, &ctx->cap_tiles, (size_t)n_tiles * sizeof(int2));
+  if (rc) return rc;
+
   TFS_CUDA(ctx, cudaMemsetAsync(ctx->bad, 0, sizeof(unsigned long long), st));
   EvalArgs a = base_args(ctx);
   a.N_seg = N_seg; a.tiles_per_seg = tps; a.n_tiles = n_tiles;
+  a.tile_table = (const int2*)ctx->buf_tiles;
+  tile_table_kernel<<<(unsigned)((n_tiles + 127) / 128), 128, 0, st>>>(ctx->vprefix, ctx->Nt, N_seg, tps, n_tiles,
+                                                                     (int2*)ctx->buf_tiles);
+  TFS_CUDA(ctx, cudaGetLastError());
+  ctx->launches += 1;
   a.partials = (float4*)ctx->buf_partials;
   for (long long off = 0; off < n; off += sub) {
     const long long nb = std::min(sub, n - off);

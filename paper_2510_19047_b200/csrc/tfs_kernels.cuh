@@ -27,6 +27,7 @@ struct EvalArgs {
   const uint8_t* __restrict__ gap;     // [Nt] 1 = valid
   const int* __restrict__ vprefix;     // [Nt+1] number of valid tranches before m
   const int* __restrict__ valid_m;     // [vprefix[Nt]] the valid tranche indices, ascending (padded to >= 1 entry)
+  const int2* __restrict__ tile_table; // [n_tiles] {i0, i1}: entries of valid_m covered by each tile
   const float4* __restrict__ lut;      // [kLutN+1] {a_F, b_F, a_G, b_G} (see fresnel_aux)
   const double* __restrict__ params;   // [n][8]
   float4* __restrict__ partials;       // [n_tiles][n] {z.re, z.im, hh, 0}
@@ -51,14 +52,17 @@ __device__ __forceinline__ void tile_range(int tile, int tps, int Nt, int N_seg,
   m1 = min(m0 + L, s1);
 }
 
-// Per-template constants derived from the parameter row (all fp64).
+// Per-template constants derived from the parameter row.
 struct TemplateConst {
-  double tc, phic_turns, inv5M, xcoef, acoef;
+  double tc, phic_turns, inv5M;
+  double xcoefDT;        // DT / (8 pi M):           x = f DT = X^{-3/8} xcoefDT
+  double ccoef;          // (3/8) DT / (5M):         c = fdot DT^2 = x ccoef / X
+  float acoef;           // amp (8 pi M)^{-2/3}:     A_m = acoef X^{-1/4}
   double TAr, TAi, TEr, TEi;
   bool ok;
 };
 
-__device__ __forceinline__ TemplateConst load_template(const double* __restrict__ p) {
+__device__ __forceinline__ TemplateConst load_template(const double* __restrict__ p, double DT) {
   TemplateConst t;
   const double Mc = p[0];
   t.tc = p[1];
@@ -69,9 +73,12 @@ __device__ __forceinline__ TemplateConst load_template(const double* __restrict_
             isfinite(t.TEr) && isfinite(t.TEi) && isfinite(amp) && (Mc > 0.0);
   const double M = (ok ? Mc : 1.0) * kMtsun;
   t.inv5M = 1.0 / (5.0 * M);
-  t.xcoef = 1.0 / (8.0 * kPi * M);                        // f = X^{-3/8} * xcoef ; x = f*DT
-  // A_m = amp f^{2/3} = amp (8 pi M)^{-2/3} X^{-1/4}
-  t.acoef = (ok ? amp : 0.0) * cbrt(t.xcoef * t.xcoef);
+  const double xcoef = 1.0 / (8.0 * kPi * M);                // f = X^{-3/8} xcoef
+  t.xcoefDT = xcoef * DT;
+  t.ccoef = 0.375 * DT * t.inv5M;
+  // A_m = amp f^{2/3} = amp xcoef^{2/3} X^{-1/4}; a common factor of the template (fp32 is enough)
+  const float cx = cbrtf((float)xcoef);
+  t.acoef = (float)(ok ? amp : 0.0) * cx * cx;
   t.phic_turns = (ok ? phic : 0.0) * (0.5 / kPi);
   t.ok = ok;
   return t;
@@ -82,27 +89,32 @@ struct TrackPoint {
   double x;        // f_m * DT  (position in bins)
   double c;        // fdot_m * DT^2 (bins swept in the tranche)
   double X58;      // X^{5/8}: phi_m = phic - 2 X^{5/8}
-  double Xm14;     // X^{-1/4}: A_m = acoef * X^{-1/4}
+  float Xm14;      // X^{-1/4}: A_m = acoef * X^{-1/4}
   bool active;
 };
 
+// All fractional powers of X come from y = X^{-1/8}: an fp32 seed y0 = 2^{-log2(X)/8} (two MUFU ops,
+// relative error d ~ 4e-7) corrected in fp64 by the binomial series of (1 - e)^{-1/8}, e = 1 - X y0^8
+// ~ 8 d, to third order: the remainder is ~0.04 e^4 < 1e-20, i.e. y is exact to fp64 rounding.
 __device__ __forceinline__ TrackPoint track_point(const TemplateConst& t, int m, double DT,
                                                   double x_lo, double x_hi, double c_max, bool valid) {
   TrackPoint r;
   const double tau = t.tc - (double)m * DT;
   bool act = valid && (tau > DT);
   const double X = act ? tau * t.inv5M : 1.0;
-  // X^{1/2}, X^{1/4}, X^{1/8} by a chain of reciprocal square roots
-  const double r1 = rsqrt(X);        // X^{-1/2}
-  const double s1 = X * r1;          // X^{ 1/2}
-  const double r2 = rsqrt(s1);       // X^{-1/4}
-  const double s2 = s1 * r2;         // X^{ 1/4}
-  const double r3 = rsqrt(s2);       // X^{-1/8}
-  const double s3 = s2 * r3;         // X^{ 1/8}
-  r.X58 = s1 * s3;
-  r.Xm14 = r2;
-  r.x = (s3 * r1) * (t.xcoef * DT);  // X^{-3/8} / (8 pi M) * DT
-  r.c = 0.375 * r.x * DT / (act ? tau : 1.0);      // fdot DT^2 = 3 f DT^2 / (8 tau)
+  double y0 = (double)exp2f(-0.125f * __log2f((float)X));
+  // X outside the fp32 range (absurd masses): fall back to the seed 1/sqrt(sqrt(sqrt(X)))
+  if (!(X > 1e-30 && X < 1e30)) y0 = rsqrt(sqrt(sqrt(X)));
+  const double p2 = y0 * y0, p4 = p2 * p2;
+  const double e = fma(-X, p4 * p4, 1.0);
+  const double y = fma(y0, e * fma(e, fma(e, 51.0 / 1024.0, 9.0 / 128.0), 0.125), y0);   // X^{-1/8}
+  const double y2 = y * y;                 // X^{-1/4}
+  const double y3 = y2 * y;                // X^{-3/8}
+  const double y4 = y2 * y2;
+  r.X58 = X * y3;
+  r.Xm14 = (float)y2;
+  r.x = y3 * t.xcoefDT;
+  r.c = r.x * t.ccoef * (y4 * y4);         // 3 f DT^2 / (8 tau), 1/tau = y^8 / (5M)
   act = act && (r.x >= x_lo) && (r.x + r.c <= x_hi) && (r.c <= c_max);
   r.active = act;
   return r;
@@ -181,19 +193,23 @@ __device__ __forceinline__ double warp_sum(double v) {
 constexpr int kLutSmemBytes = (kLutN + 1) * kLutCopies * (int)sizeof(float4);
 constexpr int kEvalSmemBytes = kLutSmemBytes + 6 * kWarpsPerCta * 32 * (int)sizeof(double);
 
-// One pixel of one tranche (a3-a5): template coefficient from the auxiliary-function form of Eq. 16
-// (DESIGN.md section 6.3), then z_alpha += Y_alpha^* h, q_alpha += W_alpha |h|^2 for both channels.
+// One pixel of one tranche (a3-a5).  The template coefficient is h = P h', P = A/sqrt(2c) exp(i phi_m)
+// constant over the tranche, and (auxiliary-function form of Eq. 16)
+//   h' = s0 G(|v0|) - s1 G(|v1|) E  [+ (1+i) exp(-i pi u^2/c) inside the swept band],  G = g + i f,
+//   E = exp(i psi), psi = pi c + 2 pi frac(x).
+// The loop accumulates z'_alpha += conj(Y_alpha) h', q'_alpha += W_alpha |h'|^2 and the factor P
+// (|P|^2 for q) is applied once per tranche.
 struct LaneTrack {      // per-lane (= per-tranche) constants of the pixel loop
   float sc;             // sqrt(2/c)
   float scc;            // sqrt(2c) = v1 - v0
   float hc;             // 1/(2c): pi u^2/c = 2 pi (u^2 hc)
-  float Pr, Pi;         // A/sqrt(2c) exp(i phi_m)
-  float Qr, Qi;         // P exp(i psi), psi = pi c + 2 pi frac(x)
+  float Er, Ei;         // exp(i psi)
 };
 
 struct LaneSums { float zAr, zAi, zEr, zEi, qA, qE; };
 
-template <int MODE>
+// INBAND: 0 = the pixel is known to lie outside the swept band, 1 = test it (v0 < 0 < v1)
+template <int MODE, int INBAND>
 __device__ __forceinline__ void pixel(const LaneTrack& L, float u, const float4 Y, const float2 Wt,
                                       unsigned lut_lane, LaneSums& s) {
   const float v0 = L.sc * u;
@@ -201,20 +217,17 @@ __device__ __forceinline__ void pixel(const LaneTrack& L, float u, const float4 
   float F0, G0, t0, F1, G1, t1;
   fresnel_aux<MODE>(v0, lut_lane, F0, G0, t0);
   fresnel_aux<MODE>(v1, lut_lane, F1, G1, t1);
-  // h = s0 G(|v0|) P - s1 G(|v1|) Q,  G = g + i f
-  const float w0r = G0 * L.Pr - F0 * L.Pi, w0i = G0 * L.Pi + F0 * L.Pr;
-  const float w1r = G1 * L.Qr - F1 * L.Qi, w1i = G1 * L.Qi + F1 * L.Qr;
-  float hr = fmaf(t0, w0r, -t1 * w1r);
-  float hi = fmaf(t0, w0i, -t1 * w1i);
-  if (v0 < 0.0f && v1 > 0.0f) {
-    // pixel inside the swept band: + (1+i) exp(-i pi u^2/c) P
+  const float w1r = G1 * L.Er - F1 * L.Ei, w1i = G1 * L.Ei + F1 * L.Er;
+  float hr = fmaf(t0, G0, -t1 * w1r);
+  float hi = fmaf(t0, F0, -t1 * w1i);
+  if (INBAND && v0 < 0.0f && v1 > 0.0f) {
+    // pixel inside the swept band: + (1+i) exp(-i pi u^2/c)
     float turns = u * u * L.hc;
     turns -= floorf(turns);
     float st, ct;
     __sincosf(6.283185307179586f * (turns - 0.5f), &st, &ct);        // = -(sin, cos)(2 pi turns)
-    const float er = -(ct + st), ei = -(ct - st);
-    hr += er * L.Pr - ei * L.Pi;
-    hi += er * L.Pi + ei * L.Pr;
+    hr -= ct + st;
+    hi -= ct - st;
   }
   s.zAr = fmaf(Y.x, hr, fmaf(Y.y, hi, s.zAr));
   s.zAi = fmaf(Y.x, hi, fmaf(-Y.y, hr, s.zAi));
@@ -225,6 +238,59 @@ __device__ __forceinline__ void pixel(const LaneTrack& L, float u, const float4 
   s.qE = fmaf(Wt.y, h2, s.qE);
 }
 
+// Generic pixel loop over window offsets [j0, j1): every lane tests its own window length Wm and the
+// in-band condition per pixel (wide or clipped windows, ragged tails).  The gather of pixel j+1 is
+// issued before the arithmetic of pixel j; lanes past their window run on zeroed data.
+template <int MODE>
+__device__ __forceinline__ void pixel_loop_generic(const EvalArgs& a, const LaneTrack& L, int j0, int j1, int Wm,
+                                                   int idx, float u, unsigned lut_lane, LaneSums& s) {
+  float4 Ya = make_float4(0.f, 0.f, 0.f, 0.f), Yb;
+  float2 Wa = make_float2(0.f, 0.f), Wb;
+  if (j0 < Wm) { Ya = __ldg(a.grid + idx); Wa = __ldg(a.wgt + idx); }
+  for (int j = j0; j < j1; j += 2) {
+    Yb = make_float4(0.f, 0.f, 0.f, 0.f); Wb = make_float2(0.f, 0.f);
+    idx += a.Nt;
+    if (j + 1 < Wm) { Yb = __ldg(a.grid + idx); Wb = __ldg(a.wgt + idx); }
+    pixel<MODE, 1>(L, u, Ya, Wa, lut_lane, s);
+    u -= 1.0f;
+    Ya = make_float4(0.f, 0.f, 0.f, 0.f); Wa = make_float2(0.f, 0.f);
+    idx += a.Nt;
+    if (j + 2 < Wm) { Ya = __ldg(a.grid + idx); Wa = __ldg(a.wgt + idx); }
+    pixel<MODE, 1>(L, u, Yb, Wb, lut_lane, s);
+    u -= 1.0f;
+  }
+}
+
+// Fast pixel loop over offsets [0, Wn), Wn <= every active lane's window length: no per-pixel window
+// test (inactive lanes never load and keep zeroed data), and the only pixel that can lie inside the
+// swept band when c < 1 -- k = ceil(x), offset jc, the same for all lanes -- is singled out by a
+// warp-uniform branch.  Loads run two pixels ahead of the arithmetic.
+template <int MODE>
+__device__ __forceinline__ void pixel_loop_fast(const EvalArgs& a, const LaneTrack& L, int Wn, int jc, bool act,
+                                                int idx, float u, unsigned lut_lane, LaneSums& s) {
+  float4 Y0 = make_float4(0.f, 0.f, 0.f, 0.f), Y1 = Y0;
+  float2 W0 = make_float2(0.f, 0.f), W1 = W0;
+  const int Nt = a.Nt;
+  if (act) {
+    Y0 = __ldg(a.grid + idx); W0 = __ldg(a.wgt + idx);
+    if (1 < Wn) { Y1 = __ldg(a.grid + idx + Nt); W1 = __ldg(a.wgt + idx + Nt); }
+  }
+  // each buffer is refilled (pixel j+2) right after the pixel that used it
+  int j = 0;
+  for (; j + 2 <= Wn; j += 2) {
+    idx += 2 * Nt;
+    if (j == jc) pixel<MODE, 1>(L, u, Y0, W0, lut_lane, s); else pixel<MODE, 0>(L, u, Y0, W0, lut_lane, s);
+    u -= 1.0f;
+    if (act && j + 2 < Wn) { Y0 = __ldg(a.grid + idx); W0 = __ldg(a.wgt + idx); }
+    if (j + 1 == jc) pixel<MODE, 1>(L, u, Y1, W1, lut_lane, s); else pixel<MODE, 0>(L, u, Y1, W1, lut_lane, s);
+    u -= 1.0f;
+    if (act && j + 3 < Wn) { Y1 = __ldg(a.grid + idx + Nt); W1 = __ldg(a.wgt + idx + Nt); }
+  }
+  if (j < Wn) {
+    if (j == jc) pixel<MODE, 1>(L, u, Y0, W0, lut_lane, s); else pixel<MODE, 0>(L, u, Y0, W0, lut_lane, s);
+  }
+}
+
 // ------------------------------------------------------------------------------------------
 // Kernel A: track + gather + per-tile sums.  Persistent: one CTA per SM, warps claim work items
 // (template, tile) in tile-major order from a global counter, kClaim at a time.
@@ -232,10 +298,21 @@ __device__ __forceinline__ void pixel(const LaneTrack& L, float u, const float4 
 // current chunk of 32, computes its track point in fp64 and then walks its own window pixel by
 // pixel.  The grid is stored time-contiguous ([k][m]), so the 32 lanes' loads of pixel offset j
 // fall on consecutive addresses wherever neighbouring tranches share k_lo (slow chirps: runs of
-// 1/c tranches).  Lanes past their window (or inactive) keep running with zeroed data: the loop has
-// no divergent branch except the rare in-band term.
+// 1/c tranches).  Chunks whose active lanes all sweep less than one bin (c < 1: the bulk of every
+// bank) and agree on the offset of bin ceil(x) take pixel_loop_fast up to the shortest window and
+// finish ragged tails in pixel_loop_generic; all other chunks run pixel_loop_generic throughout.
 // ------------------------------------------------------------------------------------------
 constexpr int kClaim = 4;
+
+// {i0, i1} = range of the compacted valid-tranche list covered by each tile (C9, C10)
+__global__ void tile_table_kernel(const int* __restrict__ vprefix, int Nt, int N_seg, int tps, int n_tiles,
+                                  int2* __restrict__ table) {
+  const int tile = blockIdx.x * blockDim.x + threadIdx.x;
+  if (tile >= n_tiles) return;
+  int m0, m1;
+  tile_range(tile, tps, Nt, N_seg, m0, m1);
+  table[tile] = make_int2(vprefix[m0], vprefix[m1]);
+}
 
 template <int MODE>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, 1)
@@ -259,16 +336,16 @@ eval_tiles_kernel(const EvalArgs a) {
     if (lane == 0) w0 = (long long)atomicAdd(a.work_counter, (unsigned long long)kClaim);
     w0 = __shfl_sync(0xffffffffu, w0, 0);
     if (w0 >= n_work) break;
-    const long long w1 = min(w0 + kClaim, n_work);
-    for (long long w = w0; w < w1; ++w) {
-      const int tile = (int)(w / a.n);
-      const long long it = w - (long long)tile * a.n;
-      int m0, m1;
-      tile_range(tile, a.tiles_per_seg, a.Nt, a.N_seg, m0, m1);
+    const int n_claim = (int)min((long long)kClaim, n_work - w0);
+    int tile = (int)(w0 / a.n);
+    long long it = w0 - (long long)tile * a.n;
+    for (int wi = 0; wi < n_claim; ++wi, ++it) {
+      if (it == a.n) { it = 0; ++tile; }
       // valid (non-gap) tranches of the tile: entries [i0, i1) of the compacted list (C10)
-      const int i0 = a.vprefix[m0], i1 = a.vprefix[m1];
+      const int2 ir = a.tile_table[tile];
+      const int i0 = ir.x, i1 = ir.y;
 
-      const TemplateConst T = load_template(a.params + it * 8);
+      const TemplateConst T = load_template(a.params + it * 8, a.DT);
       if (!T.ok) {
         if (lane == 0) {
           a.partials[(long long)tile * a.n + it] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -287,11 +364,12 @@ eval_tiles_kernel(const EvalArgs a) {
         const bool valid = i < i1;
         const int m = a.valid_m[valid ? i : i0];
         const TrackPoint tp = track_point(T, m, a.DT, a.x_lo, a.x_hi, a.c_max, valid);
-        if (__ballot_sync(0xffffffffu, tp.active) == 0u) continue;
-        int Wm = 0, idx = 0;
-        float u = 0.f;
+        const unsigned act_mask = __ballot_sync(0xffffffffu, tp.active);
+        if (act_mask == 0u) continue;
+        int Wm = 0, idx = 0, jc = -1;
+        float u = 0.f, Pr = 0.f, Pi = 0.f;
         LaneTrack L;
-        L.sc = 1.f; L.scc = 1.f; L.hc = 0.f; L.Pr = 0.f; L.Pi = 0.f; L.Qr = 0.f; L.Qi = 0.f;
+        L.sc = 1.f; L.scc = 1.f; L.hc = 0.f; L.Er = 0.f; L.Ei = 0.f;
         if (tp.active) {
           int k_lo, k_hi;
           window(tp, a.H, a.adaptive, a.Nf, k_lo, k_hi);
@@ -300,48 +378,50 @@ eval_tiles_kernel(const EvalArgs a) {
           const double flx = floor(tp.x);
           const float fracx = (float)(tp.x - flx);
           u = fracx - (float)(k_lo - (int)flx);          // cancellation-safe x - k_lo
-          // phases in turns, reduced in fp64 (phi reaches ~1e8 rad)
+          jc = (int)ceil(tp.x) - k_lo;                   // offset of bin ceil(x)
+          // phases in turns, reduced in fp64 (phi reaches ~1e8 rad), then to [-1/2, 1/2)
           double tphi = T.phic_turns - tp.X58 * (1.0 / kPi);
           tphi -= floor(tphi);
           double tpsi = 0.5 * tp.c + (tp.x - flx);
           tpsi -= floor(tpsi);
           float sphi, cphi, spsi, cpsi;
-          sincospif(2.0f * (float)tphi, &sphi, &cphi);
-          sincospif(2.0f * (float)tpsi, &spsi, &cpsi);
+          __sincosf(6.283185307179586f * ((float)tphi - 0.5f), &sphi, &cphi);     // = -(sin, cos)(2 pi tphi)
+          __sincosf(6.283185307179586f * ((float)tpsi - 0.5f), &spsi, &cpsi);
           const float cf = (float)tp.c;
-          const float pre = (float)(T.acoef * tp.Xm14) * rsqrtf(2.0f * cf);  // A_m / sqrt(2c)
+          const float pre = -(T.acoef * tp.Xm14) * rsqrtf(2.0f * cf);           // -A_m / sqrt(2c)
           L.sc = rsqrtf(0.5f * cf);
           L.scc = L.sc * cf;
           L.hc = __fdividef(0.5f, cf);
-          L.Pr = pre * cphi;
-          L.Pi = pre * sphi;
-          L.Qr = L.Pr * cpsi - L.Pi * spsi;
-          L.Qi = L.Pr * spsi + L.Pi * cpsi;
+          Pr = pre * cphi;
+          Pi = pre * sphi;
+          L.Er = -cpsi;
+          L.Ei = -spsi;
         }
+        // warp-uniform choice of the pixel loop
         const int Wmax = __reduce_max_sync(0xffffffffu, Wm);
+        const int Wmin = __reduce_min_sync(0xffffffffu, tp.active ? Wm : 0x7fffffff);
+        const int jc0 = __shfl_sync(0xffffffffu, jc, __ffs(act_mask) - 1);
+        const bool fast_lane = !tp.active || (tp.c < 1.0 && jc == jc0);
+        const bool fast = __all_sync(0xffffffffu, fast_lane) && jc0 >= 0 && jc0 < Wmin;
 
         // ---------------- pixel loop (a3-a5): lane walks its own window ----------------
-        // the gather of pixel j+1 is issued before the arithmetic of pixel j
         LaneSums s;
         s.zAr = 0.f; s.zAi = 0.f; s.zEr = 0.f; s.zEi = 0.f; s.qA = 0.f; s.qE = 0.f;
-        float4 Ya = make_float4(0.f, 0.f, 0.f, 0.f), Yb;
-        float2 Wa = make_float2(0.f, 0.f), Wb;
-        if (0 < Wm) { Ya = __ldg(a.grid + idx); Wa = __ldg(a.wgt + idx); }
-        for (int j = 0; j < Wmax; j += 2) {
-          Yb = make_float4(0.f, 0.f, 0.f, 0.f); Wb = make_float2(0.f, 0.f);
-          idx += a.Nt;
-          if (j + 1 < Wm) { Yb = __ldg(a.grid + idx); Wb = __ldg(a.wgt + idx); }
-          pixel<MODE>(L, u, Ya, Wa, lut_lane, s);
-          u -= 1.0f;
-          Ya = make_float4(0.f, 0.f, 0.f, 0.f); Wa = make_float2(0.f, 0.f);
-          idx += a.Nt;
-          if (j + 2 < Wm) { Ya = __ldg(a.grid + idx); Wa = __ldg(a.wgt + idx); }
-          pixel<MODE>(L, u, Yb, Wb, lut_lane, s);
-          u -= 1.0f;
+        if (fast) {
+          pixel_loop_fast<MODE>(a, L, Wmin, jc0, tp.active, idx, u, lut_lane, s);
+          if (Wmax > Wmin)
+            pixel_loop_generic<MODE>(a, L, Wmin, Wmax, Wm, idx + Wmin * a.Nt, u - (float)Wmin, lut_lane, s);
+        } else {
+          pixel_loop_generic<MODE>(a, L, 0, Wmax, Wm, idx, u, lut_lane, s);
         }
-        s_acc[0 * kAccStride] += s.zAr; s_acc[1 * kAccStride] += s.zAi;
-        s_acc[2 * kAccStride] += s.zEr; s_acc[3 * kAccStride] += s.zEi;
-        s_acc[4 * kAccStride] += s.qA;  s_acc[5 * kAccStride] += s.qE;
+        // apply the tranche's factor P (and |P|^2) and promote to fp64
+        const float P2 = fmaf(Pr, Pr, Pi * Pi);
+        s_acc[0 * kAccStride] += (double)(Pr * s.zAr - Pi * s.zAi);
+        s_acc[1 * kAccStride] += (double)(Pr * s.zAi + Pi * s.zAr);
+        s_acc[2 * kAccStride] += (double)(Pr * s.zEr - Pi * s.zEi);
+        s_acc[3 * kAccStride] += (double)(Pr * s.zEi + Pi * s.zEr);
+        s_acc[4 * kAccStride] += (double)(P2 * s.qA);
+        s_acc[5 * kAccStride] += (double)(P2 * s.qE);
       }
 
       const double dzAr = warp_sum(s_acc[0 * kAccStride]), dzAi = warp_sum(s_acc[1 * kAccStride]);
@@ -389,7 +469,7 @@ __global__ void count_pixels_kernel(const EvalArgs a, long long* __restrict__ co
   const int lane = threadIdx.x & 31;
   const long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= a.n) return;
-  const TemplateConst T = load_template(a.params + w * 8);
+  const TemplateConst T = load_template(a.params + w * 8, a.DT);
   long long cnt = 0;
   if (T.ok) {
     for (int m = lane; m < a.Nt; m += 32) {
