@@ -132,6 +132,12 @@ TFS_API int tfs_set_profiling(tfs_ctx* ctx, int on);
 TFS_API int tfs_get_profile(tfs_ctx* ctx, double* main_kernel_ms, long long* main_kernel_launches,
                             long long* kernel_launches);
 
+/* Measurement aid for the roofline (bench.py): allocate a zero-filled scratch buffer of `bytes`
+ * (choose it well inside the L2, e.g. 32 MiB), read it `iters` times with coalesced 16-byte loads from
+ * one 1024-thread CTA per SM, and return the sustained read bandwidth in GB/s (CUDA events around the
+ * launch; one warm-up launch first).  Synchronises `stream`.  The buffer is freed before returning. */
+TFS_API int tfs_probe_l2_bandwidth(tfs_ctx* ctx, long long bytes, int iters, double* gb_per_s, void* stream);
+
 TFS_API void tfs_destroy(tfs_ctx* ctx);
 
 /* Message of the last failure on this context (or of the last failed tfs_create when ctx is

@@ -62,6 +62,8 @@ def load_library():
     lib.tfs_set_profiling.restype = ip
     lib.tfs_get_profile.argtypes = [vp, C.POINTER(dp), C.POINTER(ll), C.POINTER(ll)]
     lib.tfs_get_profile.restype = ip
+    lib.tfs_probe_l2_bandwidth.argtypes = [vp, ll, ip, C.POINTER(dp), vp]
+    lib.tfs_probe_l2_bandwidth.restype = ip
     lib.tfs_destroy.argtypes = [vp]
     lib.tfs_destroy.restype = None
     lib.tfs_last_error.argtypes = [vp]
@@ -166,6 +168,11 @@ class Tfs:
         ms, nk, nl = C.c_double(), C.c_longlong(), C.c_longlong()
         self._check(self._lib.tfs_get_profile(self._h, C.byref(ms), C.byref(nk), C.byref(nl)))
         return dict(main_kernel_ms=ms.value, main_kernel_launches=nk.value, kernel_launches=nl.value)
+
+    def probe_l2_bandwidth(self, nbytes=32 << 20, iters=200, stream=None):
+        g = C.c_double()
+        self._check(self._lib.tfs_probe_l2_bandwidth(self._h, nbytes, iters, C.byref(g), _stream(stream)))
+        return g.value
 
     def last_error(self):
         return self._lib.tfs_last_error(self._h).decode()

@@ -561,6 +561,42 @@ int tfs_refine(tfs_ctx* ctx, const double* params, long long n, const long long*
   return TFS_OK;
 }
 
+int tfs_probe_l2_bandwidth(tfs_ctx* ctx, long long bytes, int iters, double* gb_per_s, void* stream) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_probe_l2_bandwidth: ctx is NULL");
+  if (bytes < (1 << 20) || bytes > (1ll << 32) || iters < 1 || iters > 100000 || !gb_per_s)
+    return fail(ctx, TFS_EINVAL, "tfs_probe_l2_bandwidth: need 1 MiB <= bytes <= 4 GiB, 1 <= iters <= 1e5, gb_per_s != NULL");
+  cudaStream_t st = (cudaStream_t)stream;
+  void* buf = nullptr;
+  float* sink = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  const long long n_vec = bytes / 16;
+  int rc = TFS_OK;
+  cudaError_t e;
+  auto done = [&](int code, const char* what, cudaError_t err) {
+    if (code) fail(ctx, code, "tfs_probe_l2_bandwidth: %s: %s", what, cudaGetErrorString(err));
+    if (buf) cudaFree(buf);
+    if (sink) cudaFree(sink);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    return code;
+  };
+  if ((e = cudaMalloc(&buf, (size_t)n_vec * 16)) != cudaSuccess) return done(TFS_ENOMEM, "cudaMalloc", e);
+  if ((e = cudaMalloc((void**)&sink, sizeof(float))) != cudaSuccess) return done(TFS_ENOMEM, "cudaMalloc", e);
+  if ((e = cudaMemsetAsync(buf, 0, (size_t)n_vec * 16, st)) != cudaSuccess) return done(TFS_ECUDA, "cudaMemsetAsync", e);
+  if ((e = cudaEventCreate(&e0)) != cudaSuccess || (e = cudaEventCreate(&e1)) != cudaSuccess)
+    return done(TFS_ECUDA, "cudaEventCreate", e);
+  l2_probe_kernel<<<ctx->sm_count, 1024, 0, st>>>((const float4*)buf, n_vec, 2, sink);        // warm the L2
+  cudaEventRecord(e0, st);
+  l2_probe_kernel<<<ctx->sm_count, 1024, 0, st>>>((const float4*)buf, n_vec, iters, sink);
+  cudaEventRecord(e1, st);
+  ctx->launches += 2;
+  if ((e = cudaEventSynchronize(e1)) != cudaSuccess) return done(TFS_ECUDA, "l2_probe_kernel", e);
+  float ms = 0.f;
+  if ((e = cudaEventElapsedTime(&ms, e0, e1)) != cudaSuccess) return done(TFS_ECUDA, "cudaEventElapsedTime", e);
+  *gb_per_s = (double)n_vec * 16.0 * iters / (ms * 1e-3) / 1e9;
+  return done(rc, "", cudaSuccess);
+}
+
 int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k, long long* idx, float* val, void* stream) {
   if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_topk: ctx is NULL");
   if (!upsilon || !idx || !val) return fail(ctx, TFS_EINVAL, "tfs_topk: upsilon, idx and val are required");

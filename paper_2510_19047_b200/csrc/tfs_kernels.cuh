@@ -549,6 +549,27 @@ valid_list_kernel(const uint8_t* __restrict__ gap, int Nt, int* __restrict__ vpr
 }
 
 // ------------------------------------------------------------------------------------------
+// Measurement aid (bench.py): read an L2-resident buffer over and over with
+// coalesced 16-byte loads from every SM; the resulting GB/s is the on-chip gather ceiling that the
+// roofline's L2 term is quoted against.  The sums are written so the loads cannot be dropped.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024, 1)
+l2_probe_kernel(const float4* __restrict__ buf, long long n_vec, int iters, float* __restrict__ sink) {
+  float acc = 0.f;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (int it = 0; it < iters; ++it) {
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 3 * stride < n_vec; i += 4 * stride) {
+      const float4 a = __ldcg(buf + i), b = __ldcg(buf + i + stride), c = __ldcg(buf + i + 2 * stride),
+                   d = __ldcg(buf + i + 3 * stride);
+      acc += (a.x + b.y) + (c.z + d.w);
+    }
+    for (; i < n_vec; i += stride) acc += __ldcg(buf + i).x;
+  }
+  if (acc == 123.456f) sink[0] = acc;      // never true for the zero-filled buffer; keeps the loads alive
+}
+
+// ------------------------------------------------------------------------------------------
 // Ladder refinement (a10; C19): child (a, b) of survivor j, a, b in [0, r), sits at
 //   Mc' = Mc (1 + o_a d_mc_rel),  tc' = tc + o_b d_tc,  o_i = (2i + 1 - r) / (2r)
 // (an r x r lattice, r times denser per dimension, that tiles the parent's cell); the other six

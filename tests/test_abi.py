@@ -25,7 +25,7 @@ def test_header_declares_the_boundary():
     syms = declared_symbols()
     for s in ["tfs_create", "tfs_upload_data", "tfs_eval", "tfs_topk", "tfs_destroy", "tfs_last_error",
               "tfs_count_pixels", "tfs_default_opts", "tfs_bad_param_count", "tfs_set_profiling",
-              "tfs_get_profile", "tfs_refine"]:
+              "tfs_get_profile", "tfs_refine", "tfs_probe_l2_bandwidth"]:
         assert s in syms
 
 
