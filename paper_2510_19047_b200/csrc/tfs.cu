@@ -35,6 +35,7 @@ struct tfs_ctx {
   int* vprefix = nullptr;                  // [Nt+1] valid tranches before m
   int* valid_m = nullptr;                  // [max(#valid,1)] valid tranche indices
   float4* lut = nullptr;
+  FarCoef far{};
   unsigned long long* bad = nullptr;       // device counter
   unsigned long long* work = nullptr;      // device work-item counter of the main kernel
   long long bad_host = 0;
@@ -194,8 +195,57 @@ void build_lut(std::vector<float4>& lut) {
     const double w = (double)(ip - im);                      // central difference (one-sided at the ends)
     // interpolant around node i as intercept + slope * t:  F(t) ~ F_i + (t kLutN - i) dF  (see fresnel_aux)
     const double dF = (Fp - Fm) / w, dG = (Gp - Gm) / w;
-    lut[i] = make_float4((float)(F - i * dF), (float)(kLutN * dF), (float)(G - i * dG), (float)(kLutN * dG));
+    lut[i] = make_float4((float)(G - i * dG), (float)(F - i * dF), (float)(kLutN * dG), (float)(kLutN * dF));
   }
+}
+
+// Far-zone polynomials (kernel: pixel_far).  For v >= kVFar,
+//   f(v) = w (1/pi + F1 z + F2 z^2),  g(v) = w^3 (1/pi^2 + G1 z + G2 z^2),  w = 1/v, z = w^4
+// -- the shape of the asymptotic series A&S 7.3.27-28 (f ~ 1/(pi v) - 3/(pi^3 v^5) + ...,
+// g ~ 1/(pi^2 v^3) - 15/(pi^4 v^7) + ...): the leading coefficients are kept exact, so the relative error
+// vanishes as v grows (slow chirps put their brightest pixels at v ~ 5...40), and the other two are
+// fitted by least squares on Chebyshev nodes of z in [0, z_max], weighted so that the error RELATIVE to
+// |g + i f| ~ f is minimised.  Returns the largest such relative error over the nodes.
+double fit_far(FarCoef& out) {
+  const int N = 256;
+  const double v_min = (double)kVFar * 0.98;
+  const double z_max = 1.0 / (v_min * v_min * v_min * v_min);
+  const double F0 = 1.0 / kPi, G0 = 1.0 / (kPi * kPi);
+  double Af[2][3] = {{0}}, Ag[2][3] = {{0}};        // normal equations in the scaled variable y = z/z_max
+  std::vector<double> ys(N), w1(N), tf(N), tg(N);
+  for (int i = 0; i < N; ++i) {
+    const double y = std::max(0.5 * (1.0 + std::cos(kPi * (i + 0.5) / N)), 1e-9);
+    const double z = y * z_max, w = std::sqrt(std::sqrt(z)), v = 1.0 / w;
+    double f, g;
+    fresnel_aux_host(v, f, g);
+    ys[i] = y; w1[i] = w; tf[i] = f; tg[i] = g;
+    // residuals divided by f:  (w (F0 + y a1 + y^2 a2) - f)/f  and  (w^3 (G0 + y b1 + y^2 b2) - g)/f
+    const double sf = w / f, sg = w * w * w / f;
+    const double b[2] = {y, y * y};
+    const double rf = (f - w * F0) / f, rg = (g - w * w * w * G0) / f;
+    for (int r = 0; r < 2; ++r) {
+      for (int c = 0; c < 2; ++c) { Af[r][c] += sf * b[r] * sf * b[c]; Ag[r][c] += sg * b[r] * sg * b[c]; }
+      Af[r][2] += sf * b[r] * rf;
+      Ag[r][2] += sg * b[r] * rg;
+    }
+  }
+  auto solve2 = [](double A[2][3], double x[2]) {
+    const double det = A[0][0] * A[1][1] - A[0][1] * A[1][0];
+    x[0] = (A[0][2] * A[1][1] - A[0][1] * A[1][2]) / det;
+    x[1] = (A[0][0] * A[1][2] - A[0][2] * A[1][0]) / det;
+  };
+  double cf[2], cg[2];
+  solve2(Af, cf);
+  solve2(Ag, cg);
+  double err = 0.0;
+  for (int i = 0; i < N; ++i) {
+    const double y = ys[i], w = w1[i];
+    err = std::max(err, std::fabs(w * (F0 + y * (cf[0] + y * cf[1])) - tf[i]) / tf[i]);
+    err = std::max(err, std::fabs(w * w * w * (G0 + y * (cg[0] + y * cg[1])) - tg[i]) / tf[i]);
+  }
+  out.F0 = (float)F0; out.F1 = (float)(cf[0] / z_max); out.F2 = (float)(cf[1] / (z_max * z_max));
+  out.G0 = (float)G0; out.G1 = (float)(cg[0] / z_max); out.G2 = (float)(cg[1] / (z_max * z_max));
+  return err;
 }
 
 EvalArgs base_args(const tfs_ctx* ctx) {
@@ -209,6 +259,7 @@ EvalArgs base_args(const tfs_ctx* ctx) {
   a.DT = ctx->DT;
   a.x_lo = ctx->f_lo * ctx->DT; a.x_hi = ctx->f_hi * ctx->DT;
   a.c_max = ctx->opts.c_max;
+  a.far = ctx->far;
   a.N_seg = 1; a.tiles_per_seg = 1; a.n_tiles = 1;
   return a;
 }
@@ -261,8 +312,8 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   *out = nullptr;
   if (Nt < 1 || Nf < 2 || !(dt > 0.0) || !std::isfinite(dt))
     return fail(nullptr, TFS_EINVAL, "tfs_create: need Nt >= 1, Nf >= 2, dt > 0 (got %d, %d, %g)", Nt, Nf, dt);
-  if ((long long)Nt * Nf >= (1ll << 31))
-    return fail(nullptr, TFS_EINVAL, "tfs_create: Nt*Nf must be < 2^31");
+  if ((long long)Nt * (Nf + kPadRows) >= (1ll << 31))
+    return fail(nullptr, TFS_EINVAL, "tfs_create: Nt*(Nf+%d) must be < 2^31", kPadRows);
   if (n_channels != 2)
     return fail(nullptr, TFS_EINVAL, "tfs_create: this build supports n_channels == 2 (A, E); got %d", n_channels);
   tfs_opts o;
@@ -290,9 +341,12 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   if (e != cudaSuccess) return bail(TFS_ECUDA, "cudaGetDevice (no CUDA device: libtfs has no CPU fallback)", e);
   e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
   if (e != cudaSuccess) return bail(TFS_ECUDA, "cudaDeviceGetAttribute", e);
-  const size_t npix = (size_t)Nt * Nf;
+  // kPadRows zeroed rows behind row Nf-1: the gather may read up to kPrefetch pixels past a window (pixel_loop)
+  const size_t npix = (size_t)Nt * (Nf + kPadRows);
   if ((e = cudaMalloc((void**)&ctx->grid, npix * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc grid", e);
   if ((e = cudaMalloc((void**)&ctx->wgt, npix * sizeof(float2))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc weights", e);
+  if ((e = cudaMemset(ctx->grid, 0, npix * sizeof(float4))) != cudaSuccess ||
+      (e = cudaMemset(ctx->wgt, 0, npix * sizeof(float2))) != cudaSuccess) return bail(TFS_ECUDA, "cudaMemset grid", e);
   if ((e = cudaMalloc((void**)&ctx->gap, (size_t)Nt)) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc gap", e);
   if ((e = cudaMalloc((void**)&ctx->vprefix, ((size_t)Nt + 1) * sizeof(int))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc vprefix", e);
   if ((e = cudaMalloc((void**)&ctx->valid_m, (size_t)Nt * sizeof(int))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc valid_m", e);
@@ -305,6 +359,7 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   if ((e = cudaMalloc((void**)&ctx->sel, sizeof(SelectState))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc select state", e);
   std::vector<float4> lut;
   build_lut(lut);
+  if (!(fit_far(ctx->far) < 2e-6)) return bail(TFS_ECUDA, "far-zone polynomial fit failed", cudaSuccess);
   if ((e = cudaMemcpy(ctx->lut, lut.data(), lut.size() * sizeof(float4), cudaMemcpyHostToDevice)) != cudaSuccess)
     return bail(TFS_ECUDA, "cudaMemcpy lut", e);
   *out = ctx;

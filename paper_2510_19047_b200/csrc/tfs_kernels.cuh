@@ -21,14 +21,17 @@ constexpr int kLutN = 512;          // LUT intervals in t = 1/(1+v)
 constexpr double kMtsun = 4.925490947e-6;   // G Msun / c^3 [s]
 constexpr double kPi = 3.14159265358979323846;
 
+// f(v) = w (F0 + F1 w^4 + F2 w^8), g(v) = w^3 (G0 + G1 w^4 + G2 w^8), w = 1/v, valid for |v| >= kVFar
+struct FarCoef { float F0, F1, F2, G0, G1, G2; };
+
 struct EvalArgs {
-  const float4* __restrict__ grid;     // [Nf][Nt] (time-contiguous) {Y_A.re, Y_A.im, Y_E.re, Y_E.im}, Y = W*D
+  const float4* __restrict__ grid;     // [Nf][Nt] (time-contiguous) {Y_A.re, Y_E.re, Y_A.im, Y_E.im}, Y = W*D
   const float2* __restrict__ wgt;      // [Nf][Nt] {W_A, W_E}
   const uint8_t* __restrict__ gap;     // [Nt] 1 = valid
   const int* __restrict__ vprefix;     // [Nt+1] number of valid tranches before m
   const int* __restrict__ valid_m;     // [vprefix[Nt]] the valid tranche indices, ascending (padded to >= 1 entry)
   const int2* __restrict__ tile_table; // [n_tiles] {i0, i1}: entries of valid_m covered by each tile
-  const float4* __restrict__ lut;      // [kLutN+1] {a_F, b_F, a_G, b_G} (see fresnel_aux)
+  const float4* __restrict__ lut;      // [kLutN+1] {a_G, a_F, b_G, b_F} (see fresnel_aux)
   const double* __restrict__ params;   // [n][8]
   float4* __restrict__ partials;       // [n_tiles][n] {z.re, z.im, hh, 0}
   unsigned long long* bad_count;       // templates rejected (counted on tile 0 only)
@@ -40,6 +43,7 @@ struct EvalArgs {
   double DT;
   double x_lo, x_hi;                   // band in bins: f_lo*DT, f_hi*DT
   double c_max;
+  FarCoef far;                         // far-zone polynomials of f, g (fitted at tfs_create)
 };
 
 // ----- tile geometry: segment n = tranches [ceil(n Nt/N_seg), ceil((n+1) Nt/N_seg))  (C9) -----
@@ -132,7 +136,7 @@ __device__ __forceinline__ void window(const TrackPoint& tp, int H, int adaptive
 
 // LUT of the Fresnel auxiliary functions f(v), g(v) (P:184-207 defines them through Eqs. 25-26;
 // A&S 7.3.5-6), tabulated against t = 1/(1+|v|) in (0, 1] with kLutN intervals:
-//   entry i = {a_F, b_F, a_G, b_G}: for t within half a step of i/kLutN,
+//   entry i = {a_G, a_F, b_G, b_F}: for t within half a step of i/kLutN,
 //     f(v) = t (a_F + b_F t),  g(v) = t (a_G + b_G t)
 //   (the linear interpolant of F = f/t, G = g/t around node i with central-difference slope,
 //    rewritten as intercept + slope*t so the fractional index is never formed).
@@ -155,18 +159,45 @@ __device__ __forceinline__ float4 lds128(unsigned addr) {
   return r;
 }
 
-// Returns F = f(|v|)/t, G = g(|v|)/t and ts = sign(v) t, so that sign(v) f = ts F, sign(v) g = ts G.
+// ----- packed fp32 pairs (sm_100a FFMA2 / FMUL2 / FADD2: two fp32 operations per issue slot) -----
+// A pair lives in a 64-bit register pair {lo, hi}.  ptxas folds pk(a, a) into a broadcast operand and
+// pk(-b, a) into swap / per-half negate modifiers, so these cost no extra instructions.
+typedef unsigned long long f2_t;
+__device__ __forceinline__ f2_t pk(float lo, float hi) {
+  f2_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void upk(f2_t r, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(r));
+}
+__device__ __forceinline__ f2_t ffma2(f2_t a, f2_t b, f2_t c) {
+  f2_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ f2_t fmul2(f2_t a, f2_t b) {
+  f2_t d;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ f2_t fadd2(f2_t a, f2_t b) {
+  f2_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+
+// Returns GF = {g(|v|)/t, f(|v|)/t} and ts = sign(v) t, so that Godd(v) = ts GF as a complex {re, im} pair.
 // lut_lane = shared address of this lane's LUT copy minus kMagicBits * (16 * kLutCopies)  (mod 2^32).
 template <int MODE>
-__device__ __forceinline__ void fresnel_aux(float v, unsigned lut_lane, float& F, float& G, float& ts) {
+__device__ __forceinline__ void fresnel_aux(float v, unsigned lut_lane, f2_t& GF, float& ts) {
   const float a = fabsf(v);
   if (MODE == 0) {
     const float t = rcp_approx(1.0f + a);         // MUFU.RCP
     const float q = fmaf(t, (float)kLutN, kMagic);
-    const float4 e = lds128(__float_as_uint(q) * (16u * kLutCopies) + lut_lane);
+    const float4 e = lds128(__float_as_uint(q) * (16u * kLutCopies) + lut_lane);   // {a_G, a_F, b_G, b_F}
     ts = copysignf(t, v);
-    F = fmaf(t, e.y, e.x);
-    G = fmaf(t, e.w, e.z);
+    GF = ffma2(pk(t, t), pk(e.z, e.w), pk(e.x, e.y));
   } else {
     // the paper's Eqs. 27-28 (|v| <= 6) and the plain asymptote f = 1/(pi v), g = 0 (Eqs. 23-24, |v| > 6)
     float f, g;
@@ -178,8 +209,7 @@ __device__ __forceinline__ void fresnel_aux(float v, unsigned lut_lane, float& F
       g = __fdividef(1.0f, 2.0f + a * (4.142f + a * (3.492f + 6.670f * a)));
     }
     ts = copysignf(1.0f, v);
-    F = f;
-    G = g;
+    GF = pk(g, f);
   }
 }
 
@@ -195,99 +225,172 @@ constexpr int kEvalSmemBytes = kLutSmemBytes + 6 * kWarpsPerCta * 32 * (int)size
 
 // One pixel of one tranche (a3-a5).  The template coefficient is h = P h', P = A/sqrt(2c) exp(i phi_m)
 // constant over the tranche, and (auxiliary-function form of Eq. 16)
-//   h' = s0 G(|v0|) - s1 G(|v1|) E  [+ (1+i) exp(-i pi u^2/c) inside the swept band],  G = g + i f,
-//   E = exp(i psi), psi = pi c + 2 pi frac(x).
+//   h' = Godd(v0) - Godd(v1) E  [+ (1+i) exp(-i pi u^2/c) inside the swept band],
+//   Godd(v) = sign(v) (g(|v|) + i f(|v|)),  E = exp(i psi), psi = pi c + 2 pi frac(x).
 // The loop accumulates z'_alpha += conj(Y_alpha) h', q'_alpha += W_alpha |h'|^2 and the factor P
 // (|P|^2 for q) is applied once per tranche.
+//
+// Two evaluations of Godd:
+//   FAR  (|v0|, |v1| >= kVFar):  f(v) = w Pf(w^4), g(v) = w^3 Pg(w^4), w = 1/v, Pf and Pg quadratics
+//         fitted at tfs_create (they are the asymptotic series of A&S 7.3.27-28 re-fitted on the
+//         interval; odd in v, so the sign comes for free).  No table read: 2 MUFU.RCP + 10 packed ops.
+//   NEAR (anything else): the shared-memory LUT in t = 1/(1+|v|) (fresnel_aux).
+// The far zone covers all but the ~2 pixels next to the track for the slow chirps that make up the
+// bulk of every bank (|v| = sqrt(2/c) |u|).
+constexpr float kVFar = 3.0f;
+
+
 struct LaneTrack {      // per-lane (= per-tranche) constants of the pixel loop
   float sc;             // sqrt(2/c)
-  float scc;            // sqrt(2c) = v1 - v0
+  float kap;            // sqrt(c/2) = 1/sc
+  float c;              // v1 - v0 = sc * c
   float hc;             // 1/(2c): pi u^2/c = 2 pi (u^2 hc)
   float Er, Ei;         // exp(i psi)
 };
 
-struct LaneSums { float zAr, zAi, zEr, zEi, qA, qE; };
+struct LaneSums { f2_t zr, zi, q; };     // {A, E} pairs: Re z', Im z', q'
 
-// INBAND: 0 = the pixel is known to lie outside the swept band, 1 = test it (v0 < 0 < v1)
-template <int MODE, int INBAND>
-__device__ __forceinline__ void pixel(const LaneTrack& L, float u, const float4 Y, const float2 Wt,
-                                      unsigned lut_lane, LaneSums& s) {
+// grid pixel Y = {Y_A.re, Y_E.re, Y_A.im, Y_E.im}, weights Wt = {W_A, W_E}
+__device__ __forceinline__ void mac(LaneSums& s, const float4 Y, const float2 Wt, float hr, float hi) {
+  const f2_t Yre = pk(Y.x, Y.y), Yim = pk(Y.z, Y.w);
+  s.zr = ffma2(Yre, pk(hr, hr), s.zr);            // Re conj(Y) h = Y.re hr + Y.im hi
+  s.zr = ffma2(Yim, pk(hi, hi), s.zr);
+  s.zi = ffma2(Yre, pk(hi, hi), s.zi);            // Im conj(Y) h = Y.re hi - Y.im hr
+  s.zi = ffma2(Yim, pk(-hr, -hr), s.zi);
+  const float h2 = fmaf(hr, hr, hi * hi);
+  s.q = ffma2(pk(Wt.x, Wt.y), pk(h2, h2), s.q);
+}
+
+// u = x - k; u + c is formed here, per pixel, so that it is rounded at the magnitude of u (next to the
+// track, where h' is sensitive to v1 - v0, u is small).  MASKED: msk = 0 kills the contribution of a lane
+// past its window.
+template <int MASKED>
+__device__ __forceinline__ void pixel_far(const LaneTrack& L, const FarCoef& C, float u, float msk,
+                                          float& hr, float& hi) {
+  const f2_t r = pk(rcp_approx(u), rcp_approx(u + L.c));
+  const float kap = MASKED ? L.kap * msk : L.kap;
+  const f2_t w = fmul2(r, pk(kap, kap));                         // {1/v0, 1/v1}
+  const f2_t s1 = fmul2(w, w);
+  const f2_t s2 = fmul2(s1, s1);
+  const f2_t Pf = ffma2(s2, ffma2(s2, pk(C.F2, C.F2), pk(C.F1, C.F1)), pk(C.F0, C.F0));
+  const f2_t Pg = ffma2(s2, ffma2(s2, pk(C.G2, C.G2), pk(C.G1, C.G1)), pk(C.G0, C.G0));
+  const f2_t fv = fmul2(w, Pf);
+  const f2_t gv = fmul2(fmul2(w, s1), Pg);
+  float f0, f1, g0, g1;
+  upk(fv, f0, f1);
+  upk(gv, g0, g1);
+  hr = fmaf(-L.Er, g1, fmaf(L.Ei, f1, g0));          // Godd(v0) - E Godd(v1)
+  hi = fmaf(-L.Er, f1, fmaf(-L.Ei, g1, f0));
+}
+
+template <int MODE, int MASKED>
+__device__ __forceinline__ void pixel_near(const LaneTrack& L, float u, float msk, unsigned lut_lane,
+                                           float& hr, float& hi) {
   const float v0 = L.sc * u;
-  const float v1 = v0 + L.scc;
-  float F0, G0, t0, F1, G1, t1;
-  fresnel_aux<MODE>(v0, lut_lane, F0, G0, t0);
-  fresnel_aux<MODE>(v1, lut_lane, F1, G1, t1);
-  const float w1r = G1 * L.Er - F1 * L.Ei, w1i = G1 * L.Ei + F1 * L.Er;
-  float hr = fmaf(t0, G0, -t1 * w1r);
-  float hi = fmaf(t0, F0, -t1 * w1i);
-  if (INBAND && v0 < 0.0f && v1 > 0.0f) {
+  const float v1 = fmaf(L.sc, L.c, v0);
+  f2_t GF0, GF1;
+  float t0, t1;
+  fresnel_aux<MODE>(v0, lut_lane, GF0, t0);
+  fresnel_aux<MODE>(v1, lut_lane, GF1, t1);
+  if (MASKED) { t0 *= msk; t1 *= msk; }
+  const f2_t Z0 = fmul2(pk(t0, t0), GF0);                        // Godd(v0) = {re, im}
+  const f2_t Z1 = fmul2(pk(t1, t1), GF1);
+  float z1r, z1i;
+  upk(Z1, z1r, z1i);
+  f2_t h = ffma2(pk(-L.Er, -L.Er), Z1, Z0);                      // Z0 - E Z1
+  h = ffma2(pk(L.Ei, L.Ei), pk(z1i, -z1r), h);
+  upk(h, hr, hi);
+  if (v0 < 0.0f && v1 > 0.0f) {
     // pixel inside the swept band: + (1+i) exp(-i pi u^2/c)
     float turns = u * u * L.hc;
     turns -= floorf(turns);
     float st, ct;
     __sincosf(6.283185307179586f * (turns - 0.5f), &st, &ct);        // = -(sin, cos)(2 pi turns)
-    hr -= ct + st;
-    hi -= ct - st;
-  }
-  s.zAr = fmaf(Y.x, hr, fmaf(Y.y, hi, s.zAr));
-  s.zAi = fmaf(Y.x, hi, fmaf(-Y.y, hr, s.zAi));
-  s.zEr = fmaf(Y.z, hr, fmaf(Y.w, hi, s.zEr));
-  s.zEi = fmaf(Y.z, hi, fmaf(-Y.w, hr, s.zEi));
-  const float h2 = fmaf(hr, hr, hi * hi);
-  s.qA = fmaf(Wt.x, h2, s.qA);
-  s.qE = fmaf(Wt.y, h2, s.qE);
-}
-
-// Generic pixel loop over window offsets [j0, j1): every lane tests its own window length Wm and the
-// in-band condition per pixel (wide or clipped windows, ragged tails).  The gather of pixel j+1 is
-// issued before the arithmetic of pixel j; lanes past their window run on zeroed data.
-template <int MODE>
-__device__ __forceinline__ void pixel_loop_generic(const EvalArgs& a, const LaneTrack& L, int j0, int j1, int Wm,
-                                                   int idx, float u, unsigned lut_lane, LaneSums& s) {
-  float4 Ya = make_float4(0.f, 0.f, 0.f, 0.f), Yb;
-  float2 Wa = make_float2(0.f, 0.f), Wb;
-  if (j0 < Wm) { Ya = __ldg(a.grid + idx); Wa = __ldg(a.wgt + idx); }
-  for (int j = j0; j < j1; j += 2) {
-    Yb = make_float4(0.f, 0.f, 0.f, 0.f); Wb = make_float2(0.f, 0.f);
-    idx += a.Nt;
-    if (j + 1 < Wm) { Yb = __ldg(a.grid + idx); Wb = __ldg(a.wgt + idx); }
-    pixel<MODE, 1>(L, u, Ya, Wa, lut_lane, s);
-    u -= 1.0f;
-    Ya = make_float4(0.f, 0.f, 0.f, 0.f); Wa = make_float2(0.f, 0.f);
-    idx += a.Nt;
-    if (j + 2 < Wm) { Ya = __ldg(a.grid + idx); Wa = __ldg(a.wgt + idx); }
-    pixel<MODE, 1>(L, u, Yb, Wb, lut_lane, s);
-    u -= 1.0f;
+    const float m = MASKED ? msk : 1.0f;
+    hr -= m * (ct + st);
+    hi -= m * (ct - st);
   }
 }
 
-// Fast pixel loop over offsets [0, Wn), Wn <= every active lane's window length: no per-pixel window
-// test (inactive lanes never load and keep zeroed data), and the only pixel that can lie inside the
-// swept band when c < 1 -- k = ceil(x), offset jc, the same for all lanes -- is singled out by a
-// warp-uniform branch.  Loads run two pixels ahead of the arithmetic.
-template <int MODE>
-__device__ __forceinline__ void pixel_loop_fast(const EvalArgs& a, const LaneTrack& L, int Wn, int jc, bool act,
-                                                int idx, float u, unsigned lut_lane, LaneSums& s) {
-  float4 Y0 = make_float4(0.f, 0.f, 0.f, 0.f), Y1 = Y0;
-  float2 W0 = make_float2(0.f, 0.f), W1 = W0;
-  const int Nt = a.Nt;
-  if (act) {
-    Y0 = __ldg(a.grid + idx); W0 = __ldg(a.wgt + idx);
-    if (1 < Wn) { Y1 = __ldg(a.grid + idx + Nt); W1 = __ldg(a.wgt + idx + Nt); }
+// Pixel loop of one chunk (32 tranches, one per lane): every lane walks its own window, offsets
+// j = 0 ... Wm-1 from its k_lo, in groups of kGroup offsets.  The gather is software-pipelined through
+// two register buffers: the loads of group g+1 are issued before the arithmetic of group g.  It is never
+// predicated: the grid is allocated with kPadRows rows past Nf-1, so reading up to 3 kGroup pixels past
+// the end of the shortest window stays in bounds, and an inactive lane reads pixel `idx` with stride 0
+// (its sums are multiplied by P = 0 at the end; the upload zeroes non-finite pixels, so whatever it reads
+// is finite).  Offsets [JA, JB) (warp-uniform) are the NEAR zone, evaluated from the LUT with the in-band
+// test; every other offset is FAR for every active lane, and a group that does not touch the near zone
+// runs straight-line far-zone code.  Phase 1 covers the groups that lie below Wmin (the shortest active
+// window) and needs no per-lane test at all; phase 2 finishes up to Wmax with the load offset clamped to
+// the lane's window and the contribution of lanes past their window masked to zero.
+#ifndef TFS_GROUP
+#define TFS_GROUP 2
+#endif
+constexpr int kGroup = TFS_GROUP;
+constexpr int kPadRows = 3 * kGroup;         // rows of zero padding behind the grid and the weights
+
+// ZONES: 1 = test the offset against the near zone, 0 = the offset is known to be far
+template <int MODE, int MASKED, int ZONES>
+__device__ __forceinline__ void pixel_step(const LaneTrack& L, const FarCoef& C, int jj, int Wm, int JA, int JB,
+                                           const float4 Yc, const float2 Wc, float& u, unsigned lut_lane,
+                                           LaneSums& s) {
+  const float msk = (MASKED && jj >= Wm) ? 0.0f : 1.0f;
+  float hr, hi;
+  if (ZONES && jj >= JA && jj < JB) pixel_near<MODE, MASKED>(L, u, msk, lut_lane, hr, hi);
+  else pixel_far<MASKED>(L, C, u, msk, hr, hi);
+  mac(s, Yc, Wc, hr, hi);
+  u -= 1.0f;
+}
+
+struct PixelBuf { float4 Y[kGroup]; float2 W[kGroup]; };
+
+// loads offsets j0 ... j0+kGroup-1 of the lane's window (CLAMP: not past offset jlast)
+template <int CLAMP>
+__device__ __forceinline__ void load_group(const EvalArgs& a, PixelBuf& B, int idx, int stp, int j0, int jlast) {
+#pragma unroll
+  for (int p = 0; p < kGroup; ++p) {
+    const int i = idx + (CLAMP ? min(j0 + p, jlast) : (j0 + p)) * stp;
+    B.Y[p] = __ldg(a.grid + i);
+    B.W[p] = __ldg(a.wgt + i);
   }
-  // each buffer is refilled (pixel j+2) right after the pixel that used it
+}
+
+template <int MODE, int MASKED>
+__device__ __forceinline__ void compute_group(const LaneTrack& L, const FarCoef& C, const PixelBuf& B, int j0, int Wm,
+                                              int Wmax, int JA, int JB, float& u, unsigned lut_lane, LaneSums& s) {
+  if (j0 < JB && j0 + kGroup > JA) {
+#pragma unroll
+    for (int p = 0; p < kGroup; ++p)
+      if (!MASKED || j0 + p < Wmax) pixel_step<MODE, MASKED, 1>(L, C, j0 + p, Wm, JA, JB, B.Y[p], B.W[p], u, lut_lane, s);
+  } else {
+#pragma unroll
+    for (int p = 0; p < kGroup; ++p)
+      if (!MASKED || j0 + p < Wmax) pixel_step<MODE, MASKED, 0>(L, C, j0 + p, Wm, JA, JB, B.Y[p], B.W[p], u, lut_lane, s);
+  }
+}
+
+// idx = pixel index of offset 0, stp = Nt for an active lane and 0 otherwise, Wm = window length (>= 1
+// for active lanes, 0 otherwise)
+template <int MODE>
+__device__ __forceinline__ void pixel_loop(const EvalArgs& a, const LaneTrack& L, const FarCoef& C, int Wm, int Wmin,
+                                           int Wmax, int JA, int JB, int idx, int stp, float u, unsigned lut_lane,
+                                           LaneSums& s) {
+  PixelBuf A, B;
+  const int jlast = max(Wm - 1, 0);
+  load_group<0>(a, A, idx, stp, 0, jlast);
   int j = 0;
-  for (; j + 2 <= Wn; j += 2) {
-    idx += 2 * Nt;
-    if (j == jc) pixel<MODE, 1>(L, u, Y0, W0, lut_lane, s); else pixel<MODE, 0>(L, u, Y0, W0, lut_lane, s);
-    u -= 1.0f;
-    if (act && j + 2 < Wn) { Y0 = __ldg(a.grid + idx); W0 = __ldg(a.wgt + idx); }
-    if (j + 1 == jc) pixel<MODE, 1>(L, u, Y1, W1, lut_lane, s); else pixel<MODE, 0>(L, u, Y1, W1, lut_lane, s);
-    u -= 1.0f;
-    if (act && j + 3 < Wn) { Y1 = __ldg(a.grid + idx + Nt); W1 = __ldg(a.wgt + idx + Nt); }
+  for (; j + 2 * kGroup <= Wmin; j += 2 * kGroup) {                       // phase 1
+    load_group<0>(a, B, idx, stp, j + kGroup, jlast);
+    compute_group<MODE, 0>(L, C, A, j, Wm, Wmax, JA, JB, u, lut_lane, s);
+    load_group<0>(a, A, idx, stp, j + 2 * kGroup, jlast);
+    compute_group<MODE, 0>(L, C, B, j + kGroup, Wm, Wmax, JA, JB, u, lut_lane, s);
   }
-  if (j < Wn) {
-    if (j == jc) pixel<MODE, 1>(L, u, Y0, W0, lut_lane, s); else pixel<MODE, 0>(L, u, Y0, W0, lut_lane, s);
+  for (; j < Wmax; j += 2 * kGroup) {                                    // phase 2
+    load_group<1>(a, B, idx, stp, j + kGroup, jlast);
+    compute_group<MODE, 1>(L, C, A, j, Wm, Wmax, JA, JB, u, lut_lane, s);
+    if (j + kGroup >= Wmax) break;
+    load_group<1>(a, A, idx, stp, j + 2 * kGroup, jlast);
+    compute_group<MODE, 1>(L, C, B, j + kGroup, Wm, Wmax, JA, JB, u, lut_lane, s);
   }
 }
 
@@ -298,9 +401,9 @@ __device__ __forceinline__ void pixel_loop_fast(const EvalArgs& a, const LaneTra
 // current chunk of 32, computes its track point in fp64 and then walks its own window pixel by
 // pixel.  The grid is stored time-contiguous ([k][m]), so the 32 lanes' loads of pixel offset j
 // fall on consecutive addresses wherever neighbouring tranches share k_lo (slow chirps: runs of
-// 1/c tranches).  Chunks whose active lanes all sweep less than one bin (c < 1: the bulk of every
-// bank) and agree on the offset of bin ceil(x) take pixel_loop_fast up to the shortest window and
-// finish ragged tails in pixel_loop_generic; all other chunks run pixel_loop_generic throughout.
+// 1/c tranches).  Per chunk the window offsets are split (warp-uniformly) into the NEAR zone around
+// the track, evaluated from the shared-memory LUT, and the FAR zone, evaluated from the fitted
+// asymptotic polynomials in packed fp32 (pixel_loop).
 // ------------------------------------------------------------------------------------------
 constexpr int kClaim = 4;
 
@@ -366,19 +469,19 @@ eval_tiles_kernel(const EvalArgs a) {
         const TrackPoint tp = track_point(T, m, a.DT, a.x_lo, a.x_hi, a.c_max, valid);
         const unsigned act_mask = __ballot_sync(0xffffffffu, tp.active);
         if (act_mask == 0u) continue;
-        int Wm = 0, idx = 0, jc = -1;
-        float u = 0.f, Pr = 0.f, Pi = 0.f;
-        LaneTrack L;
-        L.sc = 1.f; L.scc = 1.f; L.hc = 0.f; L.Er = 0.f; L.Ei = 0.f;
+        int Wm = 0, idx = m, stp = 0, ja = 0x7fffffff, jb = 0;
+        float u = -1.f, Pr = 0.f, Pi = 0.f;
+        LaneTrack L;        // inactive lanes: u_j = -1 - j, u_j + c = -0.5 - j (finite h' on zeroed data)
+        L.sc = 1.f; L.kap = 1.f; L.c = 0.5f; L.hc = 0.f; L.Er = 0.f; L.Ei = 0.f;
         if (tp.active) {
           int k_lo, k_hi;
           window(tp, a.H, a.adaptive, a.Nf, k_lo, k_hi);
           Wm = k_hi - k_lo + 1;
           idx = k_lo * a.Nt + m;
+          stp = a.Nt;
           const double flx = floor(tp.x);
           const float fracx = (float)(tp.x - flx);
           u = fracx - (float)(k_lo - (int)flx);          // cancellation-safe x - k_lo
-          jc = (int)ceil(tp.x) - k_lo;                   // offset of bin ceil(x)
           // phases in turns, reduced in fp64 (phi reaches ~1e8 rad), then to [-1/2, 1/2)
           double tphi = T.phic_turns - tp.X58 * (1.0 / kPi);
           tphi -= floor(tphi);
@@ -388,40 +491,41 @@ eval_tiles_kernel(const EvalArgs a) {
           __sincosf(6.283185307179586f * ((float)tphi - 0.5f), &sphi, &cphi);     // = -(sin, cos)(2 pi tphi)
           __sincosf(6.283185307179586f * ((float)tpsi - 0.5f), &spsi, &cpsi);
           const float cf = (float)tp.c;
-          const float pre = -(T.acoef * tp.Xm14) * rsqrtf(2.0f * cf);           // -A_m / sqrt(2c)
           L.sc = rsqrtf(0.5f * cf);
-          L.scc = L.sc * cf;
+          L.kap = 0.5f * cf * L.sc;                                               // sqrt(c/2)
+          L.c = cf;
           L.hc = __fdividef(0.5f, cf);
+          const float pre = -(T.acoef * tp.Xm14) * (0.5f * L.sc);               // -A_m / sqrt(2c)
           Pr = pre * cphi;
           Pi = pre * sphi;
           L.Er = -cpsi;
           L.Ei = -spsi;
+          // near zone of this lane: offsets j with |v0| < kVFar or |v1| < kVFar, i.e. -(c + d) < u - j < d
+          const float d = fmaf(kVFar, L.kap, 1e-3f);
+          ja = max((int)floorf(u - d) + 1, 0);
+          jb = (int)ceilf(u + cf + d);
         }
-        // warp-uniform choice of the pixel loop
         const int Wmax = __reduce_max_sync(0xffffffffu, Wm);
         const int Wmin = __reduce_min_sync(0xffffffffu, tp.active ? Wm : 0x7fffffff);
-        const int jc0 = __shfl_sync(0xffffffffu, jc, __ffs(act_mask) - 1);
-        const bool fast_lane = !tp.active || (tp.c < 1.0 && jc == jc0);
-        const bool fast = __all_sync(0xffffffffu, fast_lane) && jc0 >= 0 && jc0 < Wmin;
+        int JA = __reduce_min_sync(0xffffffffu, ja);
+        int JB = min(__reduce_max_sync(0xffffffffu, jb), Wmax);
+        if (MODE != 0) { JA = 0; JB = Wmax; }          // the paper's approximants are used for every pixel
+        JA = min(JA, JB);
 
         // ---------------- pixel loop (a3-a5): lane walks its own window ----------------
         LaneSums s;
-        s.zAr = 0.f; s.zAi = 0.f; s.zEr = 0.f; s.zEi = 0.f; s.qA = 0.f; s.qE = 0.f;
-        if (fast) {
-          pixel_loop_fast<MODE>(a, L, Wmin, jc0, tp.active, idx, u, lut_lane, s);
-          if (Wmax > Wmin)
-            pixel_loop_generic<MODE>(a, L, Wmin, Wmax, Wm, idx + Wmin * a.Nt, u - (float)Wmin, lut_lane, s);
-        } else {
-          pixel_loop_generic<MODE>(a, L, 0, Wmax, Wm, idx, u, lut_lane, s);
-        }
+        s.zr = pk(0.f, 0.f); s.zi = pk(0.f, 0.f); s.q = pk(0.f, 0.f);
+        pixel_loop<MODE>(a, L, a.far, Wm, Wmin, Wmax, JA, JB, idx, stp, u, lut_lane, s);
         // apply the tranche's factor P (and |P|^2) and promote to fp64
+        float zAr, zEr, zAi, zEi, qA, qE;
+        upk(s.zr, zAr, zEr); upk(s.zi, zAi, zEi); upk(s.q, qA, qE);
         const float P2 = fmaf(Pr, Pr, Pi * Pi);
-        s_acc[0 * kAccStride] += (double)(Pr * s.zAr - Pi * s.zAi);
-        s_acc[1 * kAccStride] += (double)(Pr * s.zAi + Pi * s.zAr);
-        s_acc[2 * kAccStride] += (double)(Pr * s.zEr - Pi * s.zEi);
-        s_acc[3 * kAccStride] += (double)(Pr * s.zEi + Pi * s.zEr);
-        s_acc[4 * kAccStride] += (double)(P2 * s.qA);
-        s_acc[5 * kAccStride] += (double)(P2 * s.qE);
+        s_acc[0 * kAccStride] += (double)(Pr * zAr - Pi * zAi);
+        s_acc[1 * kAccStride] += (double)(Pr * zAi + Pi * zAr);
+        s_acc[2 * kAccStride] += (double)(Pr * zEr - Pi * zEi);
+        s_acc[3 * kAccStride] += (double)(Pr * zEi + Pi * zEr);
+        s_acc[4 * kAccStride] += (double)(P2 * qA);
+        s_acc[5 * kAccStride] += (double)(P2 * qE);
       }
 
       const double dzAr = warp_sum(s_acc[0 * kAccStride]), dzAi = warp_sum(s_acc[1 * kAccStride]);
@@ -502,10 +606,14 @@ pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, 
     const int m = m0 + r, k = k0 + tx;
     if (m < Nt && k < Nf) {
       const long long i = (long long)m * Nf + k;
-      const float2 dA = coeff[i], dE = coeff[npix + i];
-      const float wA = weight ? weight[i] : 1.0f;
-      const float wE = weight ? weight[npix + i] : 1.0f;
-      sY[r][tx] = make_float4(wA * dA.x, wA * dA.y, wE * dE.x, wE * dE.y);
+      float2 dA = coeff[i], dE = coeff[npix + i];
+      float wA = weight ? weight[i] : 1.0f;
+      float wE = weight ? weight[npix + i] : 1.0f;
+      // a pixel whose product W*D is not finite carries no information: weight 0 (also keeps every
+      // value the gather can read finite, which pixel_loop relies on)
+      if (!(isfinite(wA * dA.x) && isfinite(wA * dA.y) && isfinite(wA))) { wA = 0.f; dA = make_float2(0.f, 0.f); }
+      if (!(isfinite(wE * dE.x) && isfinite(wE * dE.y) && isfinite(wE))) { wE = 0.f; dE = make_float2(0.f, 0.f); }
+      sY[r][tx] = make_float4(wA * dA.x, wE * dE.x, wA * dA.y, wE * dE.y);
       sW[r][tx] = make_float2(wA, wE);
     }
   }
