@@ -60,6 +60,9 @@ typedef struct {
                             <= 0 means the default [1*df, (Nf-1)*df]                                           */
   int    fresnel_mode;   /* 0 (default): Fresnel auxiliary functions accurate to ~1e-7;
                             1: the paper's approximants Eqs. 23-28 verbatim (C8)                    */
+  int    weight_mode;    /* 0 (default): tfs_upload_data looks for separable weights W[a,m,k] = a[m] b[k]
+                            (PSD per tranche x PSD shape; C11) and then reads no per-pixel
+                            weight in the hot loop; 1: always treat W as a general per-pixel array            */
 } tfs_opts;
 
 TFS_API void tfs_default_opts(tfs_opts* opts);
@@ -74,8 +77,9 @@ TFS_API int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels,
  *   weight   [C][Nt][Nf]    float, W >= 0 per pixel (C11)               host or device, NULL => 1
  *   gap_mask [Nt]           uint8, 1 = valid, 0 = tranche overlaps a gap (C10); NULL => all valid
  * The library keeps its own repacked copy (Y = W*D interleaved by channel, and W, both transposed
- * to time-contiguous [k][m]) plus the compacted list of valid tranches.  May be called again to
- * replace the data.  Returns after the copy out of host memory is complete. */
+ * to time-contiguous [k][m]) plus the compacted list of valid tranches, and classifies the weights
+ * (tfs_weight_structure).  A pixel whose W*D or W is not finite gets weight 0.  May be called again
+ * to replace the data.  Synchronises `stream` before returning. */
 TFS_API int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight,
                     const uint8_t* gap_mask, void* stream);
 
@@ -119,6 +123,11 @@ TFS_API int tfs_refine(tfs_ctx* ctx, const double* params, long long n, const lo
  * pixel_evals = n_channels * counts[i].  counts [n] int64, host or device.  Used by the
  * benchmark for the pixel-evals/s metric and by tests for the window logic. */
 TFS_API int tfs_count_pixels(tfs_ctx* ctx, const double* params, long long n, long long* counts, void* stream);
+
+/* How tfs_eval reads the weights of the data uploaded last (C11): 0 = general per-pixel W,
+ * 1 = separable W[a,m,k] = a[m] b[k] (|W - a b| <= 1e-6 a b on every pixel), 2 = separable with
+ * b = 1 (weights depend on the tranche only, or weight == NULL).  -1 before the first upload. */
+TFS_API int tfs_weight_structure(const tfs_ctx* ctx);
 
 /* Templates rejected (NaN/Inf/Mc<=0) by the most recent tfs_eval on this context. */
 TFS_API long long tfs_bad_param_count(const tfs_ctx* ctx);

@@ -20,7 +20,8 @@ PARAM_COLS = 8
 
 class tfs_opts(C.Structure):
     _fields_ = [("half_width", C.c_int), ("adaptive_width", C.c_int), ("c_max", C.c_double),
-                ("f_lo", C.c_double), ("f_hi", C.c_double), ("fresnel_mode", C.c_int)]
+                ("f_lo", C.c_double), ("f_hi", C.c_double), ("fresnel_mode", C.c_int),
+                ("weight_mode", C.c_int)]
 
 
 class TfsError(RuntimeError):
@@ -58,6 +59,8 @@ def load_library():
     lib.tfs_count_pixels.restype = ip
     lib.tfs_bad_param_count.argtypes = [vp]
     lib.tfs_bad_param_count.restype = ll
+    lib.tfs_weight_structure.argtypes = [vp]
+    lib.tfs_weight_structure.restype = ip
     lib.tfs_set_profiling.argtypes = [vp, ip]
     lib.tfs_set_profiling.restype = ip
     lib.tfs_get_profile.argtypes = [vp, C.POINTER(dp), C.POINTER(ll), C.POINTER(ll)]
@@ -160,6 +163,9 @@ class Tfs:
 
     def bad_param_count(self):
         return int(self._lib.tfs_bad_param_count(self._h))
+
+    def weight_structure(self):
+        return int(self._lib.tfs_weight_structure(self._h))
 
     def set_profiling(self, on=True):
         self._check(self._lib.tfs_set_profiling(self._h, int(bool(on))))

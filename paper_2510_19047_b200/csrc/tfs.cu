@@ -31,6 +31,11 @@ struct tfs_ctx {
 
   float4* grid = nullptr;
   float2* wgt = nullptr;
+  float2* wa = nullptr;                    // [Nt] separable weights: a[m]
+  float2* wb = nullptr;                    // [Nf + kPadRows] separable weights: b[k]
+  float2* colmax = nullptr;                // [Nf] scratch of the weight analysis
+  unsigned long long* wcounts = nullptr;   // [2] {pixels violating W = a b, columns with b != 1}
+  int wmode = -1;                          // kWGeneral / kWSeparable / kWTimeOnly; -1 before the first upload
   uint8_t* gap = nullptr;
   int* vprefix = nullptr;                  // [Nt+1] valid tranches before m
   int* valid_m = nullptr;                  // [max(#valid,1)] valid tranche indices
@@ -250,7 +255,7 @@ double fit_far(FarCoef& out) {
 
 EvalArgs base_args(const tfs_ctx* ctx) {
   EvalArgs a{};
-  a.grid = ctx->grid; a.wgt = ctx->wgt; a.gap = ctx->gap; a.lut = ctx->lut;
+  a.grid = ctx->grid; a.wgt = ctx->wgt; a.wa = ctx->wa; a.wb = ctx->wb; a.gap = ctx->gap; a.lut = ctx->lut;
   a.vprefix = ctx->vprefix; a.valid_m = ctx->valid_m;
   a.bad_count = ctx->bad;
   a.work_counter = ctx->work;
@@ -288,9 +293,12 @@ void tfs_default_opts(tfs_opts* o) {
   o->f_lo = 0.0;
   o->f_hi = 0.0;
   o->fresnel_mode = 0;
+  o->weight_mode = 0;
 }
 
 const char* tfs_last_error(const tfs_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
+
+int tfs_weight_structure(const tfs_ctx* ctx) { return ctx ? ctx->wmode : -1; }
 
 long long tfs_bad_param_count(const tfs_ctx* ctx) {
   if (!ctx) return 0;
@@ -320,9 +328,9 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   tfs_default_opts(&o);
   if (opts) o = *opts;
   if (o.half_width < 0 || o.half_width > 4096 || !(o.c_max >= 0.0) || o.c_max > 1e6 ||
-      (o.fresnel_mode != 0 && o.fresnel_mode != 1))
-    return fail(nullptr, TFS_EINVAL, "tfs_create: bad options (half_width %d, c_max %g, fresnel_mode %d)",
-                o.half_width, o.c_max, o.fresnel_mode);
+      (o.fresnel_mode != 0 && o.fresnel_mode != 1) || (o.weight_mode != 0 && o.weight_mode != 1))
+    return fail(nullptr, TFS_EINVAL, "tfs_create: bad options (half_width %d, c_max %g, fresnel_mode %d, weight_mode %d)",
+                o.half_width, o.c_max, o.fresnel_mode, o.weight_mode);
   tfs_ctx* ctx = new (std::nothrow) tfs_ctx();
   if (!ctx) return fail(nullptr, TFS_ENOMEM, "tfs_create: host allocation failed");
   ctx->Nt = Nt; ctx->Nf = Nf; ctx->C = n_channels; ctx->dt = dt;
@@ -345,6 +353,12 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   const size_t npix = (size_t)Nt * (Nf + kPadRows);
   if ((e = cudaMalloc((void**)&ctx->grid, npix * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc grid", e);
   if ((e = cudaMalloc((void**)&ctx->wgt, npix * sizeof(float2))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc weights", e);
+  if ((e = cudaMalloc((void**)&ctx->wa, (size_t)Nt * sizeof(float2))) != cudaSuccess ||
+      (e = cudaMalloc((void**)&ctx->wb, (size_t)(Nf + kPadRows) * sizeof(float2))) != cudaSuccess ||
+      (e = cudaMalloc((void**)&ctx->colmax, (size_t)Nf * sizeof(float2))) != cudaSuccess ||
+      (e = cudaMalloc((void**)&ctx->wcounts, 2 * sizeof(unsigned long long))) != cudaSuccess)
+    return bail(TFS_ENOMEM, "cudaMalloc weight factors", e);
+  if ((e = cudaMemset(ctx->wb, 0, (size_t)(Nf + kPadRows) * sizeof(float2))) != cudaSuccess) return bail(TFS_ECUDA, "cudaMemset wb", e);
   if ((e = cudaMemset(ctx->grid, 0, npix * sizeof(float4))) != cudaSuccess ||
       (e = cudaMemset(ctx->wgt, 0, npix * sizeof(float2))) != cudaSuccess) return bail(TFS_ECUDA, "cudaMemset grid", e);
   if ((e = cudaMalloc((void**)&ctx->gap, (size_t)Nt)) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc gap", e);
@@ -353,8 +367,10 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   if ((e = cudaMalloc((void**)&ctx->lut, (kLutN + 1) * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc lut", e);
   if ((e = cudaMalloc((void**)&ctx->bad, sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
   if ((e = cudaMalloc((void**)&ctx->work, sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
-  if ((e = cudaFuncSetAttribute(eval_tiles_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess ||
-      (e = cudaFuncSetAttribute(eval_tiles_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess)
+  if ((e = cudaFuncSetAttribute(eval_tiles_kernel<0, kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_tiles_kernel<0, kWSeparable>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_tiles_kernel<0, kWTimeOnly>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_tiles_kernel<1, kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess)
     return bail(TFS_ECUDA, "cudaFuncSetAttribute(max dynamic shared memory)", e);
   if ((e = cudaMalloc((void**)&ctx->sel, sizeof(SelectState))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc select state", e);
   std::vector<float4> lut;
@@ -392,7 +408,7 @@ int tfs_get_profile(tfs_ctx* ctx, double* main_kernel_ms, long long* main_kernel
 void tfs_destroy(tfs_ctx* ctx) {
   if (!ctx) return;
   for (auto& p : ctx->ev_pool) { cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
-  void* bufs[] = {ctx->grid, ctx->wgt, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut, ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials,
+  void* bufs[] = {ctx->grid, ctx->wgt, ctx->wa, ctx->wb, ctx->colmax, ctx->wcounts, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut, ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials,
                   ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
                   ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children, ctx->buf_tiles};
   for (void* b : bufs) if (b) cudaFree(b);
@@ -436,7 +452,20 @@ int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const
   valid_list_kernel<<<1, 1024, 0, st>>>(ctx->gap, ctx->Nt, ctx->vprefix, ctx->valid_m);
   UP_CUDA(cudaGetLastError());
   ctx->launches += 2;
-  if (tmp_c || tmp_w || (gap_mask && !is_device_ptr(gap_mask))) UP_CUDA(cudaStreamSynchronize(st));
+  // weight structure (C11): W = a[m] b[k] on every pixel?  then the hot loop reads no per-pixel weight
+  unsigned long long wc[2] = {1, 1};
+  if (ctx->opts.weight_mode == 0) {
+    UP_CUDA(cudaMemsetAsync(ctx->wcounts, 0, 2 * sizeof(unsigned long long), st));
+    weight_colmax_kernel<<<(unsigned)ctx->Nf, 256, 0, st>>>(ctx->wgt, ctx->Nt, ctx->colmax);
+    weight_rowmax_kernel<<<(unsigned)((ctx->Nt + 127) / 128), 128, 0, st>>>(ctx->wgt, ctx->Nt, ctx->Nf, ctx->wa);
+    weight_factor_kernel<<<1, 1024, 0, st>>>(ctx->colmax, ctx->Nf, ctx->wb, ctx->wcounts);
+    weight_check_kernel<<<(unsigned)((npix + 255) / 256), 256, 0, st>>>(ctx->wgt, ctx->wa, ctx->wb, ctx->Nt, ctx->Nf, ctx->wcounts);
+    UP_CUDA(cudaGetLastError());
+    ctx->launches += 4;
+    UP_CUDA(cudaMemcpyAsync(wc, ctx->wcounts, sizeof(wc), cudaMemcpyDeviceToHost, st));
+  }
+  UP_CUDA(cudaStreamSynchronize(st));
+  ctx->wmode = wc[0] != 0 ? kWGeneral : (wc[1] != 0 ? kWSeparable : kWTimeOnly);
   cleanup();
 #undef UP_CUDA
   ctx->uploaded = true;
@@ -516,10 +545,14 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
       ++ctx->ev_used;
       TFS_CUDA(ctx, cudaEventRecord(ev0, st));
     }
-    if (ctx->opts.fresnel_mode == 0)
-      eval_tiles_kernel<0><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
+    if (ctx->opts.fresnel_mode != 0)          // the paper's approximants: one variant, general weights
+      eval_tiles_kernel<1, kWGeneral><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
+    else if (ctx->wmode == kWTimeOnly)
+      eval_tiles_kernel<0, kWTimeOnly><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
+    else if (ctx->wmode == kWSeparable)
+      eval_tiles_kernel<0, kWSeparable><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
     else
-      eval_tiles_kernel<1><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
+      eval_tiles_kernel<0, kWGeneral><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
     TFS_CUDA(ctx, cudaGetLastError());
     if (ev1) TFS_CUDA(ctx, cudaEventRecord(ev1, st));
     ctx->launches += 2;     // main kernel + combine

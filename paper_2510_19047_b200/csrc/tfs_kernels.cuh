@@ -27,6 +27,8 @@ struct FarCoef { float F0, F1, F2, G0, G1, G2; };
 struct EvalArgs {
   const float4* __restrict__ grid;     // [Nf][Nt] (time-contiguous) {Y_A.re, Y_E.re, Y_A.im, Y_E.im}, Y = W*D
   const float2* __restrict__ wgt;      // [Nf][Nt] {W_A, W_E}
+  const float2* __restrict__ wa;       // [Nt] {a_A, a_E}  (separable weights: W = a[m] b[k])
+  const float2* __restrict__ wb;       // [Nf + kPadRows] {b_A, b_E}
   const uint8_t* __restrict__ gap;     // [Nt] 1 = valid
   const int* __restrict__ vprefix;     // [Nt+1] number of valid tranches before m
   const int* __restrict__ valid_m;     // [vprefix[Nt]] the valid tranche indices, ascending (padded to >= 1 entry)
@@ -250,15 +252,26 @@ struct LaneTrack {      // per-lane (= per-tranche) constants of the pixel loop
 
 struct LaneSums { f2_t zr, zi, q; };     // {A, E} pairs: Re z', Im z', q'
 
-// grid pixel Y = {Y_A.re, Y_E.re, Y_A.im, Y_E.im}, weights Wt = {W_A, W_E}
+// Weight modes (chosen by tfs_upload_data, C11):
+//   kWGeneral    per-pixel weights W[alpha,m,k], read next to every data pixel
+//   kWSeparable  W[alpha,m,k] = a_alpha[m] b_alpha[k]: b from a small [Nf] table, a applied once per tranche
+//   kWTimeOnly   b = 1: no weight is read in the pixel loop, q' = sum |h'|^2 for both channels
+constexpr int kWGeneral = 0, kWSeparable = 1, kWTimeOnly = 2;
+
+// grid pixel Y = {Y_A.re, Y_E.re, Y_A.im, Y_E.im}, weights Wt = {W_A, W_E} (or {b_A, b_E})
+template <int WMODE>
 __device__ __forceinline__ void mac(LaneSums& s, const float4 Y, const float2 Wt, float hr, float hi) {
   const f2_t Yre = pk(Y.x, Y.y), Yim = pk(Y.z, Y.w);
   s.zr = ffma2(Yre, pk(hr, hr), s.zr);            // Re conj(Y) h = Y.re hr + Y.im hi
   s.zr = ffma2(Yim, pk(hi, hi), s.zr);
   s.zi = ffma2(Yre, pk(hi, hi), s.zi);            // Im conj(Y) h = Y.re hi - Y.im hr
   s.zi = ffma2(Yim, pk(-hr, -hr), s.zi);
-  const float h2 = fmaf(hr, hr, hi * hi);
-  s.q = ffma2(pk(Wt.x, Wt.y), pk(h2, h2), s.q);
+  if (WMODE == kWTimeOnly) {
+    s.q = ffma2(pk(hr, hi), pk(hr, hi), s.q);     // {sum hr^2, sum hi^2}
+  } else {
+    const float h2 = fmaf(hr, hr, hi * hi);
+    s.q = ffma2(pk(Wt.x, Wt.y), pk(h2, h2), s.q);
+  }
 }
 
 // u = x - k; u + c is formed here, per pixel, so that it is rounded at the magnitude of u (next to the
@@ -330,7 +343,7 @@ constexpr int kGroup = TFS_GROUP;
 constexpr int kPadRows = 3 * kGroup;         // rows of zero padding behind the grid and the weights
 
 // ZONES: 1 = test the offset against the near zone, 0 = the offset is known to be far
-template <int MODE, int MASKED, int ZONES>
+template <int MODE, int WMODE, int MASKED, int ZONES>
 __device__ __forceinline__ void pixel_step(const LaneTrack& L, const FarCoef& C, int jj, int Wm, int JA, int JB,
                                            const float4 Yc, const float2 Wc, float& u, unsigned lut_lane,
                                            LaneSums& s) {
@@ -338,59 +351,67 @@ __device__ __forceinline__ void pixel_step(const LaneTrack& L, const FarCoef& C,
   float hr, hi;
   if (ZONES && jj >= JA && jj < JB) pixel_near<MODE, MASKED>(L, u, msk, lut_lane, hr, hi);
   else pixel_far<MASKED>(L, C, u, msk, hr, hi);
-  mac(s, Yc, Wc, hr, hi);
+  mac<WMODE>(s, Yc, Wc, hr, hi);
   u -= 1.0f;
 }
 
 struct PixelBuf { float4 Y[kGroup]; float2 W[kGroup]; };
 
-// loads offsets j0 ... j0+kGroup-1 of the lane's window (CLAMP: not past offset jlast)
-template <int CLAMP>
-__device__ __forceinline__ void load_group(const EvalArgs& a, PixelBuf& B, int idx, int stp, int j0, int jlast) {
+// loads offsets j0 ... j0+kGroup-1 of the lane's window (CLAMP: not past offset jlast).
+// kb = k_lo and kstp = 1 for an active lane (0, 0 otherwise): row index of the b table (kWSeparable).
+template <int CLAMP, int WMODE>
+__device__ __forceinline__ void load_group(const EvalArgs& a, PixelBuf& B, int idx, int stp, int kb, int kstp, int j0,
+                                           int jlast) {
 #pragma unroll
   for (int p = 0; p < kGroup; ++p) {
-    const int i = idx + (CLAMP ? min(j0 + p, jlast) : (j0 + p)) * stp;
+    const int jj = CLAMP ? min(j0 + p, jlast) : (j0 + p);
+    const int i = idx + jj * stp;
     B.Y[p] = __ldg(a.grid + i);
-    B.W[p] = __ldg(a.wgt + i);
+    if (WMODE == kWGeneral) B.W[p] = __ldg(a.wgt + i);
+    if (WMODE == kWSeparable) B.W[p] = __ldg(a.wb + kb + jj * kstp);
   }
 }
 
-template <int MODE, int MASKED>
+template <int MODE, int WMODE, int MASKED>
 __device__ __forceinline__ void compute_group(const LaneTrack& L, const FarCoef& C, const PixelBuf& B, int j0, int Wm,
                                               int Wmax, int JA, int JB, float& u, unsigned lut_lane, LaneSums& s) {
   if (j0 < JB && j0 + kGroup > JA) {
 #pragma unroll
     for (int p = 0; p < kGroup; ++p)
-      if (!MASKED || j0 + p < Wmax) pixel_step<MODE, MASKED, 1>(L, C, j0 + p, Wm, JA, JB, B.Y[p], B.W[p], u, lut_lane, s);
+      if (!MASKED || j0 + p < Wmax)
+        pixel_step<MODE, WMODE, MASKED, 1>(L, C, j0 + p, Wm, JA, JB, B.Y[p], B.W[p], u, lut_lane, s);
   } else {
 #pragma unroll
     for (int p = 0; p < kGroup; ++p)
-      if (!MASKED || j0 + p < Wmax) pixel_step<MODE, MASKED, 0>(L, C, j0 + p, Wm, JA, JB, B.Y[p], B.W[p], u, lut_lane, s);
+      if (!MASKED || j0 + p < Wmax)
+        pixel_step<MODE, WMODE, MASKED, 0>(L, C, j0 + p, Wm, JA, JB, B.Y[p], B.W[p], u, lut_lane, s);
   }
 }
 
 // idx = pixel index of offset 0, stp = Nt for an active lane and 0 otherwise, Wm = window length (>= 1
 // for active lanes, 0 otherwise)
-template <int MODE>
+template <int MODE, int WMODE>
 __device__ __forceinline__ void pixel_loop(const EvalArgs& a, const LaneTrack& L, const FarCoef& C, int Wm, int Wmin,
-                                           int Wmax, int JA, int JB, int idx, int stp, float u, unsigned lut_lane,
-                                           LaneSums& s) {
+                                           int Wmax, int JA, int JB, int idx, int stp, int kb, int kstp, float u,
+                                           unsigned lut_lane, LaneSums& s) {
   PixelBuf A, B;
+#pragma unroll
+  for (int p = 0; p < kGroup; ++p) { A.W[p] = make_float2(0.f, 0.f); B.W[p] = make_float2(0.f, 0.f); }
   const int jlast = max(Wm - 1, 0);
-  load_group<0>(a, A, idx, stp, 0, jlast);
+  load_group<0, WMODE>(a, A, idx, stp, kb, kstp, 0, jlast);
   int j = 0;
   for (; j + 2 * kGroup <= Wmin; j += 2 * kGroup) {                       // phase 1
-    load_group<0>(a, B, idx, stp, j + kGroup, jlast);
-    compute_group<MODE, 0>(L, C, A, j, Wm, Wmax, JA, JB, u, lut_lane, s);
-    load_group<0>(a, A, idx, stp, j + 2 * kGroup, jlast);
-    compute_group<MODE, 0>(L, C, B, j + kGroup, Wm, Wmax, JA, JB, u, lut_lane, s);
+    load_group<0, WMODE>(a, B, idx, stp, kb, kstp, j + kGroup, jlast);
+    compute_group<MODE, WMODE, 0>(L, C, A, j, Wm, Wmax, JA, JB, u, lut_lane, s);
+    load_group<0, WMODE>(a, A, idx, stp, kb, kstp, j + 2 * kGroup, jlast);
+    compute_group<MODE, WMODE, 0>(L, C, B, j + kGroup, Wm, Wmax, JA, JB, u, lut_lane, s);
   }
   for (; j < Wmax; j += 2 * kGroup) {                                    // phase 2
-    load_group<1>(a, B, idx, stp, j + kGroup, jlast);
-    compute_group<MODE, 1>(L, C, A, j, Wm, Wmax, JA, JB, u, lut_lane, s);
+    load_group<1, WMODE>(a, B, idx, stp, kb, kstp, j + kGroup, jlast);
+    compute_group<MODE, WMODE, 1>(L, C, A, j, Wm, Wmax, JA, JB, u, lut_lane, s);
     if (j + kGroup >= Wmax) break;
-    load_group<1>(a, A, idx, stp, j + 2 * kGroup, jlast);
-    compute_group<MODE, 1>(L, C, B, j + kGroup, Wm, Wmax, JA, JB, u, lut_lane, s);
+    load_group<1, WMODE>(a, A, idx, stp, kb, kstp, j + 2 * kGroup, jlast);
+    compute_group<MODE, WMODE, 1>(L, C, B, j + kGroup, Wm, Wmax, JA, JB, u, lut_lane, s);
   }
 }
 
@@ -417,7 +438,7 @@ __global__ void tile_table_kernel(const int* __restrict__ vprefix, int Nt, int N
   table[tile] = make_int2(vprefix[m0], vprefix[m1]);
 }
 
-template <int MODE>
+template <int MODE, int WMODE>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, 1)
 eval_tiles_kernel(const EvalArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -469,7 +490,7 @@ eval_tiles_kernel(const EvalArgs a) {
         const TrackPoint tp = track_point(T, m, a.DT, a.x_lo, a.x_hi, a.c_max, valid);
         const unsigned act_mask = __ballot_sync(0xffffffffu, tp.active);
         if (act_mask == 0u) continue;
-        int Wm = 0, idx = m, stp = 0, ja = 0x7fffffff, jb = 0;
+        int Wm = 0, idx = m, stp = 0, kb = 0, kstp = 0, ja = 0x7fffffff, jb = 0;
         float u = -1.f, Pr = 0.f, Pi = 0.f;
         LaneTrack L;        // inactive lanes: u_j = -1 - j, u_j + c = -0.5 - j (finite h' on zeroed data)
         L.sc = 1.f; L.kap = 1.f; L.c = 0.5f; L.hc = 0.f; L.Er = 0.f; L.Ei = 0.f;
@@ -479,6 +500,8 @@ eval_tiles_kernel(const EvalArgs a) {
           Wm = k_hi - k_lo + 1;
           idx = k_lo * a.Nt + m;
           stp = a.Nt;
+          kb = k_lo;
+          kstp = 1;
           const double flx = floor(tp.x);
           const float fracx = (float)(tp.x - flx);
           u = fracx - (float)(k_lo - (int)flx);          // cancellation-safe x - k_lo
@@ -515,10 +538,17 @@ eval_tiles_kernel(const EvalArgs a) {
         // ---------------- pixel loop (a3-a5): lane walks its own window ----------------
         LaneSums s;
         s.zr = pk(0.f, 0.f); s.zi = pk(0.f, 0.f); s.q = pk(0.f, 0.f);
-        pixel_loop<MODE>(a, L, a.far, Wm, Wmin, Wmax, JA, JB, idx, stp, u, lut_lane, s);
+        pixel_loop<MODE, WMODE>(a, L, a.far, Wm, Wmin, Wmax, JA, JB, idx, stp, kb, kstp, u, lut_lane, s);
         // apply the tranche's factor P (and |P|^2) and promote to fp64
         float zAr, zEr, zAi, zEi, qA, qE;
         upk(s.zr, zAr, zEr); upk(s.zi, zAi, zEi); upk(s.q, qA, qE);
+        if (WMODE != kWGeneral) {
+          // W = a[m] b[k]: the pixel loop summed b |h'|^2 (b = 1: {sum hr^2, sum hi^2}); apply a[m] here
+          const float2 am = __ldg(a.wa + m);
+          if (WMODE == kWTimeOnly) { qA += qE; qE = qA; }
+          qA *= am.x;
+          qE *= am.y;
+        }
         const float P2 = fmaf(Pr, Pr, Pi * Pi);
         s_acc[0 * kAccStride] += (double)(Pr * zAr - Pi * zAi);
         s_acc[1 * kAccStride] += (double)(Pr * zAi + Pi * zAr);
@@ -626,6 +656,83 @@ pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, 
       wgt[o] = sW[tx][r];
     }
   }
+}
+
+// ------------------------------------------------------------------------------------------
+// Weight structure (a0, C11).  If W[alpha,m,k] = a_alpha[m] b_alpha[k] then
+//   rowmax[m] = max_k W = a[m] max b,  colmax[k] = max_m W = b[k] max a,  gmax = max a max b,
+// so a'[m] = rowmax[m], b'[k] = colmax[k] / gmax reproduce W = a' b'.  weight_check_kernel counts the
+// pixels where that fails by more than a few ulps (or W < 0), and the columns with b' != 1.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+weight_colmax_kernel(const float2* __restrict__ wgt, int Nt, float2* __restrict__ colmax) {   // one block per k
+  __shared__ float2 sh[256];
+  const int k = blockIdx.x;
+  float2 mx = make_float2(0.f, 0.f);
+  for (int m = threadIdx.x; m < Nt; m += 256) {
+    const float2 w = wgt[(size_t)k * Nt + m];
+    mx.x = fmaxf(mx.x, w.x); mx.y = fmaxf(mx.y, w.y);
+  }
+  sh[threadIdx.x] = mx;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) {
+      sh[threadIdx.x].x = fmaxf(sh[threadIdx.x].x, sh[threadIdx.x + o].x);
+      sh[threadIdx.x].y = fmaxf(sh[threadIdx.x].y, sh[threadIdx.x + o].y);
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) colmax[k] = sh[0];
+}
+
+__global__ void weight_rowmax_kernel(const float2* __restrict__ wgt, int Nt, int Nf, float2* __restrict__ wa) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;                                         // one thread per m
+  if (m >= Nt) return;
+  float2 mx = make_float2(0.f, 0.f);
+  for (int k = 0; k < Nf; ++k) {
+    const float2 w = wgt[(size_t)k * Nt + m];
+    mx.x = fmaxf(mx.x, w.x); mx.y = fmaxf(mx.y, w.y);
+  }
+  wa[m] = mx;
+}
+
+// one block: gmax = max_k colmax[k]; wb[k] = colmax[k] / gmax (0 where gmax = 0); counts[1] += #{b' != 1}
+__global__ void __launch_bounds__(1024)
+weight_factor_kernel(const float2* __restrict__ colmax, int Nf, float2* __restrict__ wb, unsigned long long* counts) {
+  __shared__ float2 sh[1024];
+  float2 mx = make_float2(0.f, 0.f);
+  for (int k = threadIdx.x; k < Nf; k += 1024) { mx.x = fmaxf(mx.x, colmax[k].x); mx.y = fmaxf(mx.y, colmax[k].y); }
+  sh[threadIdx.x] = mx;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) {
+    if (threadIdx.x < o) {
+      sh[threadIdx.x].x = fmaxf(sh[threadIdx.x].x, sh[threadIdx.x + o].x);
+      sh[threadIdx.x].y = fmaxf(sh[threadIdx.x].y, sh[threadIdx.x + o].y);
+    }
+    __syncthreads();
+  }
+  const float2 g = sh[0];
+  unsigned long long not_one = 0;
+  for (int k = threadIdx.x; k < Nf; k += 1024) {
+    const float2 b = make_float2(g.x > 0.f ? colmax[k].x / g.x : 0.f, g.y > 0.f ? colmax[k].y / g.y : 0.f);
+    wb[k] = b;
+    not_one += (g.x > 0.f && b.x != 1.0f) + (g.y > 0.f && b.y != 1.0f);
+  }
+  if (not_one) atomicAdd(&counts[1], not_one);
+}
+
+__global__ void weight_check_kernel(const float2* __restrict__ wgt, const float2* __restrict__ wa,
+                                    const float2* __restrict__ wb, int Nt, int Nf, unsigned long long* counts) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool bad = false;
+  if (i < (size_t)Nt * Nf) {
+    const int k = (int)(i / Nt), m = (int)(i - (size_t)k * Nt);
+    const float2 w = wgt[i], a = wa[m], b = wb[k];
+    const float pA = a.x * b.x, pE = a.y * b.y;
+    bad = !(fabsf(w.x - pA) <= 1e-6f * pA) || !(fabsf(w.y - pE) <= 1e-6f * pE) || w.x < 0.f || w.y < 0.f;
+  }
+  const unsigned n_bad = __popc(__ballot_sync(0xffffffffu, bad));
+  if ((threadIdx.x & 31) == 0 && n_bad) atomicAdd(&counts[0], (unsigned long long)n_bad);
 }
 
 // Compacted list of valid (non-gap) tranches and its prefix counts (C10).  One block.

@@ -65,8 +65,9 @@ def test_cfg1_parity(api, cfg1, N_seg):
 # (start above band, merge inside the grid, never enter), several tiles, segment counts that do
 # not divide Nt, chunks with a ragged tail
 # --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("weight_mode", [0, 1])      # 0: separable weights detected, 1: forced general path
 @pytest.mark.parametrize("name,Nt,N_segs", [("cfg2", 300, (16, 7)), ("cfg3", 333, (1, 4, 64, 333))])
-def test_reduced_config_parity(api, name, Nt, N_segs):
+def test_reduced_config_parity(api, name, Nt, N_segs, weight_mode):
     w = synth.scaled(synth.WORKLOADS[name], Nt=Nt, n_templates=96)
     coeff, weight, gap = synth.make_data(w)
     # injections of the full config do not fit the short grid's time span: plant two that do
@@ -77,7 +78,9 @@ def test_reduced_config_parity(api, name, Nt, N_segs):
     params = synth.make_templates(w)
     params[:48, 1] = np.random.default_rng(5).uniform(0.0, 3.0, 48) * Tobs      # many merge in/near the grid
     params = np.vstack([params, inj[0][0][None], inj[1][0][None]])
-    ctx = _mk(api, w, coeff, weight, gap)
+    ctx = _mk(api, w, coeff, weight, gap, weight_mode=weight_mode)
+    # cfg2: W depends on the frequency only (1 = separable); cfg3: on the tranche only (2); forced: 0
+    assert ctx.weight_structure() == (0 if weight_mode else {"cfg2": 1, "cfg3": 2}[name])
     for N_seg in N_segs:
         gpu = api.eval_host(ctx, params, N_seg)
         ora = oracle_eval(coeff, weight, gap, params, w.Nt, w.Nf, w.dt, N_seg)
@@ -88,6 +91,36 @@ def test_reduced_config_parity(api, name, Nt, N_segs):
     g = O.Grid(w.Nt, w.Nf, w.dt)
     ref = np.array([O.window_pixel_counts(p[0], p[1], g, O.Opts(), gap) for p in params])
     assert np.array_equal(counts, ref)
+    ctx.destroy()
+
+
+# --------------------------------------------------------------------------------------------
+# weights: general per-pixel W (C11), a product a[m] b[k], and a product spoilt in one pixel
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind,code", [("general", 0), ("product", 1), ("spoilt", 0), ("time", 2)])
+def test_weight_structures_parity(api, kind, code):
+    w = synth.scaled(synth.WORKLOADS["cfg3"], Nt=200, n_templates=64)
+    coeff, _, gap = synth.make_data(w)
+    rng = np.random.default_rng(21)
+    a = rng.uniform(0.3, 2.0, (2, w.Nt, 1)).astype(np.float32)
+    b = rng.uniform(0.5, 1.5, (2, 1, w.Nf)).astype(np.float32)
+    if kind == "general":
+        weight = rng.uniform(0.2, 3.0, (2, w.Nt, w.Nf)).astype(np.float32)
+    elif kind == "time":
+        weight = np.ascontiguousarray(np.broadcast_to(a, (2, w.Nt, w.Nf)))
+    else:
+        weight = (a * b).astype(np.float32)
+        if kind == "spoilt":
+            weight[1, w.Nt // 2, w.Nf // 3] *= np.float32(1.001)
+    params = synth.make_templates(w)
+    params[:32, 1] = rng.uniform(0.0, 3.0, 32) * w.Nt * w.DT
+    ctx = _mk(api, w, coeff, weight, gap)
+    assert ctx.weight_structure() == code
+    for N_seg in (1, 8):
+        gpu = api.eval_host(ctx, params, N_seg)
+        ora = oracle_eval(coeff, weight, gap, params, w.Nt, w.Nf, w.dt, N_seg)
+        r = assert_parity(gpu, ora, N_seg, label=f"weights {kind} N_seg={N_seg}")
+        assert r["n_active"] >= 30
     ctx.destroy()
 
 
