@@ -26,11 +26,15 @@ if ROOT not in sys.path:
 
 from paper_2510_19047_b200 import synth  # noqa: E402
 
-ALG_BYTES_PER_PIXEL_EVAL = 12.0      # 8 B complex fp32 datum + 4 B weight
-# Algorithmic lane-instructions per window pixel (both channels): v0, v1 (2); two
-# auxiliary-function evaluations of 8 (16); G(v1) E and the combination into h' (8); z_A, z_E, |h'|^2,
-# q_A, q_E (12); gather (2 loads, 2 addresses, 1 index step: 5).
-ALG_LANE_OPS_PER_PIXEL = 43.0
+# Algorithmic bytes per pixel-eval: 8 B complex fp32 datum + 4 B weight
+# when the weights are a general per-pixel array; 8 B when they are separable W[a,m,k] = a[m] b[k]
+# (tfs_weight_structure 1 or 2: true of every BASELINE.json config), where no per-pixel weight exists to read.
+ALG_BYTES_PER_PIXEL_EVAL = {0: 12.0, 1: 8.0, 2: 8.0}
+# Algorithmic FMA-pipe lane-slots per window pixel (both channels), far-zone pixel.
+# A packed fp32 instruction (FFMA2/FMUL2/FADD2) is one issue slot but two lane-slots of the FMA pipe:
+# 10 packed for the two auxiliary-function polynomials (20), h' = Godd(v0) - E Godd(v1) (4 scalar FMA),
+# z_A, z_E (4 packed: 8), |h'|^2 and q (1 packed: 2), u + c and u - 1 (2)  ->  36; + 2 MUFU.RCP (own pipe).
+ALG_LANE_OPS_PER_PIXEL = 36.0
 SM_LANES = 128                       # lane-instructions issued per SM per clock (4 schedulers x 32 lanes)
 
 
@@ -147,6 +151,8 @@ def main():
     ap.add_argument("--n-seg", type=int, default=None)
     ap.add_argument("--cpu-sample", type=int, default=None, help="templates timed on the CPU oracle")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--weight-mode", type=int, default=0, choices=[0, 1],
+                    help="tfs_opts.weight_mode: 0 = exploit separable weights (default), 1 = general per-pixel path")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -219,7 +225,7 @@ def main():
     if world > 1:
         dist.barrier()
 
-    ctx = api.Tfs(w.Nt, w.Nf, w.dt)
+    ctx = api.Tfs(w.Nt, w.Nf, w.dt, weight_mode=args.weight_mode)
     ctx.upload_data(coeff, weight, gap)
     d_params = torch.from_numpy(params).to(dev)
     d_ups = torch.empty(n, dtype=torch.float32, device=dev)
@@ -302,7 +308,8 @@ def main():
     n_launch = max(prof["main_kernel_launches"], 1)
     kern_ms = prof["main_kernel_ms"] / n_launch                    # per main-kernel launch
     launches_per_step = n_launch / args.steps
-    bytes_per_launch = ALG_BYTES_PER_PIXEL_EVAL * pixel_evals / launches_per_step
+    wstruct = ctx.weight_structure()
+    bytes_per_launch = ALG_BYTES_PER_PIXEL_EVAL[wstruct] * pixel_evals / launches_per_step
     achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
     # roofline terms: the gathers are served by the L2 (tile-major order), so the
     # byte term is quoted against the L2 read bandwidth probed in this run; the HBM figure is given for
@@ -330,7 +337,9 @@ def main():
         "roofline": {"bound": bound, "kernel": "eval_tiles_kernel", "achieved": terms[bound]["achieved"],
                      "peak": terms[bound]["peak"], "peak_source": terms[bound]["peak_source"],
                      "unit": terms[bound]["unit"], "frac": terms[bound]["frac"], "traffic": None,
-                     "algorithmic_bytes_per_launch": bytes_per_launch, "kernel_ms_per_launch": kern_ms,
+                     "algorithmic_bytes_per_launch": bytes_per_launch,
+                     "algorithmic_bytes_per_pixel_eval": ALG_BYTES_PER_PIXEL_EVAL[wstruct],
+                     "weight_structure": wstruct, "kernel_ms_per_launch": kern_ms,
                      "kernel_share_of_step": prof["main_kernel_ms"] / ms_total, "terms": terms},
         "cpu_baseline": cpu_baseline,
         "e2e": {"value": world * n / (ms_e2e * 1e-3), "unit": "templates/s",

@@ -1,0 +1,121 @@
+"""Throughput tables for the secondary BASELINE.json configurations (markdown on stdout).
+
+    python -m paper_2510_19047_b200.report track-width     # configs[3]: throughput vs track width
+    python -m paper_2510_19047_b200.report nseg            # configs[2]: N_seg swept over {1, 4, 16, 64}
+
+Uses only the public binding (api.Tfs) and the seeded generators (synth); timing with CUDA events on
+the current stream after warm-up, inputs resident on the device.  bench.py prints the headline line;
+these tables are the "report throughput vs track width" / "N_seg swept" parts of the configs.
+"""
+from __future__ import annotations
+
+import sys
+
+import numpy as np
+
+
+def _time_eval(ctx, torch, d_params, N_seg, reps=3, warm=2):
+    n = d_params.shape[0]
+    d_ups = torch.empty(n, dtype=torch.float32, device=d_params.device)
+    for _ in range(warm):
+        ctx.eval(d_params, N_seg, d_ups)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        ctx.eval(d_params, N_seg, d_ups)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def _counts(ctx, torch, d_params):
+    c = torch.empty(d_params.shape[0], dtype=torch.int64, device=d_params.device)
+    ctx.count_pixels(d_params, c)
+    torch.cuda.synchronize()
+    return c.cpu().numpy()
+
+
+def _setup(name):
+    import torch
+    from . import api, synth
+    assert torch.cuda.is_available(), "needs cuda:0 (libtfs has no CPU fallback)"
+    torch.cuda.set_device(0)
+    w = synth.WORKLOADS[name]
+    coeff, weight, gap = synth.make_data(w)
+    ctx = api.Tfs(w.Nt, w.Nf, w.dt)
+    ctx.upload_data(coeff, weight, gap)
+    return torch, api, synth, w, ctx, (coeff, weight, gap)
+
+
+def track_width():
+    torch, api, synth, w, ctx, data = _setup("cfg4")
+    dev = torch.device("cuda:0")
+    params = synth.make_templates(w)
+    d_all = torch.from_numpy(params).to(dev)
+    pix = _counts(ctx, torch, d_all)
+    # active tranches per template from the window rule: pixels(H=10) - pixels(H=0) = 20 per active tranche
+    ctx0 = api.Tfs(w.Nt, w.Nf, w.dt, half_width=0)
+    ctx0.upload_data(*data)
+    act = (pix - _counts(ctx0, torch, d_all)) // 20
+    ctx0.destroy()
+    width = np.where(act > 0, pix / np.maximum(act, 1), 0.0)
+    print(f"# configs[3] (cfg4): throughput vs track width, N_seg = {w.N_seg}, grid {w.Nt} x {w.Nf}, "
+          f"bank of {len(params)} (80 % as cfg2, 20 % merging inside the grid)\n")
+    print("| sub-bank | templates | mean pixels / active tranche | mean active tranches | ms | templates/s | pixel-evals/s |")
+    print("|---|---:|---:|---:|---:|---:|---:|")
+
+    def row(label, p, px, ac):
+        d = torch.from_numpy(np.ascontiguousarray(p)).to(dev)
+        ms = _time_eval(ctx, torch, d, w.N_seg)
+        print(f"| {label} | {len(p)} | {px.sum() / max(ac.sum(), 1):.1f} | {ac.mean():.0f} | {ms:.2f} | "
+              f"{len(p) / ms * 1e3:.3e} | {2 * px.sum() / ms * 1e3:.3e} |")
+
+    row("whole bank", params, pix, act)
+    edges = [21, 21.5, 22, 23, 25, 30, 400]
+    for a, b in zip(edges[:-1], edges[1:]):
+        sel = (width >= a) & (width < b)
+        if sel.sum() >= 1000:
+            row(f"mean width in [{a}, {b})", params[sel], pix[sel], act[sel])
+    # short tracks: the last days before a merger inside the grid, every tranche wide
+    rng = np.random.default_rng(w.seed + 77)
+    for days, mc_lo in ((30.0, 60.0), (10.0, 60.0), (4.0, 80.0), (2.0, 90.0)):
+        p = synth.make_templates(w, n=200_000, seed=w.seed + int(days))
+        p[:, 0] = np.exp(rng.uniform(np.log(mc_lo), np.log(100.0), len(p)))
+        p[:, 1] = rng.uniform(0.3, 1.0, len(p)) * days * 86400.0
+        d = torch.from_numpy(p).to(dev)
+        px = _counts(ctx, torch, d)
+        c0 = api.Tfs(w.Nt, w.Nf, w.dt, half_width=0)
+        c0.upload_data(*data)
+        ac = (px - _counts(c0, torch, d)) // 20
+        c0.destroy()
+        row(f"Mc in [{mc_lo:.0f}, 100], merger {0.3 * days:.1f}-{days:.0f} d after the data start", p, px, ac)
+    ctx.destroy()
+
+
+def nseg():
+    torch, api, synth, w, ctx, _ = _setup("cfg3")
+    dev = torch.device("cuda:0")
+    params = synth.make_templates(w)
+    d = torch.from_numpy(params).to(dev)
+    pix = _counts(ctx, torch, d)
+    print(f"# configs[2] (cfg3): N_seg sweep, {len(params)} templates, grid {w.Nt} x {w.Nf}, "
+          f"weight structure {ctx.weight_structure()}\n")
+    print("| N_seg | time tiles | ms per tfs_eval | templates/s | pixel-evals/s |")
+    print("|---:|---:|---:|---:|---:|")
+    for N in (1, 4, 16, 64):
+        ms = _time_eval(ctx, torch, d, N)
+        seg_len = -(-w.Nt // N)
+        tiles = N * (-(-seg_len // 256))
+        print(f"| {N} | {tiles} | {ms:.2f} | {len(params) / ms * 1e3:.3e} | {2 * pix.sum() / ms * 1e3:.3e} |")
+    ctx.destroy()
+
+
+if __name__ == "__main__":
+    what = sys.argv[1] if len(sys.argv) > 1 else ""
+    if what == "track-width":
+        track_width()
+    elif what == "nseg":
+        nseg()
+    else:
+        sys.exit(__doc__)
