@@ -529,7 +529,9 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
     a.params = d_params + off * TFS_PARAM_COLS;
     a.n = nb;
     const long long n_work = nb * n_tiles;
-    const long long want = (n_work + kWarpsPerCta - 1) / kWarpsPerCta;
+    const int wm = ctx->opts.fresnel_mode != 0 ? kWGeneral : ctx->wmode;
+    const int warps = warps_per_cta(wm);
+    const long long want = (n_work + warps - 1) / warps;
     const unsigned blocks = (unsigned)std::min<long long>(want, (long long)ctx->sm_count);   // persistent, 1 CTA/SM
     TFS_CUDA(ctx, cudaMemsetAsync(ctx->work, 0, sizeof(unsigned long long), st));
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -546,13 +548,13 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
       TFS_CUDA(ctx, cudaEventRecord(ev0, st));
     }
     if (ctx->opts.fresnel_mode != 0)          // the paper's approximants: one variant, general weights
-      eval_tiles_kernel<1, kWGeneral><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
+      eval_tiles_kernel<1, kWGeneral><<<blocks, warps * 32, kEvalSmemBytes, st>>>(a);
     else if (ctx->wmode == kWTimeOnly)
-      eval_tiles_kernel<0, kWTimeOnly><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
+      eval_tiles_kernel<0, kWTimeOnly><<<blocks, warps * 32, kEvalSmemBytes, st>>>(a);
     else if (ctx->wmode == kWSeparable)
-      eval_tiles_kernel<0, kWSeparable><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
+      eval_tiles_kernel<0, kWSeparable><<<blocks, warps * 32, kEvalSmemBytes, st>>>(a);
     else
-      eval_tiles_kernel<0, kWGeneral><<<blocks, kWarpsPerCta * 32, kEvalSmemBytes, st>>>(a);
+      eval_tiles_kernel<0, kWGeneral><<<blocks, warps * 32, kEvalSmemBytes, st>>>(a);
     TFS_CUDA(ctx, cudaGetLastError());
     if (ev1) TFS_CUDA(ctx, cudaEventRecord(ev1, st));
     ctx->launches += 2;     // main kernel + combine

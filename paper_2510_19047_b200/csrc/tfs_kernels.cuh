@@ -12,10 +12,16 @@
 
 namespace tfs {
 
-#ifndef TFS_WARPS_PER_CTA
-#define TFS_WARPS_PER_CTA 24
+// Warps of the one persistent CTA per SM.  The kernel is short of warps to hide its dependent chains, so
+// it runs the most that the register file allows: 32 (64 registers per thread) when no per-pixel weight
+// is buffered, 24 (80 registers) for general weights, which need two more registers per pixel in flight.
+#ifndef TFS_WARPS_SEPARABLE
+#define TFS_WARPS_SEPARABLE 32
 #endif
-constexpr int kWarpsPerCta = TFS_WARPS_PER_CTA;   // one persistent CTA per SM
+#ifndef TFS_WARPS_GENERAL
+#define TFS_WARPS_GENERAL 24
+#endif
+constexpr int kMaxWarpsPerCta = TFS_WARPS_SEPARABLE > TFS_WARPS_GENERAL ? TFS_WARPS_SEPARABLE : TFS_WARPS_GENERAL;
 constexpr int kTileMax = 256;       // tranches per time tile (upper bound)
 constexpr int kLutN = 512;          // LUT intervals in t = 1/(1+v)
 constexpr double kMtsun = 4.925490947e-6;   // G Msun / c^3 [s]
@@ -221,9 +227,9 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// dynamic shared memory of kernel A: [LUT copies][fp64 tile sums: 6 per thread, stored [6][threads]]
+// dynamic shared memory of kernel A: [LUT copies][per-lane tile sums: 3 packed pairs per thread, stored [3][threads]]
 constexpr int kLutSmemBytes = (kLutN + 1) * kLutCopies * (int)sizeof(float4);
-constexpr int kEvalSmemBytes = kLutSmemBytes + 6 * kWarpsPerCta * 32 * (int)sizeof(double);
+constexpr int kEvalSmemBytes = kLutSmemBytes + 3 * kMaxWarpsPerCta * 32 * (int)sizeof(f2_t);
 
 // One pixel of one tranche (a3-a5).  The template coefficient is h = P h', P = A/sqrt(2c) exp(i phi_m)
 // constant over the tranche, and (auxiliary-function form of Eq. 16)
@@ -328,19 +334,21 @@ __device__ __forceinline__ void pixel_near(const LaneTrack& L, float u, float ms
 // Pixel loop of one chunk (32 tranches, one per lane): every lane walks its own window, offsets
 // j = 0 ... Wm-1 from its k_lo, in groups of kGroup offsets.  The gather is software-pipelined through
 // two register buffers: the loads of group g+1 are issued before the arithmetic of group g.  It is never
-// predicated: the grid is allocated with kPadRows rows past Nf-1, so reading up to 3 kGroup pixels past
-// the end of the shortest window stays in bounds, and an inactive lane reads pixel `idx` with stride 0
-// (its sums are multiplied by P = 0 at the end; the upload zeroes non-finite pixels, so whatever it reads
-// is finite).  Offsets [JA, JB) (warp-uniform) are the NEAR zone, evaluated from the LUT with the in-band
-// test; every other offset is FAR for every active lane, and a group that does not touch the near zone
-// runs straight-line far-zone code.  Phase 1 covers the groups that lie below Wmin (the shortest active
-// window) and needs no per-lane test at all; phase 2 finishes up to Wmax with the load offset clamped to
-// the lane's window and the contribution of lanes past their window masked to zero.
+// predicated: the grid is allocated with kPadRows zeroed rows past Nf-1, so reading a few pixels past the
+// end of a window stays in bounds, and an inactive lane reads pixel `idx` with stride 0 (its sums are
+// multiplied by P = 0 at the end; the upload zeroes non-finite pixels, so whatever it reads is finite).
+// Offsets [JA, JB) (warp-uniform) are the NEAR zone, evaluated from the LUT with the in-band test; every
+// other offset is FAR for every active lane, and a group that does not touch the near zone runs
+// straight-line far-zone code.  Groups that lie below Wmin (the shortest active window) need no per-lane
+// test at all; the groups that reach past it multiply the contribution of lanes past their own window
+// by zero.  Chunks whose windows differ by more than kRagMax pixels also clamp every load offset.
 #ifndef TFS_GROUP
 #define TFS_GROUP 2
 #endif
 constexpr int kGroup = TFS_GROUP;
-constexpr int kPadRows = 3 * kGroup;         // rows of zero padding behind the grid and the weights
+constexpr int kPadRows = 16;                 // rows of zero padding behind the grid and the weights
+constexpr int kRagMax = kPadRows - 2 * kGroup;   // largest Wmax - Wmin handled without clamping the loads
+static_assert(kRagMax >= 1, "kPadRows too small for kGroup");
 
 // ZONES: 1 = test the offset against the near zone, 0 = the offset is known to be far
 template <int MODE, int WMODE, int MASKED, int ZONES>
@@ -388,6 +396,15 @@ __device__ __forceinline__ void compute_group(const LaneTrack& L, const FarCoef&
   }
 }
 
+// one group from buffer B: unmasked while the whole group lies below Wmin
+template <int MODE, int WMODE>
+__device__ __forceinline__ void compute_group_auto(const LaneTrack& L, const FarCoef& C, const PixelBuf& B, int j0,
+                                                   int Wm, int Wmin, int Wmax, int JA, int JB, float& u,
+                                                   unsigned lut_lane, LaneSums& s) {
+  if (j0 + kGroup <= Wmin) compute_group<MODE, WMODE, 0>(L, C, B, j0, Wm, Wmax, JA, JB, u, lut_lane, s);
+  else compute_group<MODE, WMODE, 1>(L, C, B, j0, Wm, Wmax, JA, JB, u, lut_lane, s);
+}
+
 // idx = pixel index of offset 0, stp = Nt for an active lane and 0 otherwise, Wm = window length (>= 1
 // for active lanes, 0 otherwise)
 template <int MODE, int WMODE>
@@ -398,20 +415,28 @@ __device__ __forceinline__ void pixel_loop(const EvalArgs& a, const LaneTrack& L
 #pragma unroll
   for (int p = 0; p < kGroup; ++p) { A.W[p] = make_float2(0.f, 0.f); B.W[p] = make_float2(0.f, 0.f); }
   const int jlast = max(Wm - 1, 0);
-  load_group<0, WMODE>(a, A, idx, stp, kb, kstp, 0, jlast);
-  int j = 0;
-  for (; j + 2 * kGroup <= Wmin; j += 2 * kGroup) {                       // phase 1
-    load_group<0, WMODE>(a, B, idx, stp, kb, kstp, j + kGroup, jlast);
-    compute_group<MODE, WMODE, 0>(L, C, A, j, Wm, Wmax, JA, JB, u, lut_lane, s);
-    load_group<0, WMODE>(a, A, idx, stp, kb, kstp, j + 2 * kGroup, jlast);
-    compute_group<MODE, WMODE, 0>(L, C, B, j + kGroup, Wm, Wmax, JA, JB, u, lut_lane, s);
-  }
-  for (; j < Wmax; j += 2 * kGroup) {                                    // phase 2
-    load_group<1, WMODE>(a, B, idx, stp, kb, kstp, j + kGroup, jlast);
-    compute_group<MODE, WMODE, 1>(L, C, A, j, Wm, Wmax, JA, JB, u, lut_lane, s);
-    if (j + kGroup >= Wmax) break;
-    load_group<1, WMODE>(a, A, idx, stp, kb, kstp, j + 2 * kGroup, jlast);
-    compute_group<MODE, WMODE, 1>(L, C, B, j + kGroup, Wm, Wmax, JA, JB, u, lut_lane, s);
+  if (Wmax - Wmin <= kRagMax) {
+    // windows of (nearly) equal length, the usual case: nothing is clamped (the loads stay within
+    // kRagMax + 2 kGroup rows of every lane's window: zeroed pad rows), only the groups that reach
+    // past Wmin are masked
+    load_group<0, WMODE>(a, A, idx, stp, kb, kstp, 0, jlast);
+    for (int j = 0; j < Wmax; j += 2 * kGroup) {
+      load_group<0, WMODE>(a, B, idx, stp, kb, kstp, j + kGroup, jlast);
+      compute_group_auto<MODE, WMODE>(L, C, A, j, Wm, Wmin, Wmax, JA, JB, u, lut_lane, s);
+      if (j + kGroup >= Wmax) break;
+      load_group<0, WMODE>(a, A, idx, stp, kb, kstp, j + 2 * kGroup, jlast);
+      compute_group_auto<MODE, WMODE>(L, C, B, j + kGroup, Wm, Wmin, Wmax, JA, JB, u, lut_lane, s);
+    }
+  } else {
+    // very ragged chunk (wide tracks next to narrow ones): every load clamped, every step masked
+    load_group<1, WMODE>(a, A, idx, stp, kb, kstp, 0, jlast);
+    for (int j = 0; j < Wmax; j += 2 * kGroup) {
+      load_group<1, WMODE>(a, B, idx, stp, kb, kstp, j + kGroup, jlast);
+      compute_group<MODE, WMODE, 1>(L, C, A, j, Wm, Wmax, JA, JB, u, lut_lane, s);
+      if (j + kGroup >= Wmax) break;
+      load_group<1, WMODE>(a, A, idx, stp, kb, kstp, j + 2 * kGroup, jlast);
+      compute_group<MODE, WMODE, 1>(L, C, B, j + kGroup, Wm, Wmax, JA, JB, u, lut_lane, s);
+    }
   }
 }
 
@@ -438,13 +463,17 @@ __global__ void tile_table_kernel(const int* __restrict__ vprefix, int Nt, int N
   table[tile] = make_int2(vprefix[m0], vprefix[m1]);
 }
 
+__host__ __device__ constexpr int warps_per_cta(int wmode) {
+  return wmode == 0 ? TFS_WARPS_GENERAL : TFS_WARPS_SEPARABLE;      // 0 = kWGeneral (declared below)
+}
+
 template <int MODE, int WMODE>
-__global__ void __launch_bounds__(kWarpsPerCta * 32, 1)
+__global__ void __launch_bounds__(warps_per_cta(WMODE) * 32, 1)
 eval_tiles_kernel(const EvalArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* s_lut = reinterpret_cast<float4*>(smem_raw);
-  double* s_acc = reinterpret_cast<double*>(smem_raw + kLutSmemBytes) + threadIdx.x;   // [6][blockDim]
-  constexpr int kAccStride = kWarpsPerCta * 32;
+  f2_t* s_acc = reinterpret_cast<f2_t*>(smem_raw + kLutSmemBytes) + threadIdx.x;       // [3][blockDim]
+  constexpr int kAccStride = warps_per_cta(WMODE) * 32;
 
   const int lane = threadIdx.x & 31;
   if (MODE == 0) {
@@ -478,9 +507,10 @@ eval_tiles_kernel(const EvalArgs a) {
         continue;
       }
 
-      // fp64 per-lane running sums over the tile (z_A, z_E complex, q_A, q_E) live in shared memory
+      // per-lane running sums over the tile ({A, E} pairs of Re z, Im z, q; <= kTileMax/32 chunk sums each, fp32)
+      // live in shared memory; lanes, tiles and segments are then summed in fp64
 #pragma unroll
-      for (int v = 0; v < 6; ++v) s_acc[v * kAccStride] = 0.0;
+      for (int v = 0; v < 3; ++v) s_acc[v * kAccStride] = pk(0.f, 0.f);
 
       for (int ic = i0; ic < i1; ic += 32) {
         // ---------------- track point of this lane's tranche (a2) ----------------
@@ -539,28 +569,36 @@ eval_tiles_kernel(const EvalArgs a) {
         LaneSums s;
         s.zr = pk(0.f, 0.f); s.zi = pk(0.f, 0.f); s.q = pk(0.f, 0.f);
         pixel_loop<MODE, WMODE>(a, L, a.far, Wm, Wmin, Wmax, JA, JB, idx, stp, kb, kstp, u, lut_lane, s);
-        // apply the tranche's factor P (and |P|^2) and promote to fp64
-        float zAr, zEr, zAi, zEi, qA, qE;
-        upk(s.zr, zAr, zEr); upk(s.zi, zAi, zEi); upk(s.q, qA, qE);
-        if (WMODE != kWGeneral) {
-          // W = a[m] b[k]: the pixel loop summed b |h'|^2 (b = 1: {sum hr^2, sum hi^2}); apply a[m] here
-          const float2 am = __ldg(a.wa + m);
-          if (WMODE == kWTimeOnly) { qA += qE; qE = qA; }
-          qA *= am.x;
-          qE *= am.y;
-        }
+        // apply the tranche's factor P to z' and |P|^2 (times a[m] for separable weights) to q'
         const float P2 = fmaf(Pr, Pr, Pi * Pi);
-        s_acc[0 * kAccStride] += (double)(Pr * zAr - Pi * zAi);
-        s_acc[1 * kAccStride] += (double)(Pr * zAi + Pi * zAr);
-        s_acc[2 * kAccStride] += (double)(Pr * zEr - Pi * zEi);
-        s_acc[3 * kAccStride] += (double)(Pr * zEi + Pi * zEr);
-        s_acc[4 * kAccStride] += (double)(P2 * qA);
-        s_acc[5 * kAccStride] += (double)(P2 * qE);
+        f2_t qs = s.q, qc = pk(P2, P2);
+        if (WMODE != kWGeneral) {
+          // W = a[m] b[k]: the pixel loop summed b |h'|^2 (b = 1: {sum hr^2, sum hi^2})
+          const float2 am = __ldg(a.wa + m);
+          qc = pk(P2 * am.x, P2 * am.y);
+          if (WMODE == kWTimeOnly) {
+            float q0, q1;
+            upk(s.q, q0, q1);
+            qs = pk(q0 + q1, q0 + q1);
+          }
+        }
+        f2_t accr = s_acc[0 * kAccStride], acci = s_acc[1 * kAccStride];
+        accr = ffma2(pk(Pr, Pr), s.zr, accr);            // Re (P z') = Pr zr - Pi zi
+        accr = ffma2(pk(-Pi, -Pi), s.zi, accr);
+        acci = ffma2(pk(Pr, Pr), s.zi, acci);            // Im (P z') = Pr zi + Pi zr
+        acci = ffma2(pk(Pi, Pi), s.zr, acci);
+        s_acc[0 * kAccStride] = accr;
+        s_acc[1 * kAccStride] = acci;
+        s_acc[2 * kAccStride] = ffma2(qc, qs, s_acc[2 * kAccStride]);
       }
 
-      const double dzAr = warp_sum(s_acc[0 * kAccStride]), dzAi = warp_sum(s_acc[1 * kAccStride]);
-      const double dzEr = warp_sum(s_acc[2 * kAccStride]), dzEi = warp_sum(s_acc[3 * kAccStride]);
-      const double dqA = warp_sum(s_acc[4 * kAccStride]),  dqE = warp_sum(s_acc[5 * kAccStride]);
+      float tzAr, tzEr, tzAi, tzEi, tqA, tqE;
+      upk(s_acc[0 * kAccStride], tzAr, tzEr);
+      upk(s_acc[1 * kAccStride], tzAi, tzEi);
+      upk(s_acc[2 * kAccStride], tqA, tqE);
+      const double dzAr = warp_sum((double)tzAr), dzAi = warp_sum((double)tzAi);
+      const double dzEr = warp_sum((double)tzEr), dzEi = warp_sum((double)tzEi);
+      const double dqA = warp_sum((double)tqA),  dqE = warp_sum((double)tqE);
       if (lane == 0) {
         // z = T_A z_A + T_E z_E ; hh = |T_A|^2 q_A + |T_E|^2 q_E   (Eq. 29, Eq. 31)
         const double zr = T.TAr * dzAr - T.TAi * dzAi + T.TEr * dzEr - T.TEi * dzEi;
