@@ -155,7 +155,8 @@ def test_wide_tracks_parity(api):
 # options: paper-strict 21 bins, other half widths, restricted band, paper Fresnel approximants
 # --------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("opts", [dict(adaptive_width=0), dict(half_width=4), dict(half_width=15, c_max=20.0),
-                                  dict(f_lo=0.012, f_hi=0.05)])
+                                  dict(f_lo=0.012, f_hi=0.05), dict(half_width=0), dict(half_width=1),
+                                  dict(half_width=1, adaptive_width=0), dict(half_width=40, weight_mode=1)])
 def test_options_parity(api, opts):
     w = synth.scaled(synth.WORKLOADS["cfg2"], Nt=128, Nf=1024, n_templates=64)
     coeff, weight, gap = synth.make_data(w)
@@ -163,7 +164,8 @@ def test_options_parity(api, opts):
     params[:32, 1] = np.random.default_rng(2).uniform(0.2, 2.0, 32) * w.Nt * w.DT
     ctx = _mk(api, w, coeff, weight, gap, **opts)
     gpu = api.eval_host(ctx, params, 8)
-    ora = oracle_eval(coeff, weight, gap, params, w.Nt, w.Nf, w.dt, 8, **opts)
+    ora_opts = {k: v for k, v in opts.items() if k != "weight_mode"}        # a library-side choice, same result
+    ora = oracle_eval(coeff, weight, gap, params, w.Nt, w.Nf, w.dt, 8, **ora_opts)
     assert_parity(gpu, ora, 8, label=str(opts))
     ctx.destroy()
 
