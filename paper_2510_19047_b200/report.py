@@ -2,6 +2,7 @@
 
     python -m paper_2510_19047_b200.report track-width     # configs[3]: throughput vs track width
     python -m paper_2510_19047_b200.report nseg            # configs[2]: N_seg swept over {1, 4, 16, 64}
+    python -m paper_2510_19047_b200.report ladder          # configs[4]: the 64 -> 16 -> 4 -> 1 ladder at full size
 
 Uses only the public binding (api.Tfs) and the seeded generators (synth); timing with CUDA events on
 the current stream after warm-up, inputs resident on the device.  bench.py prints the headline line;
@@ -111,11 +112,41 @@ def nseg():
     ctx.destroy()
 
 
+def ladder_report():
+    """Full-size configs[4]: 10^6 templates on the cfg5 grid, stages N_seg = 64, 16, 4, 1, top 1 % kept and
+    replaced by 4 x 4 children per survivor.  Noise only (injections are made by the oracle, which this
+    package never imports): this table times the stages; recovery is tested in tests/test_gpu_ladder.py."""
+    torch, api, synth, w, ctx, _ = _setup("cfg5")
+    from . import ladder
+    dev = torch.device("cuda:0")
+    d = torch.from_numpy(synth.make_templates(w)).to(dev)
+    d_mc, d_tc = 2e-4, 1.0e4          # stage-0 lattice steps (relative Mc step, tc step in s)
+    for _ in range(2):
+        ladder.run(ctx, d, d_mc, d_tc)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    st = ladder.run(ctx, d, d_mc, d_tc)
+    e1.record()
+    torch.cuda.synchronize()
+    print(f"# configs[4] (cfg5): ladder at full size, grid {w.Nt} x {w.Nf}, keep 1 %, 4 x 4 children per survivor\n")
+    print(f"whole ladder (4 x tfs_eval + 4 x tfs_topk + 3 x tfs_refine): {e0.elapsed_time(e1):.2f} ms\n")
+    print("| stage | N_seg | templates | kept | ms per tfs_eval | templates/s | best Upsilon |")
+    print("|---:|---:|---:|---:|---:|---:|---:|")
+    for i, s in enumerate(st):
+        ms = _time_eval(ctx, torch, s.params, s.N_seg, reps=2, warm=1)
+        print(f"| {i} | {s.N_seg} | {s.params.shape[0]} | {s.top_idx.shape[0]} | {ms:.2f} | "
+              f"{s.params.shape[0] / ms * 1e3:.3e} | {float(s.top_val[0]):.1f} |")
+    ctx.destroy()
+
+
 if __name__ == "__main__":
     what = sys.argv[1] if len(sys.argv) > 1 else ""
     if what == "track-width":
         track_width()
     elif what == "nseg":
         nseg()
+    elif what == "ladder":
+        ladder_report()
     else:
         sys.exit(__doc__)
