@@ -17,7 +17,7 @@ namespace {
 
 thread_local char g_create_err[512] = "";
 
-constexpr size_t kScratchBytes = 1ull << 30;  // cap for the tile-partials buffer per sub-batch
+constexpr size_t kScratchBytes = 2ull << 30;  // cap for the piece-partials buffer per sub-batch
 
 }  // namespace
 
@@ -36,6 +36,10 @@ struct tfs_ctx {
   float2* colmax = nullptr;                // [Nf] scratch of the weight analysis
   unsigned long long* wcounts = nullptr;   // [2] {pixels violating W = a b, columns with b != 1}
   int wmode = -1;                          // kWGeneral / kWSeparable / kWTimeOnly; -1 before the first upload
+  int n_valid = 0;                         // valid (non-gap) tranches of the data uploaded last
+  // piece tables (tile x segment cuts of the valid-tranche list), cached per N_seg until the next upload
+  struct PieceTable { int N_seg; int n_tiles; int* tile_first; int* piece_end; int* piece_seg; cudaEvent_t ready; };
+  std::vector<PieceTable> piece_tables;
   uint8_t* gap = nullptr;
   int* vprefix = nullptr;                  // [Nt+1] valid tranches before m
   int* valid_m = nullptr;                  // [max(#valid,1)] valid tranche indices
@@ -253,6 +257,47 @@ double fit_far(FarCoef& out) {
   return err;
 }
 
+void free_piece_tables(tfs_ctx* ctx) {
+  for (auto& t : ctx->piece_tables) {
+    cudaFree(t.tile_first); cudaFree(t.piece_end); cudaFree(t.piece_seg);
+    if (t.ready) cudaEventDestroy(t.ready);
+  }
+  ctx->piece_tables.clear();
+}
+
+// piece table for N_seg (built on `st` on first use; later users on other streams wait for the build event)
+int get_piece_table(tfs_ctx* ctx, int N_seg, cudaStream_t st, const tfs_ctx::PieceTable** out) {
+  for (auto& t : ctx->piece_tables)
+    if (t.N_seg == N_seg) {
+      TFS_CUDA(ctx, cudaStreamWaitEvent(st, t.ready, 0));
+      *out = &t;
+      return TFS_OK;
+    }
+  if (ctx->piece_tables.size() >= 64) free_piece_tables(ctx);         // a sweep over many N_seg: start over
+  tfs_ctx::PieceTable t{};
+  t.N_seg = N_seg;
+  t.n_tiles = std::max(1, (ctx->n_valid + kTileMax - 1) / kTileMax);
+  const size_t max_pieces = (size_t)t.n_tiles + (size_t)N_seg;
+  cudaError_t e;
+  if ((e = cudaMalloc((void**)&t.tile_first, (t.n_tiles + 1) * sizeof(int))) != cudaSuccess ||
+      (e = cudaMalloc((void**)&t.piece_end, max_pieces * sizeof(int))) != cudaSuccess ||
+      (e = cudaMalloc((void**)&t.piece_seg, max_pieces * sizeof(int))) != cudaSuccess ||
+      (e = cudaEventCreateWithFlags(&t.ready, cudaEventDisableTiming)) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(t.tile_first); cudaFree(t.piece_end); cudaFree(t.piece_seg);
+    return fail(ctx, TFS_ENOMEM, "piece table allocation failed: %s", cudaGetErrorString(e));
+  }
+  piece_table_kernel<<<1, 1, 0, st>>>(ctx->vprefix, ctx->valid_m, ctx->Nt, N_seg, ctx->n_valid, t.n_tiles,
+                                      t.tile_first, t.piece_end, t.piece_seg);
+  ctx->launches += 1;
+  e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaEventRecord(t.ready, st);
+  ctx->piece_tables.push_back(t);
+  if (e != cudaSuccess) return fail(ctx, TFS_ECUDA, "piece_table_kernel failed: %s", cudaGetErrorString(e));
+  *out = &ctx->piece_tables.back();
+  return TFS_OK;
+}
+
 EvalArgs base_args(const tfs_ctx* ctx) {
   EvalArgs a{};
   a.grid = ctx->grid; a.wgt = ctx->wgt; a.wa = ctx->wa; a.wb = ctx->wb; a.gap = ctx->gap; a.lut = ctx->lut;
@@ -265,7 +310,7 @@ EvalArgs base_args(const tfs_ctx* ctx) {
   a.x_lo = ctx->f_lo * ctx->DT; a.x_hi = ctx->f_hi * ctx->DT;
   a.c_max = ctx->opts.c_max;
   a.far = ctx->far;
-  a.N_seg = 1; a.tiles_per_seg = 1; a.n_tiles = 1;
+  a.n_valid = ctx->n_valid; a.n_tiles = 1;
   return a;
 }
 
@@ -412,6 +457,7 @@ void tfs_destroy(tfs_ctx* ctx) {
                   ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
                   ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children, ctx->buf_tiles};
   for (void* b : bufs) if (b) cudaFree(b);
+  free_piece_tables(ctx);
   delete ctx;
 }
 
@@ -464,7 +510,11 @@ int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const
     ctx->launches += 4;
     UP_CUDA(cudaMemcpyAsync(wc, ctx->wcounts, sizeof(wc), cudaMemcpyDeviceToHost, st));
   }
+  int n_valid = 0;
+  UP_CUDA(cudaMemcpyAsync(&n_valid, ctx->vprefix + ctx->Nt, sizeof(int), cudaMemcpyDeviceToHost, st));
   UP_CUDA(cudaStreamSynchronize(st));
+  ctx->n_valid = n_valid;
+  free_piece_tables(ctx);                  // cut for the previous gap mask
   ctx->wmode = wc[0] != 0 ? kWGeneral : (wc[1] != 0 ? kWSeparable : kWTimeOnly);
   cleanup();
 #undef UP_CUDA
@@ -502,27 +552,23 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
     dev[i] = (float*)ctx->buf_out[i];
   }
 
-  // tiling: each segment is cut into tiles_per_seg tiles of <= kTileMax tranches
-  const int max_seg_len = (ctx->Nt + N_seg - 1) / N_seg;
-  const int tps = (max_seg_len + kTileMax - 1) / kTileMax;
-  const int n_tiles = N_seg * tps;
-  long long sub = (long long)(kScratchBytes / ((size_t)n_tiles * sizeof(float4)));
+  // tiling: tiles of kTileMax valid tranches, cut by the segment boundaries into pieces (one partial each)
+  const tfs_ctx::PieceTable* pt = nullptr;
+  rc = get_piece_table(ctx, N_seg, st, &pt);
+  if (rc) return rc;
+  const int n_tiles = pt->n_tiles;
+  const size_t max_pieces = (size_t)n_tiles + (size_t)N_seg;
+  long long sub = (long long)(kScratchBytes / (max_pieces * sizeof(float4)));
   sub = std::max<long long>(sub, 1024);
   sub = std::min<long long>(sub, n);
-  rc = ensure(ctx, &ctx->buf_partials, &ctx->cap_partials, (size_t)sub * n_tiles * sizeof(float4));
-  if (rc) return rc;
-
-  rc = ensure(ctx, &ctx->buf_tiles, &ctx->cap_tiles, (size_t)n_tiles * sizeof(int2));
+  rc = ensure(ctx, &ctx->buf_partials, &ctx->cap_partials, (size_t)sub * max_pieces * sizeof(float4));
   if (rc) return rc;
 
   TFS_CUDA(ctx, cudaMemsetAsync(ctx->bad, 0, sizeof(unsigned long long), st));
   EvalArgs a = base_args(ctx);
-  a.N_seg = N_seg; a.tiles_per_seg = tps; a.n_tiles = n_tiles;
-  a.tile_table = (const int2*)ctx->buf_tiles;
-  tile_table_kernel<<<(unsigned)((n_tiles + 127) / 128), 128, 0, st>>>(ctx->vprefix, ctx->Nt, N_seg, tps, n_tiles,
-                                                                     (int2*)ctx->buf_tiles);
-  TFS_CUDA(ctx, cudaGetLastError());
-  ctx->launches += 1;
+  a.n_tiles = n_tiles;
+  a.tile_first = pt->tile_first;
+  a.piece_end = pt->piece_end;
   a.partials = (float4*)ctx->buf_partials;
   for (long long off = 0; off < n; off += sub) {
     const long long nb = std::min(sub, n - off);
@@ -560,7 +606,7 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
     ctx->launches += 2;     // main kernel + combine
     const int threads = 128;
     combine_kernel<<<(unsigned)((nb + threads - 1) / threads), threads, 0, st>>>(
-        a.partials, nb, N_seg, tps, dev[0] + off, dev[1] ? dev[1] + off * per[1] : nullptr,
+        a.partials, nb, N_seg, pt->tile_first, n_tiles, pt->piece_seg, dev[0] + off, dev[1] ? dev[1] + off * per[1] : nullptr,
         dev[2] ? dev[2] + off * per[2] : nullptr, dev[3] ? dev[3] + off * per[3] : nullptr);
     TFS_CUDA(ctx, cudaGetLastError());
   }

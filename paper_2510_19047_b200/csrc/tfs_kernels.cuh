@@ -2,8 +2,9 @@
 // DESIGN.md section 6 for the kernel design.  Citations: P:<line> of PAPER.md, C<n> = DESIGN.md.
 //
 // Work decomposition: one WARP evaluates one (template, time tile) pair.  A time tile is a run
-// of <= kTileMax consecutive tranches inside one segment; work items are ordered tile-major so
-// that all templates sweep the same slab of the grid together and the slab stays L2-resident.
+// of kTileMax consecutive VALID (non-gap) tranches, whatever N_seg is; work items are ordered
+// tile-major so that all templates sweep the same slab of the grid together and the slab stays
+// L2-resident.  Segment boundaries cut a tile into PIECES; the warp writes one partial per piece.
 // Inside a tile lanes are tranches (32 at a time): fp64 0PN track per lane, then each lane walks
 // its own window; the grid is stored time-contiguous so those loads coalesce across lanes.
 #pragma once
@@ -22,7 +23,7 @@ namespace tfs {
 #define TFS_WARPS_GENERAL 24
 #endif
 constexpr int kMaxWarpsPerCta = TFS_WARPS_SEPARABLE > TFS_WARPS_GENERAL ? TFS_WARPS_SEPARABLE : TFS_WARPS_GENERAL;
-constexpr int kTileMax = 256;       // tranches per time tile (upper bound)
+constexpr int kTileMax = 256;       // valid tranches per time tile (8 chunks of 32 lanes)
 constexpr int kLutN = 512;          // LUT intervals in t = 1/(1+v)
 constexpr double kMtsun = 4.925490947e-6;   // G Msun / c^3 [s]
 constexpr double kPi = 3.14159265358979323846;
@@ -38,31 +39,22 @@ struct EvalArgs {
   const uint8_t* __restrict__ gap;     // [Nt] 1 = valid
   const int* __restrict__ vprefix;     // [Nt+1] number of valid tranches before m
   const int* __restrict__ valid_m;     // [vprefix[Nt]] the valid tranche indices, ascending (padded to >= 1 entry)
-  const int2* __restrict__ tile_table; // [n_tiles] {i0, i1}: entries of valid_m covered by each tile
+  const int* __restrict__ tile_first;  // [n_tiles+1] first piece of each tile (pieces are numbered in time order)
+  const int* __restrict__ piece_end;   // [n_pieces] entry of valid_m where the piece ends (exclusive)
   const float4* __restrict__ lut;      // [kLutN+1] {a_G, a_F, b_G, b_F} (see fresnel_aux)
   const double* __restrict__ params;   // [n][8]
-  float4* __restrict__ partials;       // [n_tiles][n] {z.re, z.im, hh, 0}
+  float4* __restrict__ partials;       // [n_pieces][n] {z.re, z.im, hh, 0}
   unsigned long long* bad_count;       // templates rejected (counted on tile 0 only)
   unsigned long long* work_counter;    // next unclaimed work item (zeroed before each launch)
   long long n;                         // templates in this launch
   int Nt, Nf;
-  int N_seg, tiles_per_seg, n_tiles;
+  int n_valid, n_tiles;                // valid tranches, ceil(n_valid / kTileMax) (>= 1)
   int H, adaptive;
   double DT;
   double x_lo, x_hi;                   // band in bins: f_lo*DT, f_hi*DT
   double c_max;
   FarCoef far;                         // far-zone polynomials of f, g (fitted at tfs_create)
 };
-
-// ----- tile geometry: segment n = tranches [ceil(n Nt/N_seg), ceil((n+1) Nt/N_seg))  (C9) -----
-__device__ __forceinline__ void tile_range(int tile, int tps, int Nt, int N_seg, int& m0, int& m1) {
-  const int n = tile / tps, t = tile - n * tps;
-  const int s0 = (int)(((long long)n * Nt + N_seg - 1) / N_seg);
-  const int s1 = (int)(((long long)(n + 1) * Nt + N_seg - 1) / N_seg);
-  const int L = (s1 - s0 + tps - 1) / tps;
-  m0 = min(s0 + t * L, s1);
-  m1 = min(m0 + L, s1);
-}
 
 // Per-template constants derived from the parameter row.
 struct TemplateConst {
@@ -453,14 +445,32 @@ __device__ __forceinline__ void pixel_loop(const EvalArgs& a, const LaneTrack& L
 // ------------------------------------------------------------------------------------------
 constexpr int kClaim = 4;
 
-// {i0, i1} = range of the compacted valid-tranche list covered by each tile (C9, C10)
-__global__ void tile_table_kernel(const int* __restrict__ vprefix, int Nt, int N_seg, int tps, int n_tiles,
-                                  int2* __restrict__ table) {
-  const int tile = blockIdx.x * blockDim.x + threadIdx.x;
-  if (tile >= n_tiles) return;
-  int m0, m1;
-  tile_range(tile, tps, Nt, N_seg, m0, m1);
-  table[tile] = make_int2(vprefix[m0], vprefix[m1]);
+// Piece table (C9, C10).  Segment n = tranches [ceil(n Nt/N_seg), ceil((n+1) Nt/N_seg)), i.e. n(m) =
+// floor(m N_seg / Nt).  Tile t = entries [t kTileMax, (t+1) kTileMax) of the compacted valid-tranche list.
+// A piece is a maximal run of entries inside one tile and one segment; pieces are numbered in time order.
+// One thread walks the list (<= n_tiles + N_seg pieces); the table is cached per N_seg by the host.
+//   tile_first[t] = first piece of tile t, tile_first[n_tiles] = number of pieces
+//   piece_end[p]  = entry where piece p ends (exclusive);  piece_seg[p] = its segment
+__global__ void piece_table_kernel(const int* __restrict__ vprefix, const int* __restrict__ valid_m, int Nt, int N_seg,
+                                   int n_valid, int n_tiles, int* __restrict__ tile_first,
+                                   int* __restrict__ piece_end, int* __restrict__ piece_seg) {
+  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  int p = 0;
+  for (int t = 0; t < n_tiles; ++t) {
+    tile_first[t] = p;
+    int i = t * kTileMax;
+    const int iend = min(i + kTileMax, n_valid);
+    while (i < iend) {
+      const int seg = (int)(((long long)valid_m[i] * N_seg) / Nt);
+      const int s1 = (int)(((long long)(seg + 1) * Nt + N_seg - 1) / N_seg);     // first tranche of the next segment
+      const int e = min(vprefix[min(s1, Nt)], iend);
+      piece_seg[p] = seg;
+      piece_end[p] = e;
+      ++p;
+      i = e;
+    }
+  }
+  tile_first[n_tiles] = p;
 }
 
 __host__ __device__ constexpr int warps_per_cta(int wmode) {
@@ -494,23 +504,48 @@ eval_tiles_kernel(const EvalArgs a) {
     long long it = w0 - (long long)tile * a.n;
     for (int wi = 0; wi < n_claim; ++wi, ++it) {
       if (it == a.n) { it = 0; ++tile; }
-      // valid (non-gap) tranches of the tile: entries [i0, i1) of the compacted list (C10)
-      const int2 ir = a.tile_table[tile];
-      const int i0 = ir.x, i1 = ir.y;
+      // valid (non-gap) tranches of the tile: entries [i0, i1) of the compacted list (C10), cut by the
+      // segment boundaries into pieces [p, p_last]
+      const int i0 = tile * kTileMax, i1 = min(i0 + kTileMax, a.n_valid);
+      int p = a.tile_first[tile];
+      const int p_stop = a.tile_first[tile + 1];
 
       const TemplateConst T = load_template(a.params + it * 8, a.DT);
       if (!T.ok) {
-        if (lane == 0) {
-          a.partials[(long long)tile * a.n + it] = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (tile == 0) atomicAdd(a.bad_count, 1ULL);
-        }
+        for (int q = p + lane; q < p_stop; q += 32) a.partials[(long long)q * a.n + it] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (lane == 0 && tile == 0) atomicAdd(a.bad_count, 1ULL);
         continue;
       }
+      int pend = p < p_stop ? a.piece_end[p] : i1;
 
-      // per-lane running sums over the tile ({A, E} pairs of Re z, Im z, q; <= kTileMax/32 chunk sums each, fp32)
-      // live in shared memory; lanes, tiles and segments are then summed in fp64
+      // per-lane running sums over the current piece ({A, E} pairs of Re z, Im z, q; <= kTileMax/32 chunk sums
+      // each, fp32) live in shared memory; lanes, pieces and segments are then summed in fp64
 #pragma unroll
       for (int v = 0; v < 3; ++v) s_acc[v * kAccStride] = pk(0.f, 0.f);
+
+      // close piece p: sum its per-lane sums over the warp (packed fp32 butterfly: 32 terms), combine the
+      // channels in fp64, store, reset
+      auto flush = [&]() {
+        f2_t r0 = s_acc[0 * kAccStride], r1 = s_acc[1 * kAccStride], r2 = s_acc[2 * kAccStride];
+#pragma unroll
+        for (int v = 0; v < 3; ++v) s_acc[v * kAccStride] = pk(0.f, 0.f);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          r0 = fadd2(r0, __shfl_xor_sync(0xffffffffu, r0, o));
+          r1 = fadd2(r1, __shfl_xor_sync(0xffffffffu, r1, o));
+          r2 = fadd2(r2, __shfl_xor_sync(0xffffffffu, r2, o));
+        }
+        if (lane == 0) {
+          float zAr, zEr, zAi, zEi, qA, qE;
+          upk(r0, zAr, zEr); upk(r1, zAi, zEi); upk(r2, qA, qE);
+          const double dzAr = zAr, dzAi = zAi, dzEr = zEr, dzEi = zEi, dqA = qA, dqE = qE;
+          // z = T_A z_A + T_E z_E ; hh = |T_A|^2 q_A + |T_E|^2 q_E   (Eq. 29, Eq. 31)
+          const double zr = T.TAr * dzAr - T.TAi * dzAi + T.TEr * dzEr - T.TEi * dzEi;
+          const double zi = T.TAr * dzAi + T.TAi * dzAr + T.TEr * dzEi + T.TEi * dzEr;
+          const double hh = (T.TAr * T.TAr + T.TAi * T.TAi) * dqA + (T.TEr * T.TEr + T.TEi * T.TEi) * dqE;
+          a.partials[(long long)p * a.n + it] = make_float4((float)zr, (float)zi, (float)hh, 0.f);
+        }
+      };
 
       for (int ic = i0; ic < i1; ic += 32) {
         // ---------------- track point of this lane's tranche (a2) ----------------
@@ -519,7 +554,10 @@ eval_tiles_kernel(const EvalArgs a) {
         const int m = a.valid_m[valid ? i : i0];
         const TrackPoint tp = track_point(T, m, a.DT, a.x_lo, a.x_hi, a.c_max, valid);
         const unsigned act_mask = __ballot_sync(0xffffffffu, tp.active);
-        if (act_mask == 0u) continue;
+        const int cend = min(ic + 32, i1);
+        const bool closes = p < p_stop && pend <= cend;   // a piece ends inside this chunk (warp-uniform)
+        f2_t vr = pk(0.f, 0.f), vi = vr, vq = vr;          // this chunk's per-lane contribution (P z', |P|^2 a q')
+        if (act_mask != 0u) {
         int Wm = 0, idx = m, stp = 0, kb = 0, kstp = 0, ja = 0x7fffffff, jb = 0;
         float u = -1.f, Pr = 0.f, Pi = 0.f;
         LaneTrack L;        // inactive lanes: u_j = -1 - j, u_j + c = -0.5 - j (finite h' on zeroed data)
@@ -582,48 +620,67 @@ eval_tiles_kernel(const EvalArgs a) {
             qs = pk(q0 + q1, q0 + q1);
           }
         }
-        f2_t accr = s_acc[0 * kAccStride], acci = s_acc[1 * kAccStride];
-        accr = ffma2(pk(Pr, Pr), s.zr, accr);            // Re (P z') = Pr zr - Pi zi
-        accr = ffma2(pk(-Pi, -Pi), s.zi, accr);
-        acci = ffma2(pk(Pr, Pr), s.zi, acci);            // Im (P z') = Pr zi + Pi zr
-        acci = ffma2(pk(Pi, Pi), s.zr, acci);
-        s_acc[0 * kAccStride] = accr;
-        s_acc[1 * kAccStride] = acci;
-        s_acc[2 * kAccStride] = ffma2(qc, qs, s_acc[2 * kAccStride]);
-      }
-
-      float tzAr, tzEr, tzAi, tzEi, tqA, tqE;
-      upk(s_acc[0 * kAccStride], tzAr, tzEr);
-      upk(s_acc[1 * kAccStride], tzAi, tzEi);
-      upk(s_acc[2 * kAccStride], tqA, tqE);
-      const double dzAr = warp_sum((double)tzAr), dzAi = warp_sum((double)tzAi);
-      const double dzEr = warp_sum((double)tzEr), dzEi = warp_sum((double)tzEi);
-      const double dqA = warp_sum((double)tqA),  dqE = warp_sum((double)tqE);
-      if (lane == 0) {
-        // z = T_A z_A + T_E z_E ; hh = |T_A|^2 q_A + |T_E|^2 q_E   (Eq. 29, Eq. 31)
-        const double zr = T.TAr * dzAr - T.TAi * dzAi + T.TEr * dzEr - T.TEi * dzEi;
-        const double zi = T.TAr * dzAi + T.TAi * dzAr + T.TEr * dzEi + T.TEi * dzEr;
-        const double hh = (T.TAr * T.TAr + T.TAi * T.TAi) * dqA + (T.TEr * T.TEr + T.TEi * T.TEi) * dqE;
-        a.partials[(long long)tile * a.n + it] = make_float4((float)zr, (float)zi, (float)hh, 0.f);
+        if (!closes) {
+          // the usual case: the whole chunk belongs to the current piece
+          f2_t accr = s_acc[0 * kAccStride], acci = s_acc[1 * kAccStride];
+          accr = ffma2(pk(Pr, Pr), s.zr, accr);          // Re (P z') = Pr zr - Pi zi
+          accr = ffma2(pk(-Pi, -Pi), s.zi, accr);
+          acci = ffma2(pk(Pr, Pr), s.zi, acci);          // Im (P z') = Pr zi + Pi zr
+          acci = ffma2(pk(Pi, Pi), s.zr, acci);
+          s_acc[0 * kAccStride] = accr;
+          s_acc[1 * kAccStride] = acci;
+          s_acc[2 * kAccStride] = ffma2(qc, qs, s_acc[2 * kAccStride]);
+        } else {
+          vr = fmul2(pk(Pr, Pr), s.zr);
+          vr = ffma2(pk(-Pi, -Pi), s.zi, vr);
+          vi = fmul2(pk(Pr, Pr), s.zi);
+          vi = ffma2(pk(Pi, Pi), s.zr, vi);
+          vq = fmul2(qc, qs);
+        }
+        }
+        if (closes) {
+          // every piece that ends inside this chunk (a segment boundary, or the end of the tile) takes the
+          // lanes before its end and is closed; the lanes behind the last such end open the next piece
+          int lo = 0;
+          for (;;) {
+            const bool ends = p < p_stop && pend <= cend;
+            const int hi = ends ? pend - ic : 32;
+            if (lane >= lo && lane < hi) {
+              s_acc[0 * kAccStride] = fadd2(s_acc[0 * kAccStride], vr);
+              s_acc[1 * kAccStride] = fadd2(s_acc[1 * kAccStride], vi);
+              s_acc[2 * kAccStride] = fadd2(s_acc[2 * kAccStride], vq);
+            }
+            if (!ends) break;
+            flush();
+            ++p;
+            if (p < p_stop) pend = a.piece_end[p];
+            lo = hi;
+          }
+        }
       }
     }
   }
 }
 
 // ------------------------------------------------------------------------------------------
-// Kernel B: sum tile partials per segment, P_n = |z_n|^2/hh_n, Upsilon = sum_n P_n (Eq. 8, 9).
+// Kernel B: sum the piece partials of each segment, P_n = |z_n|^2/hh_n, Upsilon = sum_n P_n (Eq. 8, 9).
+// Pieces are in time order, so the pieces of a segment are consecutive; a segment without a valid
+// tranche has no piece and contributes 0.
 // ------------------------------------------------------------------------------------------
-__global__ void combine_kernel(const float4* __restrict__ partials, long long n, int N_seg, int tps,
+__global__ void combine_kernel(const float4* __restrict__ partials, long long n, int N_seg,
+                               const int* __restrict__ tile_first, int n_tiles, const int* __restrict__ piece_seg,
                                float* __restrict__ upsilon, float* __restrict__ seg_power,
                                float* __restrict__ seg_dh, float* __restrict__ seg_hh) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
+  const int n_pieces = tile_first[n_tiles];
   double ups = 0.0;
+  int p = 0;
   for (int s = 0; s < N_seg; ++s) {
     double zr = 0, zi = 0, hh = 0;
-    for (int t = 0; t < tps; ++t) {
-      const float4 p = partials[(long long)(s * tps + t) * n + i];
-      zr += p.x; zi += p.y; hh += p.z;
+    for (; p < n_pieces && piece_seg[p] == s; ++p) {
+      const float4 v = partials[(long long)p * n + i];
+      zr += v.x; zi += v.y; hh += v.z;
     }
     const double P = hh > 0.0 ? (zr * zr + zi * zi) / hh : 0.0;
     ups += P;

@@ -95,20 +95,20 @@ def track_width():
 
 
 def nseg():
-    torch, api, synth, w, ctx, _ = _setup("cfg3")
+    torch, api, synth, w, ctx, data = _setup("cfg3")
     dev = torch.device("cuda:0")
+    n_valid = int(np.count_nonzero(data[2]))
     params = synth.make_templates(w)
     d = torch.from_numpy(params).to(dev)
     pix = _counts(ctx, torch, d)
     print(f"# configs[2] (cfg3): N_seg sweep, {len(params)} templates, grid {w.Nt} x {w.Nf}, "
-          f"weight structure {ctx.weight_structure()}\n")
-    print("| N_seg | time tiles | ms per tfs_eval | templates/s | pixel-evals/s |")
-    print("|---:|---:|---:|---:|---:|")
+          f"weight structure {ctx.weight_structure()}, {n_valid} valid tranches = {-(-n_valid // 256)} time tiles "
+          f"of 256 for every N_seg\n")
+    print("| N_seg | ms per tfs_eval | templates/s | pixel-evals/s |")
+    print("|---:|---:|---:|---:|")
     for N in (1, 4, 16, 64):
         ms = _time_eval(ctx, torch, d, N)
-        seg_len = -(-w.Nt // N)
-        tiles = N * (-(-seg_len // 256))
-        print(f"| {N} | {tiles} | {ms:.2f} | {len(params) / ms * 1e3:.3e} | {2 * pix.sum() / ms * 1e3:.3e} |")
+        print(f"| {N} | {ms:.2f} | {len(params) / ms * 1e3:.3e} | {2 * pix.sum() / ms * 1e3:.3e} |")
     ctx.destroy()
 
 
