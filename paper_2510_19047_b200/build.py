@@ -16,11 +16,21 @@ DEPS = SOURCES + [os.path.join(CSRC, "tfs_kernels.cuh"),
                   os.path.join(os.path.dirname(HERE), "include", "tfs.h")]
 
 
-def nvcc_cmd(extra=()):
+def nvcc_cmd(extra=(), out=None):
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     return [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
             "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",
-            "-DTFS_BUILD", *extra, "-o", LIB, *SOURCES, "-lcudart"]
+            "-DTFS_BUILD", *extra, "-o", out or LIB, *SOURCES, "-lcudart"]
+
+
+def build_variant(out: str, defines=()) -> str:
+    """Compile a variant of the library (e.g. -DTFS_BOUNDS_CHECK, the debug build whose gather traps on an
+    out-of-range index) to `out`; select it with the TFS_LIB_PATH environment variable."""
+    cmd = nvcc_cmd([f"-D{d}" for d in defines], out=out)
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
+    return out
 
 
 def up_to_date() -> bool:

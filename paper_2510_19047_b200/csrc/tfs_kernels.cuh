@@ -14,13 +14,13 @@
 namespace tfs {
 
 // Warps of the one persistent CTA per SM.  The kernel is short of warps to hide its dependent chains, so
-// it runs the most that the register file allows: 32 (64 registers per thread) when no per-pixel weight
-// is buffered, 24 (80 registers) for general weights, which need two more registers per pixel in flight.
+// it runs the most a CTA can hold: 32 warps at 64 registers per thread (measured against 20, 24, 26, 28
+// for both the separable- and the general-weights variants).
 #ifndef TFS_WARPS_SEPARABLE
 #define TFS_WARPS_SEPARABLE 32
 #endif
 #ifndef TFS_WARPS_GENERAL
-#define TFS_WARPS_GENERAL 24
+#define TFS_WARPS_GENERAL 32
 #endif
 constexpr int kMaxWarpsPerCta = TFS_WARPS_SEPARABLE > TFS_WARPS_GENERAL ? TFS_WARPS_SEPARABLE : TFS_WARPS_GENERAL;
 constexpr int kTileMax = 256;       // valid tranches per time tile (8 chunks of 32 lanes)
@@ -366,6 +366,13 @@ __device__ __forceinline__ void load_group(const EvalArgs& a, PixelBuf& B, int i
   for (int p = 0; p < kGroup; ++p) {
     const int jj = CLAMP ? min(j0 + p, jlast) : (j0 + p);
     const int i = idx + jj * stp;
+#ifdef TFS_BOUNDS_CHECK
+#ifndef TFS_BOUNDS_PAD
+#define TFS_BOUNDS_PAD kPadRows   // (a smaller value makes the check fail on purpose: tests the checker)
+#endif
+    // debug builds only: the gather is unpredicated, so prove it stays inside the padded arrays
+    if (i < 0 || i >= (a.Nf + TFS_BOUNDS_PAD) * a.Nt || kb + jj * kstp < 0 || kb + jj * kstp >= a.Nf + TFS_BOUNDS_PAD) __trap();
+#endif
     B.Y[p] = __ldg(a.grid + i);
     if (WMODE == kWGeneral) B.W[p] = __ldg(a.wgt + i);
     if (WMODE == kWSeparable) B.W[p] = __ldg(a.wb + kb + jj * kstp);

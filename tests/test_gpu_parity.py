@@ -368,3 +368,46 @@ def test_full_size_cfg3_sampled_parity(api):
     r = assert_parity(gpu, ora, N_seg, label="cfg3 full size, sampled rows")
     assert r["n_active"] == len(sample)
     ctx.destroy()
+
+
+# --------------------------------------------------------------------------------------------
+# The gather of the main kernel is unpredicated and software-pipelined: it reads a few pixels past
+# the end of a window and relies on zeroed pad rows.  A debug build (-DTFS_BOUNDS_CHECK) traps on any
+# index outside the padded arrays; run the shapes that stress it (windows clipped at both band edges,
+# wide and ragged chunks, large half widths, every weight mode) through that build in a subprocess.
+# --------------------------------------------------------------------------------------------
+_BOUNDS_SCRIPT = r"""
+import numpy as np, torch
+from paper_2510_19047_b200 import api, synth
+assert "boundscheck" in api.LIB_PATH
+for name, Nt, Nf, opts in (("cfg4", 160, 1024, {}), ("cfg4", 96, 512, dict(half_width=40)),
+                           ("cfg2", 200, 768, dict(half_width=0)), ("cfg3", 333, 1024, dict(weight_mode=1)),
+                           ("cfg3", 300, 640, dict(c_max=1000.0, half_width=25))):
+    w = synth.scaled(synth.WORKLOADS[name], Nt=Nt, Nf=Nf, n_templates=512)
+    coeff, weight, gap = synth.make_data(w)
+    p = synth.make_templates(w)
+    rng = np.random.default_rng(3)
+    p[::2, 0] = np.exp(rng.uniform(np.log(5.0), np.log(100.0), len(p[::2])))
+    p[::2, 1] = rng.uniform(0.0, 1.5, len(p[::2])) * w.Nt * w.DT          # many merge inside the grid
+    ctx = api.Tfs(w.Nt, w.Nf, w.dt, **opts)
+    ctx.upload_data(coeff, weight, gap)
+    for N_seg in (1, 7, w.Nt):
+        r = api.eval_host(ctx, p, N_seg, segments=False)
+        assert np.isfinite(r["upsilon"]).all()
+    torch.cuda.synchronize()
+    ctx.destroy()
+print("bounds ok")
+"""
+
+
+def test_gather_stays_inside_the_padded_grid(api, tmp_path):
+    import os
+    import subprocess
+    import sys
+    from paper_2510_19047_b200 import build
+    lib = build.build_variant(str(tmp_path / "libtfs_boundscheck.so"), ["TFS_BOUNDS_CHECK"])
+    env = dict(os.environ, TFS_LIB_PATH=lib)
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", _BOUNDS_SCRIPT], cwd=root, env=env, capture_output=True, text=True,
+                       timeout=900)
+    assert r.returncode == 0 and "bounds ok" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
