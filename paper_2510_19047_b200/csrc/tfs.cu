@@ -59,7 +59,6 @@ struct tfs_ctx {
   void* buf_tk_val = nullptr;   size_t cap_tk_val = 0;
   void* buf_counts = nullptr;   size_t cap_counts = 0;
   void* buf_children = nullptr; size_t cap_children = 0;
-  void* buf_tiles = nullptr;    size_t cap_tiles = 0;
   SelectState* sel = nullptr;
 
   // measurement hooks
@@ -455,7 +454,7 @@ void tfs_destroy(tfs_ctx* ctx) {
   for (auto& p : ctx->ev_pool) { cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
   void* bufs[] = {ctx->grid, ctx->wgt, ctx->wa, ctx->wb, ctx->colmax, ctx->wcounts, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut, ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials,
                   ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
-                  ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children, ctx->buf_tiles};
+                  ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children};
   for (void* b : bufs) if (b) cudaFree(b);
   free_piece_tables(ctx);
   delete ctx;
@@ -782,11 +781,17 @@ int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k, long long* 
     bitonic_small_kernel<<<1, 1024, P * sizeof(unsigned long long), st>>>(keys, P);
     ctx->launches += 1;
   } else {
-    for (unsigned size = 2; size <= P; size <<= 1)
-      for (unsigned stride = size >> 1; stride > 0; stride >>= 1) {
+    // sizes up to the block: one launch; larger sizes: the strides that leave a block one by one, the rest per block
+    bitonic_block_kernel<<<P / kBitonicBlock, 1024, 0, st>>>(keys, 2u, kBitonicBlock);
+    ctx->launches += 1;
+    for (unsigned size = 2 * kBitonicBlock; size <= P && size != 0; size <<= 1) {
+      for (unsigned stride = size >> 1; stride > kBitonicBlock / 2; stride >>= 1) {
         bitonic_step_kernel<<<(P / 2 + threads - 1) / threads, threads, 0, st>>>(keys, P, size, stride);
         ctx->launches += 1;
       }
+      bitonic_block_kernel<<<P / kBitonicBlock, 1024, 0, st>>>(keys, size, size);
+      ctx->launches += 1;
+    }
   }
   topk_emit_kernel<<<(k + threads - 1) / threads, threads, 0, st>>>(keys, d_in, k, d_idx, d_val);
   TFS_CUDA(ctx, cudaGetLastError());

@@ -1023,6 +1023,31 @@ __global__ void bitonic_small_kernel(unsigned long long* keys, unsigned P) {
   for (unsigned i = threadIdx.x; i < P; i += blockDim.x) keys[i] = sk[i];
 }
 
+// P > 4096: each block owns kBitonicBlock consecutive keys in shared memory and runs every compare-exchange
+// step whose stride stays inside the block (stride <= kBitonicBlock/2) for the sizes size_first ... size_last;
+// the few steps with a larger stride run in bitonic_step_kernel.  Directions use the global index.
+constexpr unsigned kBitonicBlock = 4096;
+__global__ void __launch_bounds__(1024)
+bitonic_block_kernel(unsigned long long* keys, unsigned size_first, unsigned size_last) {
+  __shared__ unsigned long long sk[kBitonicBlock];
+  const unsigned base = blockIdx.x * kBitonicBlock;
+  for (unsigned i = threadIdx.x; i < kBitonicBlock; i += blockDim.x) sk[i] = keys[base + i];
+  __syncthreads();
+  for (unsigned size = size_first; size <= size_last && size != 0; size <<= 1) {
+    for (unsigned stride = min(size >> 1, kBitonicBlock / 2); stride > 0; stride >>= 1) {
+      for (unsigned t = threadIdx.x; t < kBitonicBlock / 2; t += blockDim.x) {
+        const unsigned lo = 2 * stride * (t / stride) + (t % stride);
+        const unsigned hi = lo + stride;
+        const bool desc = (((base + lo) & size) == 0);
+        const unsigned long long a = sk[lo], b = sk[hi];
+        if ((a < b) == desc) { sk[lo] = b; sk[hi] = a; }
+      }
+      __syncthreads();
+    }
+  }
+  for (unsigned i = threadIdx.x; i < kBitonicBlock; i += blockDim.x) keys[base + i] = sk[i];
+}
+
 __global__ void topk_emit_kernel(const unsigned long long* __restrict__ keys, const float* __restrict__ v,
                                  int k, long long* __restrict__ idx, float* __restrict__ val) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
