@@ -411,3 +411,20 @@ def test_gather_stays_inside_the_padded_grid(api, tmp_path):
     r = subprocess.run([sys.executable, "-c", _BOUNDS_SCRIPT], cwd=root, env=env, capture_output=True, text=True,
                        timeout=900)
     assert r.returncode == 0 and "bounds ok" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
+
+
+def test_sub_batches_match_separate_calls(api):
+    """A bank whose piece partials exceed the scratch cap is cut into sub-batches inside one tfs_eval call;
+    the results must be bit-identical to evaluating the same rows in separate, smaller calls."""
+    w = synth.scaled(synth.WORKLOADS["cfg3"], Nt=1024, Nf=1024, n_templates=300_000)
+    coeff, weight, gap = synth.make_data(w)
+    params = synth.make_templates(w)
+    params[:, 1] = np.random.default_rng(4).uniform(0.0, 3.0, len(params)) * w.Nt * w.DT
+    ctx = _mk(api, w, coeff, weight, gap)
+    N_seg = w.Nt                       # one segment per tranche: ~1030 pieces -> 16.5 KB of partials per template
+    whole = api.eval_host(ctx, params, N_seg, segments=False)["upsilon"]
+    parts = [api.eval_host(ctx, params[i:i + 60_000], N_seg, segments=False)["upsilon"]
+             for i in range(0, len(params), 60_000)]
+    assert np.array_equal(whole, np.concatenate(parts))
+    assert (whole > 0).sum() > 100_000
+    ctx.destroy()
