@@ -83,6 +83,25 @@ TFS_API int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels,
 TFS_API int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight,
                     const uint8_t* gap_mask, void* stream);
 
+/* Time-series front end (the step before the path): window every tranche of N = 2*Nf samples
+ * with a Tukey window of shape parameter tukey_alpha (the paper uses 0.1; 0 = boxcar), Fourier-transform
+ * it, attach the noise weights of a one-sided PSD model and turn sample gaps into the tranche mask; then
+ * proceed exactly as tfs_upload_data:
+ *     D[a,m,k] = (1/N) sum_n w[n] x[a, m*N + n] exp(-2 pi i k n / N),   k = 0 ... Nf-1
+ *                (= dt*DFT/DT: the continuous-FT convention with the common factor DT dropped, C16)
+ *     W[a,m,k] = 4*DT / S_a[k]   (0 where S is not positive and finite; 1 everywhere if psd == NULL),
+ *                so that E[W |D|^2] = 2 <w^2> for noise of that PSD
+ *     g[m]     = 1 iff every sample of tranche m is valid
+ *   x           [C][Nt*2*Nf] float, real TDI series at cadence dt            host or device, required
+ *   sample_mask [Nt*2*Nf]    uint8, 1 = valid sample; NULL => all valid        host or device
+ *   psd         [C][Nf]      float, one-sided PSD [1/Hz] at f_k = k/DT; NULL => W = 1   host or device
+ *   coeff_out [C][Nt][Nf][2], weight_out [C][Nt][Nf], gap_out [Nt]: nullable copies of D, W, g
+ *                (host or device), e.g. to draw the whitened spectrogram of Fig. 3
+ * Nf must factor into 2, 3 and 5 (shared-memory FFT) and be <= 12800.  Synchronises `stream`. */
+TFS_API int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_mask, const float* psd,
+                                  double tukey_alpha, float* coeff_out, float* weight_out, uint8_t* gap_out,
+                                  void* stream);
+
 /* Evaluate Upsilon_{N_seg} for n templates.
  *   params  [n][8] double: Mc [Msun], tc [s after data start], phic [rad],
  *                          T_A.re, T_A.im, T_E.re, T_E.im (Eq. 29, constant per template, C5),

@@ -49,6 +49,8 @@ def load_library():
     lib.tfs_create.restype = ip
     lib.tfs_upload_data.argtypes = [vp, vp, vp, vp, vp]
     lib.tfs_upload_data.restype = ip
+    lib.tfs_upload_timeseries.argtypes = [vp, vp, vp, vp, dp, vp, vp, vp, vp]
+    lib.tfs_upload_timeseries.restype = ip
     lib.tfs_eval.argtypes = [vp, vp, ll, ip, vp, vp, vp, vp, vp]
     lib.tfs_eval.restype = ip
     lib.tfs_topk.argtypes = [vp, vp, ll, ip, vp, vp, vp]
@@ -131,6 +133,15 @@ class Tfs:
         self._check(self._lib.tfs_upload_data(self._h, _ptr(coeff, np.float32, 2 * npix),
                                               _ptr(weight, np.float32, npix),
                                               _ptr(gap_mask, np.uint8, self.Nt), _stream(stream)))
+
+    def upload_timeseries(self, x, sample_mask=None, psd=None, tukey_alpha=0.1, coeff_out=None, weight_out=None,
+                          gap_out=None, stream=None):
+        nsamp = self.Nt * 2 * self.Nf
+        npix = self.C * self.Nt * self.Nf
+        self._check(self._lib.tfs_upload_timeseries(
+            self._h, _ptr(x, np.float32, self.C * nsamp), _ptr(sample_mask, np.uint8, nsamp),
+            _ptr(psd, np.float32, self.C * self.Nf), float(tukey_alpha), _ptr(coeff_out, np.float32, 2 * npix),
+            _ptr(weight_out, np.float32, npix), _ptr(gap_out, np.uint8, self.Nt), _stream(stream)))
 
     def eval(self, params, N_seg, upsilon, seg_power=None, seg_dh=None, seg_hh=None, n=None, stream=None):
         if n is None:

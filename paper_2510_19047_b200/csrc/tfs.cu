@@ -2,6 +2,7 @@
 // No torch, no third-party libraries: CUDA runtime only.
 #include "../../include/tfs.h"
 #include "tfs_kernels.cuh"
+#include "tfs_frontend.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -502,7 +503,8 @@ int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const
   if (ctx->opts.weight_mode == 0) {
     UP_CUDA(cudaMemsetAsync(ctx->wcounts, 0, 2 * sizeof(unsigned long long), st));
     weight_colmax_kernel<<<(unsigned)ctx->Nf, 256, 0, st>>>(ctx->wgt, ctx->Nt, ctx->colmax);
-    weight_rowmax_kernel<<<(unsigned)((ctx->Nt + 127) / 128), 128, 0, st>>>(ctx->wgt, ctx->Nt, ctx->Nf, ctx->wa);
+    UP_CUDA(cudaMemsetAsync(ctx->wa, 0, (size_t)ctx->Nt * sizeof(float2), st));
+    weight_rowmax_kernel<<<dim3((unsigned)((ctx->Nt + 127) / 128), 32), 128, 0, st>>>(ctx->wgt, ctx->Nt, ctx->Nf, ctx->wa);
     weight_factor_kernel<<<1, 1024, 0, st>>>(ctx->colmax, ctx->Nf, ctx->wb, ctx->wcounts);
     weight_check_kernel<<<(unsigned)((npix + 255) / 256), 256, 0, st>>>(ctx->wgt, ctx->wa, ctx->wb, ctx->Nt, ctx->Nf, ctx->wcounts);
     UP_CUDA(cudaGetLastError());
@@ -518,6 +520,80 @@ int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const
   cleanup();
 #undef UP_CUDA
   ctx->uploaded = true;
+  return rc;
+}
+
+int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_mask, const float* psd,
+                          double tukey_alpha, float* coeff_out, float* weight_out, uint8_t* gap_out, void* stream) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_upload_timeseries: ctx is NULL");
+  if (!x) return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: x is NULL");
+  if (!(tukey_alpha >= 0.0 && tukey_alpha <= 1.0))
+    return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: tukey_alpha must be in [0, 1] (got %g)", tukey_alpha);
+  cudaStream_t st = (cudaStream_t)stream;
+  const int C = ctx->C, Nt = ctx->Nt, Nf = ctx->Nf, N = 2 * ctx->Nf;
+  // radices of the length-Nf complex FFT behind the packed real transform
+  FeRadices rad{};
+  {
+    int L = Nf;
+    const int primes[4] = {4, 2, 3, 5};
+    for (int pi = 0; pi < 4; ++pi)
+      while (L % primes[pi] == 0 && rad.n < kFeMaxStages) { rad.r[rad.n++] = primes[pi]; L /= primes[pi]; }
+    if (L != 1) return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: Nf = %d must factor into 2, 3 and 5", Nf);
+  }
+  const size_t smem = 2 * (size_t)Nf * sizeof(float2);
+  if (smem > 200 * 1024) return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: Nf = %d is too long for the shared-memory FFT", Nf);
+  const size_t nsamp = (size_t)Nt * N, npix = (size_t)Nt * Nf;
+  void* tmp[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // x, mask, psd, tables, coeff, weight
+  uint8_t* d_gap = nullptr;
+  auto cleanup = [&]() { for (void* t : tmp) if (t) cudaFree(t); if (d_gap) cudaFree(d_gap); };
+#define FE_CUDA(expr)                                                                      \
+  do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { cleanup();                       \
+       return fail(ctx, e_ == cudaErrorMemoryAllocation ? TFS_ENOMEM : TFS_ECUDA,          \
+                   "%s failed: %s", #expr, cudaGetErrorString(e_)); } } while (0)
+  const float* d_x = x;
+  if (!is_device_ptr(x) || ((uintptr_t)x & 7u)) {
+    FE_CUDA(cudaMalloc(&tmp[0], C * nsamp * sizeof(float)));
+    FE_CUDA(cudaMemcpyAsync(tmp[0], x, C * nsamp * sizeof(float), cudaMemcpyDefault, st));
+    d_x = (const float*)tmp[0];
+  }
+  const uint8_t* d_mask = sample_mask;
+  if (sample_mask && !is_device_ptr(sample_mask)) {
+    FE_CUDA(cudaMalloc(&tmp[1], nsamp));
+    FE_CUDA(cudaMemcpyAsync(tmp[1], sample_mask, nsamp, cudaMemcpyHostToDevice, st));
+    d_mask = (const uint8_t*)tmp[1];
+  }
+  const float* d_psd = psd;
+  if (psd && !is_device_ptr(psd)) {
+    FE_CUDA(cudaMalloc(&tmp[2], (size_t)C * Nf * sizeof(float)));
+    FE_CUDA(cudaMemcpyAsync(tmp[2], psd, (size_t)C * Nf * sizeof(float), cudaMemcpyHostToDevice, st));
+    d_psd = (const float*)tmp[2];
+  }
+  FE_CUDA(cudaMalloc(&tmp[3], (size_t)Nf * sizeof(float2) + (size_t)N * sizeof(float)));
+  float2* d_tw = (float2*)tmp[3];
+  float* d_win = (float*)(d_tw + Nf);
+  FE_CUDA(cudaMalloc(&tmp[4], C * npix * sizeof(float2)));
+  FE_CUDA(cudaMalloc(&tmp[5], C * npix * sizeof(float)));
+  FE_CUDA(cudaMalloc((void**)&d_gap, (size_t)Nt));
+  float2* d_coeff = (float2*)tmp[4];
+  float* d_weight = (float*)tmp[5];
+
+  fe_tables_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(d_tw, Nf, d_win, N, tukey_alpha);
+  FE_CUDA(cudaGetLastError());
+  FE_CUDA(cudaFuncSetAttribute(fe_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  fe_fft_kernel<<<dim3((unsigned)Nt, (unsigned)C), kFeThreads, smem, st>>>(d_x, d_win, d_tw, rad, Nt, Nf, d_coeff);
+  FE_CUDA(cudaGetLastError());
+  fe_weight_kernel<<<(unsigned)((C * npix + 255) / 256), 256, 0, st>>>(d_psd, C, Nt, Nf, ctx->DT, d_weight);
+  FE_CUDA(cudaGetLastError());
+  fe_gap_kernel<<<(unsigned)Nt, 256, 0, st>>>(d_mask, N, d_gap);
+  FE_CUDA(cudaGetLastError());
+  ctx->launches += 4;
+  if (coeff_out) FE_CUDA(cudaMemcpyAsync(coeff_out, d_coeff, C * npix * sizeof(float2), cudaMemcpyDefault, st));
+  if (weight_out) FE_CUDA(cudaMemcpyAsync(weight_out, d_weight, C * npix * sizeof(float), cudaMemcpyDefault, st));
+  if (gap_out) FE_CUDA(cudaMemcpyAsync(gap_out, d_gap, (size_t)Nt, cudaMemcpyDefault, st));
+#undef FE_CUDA
+  // the rest is the ordinary upload, from device buffers (it synchronises the stream before returning)
+  const int rc = tfs_upload_data(ctx, (const float*)d_coeff, d_weight, d_gap, stream);
+  cleanup();
   return rc;
 }
 

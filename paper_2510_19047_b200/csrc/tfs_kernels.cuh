@@ -787,15 +787,21 @@ weight_colmax_kernel(const float2* __restrict__ wgt, int Nt, float2* __restrict_
   if (threadIdx.x == 0) colmax[k] = sh[0];
 }
 
+// wa must be zeroed first; grid (ceil(Nt/128), k-slices): weights are >= 0 (or zeroed at upload), so their
+// bit patterns order like integers and atomicMax on them is the float maximum
 __global__ void weight_rowmax_kernel(const float2* __restrict__ wgt, int Nt, int Nf, float2* __restrict__ wa) {
-  const int m = blockIdx.x * blockDim.x + threadIdx.x;                                         // one thread per m
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;
   if (m >= Nt) return;
+  const int per = (Nf + gridDim.y - 1) / gridDim.y;
+  const int k0 = blockIdx.y * per, k1 = min(k0 + per, Nf);
   float2 mx = make_float2(0.f, 0.f);
-  for (int k = 0; k < Nf; ++k) {
+  for (int k = k0; k < k1; ++k) {
     const float2 w = wgt[(size_t)k * Nt + m];
     mx.x = fmaxf(mx.x, w.x); mx.y = fmaxf(mx.y, w.y);
   }
-  wa[m] = mx;
+  int* out = reinterpret_cast<int*>(wa + m);
+  atomicMax(out, __float_as_int(fmaxf(mx.x, 0.f)));
+  atomicMax(out + 1, __float_as_int(fmaxf(mx.y, 0.f)));
 }
 
 // one block: gmax = max_k colmax[k]; wb[k] = colmax[k] / gmax (0 where gmax = 0); counts[1] += #{b' != 1}

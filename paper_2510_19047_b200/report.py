@@ -3,6 +3,7 @@
     python -m paper_2510_19047_b200.report track-width     # configs[3]: throughput vs track width
     python -m paper_2510_19047_b200.report nseg            # configs[2]: N_seg swept over {1, 4, 16, 64}
     python -m paper_2510_19047_b200.report ladder          # configs[4]: the 64 -> 16 -> 4 -> 1 ladder at full size
+    python -m paper_2510_19047_b200.report frontend        # NEXT-2: time series -> TF grid at the 2-year-shaped size
 
 Uses only the public binding (api.Tfs) and the seeded generators (synth); timing with CUDA events on
 the current stream after warm-up, inputs resident on the device.  bench.py prints the headline line;
@@ -140,6 +141,39 @@ def ladder_report():
     ctx.destroy()
 
 
+def frontend_report():
+    """tfs_upload_timeseries at the cfg3 size (2 channels x 4096 tranches x 6144 samples), device-resident input.
+    The call = window + FFT + weights + gap mask (4 kernels) followed by the ordinary upload (pack, valid list,
+    weight analysis) and a stream synchronisation.  Bytes that must cross HBM: read x, write and re-read D and W,
+    write the packed grid and weights."""
+    import torch
+    from . import api, synth
+    torch.cuda.set_device(0)
+    w = synth.WORKLOADS["cfg3"]
+    x, mask, psd = synth.make_timeseries(w)
+    dev = torch.device("cuda:0")
+    tx, tm, tp = torch.from_numpy(x).to(dev), torch.from_numpy(mask).to(dev), torch.from_numpy(psd).to(dev)
+    ctx = api.Tfs(w.Nt, w.Nf, w.dt)
+    for _ in range(2):
+        ctx.upload_timeseries(tx, tm, tp, 0.1)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = 5
+    e0.record()
+    for _ in range(reps):
+        ctx.upload_timeseries(tx, tm, tp, 0.1)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    npix = 2 * w.Nt * w.Nf
+    mandatory = x.nbytes + mask.nbytes + 2 * (npix * 8 + npix * 4) + npix * 8 + npix * 4
+    print(f"# NEXT-2 front end at the cfg3 size: {w.Nt} tranches x {2 * w.Nf} samples x 2 channels\n")
+    print(f"tfs_upload_timeseries (device input, Tukey 0.1, PSD weights, gap mask; includes the ordinary upload and "
+          f"its synchronisation): {ms:.2f} ms per call; {mandatory / 1e9:.2f} GB must cross HBM "
+          f"({mandatory / ms / 1e6:.0f} GB/s); weight structure {ctx.weight_structure()}, "
+          f"{x.shape[1] * 2 / ms / 1e6:.1f} G samples/s")
+    ctx.destroy()
+
+
 if __name__ == "__main__":
     what = sys.argv[1] if len(sys.argv) > 1 else ""
     if what == "track-width":
@@ -148,5 +182,7 @@ if __name__ == "__main__":
         nseg()
     elif what == "ladder":
         ladder_report()
+    elif what == "frontend":
+        frontend_report()
     else:
         sys.exit(__doc__)

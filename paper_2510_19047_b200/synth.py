@@ -170,3 +170,35 @@ def injection_params(w: Workload):
             v = np.array([T[0].real, T[0].imag, T[1].real, T[1].imag])
         out.append((np.array([mc, tc_yr * YEAR_S, phic, v[0], v[1], v[2], v[3], 1.0]), rho))
     return out
+
+
+def make_timeseries(w: Workload, seed=None):
+    """Seeded real time series for the front end (tfs_upload_timeseries): x [2][Nt*2*Nf] float32 at cadence dt
+    (white Gaussian noise of unit variance plus a few steady tones at frequencies that do not sit on a bin),
+    a sample-validity mask [Nt*2*Nf] uint8 (6-hour gaps at random times adding up to 15 % of the samples, as
+    in the paper's gap experiment P:297, plus a few short gaps inside tranches) and a smooth one-sided PSD model [2][Nf] (white level 2*dt with a red rise below
+    5 mHz).  Inputs only: no window, no transform, no weights are formed here."""
+    rng = np.random.default_rng((w.seed if seed is None else seed) + 3000)
+    N = 2 * w.Nf
+    ns = w.Nt * N
+    x = rng.standard_normal((2, ns)).astype(np.float32)
+    t = np.arange(ns, dtype=np.float64) * w.dt
+    for a in range(2):
+        for j in range(3):
+            f = (0.13 + 0.27 * j + 0.05 * a) * 0.5 / w.dt * 0.9          # inside (0, Nyquist)
+            x[a] += (3.0 / (1 + j) * np.cos(2 * np.pi * f * t + 0.3 * j + a)).astype(np.float32)
+    mask = np.ones(ns, dtype=np.uint8)
+    if w.gaps:
+        # the paper's gap experiment (P:297): 6-hour gaps at random times, 15 % of the samples in total
+        glen = max(1, int(round(6 * 3600.0 / w.dt)))
+        for s in rng.integers(0, ns, size=max(1, int(round(0.15 * ns / glen)))):
+            mask[s: s + glen] = 0
+    for m in rng.choice(w.Nt, size=max(1, w.Nt // 16), replace=False):    # short gaps inside a tranche
+        s = int(rng.integers(0, max(1, N - 8)))
+        mask[m * N + s: min(m * N + s + int(rng.integers(1, 8)), (m + 1) * N)] = 0
+    fk = np.arange(w.Nf) * w.df
+    with np.errstate(divide="ignore"):
+        S = 2.0 * w.dt * (1.0 + (5e-3 / fk) ** 4)
+    S[0] = np.inf
+    psd = np.stack([S, 1.7 * S]).astype(np.float32)
+    return x, mask, psd
