@@ -539,6 +539,8 @@ int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_ma
     for (int pi = 0; pi < 4; ++pi)
       while (L % primes[pi] == 0 && rad.n < kFeMaxStages) { rad.r[rad.n++] = primes[pi]; L /= primes[pi]; }
     if (L != 1) return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: Nf = %d must factor into 2, 3 and 5", Nf);
+    int Ns = 1;
+    for (int s = 0; s < rad.n; ++s) { rad.off[s] = rad.total; rad.total += (rad.r[s] - 1) * Ns; Ns *= rad.r[s]; }
   }
   const size_t smem = 2 * (size_t)Nf * sizeof(float2);
   if (smem > 200 * 1024) return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: Nf = %d is too long for the shared-memory FFT", Nf);
@@ -568,16 +570,16 @@ int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_ma
     FE_CUDA(cudaMemcpyAsync(tmp[2], psd, (size_t)C * Nf * sizeof(float), cudaMemcpyHostToDevice, st));
     d_psd = (const float*)tmp[2];
   }
-  FE_CUDA(cudaMalloc(&tmp[3], (size_t)Nf * sizeof(float2) + (size_t)N * sizeof(float)));
+  FE_CUDA(cudaMalloc(&tmp[3], (size_t)(rad.total + 2) * sizeof(float2) + (size_t)N * sizeof(float)));
   float2* d_tw = (float2*)tmp[3];
-  float* d_win = (float*)(d_tw + Nf);
+  float* d_win = (float*)(d_tw + rad.total + 2);
   FE_CUDA(cudaMalloc(&tmp[4], C * npix * sizeof(float2)));
   FE_CUDA(cudaMalloc(&tmp[5], C * npix * sizeof(float)));
   FE_CUDA(cudaMalloc((void**)&d_gap, (size_t)Nt));
   float2* d_coeff = (float2*)tmp[4];
   float* d_weight = (float*)tmp[5];
 
-  fe_tables_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(d_tw, Nf, d_win, N, tukey_alpha);
+  fe_tables_kernel<<<(unsigned)((std::max(N, rad.total) + 255) / 256), 256, 0, st>>>(d_tw, rad, d_win, N, tukey_alpha);
   FE_CUDA(cudaGetLastError());
   FE_CUDA(cudaFuncSetAttribute(fe_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   fe_fft_kernel<<<dim3((unsigned)Nt, (unsigned)C), kFeThreads, smem, st>>>(d_x, d_win, d_tw, rad, Nt, Nf, d_coeff);

@@ -15,18 +15,26 @@
 namespace tfs {
 
 constexpr int kFeMaxStages = 24;
-struct FeRadices { int n; int r[kFeMaxStages]; };
+// radices of the stages, and for each stage the offset of its twiddle block in the table: stage s (radix R,
+// Ns = product of the earlier radices) owns (R-1)*Ns entries, entry (t-1)*Ns + k = exp(-2 pi i t k / (Ns R)),
+// so that consecutive butterflies (consecutive k) read consecutive twiddles
+struct FeRadices { int n; int r[kFeMaxStages]; int off[kFeMaxStages]; int total; };
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
   return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
 
-// tw[q] = exp(-2 pi i q / L), q = 0 ... L-1;  win[n] = Tukey(N, alpha)[n] (symmetric form), both from fp64
-__global__ void fe_tables_kernel(float2* __restrict__ tw, int L, float* __restrict__ win, int N, double alpha) {
+// per-stage twiddle blocks (see FeRadices) and win[n] = Tukey(N, alpha)[n] (symmetric form), both from fp64
+__global__ void fe_tables_kernel(float2* __restrict__ tw, const FeRadices rad, float* __restrict__ win, int N,
+                                 double alpha) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < L) {
+  if (i < rad.total) {
+    int st = 0, Ns = 1;
+    while (st + 1 < rad.n && i >= rad.off[st + 1]) { Ns *= rad.r[st]; ++st; }
+    const int e = i - rad.off[st];
+    const int t = e / Ns + 1, k = e - (t - 1) * Ns;
     double s, c;
-    sincospi(-2.0 * (double)i / (double)L, &s, &c);
+    sincospi(-2.0 * (double)t * (double)k / ((double)Ns * (double)rad.r[st]), &s, &c);
     tw[i] = make_float2((float)c, (float)s);
   }
   if (i < N) {
@@ -79,25 +87,31 @@ __device__ __forceinline__ void small_dft(float2* v) {
   }
 }
 
-// one Stockham stage of radix R: Ns = product of the radices of the stages already done
+// shared-memory index swizzle: XOR the low 4 bits with the next 4.  Consecutive elements stay a permutation
+// of their aligned block of 16 (conflict-free loads), while the strided stores of the first stages
+// (out[4 j + t], out[16 a + b + 4 t]) spread over the banks: 2304 -> 1344 store wavefronts per transform at
+// L = 3072 (1152 is the minimum).  smask = 15 when L is a multiple of 16, else 0 (no swizzle).
+__device__ __forceinline__ int fe_swz(int e, int smask) { return e ^ ((e >> 4) & smask); }
+
+// one Stockham stage of radix R: Ns = product of the radices of the stages already done, tw = this stage's
+// twiddle block
 template <int R>
 __device__ __forceinline__ void stockham_stage(const float2* __restrict__ in, float2* __restrict__ out, int L, int Ns,
-                                               const float2* __restrict__ tw) {
+                                               const float2* __restrict__ tw, int smask) {
   const int LR = L / R;
-  const int tstep = L / (Ns * R);
   const bool pow2 = (Ns & (Ns - 1)) == 0;        // the host puts the odd radices last, so this is the usual case
   for (int j = threadIdx.x; j < LR; j += blockDim.x) {
     const int k = pow2 ? (j & (Ns - 1)) : (j % Ns);
     float2 v[R];
 #pragma unroll
     for (int t = 0; t < R; ++t) {
-      v[t] = in[j + t * LR];
-      if (t > 0 && k > 0) v[t] = cmul(v[t], __ldg(tw + t * k * tstep));
+      v[t] = in[fe_swz(j + t * LR, smask)];
+      if (t > 0) v[t] = cmul(v[t], __ldg(tw + (t - 1) * Ns + k));
     }
     small_dft<R>(v);
     const int j0 = (j - k) * R + k;
 #pragma unroll
-    for (int t = 0; t < R; ++t) out[j0 + t * Ns] = v[t];
+    for (int t = 0; t < R; ++t) out[fe_swz(j0 + t * Ns, smask)] = v[t];
   }
 }
 
@@ -117,18 +131,19 @@ fe_fft_kernel(const float* __restrict__ x, const float* __restrict__ win, const 
   float2* nxt = fe_smem + L;
   const float2* xs = reinterpret_cast<const float2*>(x + ((size_t)a * Nt + m) * N);      // N is even: 8-byte aligned
   const float2* ws = reinterpret_cast<const float2*>(win);
+  const int smask = (L & 15) == 0 ? 15 : 0;
   for (int n = threadIdx.x; n < L; n += blockDim.x) {
     const float2 s = __ldg(xs + n), w = __ldg(ws + n);
-    cur[n] = make_float2(s.x * w.x, s.y * w.y);
+    cur[fe_swz(n, smask)] = make_float2(s.x * w.x, s.y * w.y);
   }
   __syncthreads();
   int Ns = 1;
   for (int st = 0; st < rad.n; ++st) {
     const int R = rad.r[st];
-    if (R == 4) stockham_stage<4>(cur, nxt, L, Ns, tw);
-    else if (R == 2) stockham_stage<2>(cur, nxt, L, Ns, tw);
-    else if (R == 3) stockham_stage<3>(cur, nxt, L, Ns, tw);
-    else stockham_stage<5>(cur, nxt, L, Ns, tw);
+    if (R == 4) stockham_stage<4>(cur, nxt, L, Ns, tw + rad.off[st], smask);
+    else if (R == 2) stockham_stage<2>(cur, nxt, L, Ns, tw + rad.off[st], smask);
+    else if (R == 3) stockham_stage<3>(cur, nxt, L, Ns, tw + rad.off[st], smask);
+    else stockham_stage<5>(cur, nxt, L, Ns, tw + rad.off[st], smask);
     Ns *= R;
     __syncthreads();
     float2* t = cur; cur = nxt; nxt = t;
@@ -136,7 +151,7 @@ fe_fft_kernel(const float* __restrict__ x, const float* __restrict__ win, const 
   const float invN = 1.0f / (float)N;
   float2* out = coeff_out + ((size_t)a * Nt + m) * Nf;
   for (int k = threadIdx.x; k < L; k += blockDim.x) {
-    const float2 zk = cur[k], zc = cur[k == 0 ? 0 : L - k];
+    const float2 zk = cur[fe_swz(k, smask)], zc = cur[fe_swz(k == 0 ? 0 : L - k, smask)];
     const float2 E = make_float2(0.5f * (zk.x + zc.x), 0.5f * (zk.y - zc.y));      // (Z[k] + conj Z[L-k]) / 2
     const float2 O = make_float2(0.5f * (zk.x - zc.x), 0.5f * (zk.y + zc.y));      // (Z[k] - conj Z[L-k]) / 2
     float s, c;
