@@ -428,3 +428,21 @@ def test_sub_batches_match_separate_calls(api):
     assert np.array_equal(whole, np.concatenate(parts))
     assert (whole > 0).sum() > 100_000
     ctx.destroy()
+
+
+def test_eval_is_bitwise_reproducible(api):
+    """Work items are claimed dynamically, but every partial has one writer and the sums have a fixed order:
+    repeated calls (and a fresh context) give bit-identical outputs."""
+    w = synth.scaled(synth.WORKLOADS["cfg3"], Nt=700, Nf=1024, n_templates=20_000)
+    coeff, weight, gap = synth.make_data(w)
+    params = synth.make_templates(w)
+    params[:, 1] = np.random.default_rng(8).uniform(0.0, 3.0, len(params)) * w.Nt * w.DT
+    ctx = _mk(api, w, coeff, weight, gap)
+    a = api.eval_host(ctx, params, 16)
+    b = api.eval_host(ctx, params, 16)
+    ctx2 = _mk(api, w, coeff, weight, gap)
+    c = api.eval_host(ctx2, params, 16)
+    for k in ("upsilon", "seg_power", "seg_dh", "seg_hh"):
+        assert np.array_equal(a[k], b[k]) and np.array_equal(a[k], c[k]), k
+    ctx.destroy()
+    ctx2.destroy()
