@@ -60,6 +60,7 @@ struct tfs_ctx {
   void* buf_tk_val = nullptr;   size_t cap_tk_val = 0;
   void* buf_counts = nullptr;   size_t cap_counts = 0;
   void* buf_children = nullptr; size_t cap_children = 0;
+  void* buf_fe = nullptr;       size_t cap_fe = 0;        // front-end temporaries (tfs_upload_timeseries)
   SelectState* sel = nullptr;
 
   // measurement hooks
@@ -455,7 +456,7 @@ void tfs_destroy(tfs_ctx* ctx) {
   for (auto& p : ctx->ev_pool) { cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
   void* bufs[] = {ctx->grid, ctx->wgt, ctx->wa, ctx->wb, ctx->colmax, ctx->wcounts, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut, ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials,
                   ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
-                  ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children};
+                  ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children, ctx->buf_fe};
   for (void* b : bufs) if (b) cudaFree(b);
   free_piece_tables(ctx);
   delete ctx;
@@ -545,46 +546,50 @@ int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_ma
   const size_t smem = 2 * (size_t)Nf * sizeof(float2);
   if (smem > 200 * 1024) return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: Nf = %d is too long for the shared-memory FFT", Nf);
   const size_t nsamp = (size_t)Nt * N, npix = (size_t)Nt * Nf;
-  void* tmp[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // x, mask, psd, tables, coeff, weight
-  uint8_t* d_gap = nullptr;
-  auto cleanup = [&]() { for (void* t : tmp) if (t) cudaFree(t); if (d_gap) cudaFree(d_gap); };
-#define FE_CUDA(expr)                                                                      \
-  do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { cleanup();                       \
-       return fail(ctx, e_ == cudaErrorMemoryAllocation ? TFS_ENOMEM : TFS_ECUDA,          \
-                   "%s failed: %s", #expr, cudaGetErrorString(e_)); } } while (0)
+  // one pooled scratch allocation, kept in the context (a second dataset of the same size costs no cudaMalloc)
+  const bool copy_x = !is_device_ptr(x) || ((uintptr_t)x & 7u);
+  const bool copy_mask = sample_mask && !is_device_ptr(sample_mask);
+  const bool copy_psd = psd && !is_device_ptr(psd);
+  auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
+  const size_t sz[7] = {copy_x ? al(C * nsamp * sizeof(float)) : 0, copy_mask ? al(nsamp) : 0,
+                        copy_psd ? al((size_t)C * Nf * sizeof(float)) : 0, al((size_t)(rad.total + 2) * sizeof(float2)),
+                        al((size_t)N * sizeof(float)), al(C * npix * sizeof(float2)), al(C * npix * sizeof(float))};
+  size_t total = al((size_t)Nt);
+  for (size_t b : sz) total += b;
+  int rc0 = ensure(ctx, &ctx->buf_fe, &ctx->cap_fe, total);
+  if (rc0) return rc0;
+  char* base = (char*)ctx->buf_fe;
+  char* part[8];
+  for (int i = 0; i < 7; ++i) { part[i] = base; base += sz[i]; }
+  part[7] = base;
+#define FE_CUDA(expr) TFS_CUDA(ctx, expr)
   const float* d_x = x;
-  if (!is_device_ptr(x) || ((uintptr_t)x & 7u)) {
-    FE_CUDA(cudaMalloc(&tmp[0], C * nsamp * sizeof(float)));
-    FE_CUDA(cudaMemcpyAsync(tmp[0], x, C * nsamp * sizeof(float), cudaMemcpyDefault, st));
-    d_x = (const float*)tmp[0];
+  if (copy_x) {
+    FE_CUDA(cudaMemcpyAsync(part[0], x, C * nsamp * sizeof(float), cudaMemcpyDefault, st));
+    d_x = (const float*)part[0];
   }
   const uint8_t* d_mask = sample_mask;
-  if (sample_mask && !is_device_ptr(sample_mask)) {
-    FE_CUDA(cudaMalloc(&tmp[1], nsamp));
-    FE_CUDA(cudaMemcpyAsync(tmp[1], sample_mask, nsamp, cudaMemcpyHostToDevice, st));
-    d_mask = (const uint8_t*)tmp[1];
+  if (copy_mask) {
+    FE_CUDA(cudaMemcpyAsync(part[1], sample_mask, nsamp, cudaMemcpyHostToDevice, st));
+    d_mask = (const uint8_t*)part[1];
   }
   const float* d_psd = psd;
-  if (psd && !is_device_ptr(psd)) {
-    FE_CUDA(cudaMalloc(&tmp[2], (size_t)C * Nf * sizeof(float)));
-    FE_CUDA(cudaMemcpyAsync(tmp[2], psd, (size_t)C * Nf * sizeof(float), cudaMemcpyHostToDevice, st));
-    d_psd = (const float*)tmp[2];
+  if (copy_psd) {
+    FE_CUDA(cudaMemcpyAsync(part[2], psd, (size_t)C * Nf * sizeof(float), cudaMemcpyHostToDevice, st));
+    d_psd = (const float*)part[2];
   }
-  FE_CUDA(cudaMalloc(&tmp[3], (size_t)(rad.total + 2) * sizeof(float2) + (size_t)N * sizeof(float)));
-  float2* d_tw = (float2*)tmp[3];
-  float* d_win = (float*)(d_tw + rad.total + 2);
-  FE_CUDA(cudaMalloc(&tmp[4], C * npix * sizeof(float2)));
-  FE_CUDA(cudaMalloc(&tmp[5], C * npix * sizeof(float)));
-  FE_CUDA(cudaMalloc((void**)&d_gap, (size_t)Nt));
-  float2* d_coeff = (float2*)tmp[4];
-  float* d_weight = (float*)tmp[5];
+  float2* d_tw = (float2*)part[3];
+  float* d_win = (float*)part[4];
+  float2* d_coeff = (float2*)part[5];
+  float* d_weight = (float*)part[6];
+  uint8_t* d_gap = (uint8_t*)part[7];
 
   fe_tables_kernel<<<(unsigned)((std::max(N, rad.total) + 255) / 256), 256, 0, st>>>(d_tw, rad, d_win, N, tukey_alpha);
   FE_CUDA(cudaGetLastError());
   FE_CUDA(cudaFuncSetAttribute(fe_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   fe_fft_kernel<<<dim3((unsigned)Nt, (unsigned)C), kFeThreads, smem, st>>>(d_x, d_win, d_tw, rad, Nt, Nf, d_coeff);
   FE_CUDA(cudaGetLastError());
-  fe_weight_kernel<<<(unsigned)((C * npix + 255) / 256), 256, 0, st>>>(d_psd, C, Nt, Nf, ctx->DT, d_weight);
+  fe_weight_kernel<<<dim3((unsigned)((Nf + 255) / 256), (unsigned)Nt, (unsigned)C), 256, 0, st>>>(d_psd, Nt, Nf, ctx->DT, d_weight);
   FE_CUDA(cudaGetLastError());
   fe_gap_kernel<<<(unsigned)Nt, 256, 0, st>>>(d_mask, N, d_gap);
   FE_CUDA(cudaGetLastError());
@@ -594,9 +599,7 @@ int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_ma
   if (gap_out) FE_CUDA(cudaMemcpyAsync(gap_out, d_gap, (size_t)Nt, cudaMemcpyDefault, st));
 #undef FE_CUDA
   // the rest is the ordinary upload, from device buffers (it synchronises the stream before returning)
-  const int rc = tfs_upload_data(ctx, (const float*)d_coeff, d_weight, d_gap, stream);
-  cleanup();
-  return rc;
+  return tfs_upload_data(ctx, (const float*)d_coeff, d_weight, d_gap, stream);
 }
 
 int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* upsilon, float* seg_power,

@@ -161,19 +161,16 @@ fe_fft_kernel(const float* __restrict__ x, const float* __restrict__ win, const 
   }
 }
 
-// W[alpha,m,k] = 4 DT / S_alpha[k] (0 where S is not positive and finite), or 1 without a PSD
-__global__ void fe_weight_kernel(const float* __restrict__ psd, int C, int Nt, int Nf, double DT,
-                                 float* __restrict__ weight_out) {
-  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t total = (size_t)C * Nt * Nf;
-  if (i >= total) return;
+// W[alpha,m,k] = 4 DT / S_alpha[k] (0 where S is not positive and finite), or 1 without a PSD; grid (k blocks, Nt, C)
+__global__ void fe_weight_kernel(const float* __restrict__ psd, int Nt, int Nf, double DT, float* __restrict__ weight_out) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y, a = blockIdx.z;
+  if (k >= Nf) return;
   float w = 1.0f;
   if (psd) {
-    const int k = (int)(i % Nf), a = (int)(i / ((size_t)Nt * Nf));
     const float S = psd[(size_t)a * Nf + k];
     w = (isfinite(S) && S > 0.0f) ? (float)(4.0 * DT / (double)S) : 0.0f;
   }
-  weight_out[i] = w;
+  weight_out[((size_t)a * Nt + m) * Nf + k] = w;
 }
 
 // g[m] = 1 iff every sample of tranche m is valid; one block per tranche
