@@ -23,7 +23,10 @@
  * owns every array it passes and the library never keeps a caller pointer after the call
  * returns (device-pointer work is only ENQUEUED on `stream`: the caller must keep those
  * arrays alive and unchanged until it has synchronised that stream).  Host outputs imply a
- * stream synchronisation inside the call.  A context must not be used from two threads at once.
+ * stream synchronisation inside the call.  A context must not be used from two threads at once, and
+ * its calls share scratch buffers: work enqueued on one stream must have completed (or be ordered
+ * before) the next call on another stream; tfs_upload_data / tfs_upload_timeseries must not be
+ * called while a tfs_eval of the same context is still running.
  */
 #ifndef TFS_H
 #define TFS_H
