@@ -446,3 +446,42 @@ def test_eval_is_bitwise_reproducible(api):
         assert np.array_equal(a[k], b[k]) and np.array_equal(a[k], c[k]), k
     ctx.destroy()
     ctx2.destroy()
+
+
+# --------------------------------------------------------------------------------------------
+# Seeded sweep over odd shapes: grid sizes that are not multiples of anything, random gap masks (including
+# segments with no valid tranche and tiles that end inside a chunk), segment counts that do not divide Nt,
+# every half width from 0 to 12, the three weight structures, banks that start above the band, merge inside
+# the grid or sweep hundreds of bins per tranche.
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("case", range(12))
+def test_seeded_shape_sweep(api, case):
+    rng = np.random.default_rng(1234 + case)
+    Nt = int(rng.integers(33, 420))
+    Nf = int(rng.integers(160, 900))
+    w = synth.scaled(synth.WORKLOADS["cfg2"], Nt=Nt, Nf=Nf, n_templates=28)
+    coeff, _, _ = synth.make_data(w)
+    kind = case % 3
+    if kind == 0:
+        weight = rng.uniform(0.2, 3.0, (2, Nt, Nf)).astype(np.float32)
+    elif kind == 1:
+        weight = (rng.uniform(0.3, 2.0, (2, Nt, 1)) * rng.uniform(0.5, 1.5, (2, 1, Nf))).astype(np.float32)
+    else:
+        weight = np.ascontiguousarray(np.broadcast_to(rng.uniform(0.3, 2.0, (2, Nt, 1)).astype(np.float32), (2, Nt, Nf)))
+    gap = (rng.uniform(size=Nt) > rng.choice([0.0, 0.1, 0.5])).astype(np.uint8)
+    a = int(rng.integers(0, Nt - 8))
+    gap[a:a + int(rng.integers(1, 40))] = 0                                 # one long gap: segments with nothing valid
+    params = synth.make_templates(w)
+    Tobs = Nt * w.DT
+    params[:, 0] = np.exp(rng.uniform(np.log(5.0), np.log(100.0), len(params)))
+    params[:, 1] = rng.uniform(0.02, 2.5, len(params)) * Tobs
+    opts = dict(half_width=int(rng.integers(0, 13)))
+    if case % 4 == 3:
+        opts["adaptive_width"] = 0
+    ctx = _mk(api, w, coeff, weight, gap, **opts)
+    assert ctx.weight_structure() == kind
+    for N_seg in sorted({1, int(rng.integers(2, 12)), int(rng.integers(12, Nt)), Nt}):
+        gpu = api.eval_host(ctx, params, N_seg)
+        ora = oracle_eval(coeff, weight, gap, params, Nt, Nf, w.dt, N_seg, **opts)
+        assert_parity(gpu, ora, N_seg, label=f"sweep case {case} Nt={Nt} Nf={Nf} N_seg={N_seg} {opts}")
+    ctx.destroy()
