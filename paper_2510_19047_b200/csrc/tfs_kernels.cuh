@@ -423,10 +423,10 @@ __device__ __forceinline__ void pixel_loop(const EvalArgs& a, const LaneTrack& L
     // past Wmin are masked
     load_group<0, WMODE>(a, A, idx, stp, kb, kstp, 0, jlast);
     for (int j = 0; j < Wmax; j += 2 * kGroup) {
-      load_group<0, WMODE>(a, B, idx, stp, kb, kstp, j + kGroup, jlast);
+      if (j + kGroup < Wmax) load_group<0, WMODE>(a, B, idx, stp, kb, kstp, j + kGroup, jlast);
       compute_group_auto<MODE, WMODE>(L, C, A, j, Wm, Wmin, Wmax, JA, JB, u, lut_lane, s);
       if (j + kGroup >= Wmax) break;
-      load_group<0, WMODE>(a, A, idx, stp, kb, kstp, j + 2 * kGroup, jlast);
+      if (j + 2 * kGroup < Wmax) load_group<0, WMODE>(a, A, idx, stp, kb, kstp, j + 2 * kGroup, jlast);
       compute_group_auto<MODE, WMODE>(L, C, B, j + kGroup, Wm, Wmin, Wmax, JA, JB, u, lut_lane, s);
     }
   } else {
