@@ -117,7 +117,7 @@ TFS_API int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* s
  *   seg_hh    [n][N_seg]    float   nullable      hh_n
  * 1 <= N_seg <= Nt.  Rows containing NaN/Inf or Mc <= 0 yield zeros and are counted
  * (tfs_bad_param_count), not fatal.  n == 0 is a no-op.  Arithmetic: fp64 track, fp32 pixels,
- * fp32 sums within a piece (<= 256 tranches of one segment), fp64 across pieces and segments, fp32 stores. */
+ * fp32 sums within a piece (<= 512 tranches of one segment), fp64 across pieces and segments, fp32 stores. */
 TFS_API int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg,
              float* upsilon, float* seg_power, float* seg_dh, float* seg_hh, void* stream);
 

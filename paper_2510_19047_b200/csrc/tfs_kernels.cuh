@@ -24,9 +24,9 @@ namespace tfs {
 #endif
 constexpr int kMaxWarpsPerCta = TFS_WARPS_SEPARABLE > TFS_WARPS_GENERAL ? TFS_WARPS_SEPARABLE : TFS_WARPS_GENERAL;
 #ifndef TFS_TILE
-#define TFS_TILE 256
+#define TFS_TILE 512
 #endif
-constexpr int kTileMax = TFS_TILE;       // valid tranches per time tile (8 chunks of 32 lanes)
+constexpr int kTileMax = TFS_TILE;       // valid tranches per time tile (16 chunks of 32 lanes)
 constexpr int kLutN = 512;          // LUT intervals in t = 1/(1+v)
 constexpr double kMtsun = 4.925490947e-6;   // G Msun / c^3 [s]
 constexpr double kPi = 3.14159265358979323846;

@@ -103,8 +103,8 @@ def nseg():
     d = torch.from_numpy(params).to(dev)
     pix = _counts(ctx, torch, d)
     print(f"# configs[2] (cfg3): N_seg sweep, {len(params)} templates, grid {w.Nt} x {w.Nf}, "
-          f"weight structure {ctx.weight_structure()}, {n_valid} valid tranches = {-(-n_valid // 256)} time tiles "
-          f"of 256 for every N_seg\n")
+          f"weight structure {ctx.weight_structure()}, {n_valid} valid tranches = {-(-n_valid // 512)} time tiles "
+          f"of 512 for every N_seg\n")
     print("| N_seg | ms per tfs_eval | templates/s | pixel-evals/s |")
     print("|---:|---:|---:|---:|")
     for N in (1, 4, 16, 64):
