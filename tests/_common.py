@@ -17,12 +17,39 @@ def oracle_eval(coeff, weight, gap, params, Nt, Nf, dt, N_seg, **opts):
     return O.evaluate(params, to_complex(coeff), W, gap, g, N_seg, O.Opts(**opts))
 
 
-def add_injections(coeff, weight, gap, inj_list, Nt, Nf, dt, **opts):
-    """coeff += injected signals (oracle-made, untruncated dense templates); float32 in, float32 out."""
+def oracle_eval_multi(coeff, weight, gap, params, Nt, Nf, dt, N_segs, **opts):
+    """Oracle results for several N_seg at once: the dense template of a row is built once
+    (O.dense_template) and O.segment_products / O.combine run once per N_seg -- the same calls
+    O.evaluate makes, so the values are identical to calling it per N_seg.  Returns {N_seg: dict}."""
+    g = O.Grid(Nt, Nf, dt)
+    o = O.Opts(**opts)
+    D = to_complex(coeff)
+    W = None if weight is None else np.asarray(weight, dtype=np.float64)
+    params = np.atleast_2d(np.asarray(params, dtype=np.float64))
+    n = len(params)
+    out = {N: dict(upsilon=np.zeros(n), seg_power=np.zeros((n, N)), seg_dh=np.zeros((n, N), dtype=np.complex128),
+                   seg_hh=np.zeros((n, N))) for N in N_segs}
+    for i, p in enumerate(params):
+        if not np.all(np.isfinite(p)) or p[0] <= 0:
+            continue
+        Hd = O.dense_template(p[0], p[1], p[2], p[7], g, o, gap, truncate=True)
+        T = np.array([p[3] + 1j * p[4], p[5] + 1j * p[6]])
+        for N in N_segs:
+            z, hh = O.segment_products(Hd, T[: D.shape[0]], D, W, gap, N)
+            P, U = O.combine(z, hh)
+            r = out[N]
+            r["upsilon"][i], r["seg_power"][i], r["seg_dh"][i], r["seg_hh"][i] = U, P, z, hh
+    return out
+
+
+def add_injections(coeff, weight, gap, inj_list, Nt, Nf, dt, truncate=False, **opts):
+    """coeff += injected signals (oracle-made dense templates: untruncated by default; truncate=True keeps
+    only the window that `opts` defines, e.g. half_width=100 at full size where filling every bin of a
+    4096 x 3072 grid takes minutes per signal); float32 in, float32 out."""
     g = O.Grid(Nt, Nf, dt)
     W = None if weight is None else np.asarray(weight, dtype=np.float64)
     for p, rho in inj_list:
-        S = O.injection(p, rho, W, gap, g, O.Opts(**opts))
+        S = O.injection(p, rho, W, gap, g, O.Opts(**opts), truncate=truncate)
         coeff[..., 0] += S.real.astype(np.float32)
         coeff[..., 1] += S.imag.astype(np.float32)
     return coeff

@@ -62,8 +62,8 @@ def test_cfg1_parity(api, cfg1, N_seg):
 
 # --------------------------------------------------------------------------------------------
 # reduced configs[1]/[2]: PSD weights / non-stationary noise + gaps, random bank with ragged tracks
-# (start above band, merge inside the grid, never enter), several tiles, segment counts that do
-# not divide Nt, chunks with a ragged tail
+# (start above band, merge inside the grid, never enter), segment counts that do not divide Nt, chunks
+# with a ragged tail (several time tiles: test_many_tiles_heavy_gaps_parity and the full-size test)
 # --------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("weight_mode", [0, 1])      # 0: separable weights detected, 1: forced general path
 @pytest.mark.parametrize("name,Nt,N_segs", [("cfg2", 300, (16, 7)), ("cfg3", 333, (1, 4, 64, 333))])
@@ -309,64 +309,167 @@ def test_topk_nan_sorts_last(api):
 
 # --------------------------------------------------------------------------------------------
 # BASELINE.json's full size, in the launch configuration bench.py times: the 2-year-shaped grid
-# (Nt = 4096 x Nf = 3072, non-stationary noise, gaps), the 10^6-template bank, N_seg = 16, one
-# tfs_eval call + tfs_topk of the top 1 %.  The dense oracle needs ~1 s per template at this
-# size, so it checks a sample: random rows, the GPU's best rows, and rows that merge inside the grid.
-# Properties that hold at any size cover the rest: Cauchy-Schwarz across N_seg on every row (P8),
-# zeros exactly where the track never enters the band, and tfs_topk against a CPU sort of all 10^6.
+# (Nt = 4096 x Nf = 3072, non-stationary noise, gaps) with the config's three injections planted, the
+# 10^6-template bank (+ the three true-parameter rows), one tfs_eval call per N_seg in {1, 16, 64} and
+# tfs_topk of the top 1 %.  The dense oracle needs ~1 s per template and N_seg at this size, so it checks
+# a sample of >= 64 rows: random active rows, the GPU's top 16, rows that merge inside the grid, the
+# widest tracks and the injections' own parameters.  Properties that hold at any size cover the rest:
+# Cauchy-Schwarz across N_seg on every row (P8), zeros exactly where the track never enters the band, and
+# tfs_topk against a CPU sort of all 10^6.  Then the same bank through the other two weight structures
+# at full size: general per-pixel weights (weight_mode = 1) and separable weights with a b[k] table.
 # --------------------------------------------------------------------------------------------
+def _full_size_gpu(api, ctx, d_params, n, N, want_segments):
+    import torch
+    dev = d_params.device
+    d_ups = torch.empty(n, dtype=torch.float32, device=dev)
+    extra = {}
+    if want_segments:
+        extra = dict(seg_power=torch.empty(n * N, dtype=torch.float32, device=dev),
+                     seg_dh=torch.empty(n * N * 2, dtype=torch.float32, device=dev),
+                     seg_hh=torch.empty(n * N, dtype=torch.float32, device=dev))
+    ctx.eval(d_params, N, d_ups, **extra)
+    torch.cuda.synchronize()
+    return d_ups.cpu().numpy(), extra
+
+
+def _rows(ups, extra, n, N, sample):
+    """Sampled rows (device index tensor `sample`) of device outputs as the dict assert_parity expects."""
+    P = extra["seg_power"].view(n, N)[sample].cpu().numpy()
+    z = extra["seg_dh"].view(n, N, 2)[sample].cpu().numpy()
+    hh = extra["seg_hh"].view(n, N)[sample].cpu().numpy()
+    return dict(upsilon=ups[sample.cpu().numpy()], seg_power=P, seg_dh=z[..., 0] + 1j * z[..., 1], seg_hh=hh)
+
+
 def test_full_size_cfg3_sampled_parity(api):
     import torch
+    from tests._common import oracle_eval_multi
     w = synth.WORKLOADS["cfg3"]
     coeff, weight, gap = synth.make_data(w)
-    params = synth.make_templates(w)
+    inj = synth.injection_params(w)
+    assert len(inj) == 3
+    # the injections: dense templates over a +-100-bin window around the track (> 99.9 % of their power)
+    add_injections(coeff, weight, gap, inj, w.Nt, w.Nf, w.dt, truncate=True, half_width=100)
+    params = np.vstack([synth.make_templates(w)] + [p[None] for p, _ in inj])
     n = len(params)
-    assert (w.Nt, w.Nf, n) == (4096, 3072, 1_000_000)
+    assert (w.Nt, w.Nf, n) == (4096, 3072, 1_000_003)
     ctx = _mk(api, w, coeff, weight, gap)
     assert ctx.weight_structure() == 2
     dev = torch.device("cuda:0")
     d_params = torch.from_numpy(params).to(dev)
-    N_seg = 16
-    ups = {}
-    for N in (16, 64):
-        d_ups = torch.empty(n, dtype=torch.float32, device=dev)
-        extra = {}
-        if N == N_seg:
-            extra = dict(seg_power=torch.empty(n * N, dtype=torch.float32, device=dev),
-                         seg_dh=torch.empty(n * N * 2, dtype=torch.float32, device=dev),
-                         seg_hh=torch.empty(n * N, dtype=torch.float32, device=dev))
-        ctx.eval(d_params, N, d_ups, **extra)
-        torch.cuda.synchronize()
-        ups[N] = d_ups.cpu().numpy()
-        if N == N_seg:
-            full = {k: v.cpu().numpy() for k, v in extra.items()}
-    u16 = ups[16]
-    assert ctx.bad_param_count() == 0
-    assert np.isfinite(u16).all() and (u16 >= 0).all()
-    # P8 on every row: Upsilon_16 <= Upsilon_64 (fp32 outputs: allow rounding)
-    assert (u16 <= ups[64] * (1 + 1e-5) + 1e-4).all()
-    # rows whose track never enters the band are exactly zero, and only those
+    sample_t = None
+    ups, rows = {}, {}
     counts = torch.empty(n, dtype=torch.int64, device=dev)
     ctx.count_pixels(d_params, counts)
     cnt = counts.cpu().numpy()
-    assert ((cnt == 0) == (u16 == 0)).all()
-    # top-k of the whole vector, exactly
-    k = n // 100
-    idx, val = api.topk_host(ctx, u16, k)
-    order = np.lexsort((np.arange(n), -u16.astype(np.float64)))[:k]
-    assert np.array_equal(idx, order) and np.array_equal(val, u16[order])
-    # sampled rows against the dense oracle
-    rng = np.random.default_rng(77)
-    Tobs = w.Nt * w.DT
-    merging = np.flatnonzero((params[:, 1] < Tobs) & (cnt > 0))
-    sample = np.unique(np.concatenate([rng.choice(np.flatnonzero(cnt > 0), 5, replace=False), idx[:3],
-                                       rng.choice(merging, 2, replace=False)]))
-    ora = oracle_eval(coeff, weight, gap, params[sample], w.Nt, w.Nf, w.dt, N_seg)
-    gpu = dict(upsilon=u16[sample], seg_power=full["seg_power"].reshape(n, N_seg)[sample],
-               seg_dh=full["seg_dh"].reshape(n, N_seg, 2)[sample], seg_hh=full["seg_hh"].reshape(n, N_seg)[sample])
-    gpu["seg_dh"] = gpu["seg_dh"][..., 0] + 1j * gpu["seg_dh"][..., 1]
-    r = assert_parity(gpu, ora, N_seg, label="cfg3 full size, sampled rows")
-    assert r["n_active"] == len(sample)
+    for N in (16, 1, 64):
+        ups[N], extra = _full_size_gpu(api, ctx, d_params, n, N, True)
+        if sample_t is None:
+            # the sample (chosen once, from the N_seg = 16 run): 40 random active rows, the GPU's top 16,
+            # 6 rows that merge inside the grid, the 4 rows with the most window pixels per active tranche
+            # (widest tracks), and the three injections' own parameters
+            k = n // 100
+            idx, val = api.topk_host(ctx, ups[16], k)
+            order = np.lexsort((np.arange(n), -ups[16].astype(np.float64)))[:k]
+            assert np.array_equal(idx, order) and np.array_equal(val, ups[16][order])
+            rng = np.random.default_rng(77)
+            Tobs = w.Nt * w.DT
+            active = np.flatnonzero(cnt > 0)
+            merging = np.flatnonzero((params[:, 1] < Tobs) & (cnt > 0))
+            widest = active[np.argsort(-cnt[active] / np.maximum(np.minimum(params[active, 1], Tobs) / w.DT, 1.0))[:4]]
+            sample = np.unique(np.concatenate([rng.choice(active, 40, replace=False), idx[:16],
+                                               rng.choice(merging, 6, replace=False), widest,
+                                               np.arange(n - 3, n)]))
+            assert len(sample) >= 64
+            sample_t = torch.from_numpy(sample).to(dev)
+        rows[N] = _rows(ups[N], extra, n, N, sample_t)
+        del extra
+    assert ctx.bad_param_count() == 0
+    u1, u16, u64 = ups[1], ups[16], ups[64]
+    assert np.isfinite(u16).all() and (u16 >= 0).all()
+    # P8 on every row: Upsilon_1 <= Upsilon_16 <= Upsilon_64 (fp32 outputs: allow rounding)
+    assert (u1 <= u16 * (1 + 1e-5) + 1e-4).all() and (u16 <= u64 * (1 + 1e-5) + 1e-4).all()
+    # rows whose track never enters the band are exactly zero, and only those
+    assert ((cnt == 0) == (u16 == 0)).all() and ((cnt == 0) == (u1 == 0)).all()
+    # sampled rows against the dense oracle, N_seg = 1, 16, 64
+    ora = oracle_eval_multi(coeff, weight, gap, params[sample], w.Nt, w.Nf, w.dt, (1, 16, 64))
+    for N in (1, 16, 64):
+        r = assert_parity(rows[N], ora[N], N, label=f"cfg3 full size, {len(sample)} sampled rows, N_seg={N}")
+        assert r["n_active"] == len(sample)
+    # the injections are recovered at their true parameters (P:104: Upsilon_N ~ non-central chi^2 with 2N
+    # degrees of freedom and non-centrality ~ rho^2 x duty cycle; the planted signal lost its gap tranches
+    # before scaling, so the non-centrality is rho^2 up to the template's truncation), and they top the bank
+    for j, (p, rho) in enumerate(inj):
+        i = n - 3 + j
+        for N in (1, 16, 64):
+            lam = rho * rho
+            assert abs(ups[N][i] - (lam + 2 * N)) < 5 * np.sqrt(4 * N + 4 * lam) + 0.03 * lam, (j, N, ups[N][i])
+    assert set(idx[:2]) <= {n - 3, n - 2, n - 1}           # rho = 25 and 15 lead at N_seg = 16
+    ctx.destroy()
+    # ---- the other weight structures at full size, N_seg = 16, 16 sampled rows each ----
+    sub = np.unique(np.concatenate([sample[::6], np.arange(n - 3, n)]))[:16]
+    sub_t = torch.from_numpy(sub).to(dev)
+    # (a) the same data through the general per-pixel path
+    ctx = _mk(api, w, coeff, weight, gap, weight_mode=1)
+    assert ctx.weight_structure() == 0
+    u, extra = _full_size_gpu(api, ctx, d_params, n, 16, True)
+    assert_parity(_rows(u, extra, n, 16, sub_t), {k: v[np.searchsorted(sample, sub)] for k, v in ora[16].items()}, 16,
+                  label="cfg3 full size, weight_mode=1")
+    # the two paths agree on every row (same arithmetic up to where the weight is applied)
+    assert np.max(np.abs(u - u16) / np.maximum(u16, 32.0)) < 2e-5
+    del extra
+    ctx.destroy()
+    # (b) a cfg2-style PSD shape b[k] on top of the per-tranche levels: separable with a b table
+    fk = np.arange(w.Nf) * w.df
+    with np.errstate(divide="ignore"):
+        b = (1.0 / (1.0 + (5e-3 / fk) ** 4)).astype(np.float32)
+    weight_b = weight * b[None, None, :]
+    ctx = _mk(api, w, coeff, weight_b, gap)
+    assert ctx.weight_structure() == 1
+    u, extra = _full_size_gpu(api, ctx, d_params, n, 16, True)
+    ora_b = oracle_eval(coeff, weight_b, gap, params[sub], w.Nt, w.Nf, w.dt, 16)
+    assert_parity(_rows(u, extra, n, 16, sub_t), ora_b, 16, label="cfg3 full size, separable b[k] weights")
+    ctx.destroy()
+
+
+# --------------------------------------------------------------------------------------------
+# Several time tiles at the default tile length, against the oracle: Nt = 1400 with a heavy random gap
+# mask (tiles and chunks end anywhere, segments with no valid tranche, pieces of one tranche), N_seg in
+# {1, 7, 64, Nt}, the three weight structures, 48 rows that start above the band, merge inside the grid
+# or cross the whole grid.
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", ["time", "product", "general"])
+def test_many_tiles_heavy_gaps_parity(api, kind):
+    Nt, Nf = 1400, 512
+    w = synth.scaled(synth.WORKLOADS["cfg3"], Nt=Nt, Nf=Nf, n_templates=48)
+    coeff, _, _ = synth.make_data(w)
+    rng = np.random.default_rng(4242)
+    a = rng.uniform(0.3, 2.0, (2, Nt, 1)).astype(np.float32)
+    b = rng.uniform(0.5, 1.5, (2, 1, Nf)).astype(np.float32)
+    if kind == "time":
+        weight, code = np.ascontiguousarray(np.broadcast_to(a, (2, Nt, Nf))), 2
+    elif kind == "product":
+        weight, code = (a * b).astype(np.float32), 1
+    else:
+        weight, code = rng.uniform(0.2, 3.0, (2, Nt, Nf)).astype(np.float32), 0
+    gap = (rng.uniform(size=Nt) > 0.35).astype(np.uint8)              # 35 % of the tranches masked at random
+    for s, l in ((100, 90), (700, 33), (1290, 70)):                    # plus long gaps (whole segments empty)
+        gap[s:s + l] = 0
+    Tobs = Nt * w.DT
+    params = synth.make_templates(w)
+    params[:, 0] = np.exp(rng.uniform(np.log(8.0), np.log(100.0), len(params)))
+    params[:, 1] = rng.uniform(0.05, 4.0, len(params)) * Tobs
+    inj = [(np.array([40.0, 1.7 * Tobs, 0.4, 0.5, 0.2, -0.3, 0.6, 1.0]), 18.0)]
+    add_injections(coeff, weight, gap, inj, Nt, Nf, w.dt)
+    params = np.vstack([params, inj[0][0][None]])
+    ctx = _mk(api, w, coeff, weight, gap)
+    assert ctx.weight_structure() == code
+    from tests._common import oracle_eval_multi
+    N_segs = (1, 7, 64, Nt)
+    ora = oracle_eval_multi(coeff, weight, gap, params, Nt, Nf, w.dt, N_segs)
+    for N_seg in N_segs:
+        gpu = api.eval_host(ctx, params, N_seg)
+        r = assert_parity(gpu, ora[N_seg], N_seg, label=f"many tiles, {kind} weights, N_seg={N_seg}")
+        assert r["n_active"] >= 30
     ctx.destroy()
 
 
