@@ -24,7 +24,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2510_19047_b200 import synth  # noqa: E402
+from paper_2510_19047_b200 import replicas, synth  # noqa: E402
 
 # Algorithmic bytes per pixel-eval: 8 B complex fp32 datum + 4 B weight
 # when the weights are a general per-pixel array; 8 B when they are separable W[a,m,k] = a[m] b[k]
@@ -36,6 +36,7 @@ ALG_BYTES_PER_PIXEL_EVAL = {0: 12.0, 1: 8.0, 2: 8.0}
 # z_A, z_E (4 packed: 8), |h'|^2 and q (1 packed: 2), u + c and u - 1 (2)  ->  36; + 2 MUFU.RCP (own pipe).
 ALG_LANE_OPS_PER_PIXEL = 36.0
 SM_LANES = 128                       # lane-instructions issued per SM per clock (4 schedulers x 32 lanes)
+SMEM_BYTES_PER_CLK = 128             # shared-memory bandwidth per SM per clock (B300_MICROARCH.md: 128/N B/clk/SM)
 
 
 def measured_peaks():
@@ -110,7 +111,42 @@ def _oracle_one(i):
     from oracle import tfs_oracle as O
     d = _ORA
     r = O.evaluate(d["params"][i:i + 1], d["D"], d["W"], d["gap"], d["grid"], d["N_seg"])
-    return float(r["upsilon"][0])
+    return float(r["upsilon"][0]), int((r["seg_hh"][0] > 0).sum())
+
+
+def sparse_cpu_rate(w, coeff, weight, gap, params, N_seg, budget_s=6.0):
+    """The analogue of the paper's single-core CPU curve (Fig. 1): the same statistic evaluated
+    on the track's window pixels only, one template at a time on ONE core, with the oracle's own track,
+    kernel and combine routines (numpy fp64) -- a labelled second CPU line, not the oracle (which sums
+    over every pixel).  Returns (templates/s, templates timed)."""
+    from oracle import tfs_oracle as O
+    g = O.Grid(w.Nt, w.Nf, w.dt)
+    o = O.Opts()
+    seg = O.segment_of_bin(np.arange(w.Nt), w.Nt, N_seg)
+    t0 = time.perf_counter()
+    done = 0
+    for p in params:
+        tr = O.track(p[0], p[1], p[2], p[7], g, o, gap)
+        ms = np.nonzero(tr["active"])[0]
+        z = np.zeros(N_seg, dtype=np.complex128)
+        hh = np.zeros(N_seg)
+        if ms.size:
+            lo, hi = tr["k_lo"][ms], tr["k_hi"][ms]
+            mm = np.repeat(ms, hi - lo + 1)
+            kk = np.concatenate([np.arange(a, b + 1) for a, b in zip(lo, hi)])
+            H = O.kernel_pixels(tr["x"][mm], tr["c"][mm], tr["phi"][mm], tr["A"][mm], kk)
+            T = (p[3] + 1j * p[4], p[5] + 1j * p[6])
+            for a in range(2):
+                D = coeff[a, mm, kk, 0].astype(np.float64) + 1j * coeff[a, mm, kk, 1]
+                Wp = weight[a, mm, kk].astype(np.float64)
+                z += T[a] * (np.bincount(seg[mm], weights=(Wp * np.conj(D) * H).real, minlength=N_seg) +
+                             1j * np.bincount(seg[mm], weights=(Wp * np.conj(D) * H).imag, minlength=N_seg))
+                hh += abs(T[a]) ** 2 * np.bincount(seg[mm], weights=Wp * np.abs(H) ** 2, minlength=N_seg)
+        O.combine(z, hh)
+        done += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    return done / (time.perf_counter() - t0), done
 
 
 def oracle_throughput(w, coeff, weight, gap, params, N_seg, n_sample, procs):
@@ -140,6 +176,67 @@ def host_cores():
         return os.cpu_count() or 1
 
 
+def time_leg(api, torch, ctx, w, d_params, n, N_seg, k_top, steps, warmup, info, dev, sample_clocks):
+    """Device-timed leg: `warmup` untimed steps, then exactly `steps` steps bracketed by barrier + synchronize.
+    Returns dict(ms_step, prof, clocks, d_ups)."""
+    d_ups = torch.empty(n, dtype=torch.float32, device=dev)
+    d_idx = torch.empty(k_top, dtype=torch.int64, device=dev)
+    d_val = torch.empty(k_top, dtype=torch.float32, device=dev)
+
+    def step():
+        ctx.eval(d_params, N_seg, d_ups)
+        ctx.topk(d_ups, k_top, d_idx, d_val)
+
+    def barrier():
+        replicas.barrier(info)
+        torch.cuda.synchronize()
+
+    for _ in range(warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(info.local_rank)
+    if sample_clocks:
+        sampler.start()
+    ctx.set_profiling(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    prof = ctx.get_profile_kernels()
+    ctx.set_profiling(False)
+    clocks = sampler.stop() if sample_clocks else None
+    ms_total = replicas.max_over_ranks(ms_total, info, dev)
+    return dict(ms_step=ms_total / steps, ms_total=ms_total, prof=prof, clocks=clocks, d_ups=d_ups, d_idx=d_idx, d_val=d_val)
+
+
+def roofline_terms(leg, steps, pixels, wstruct, l2_gbs, peaks, peak_src, sm_count, sm_mhz):
+    """The roofline terms of the evaluation kernels (eval_list_kernel + eval_slab_kernel, one pair per step)."""
+    n_launch = max(leg["prof"]["eval_launches"], 1)
+    kern_ms = (leg["prof"]["slab_kernel_ms"] + leg["prof"]["list_kernel_ms"]) / n_launch
+    per_step = n_launch / steps
+    bytes_per_launch = ALG_BYTES_PER_PIXEL_EVAL[wstruct] * 2 * pixels / per_step
+    achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
+    smem_peak = sm_count * SMEM_BYTES_PER_CLK * sm_mhz * 1e6 / 1e9
+    alu_peak = sm_count * SM_LANES * sm_mhz * 1e6 / 1e12           # T lane-instructions / s
+    alu_ach = ALG_LANE_OPS_PER_PIXEL * pixels / per_step / (kern_ms * 1e-3) / 1e12
+    terms = {
+        "l2": {"achieved": achieved, "peak": l2_gbs, "unit": "GB/s", "frac": achieved / l2_gbs,
+               "peak_source": "tfs_probe_l2_bandwidth, 32 MiB buffer, this run (the SM's L1 -> register return path)"},
+        "smem": {"achieved": achieved, "peak": smem_peak, "unit": "GB/s", "frac": achieved / smem_peak,
+                 "peak_source": f"{sm_count} SMs x {SMEM_BYTES_PER_CLK} B/clk x {sm_mhz:.0f} MHz (sampled): where the slab "
+                                "kernel's gathers are served"},
+        "hbm_if_every_gather_missed_l2": {"achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                          "frac": achieved / peaks["hbm_gbs"], "peak_source": peak_src},
+        "alu": {"achieved": alu_ach, "peak": alu_peak, "unit": "T lane-instr/s", "frac": alu_ach / alu_peak,
+                "peak_source": f"{sm_count} SMs x {SM_LANES} lanes x {sm_mhz:.0f} MHz (sampled)"},
+    }
+    return terms, kern_ms, bytes_per_launch
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -151,22 +248,28 @@ def main():
     ap.add_argument("--n-seg", type=int, default=None)
     ap.add_argument("--cpu-sample", type=int, default=None, help="templates timed on the CPU oracle")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-general-leg", action="store_true",
+                    help="skip the second timed leg with general per-pixel weights (weight_mode = 1)")
     ap.add_argument("--weight-mode", type=int, default=0, choices=[0, 1],
-                    help="tfs_opts.weight_mode: 0 = exploit separable weights (default), 1 = general per-pixel path")
+                    help="tfs_opts.weight_mode of the headline leg: 0 = exploit separable weights (default), 1 = general per-pixel path")
     args = ap.parse_args()
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    info = replicas.RankInfo.from_env()
+    rank, world, local_rank = info.rank, info.world, info.local_rank
 
     w = synth.WORKLOADS[args.workload]
     n = args.n_templates or w.n_templates
     N_seg = args.n_seg or w.N_seg
     k_top = max(1, n // 100)
+    grid_bytes = int(w.Nt * w.Nf * 24)
     cfg = {"workload": f"{w.name}: Nt={w.Nt} x Nf={w.Nf} x 2 channels (A,E), dt={w.dt:g} s, noise={w.noise}, "
                        f"gaps={w.gaps}, {n} templates, N_seg={N_seg}, top-k k={k_top}",
-           "grid_bytes": int(w.Nt * w.Nf * 24), "l2": "inputs larger than L2 (grid 302 MB at cfg3 > 126 MB L2)",
-           "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no collective)"}
+           "grid_bytes": grid_bytes,
+           "l2": (f"inputs larger than L2 (grid {grid_bytes / 1e6:.0f} MB + {n * 64 / 1e6:.0f} MB of parameters + the step's "
+                  "partials/lists > 126 MB L2)" if grid_bytes + n * 64 > 126e6 else
+                  f"inputs fit the L2 (grid {grid_bytes / 1e6:.0f} MB): the step's own scratch (partials, item lists) is rewritten "
+                  "every step"),
+           "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no collective), one seeded bank per rank"}
 
     # ---------------- reference arm: the CPU oracle, rank 0 only ----------------
     if args.impl == "reference":
@@ -199,17 +302,24 @@ def main():
 
     # ---------------- our arm ----------------
     coeff, weight, gap = synth.make_data(w)
-    params = synth.make_templates(w, n)
+    # every rank its own seeded bank (rank 0 = the 1-GPU bank)
+    params = synth.make_templates(w, n, seed=replicas.bank_seed(w.seed, rank))
 
     cpu_baseline = None
+    ora = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cores = host_cores()
         procs = max(1, min(cores, 16))
-        ns = args.cpu_sample or 12 * procs      # ~10-30 s of CPU work at cfg3
-        r, dt, ups_cpu = oracle_throughput(w, coeff, weight, gap, params[:ns], N_seg, ns, procs)   # before CUDA init
+        ns = args.cpu_sample or 64 * procs      # ~60 s of CPU work at cfg3 on 16 cores (why not 4096)
+        r, dt, ora = oracle_throughput(w, coeff, weight, gap, params[:ns], N_seg, ns, procs)   # before CUDA init
+        sp_rate, sp_n = sparse_cpu_rate(w, coeff, weight, gap, params[:ns], N_seg)
         cpu_baseline = {"value": r, "unit": "templates/s", "cores": procs, "kind": "oracle",
                         "sample": f"first {ns} templates of the bank, {dt:.1f} s wall (dense fp64 oracle, {procs} "
-                                  f"processes of {cores} cores)"}
+                                  f"processes of {cores} cores)",
+                        "sparse_single_core": {"value": sp_rate, "unit": "templates/s", "cores": 1, "templates": sp_n,
+                                               "what": "window pixels only, one template at a time with the oracle's "
+                                                       "track/kernel routines (analogue of the paper's Fig. 1 CPU "
+                                                       "curve, P:243); not the oracle"}}
 
     import torch
     from paper_2510_19047_b200 import api, build
@@ -217,20 +327,14 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: libtfs has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
+    replicas.init(info, "nccl", dev)
     if rank == 0:
         build.build()
-    if world > 1:
-        dist.barrier()
+    replicas.barrier(info)
 
     ctx = api.Tfs(w.Nt, w.Nf, w.dt, weight_mode=args.weight_mode)
     ctx.upload_data(coeff, weight, gap)
     d_params = torch.from_numpy(params).to(dev)
-    d_ups = torch.empty(n, dtype=torch.float32, device=dev)
-    d_idx = torch.empty(k_top, dtype=torch.int64, device=dev)
-    d_val = torch.empty(k_top, dtype=torch.float32, device=dev)
     counts = torch.empty(n, dtype=torch.int64, device=dev)
     ctx.count_pixels(d_params, counts)
     torch.cuda.synchronize()
@@ -238,39 +342,21 @@ def main():
     pixel_evals = 2 * pixels
     l2_gbs = ctx.probe_l2_bandwidth(32 << 20, 200)
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    warm = max(args.warmup, 3)
 
-    def step():
-        ctx.eval(d_params, N_seg, d_ups)
-        ctx.topk(d_ups, k_top, d_idx, d_val)
+    leg = time_leg(api, torch, ctx, w, d_params, n, N_seg, k_top, args.steps, warm, info, dev, rank == 0)
+    ms_step, clocks, d_ups = leg["ms_step"], leg["clocks"], leg["d_ups"]
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
-        sampler.start()
-    ctx.set_profiling(True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record()
-    for _ in range(args.steps):
-        step()
-    e1.record()
-    barrier()
-    ms_total = e0.elapsed_time(e1)
-    prof = ctx.get_profile()
-    ctx.set_profiling(False)
-    clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    ms_step = ms_total / args.steps
+    # ---------------- parity of the timed output with the oracle values computed above ----------------
+    parity = None
+    if ora is not None:
+        uo = np.array([u for u, _ in ora])
+        neff = np.maximum(np.array([e for _, e in ora]), 1)
+        ug = d_ups[:len(uo)].cpu().numpy().astype(np.float64)
+        err = np.abs(ug - uo) / np.maximum(uo, 2.0 * neff)
+        parity = {"n": int(len(uo)), "max_norm_err": float(err.max()), "tolerance": 1e-4,
+                  "criterion": "C12: |dUpsilon| <= 1e-4 max(Upsilon, 2 N_eff), GPU output of the timed run vs oracle/",
+                  "ok": bool(err.max() <= 1e-4)}
 
     # ---------------- e2e: host buffers through the C ABI, copies inside the timed region ----------------
     h_params = torch.from_numpy(params).pin_memory()
@@ -281,6 +367,10 @@ def main():
     def step_e2e():
         ctx.eval(h_params.numpy(), N_seg, h_ups.numpy())
         ctx.topk(h_ups.numpy(), k_top, h_idx.numpy(), h_val.numpy())
+
+    def barrier():
+        replicas.barrier(info)
+        torch.cuda.synchronize()
 
     step_e2e()
     barrier()
@@ -293,71 +383,87 @@ def main():
     barrier()
     wall_e2e = time.perf_counter() - t0
     ms_e2e = max(e2.elapsed_time(e3), 1e3 * wall_e2e) / args.steps
-    if world > 1:
-        t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
+    ms_e2e = replicas.max_over_ranks(ms_e2e, info, dev)
     same = bool(np.array_equal(h_ups.numpy(), d_ups.cpu().numpy()))
+    wstruct = ctx.weight_structure()
+    launches_total = int(leg["prof"]["kernel_launches"])
+    ctx.destroy()
+
+    # ---------------- second leg: the same bank with general per-pixel weights (12 B per pixel-eval) ----------------
+    general = None
+    if world == 1 and wstruct != 0 and not args.no_general_leg:
+        ctx1 = api.Tfs(w.Nt, w.Nf, w.dt, weight_mode=1)
+        ctx1.upload_data(coeff, weight, gap)
+        leg1 = time_leg(api, torch, ctx1, w, d_params, n, N_seg, k_top, args.steps, warm, info, dev, True)
+        general = (leg1, float(np.max(np.abs(leg1["d_ups"].cpu().numpy() - d_ups.cpu().numpy()) /
+                                      np.maximum(d_ups.cpu().numpy(), 2.0 * N_seg))))
+        ctx1.destroy()
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        replicas.finish(info)
         return 0
 
     peaks, peak_src = measured_peaks()
-    n_launch = max(prof["main_kernel_launches"], 1)
-    kern_ms = prof["main_kernel_ms"] / n_launch                    # per main-kernel launch
-    launches_per_step = n_launch / args.steps
-    wstruct = ctx.weight_structure()
-    bytes_per_launch = ALG_BYTES_PER_PIXEL_EVAL[wstruct] * pixel_evals / launches_per_step
-    achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
-    # roofline terms: the gathers are served by the L2 (tile-major order), so the
-    # byte term is quoted against the L2 read bandwidth probed in this run; the HBM figure is given for
-    # context (what the same bytes would cost if every gather missed the L2); the ALU term is the
-    # algorithmic instruction count against the issue rate at the clock seen during the timed region.
     sm_mhz = (clocks or {}).get("sm_mhz") or peaks.get("sm_max_mhz", 1965.0)
-    alu_peak = sm_count * SM_LANES * sm_mhz * 1e6 / 1e12           # T lane-instructions / s
-    alu_ach = ALG_LANE_OPS_PER_PIXEL * pixels / launches_per_step / (kern_ms * 1e-3) / 1e12
-    terms = {
-        "l2": {"achieved": achieved, "peak": l2_gbs, "unit": "GB/s", "frac": achieved / l2_gbs,
-               "peak_source": "tfs_probe_l2_bandwidth, 32 MiB buffer, this run"},
-        "hbm_if_every_gather_missed_l2": {"achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                                          "frac": achieved / peaks["hbm_gbs"], "peak_source": peak_src},
-        "alu": {"achieved": alu_ach, "peak": alu_peak, "unit": "T lane-instr/s", "frac": alu_ach / alu_peak,
-                "peak_source": f"{sm_count} SMs x {SM_LANES} lanes x {sm_mhz:.0f} MHz (sampled)"},
-    }
-    bound = "l2" if terms["l2"]["frac"] >= terms["alu"]["frac"] else "alu"
+    terms, kern_ms, bytes_per_launch = roofline_terms(leg, args.steps, pixels, wstruct, l2_gbs, peaks, peak_src, sm_count, sm_mhz)
+    # the larger of the byte term -- against the level that serves the gathers: shared memory for the slab
+    # kernel -- and the arithmetic term (BASELINE.json north_star); the L1/L2 and HBM figures are context
+    bound = "smem" if terms["smem"]["frac"] >= terms["alu"]["frac"] else "alu"
+    prof = leg["prof"]
+    n_launch = max(prof["eval_launches"], 1)
     line = {
         "metric": "templates/sec", "value": world * n / (ms_step * 1e-3), "unit": "templates/s",
-        "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
+        "n_gpus": world, "steps": args.steps, "warmup": warm, "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "config": cfg,
         "pixel_evals_per_sec": world * pixel_evals / (ms_step * 1e-3),
         "pixel_evals_per_template": pixel_evals / n,
-        "roofline": {"bound": bound, "kernel": "eval_tiles_kernel", "achieved": terms[bound]["achieved"],
+        "roofline": {"bound": bound, "kernel": "eval_list_kernel + eval_slab_kernel (one pair per step)",
+                     "achieved": terms[bound]["achieved"],
                      "peak": terms[bound]["peak"], "peak_source": terms[bound]["peak_source"],
                      "unit": terms[bound]["unit"], "frac": terms[bound]["frac"], "traffic": None,
                      "algorithmic_bytes_per_launch": bytes_per_launch,
                      "algorithmic_bytes_per_pixel_eval": ALG_BYTES_PER_PIXEL_EVAL[wstruct],
+                     "algorithmic_lane_ops_per_pixel": ALG_LANE_OPS_PER_PIXEL,
                      "weight_structure": wstruct, "kernel_ms_per_launch": kern_ms,
-                     "kernel_share_of_step": prof["main_kernel_ms"] / ms_total, "terms": terms},
+                     "slab_kernel_ms": prof["slab_kernel_ms"] / n_launch, "list_kernel_ms": prof["list_kernel_ms"] / n_launch,
+                     "kernel_share_of_step": (prof["slab_kernel_ms"] + prof["list_kernel_ms"]) / leg["ms_total"],
+                     "terms": terms},
         "cpu_baseline": cpu_baseline,
+        "parity": parity,
         "e2e": {"value": world * n / (ms_e2e * 1e-3), "unit": "templates/s",
                 "h2d_bytes_per_step": int(params.nbytes + h_ups.numpy().nbytes),
                 "d2h_bytes_per_step": int(h_ups.numpy().nbytes + h_idx.numpy().nbytes + h_val.numpy().nbytes),
                 "ms_per_step": ms_e2e, "matches_device_path": same},
-        "gpu_launches": int(prof["kernel_launches"]),
+        "gpu_launches": launches_total,
         "clocks": clocks,
     }
-    extra = os.path.join(ROOT, "profiles", "roofline_traffic.json")      # ncu-derived, committed by hand
+    if general is not None:
+        leg1, dmax = general
+        mhz1 = (leg1["clocks"] or {}).get("sm_mhz") or sm_mhz
+        t1, k1, b1 = roofline_terms(leg1, args.steps, pixels, 0, l2_gbs, peaks, peak_src, sm_count, mhz1)
+        line["general_weights_leg"] = {
+            "what": "the same bank and data with tfs_opts.weight_mode = 1: W read next to every data pixel (12 B per pixel-eval)",
+            "value": n / (leg1["ms_step"] * 1e-3), "unit": "templates/s", "ms_per_step": leg1["ms_step"],
+            "kernel_ms_per_launch": k1, "algorithmic_bytes_per_launch": b1,
+            "frac_smem": t1["smem"]["frac"], "frac_l2": t1["l2"]["frac"], "frac_alu": t1["alu"]["frac"],
+            "max_norm_diff_vs_separable_leg": dmax, "clocks": leg1["clocks"]}
+    extra = os.path.join(ROOT, "profiles", "roofline_traffic.json")      # ncu-derived, committed with the capture
     if os.path.exists(extra):
         try:
-            line["roofline"].update(json.load(open(extra)).get(w.name, {}))
+            t = json.load(open(extra)).get(w.name, {})
+            # the capture is stamped with the hash of the kernel source it was taken at
+            import hashlib
+            src = os.path.join(ROOT, "paper_2510_19047_b200", "csrc", "tfs_kernels.cuh")
+            cur = hashlib.sha256(open(src, "rb").read()).hexdigest()[:16]
+            if t.get("kernel_source_sha256_16") == cur:
+                line["roofline"].update({k: v for k, v in t.items() if k != "kernel_source_sha256_16"})
+            else:
+                line["roofline"].update({"traffic": None, "traffic_stale": True})
         except Exception:
             pass
     print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    replicas.finish(info)
     return 0
 
 

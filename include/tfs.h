@@ -71,8 +71,11 @@ typedef struct {
 TFS_API void tfs_default_opts(tfs_opts* opts);
 
 /* Create a context for an Nt x Nf grid sampled at dt seconds with n_channels TDI channels
- * (this build supports n_channels == 2, the A and E channels).  Uses the current CUDA
- * device.  *out is set to NULL on failure (the reason is then in tfs_last_error(NULL)). */
+ * (Eq. 3 sums alpha = 1..3; the paper uses A, E, T; BASELINE.json's configs use A, E):
+ * n_channels = 1, 2 or 3.  Channels are stored in pairs (0, 1) and (2, -); an odd last channel costs
+ * as much as a pair.  Uses the current CUDA device, which must also be current in every later call on
+ * this context (TFS_ESTATE otherwise).  Nt <= 2000000 and Nt*(Nf+16) < 2^31.
+ * *out is set to NULL on failure (the reason is then in tfs_last_error(NULL)). */
 TFS_API int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const tfs_opts* opts);
 
 /* Upload (copy + repack) the TF data product.
@@ -117,11 +120,27 @@ TFS_API int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* s
  *   seg_hh    [n][N_seg]    float   nullable      hh_n
  * 1 <= N_seg <= Nt.  Rows containing NaN/Inf or Mc <= 0 yield zeros and are counted
  * (tfs_bad_param_count), not fatal.  n == 0 is a no-op.  Arithmetic: fp64 track, fp32 pixels,
- * fp32 sums within a piece (<= 512 tranches of one segment), fp64 across pieces and segments, fp32 stores. */
+ * fp32 sums within a piece (<= 64 tranches of one segment), fp64 across pieces and segments, fp32 stores.
+ * On a 1-channel context T_E is ignored; on a 3-channel context T_T = 0 (see tfs_eval_tf). */
 TFS_API int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg,
              float* upsilon, float* seg_power, float* seg_dh, float* seg_hh, void* stream);
 
-/* Indices and values of the k largest entries of upsilon[0..n), descending; equal values are
+/* The same evaluation with a frequency-dependent transfer factor per template (Eq. 7 and P:213 Eq. 29:
+ * T_alpha(f_nm), "computed once per tranche for all frequency bins"): template i carries, for each of the
+ * context's C channels, a table of n_knots complex values at the frequencies f_knot0 + j*f_knot_step; the factor
+ * of tranche m is the table interpolated linearly at f_m (the tranche-start frequency, C6), held at the end
+ * values outside the knots; n_knots == 1 means one constant per channel.  The columns T_A, T_E of `params` are
+ * then ignored (they must still be finite).  This is also how the third channel gets a transfer factor: tfs_eval
+ * on a 3-channel context uses T_A, T_E of `params` and T_T = 0.
+ *   transfer [n][C][n_knots][2] float (re, im)       host or device, required
+ *   1 <= n_knots <= 65536; f_knot_step > 0 [Hz] when n_knots > 1.
+ * The factors are applied in fp32 once per tranche; everything else is as in tfs_eval. */
+TFS_API int tfs_eval_tf(tfs_ctx* ctx, const double* params, long long n, int N_seg,
+                const float* transfer, int n_knots, double f_knot0, double f_knot_step,
+                float* upsilon, float* seg_power, float* seg_dh, float* seg_hh, void* stream);
+
+/* Top-k of a batch (BASELINE.json north_star (3); the optimiser keeps the best parameter sets of each
+ * iteration).  Indices and values of the k largest entries of upsilon[0..n), descending; equal values are
  * ordered by lower index first; NaN sorts below everything.  1 <= k <= n.
  *   upsilon host or device;  idx [k] int64 and val [k] float, host or device, required. */
 TFS_API int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k,
@@ -154,14 +173,19 @@ TFS_API int tfs_weight_structure(const tfs_ctx* ctx);
 /* Templates rejected (NaN/Inf/Mc<=0) by the most recent tfs_eval on this context. */
 TFS_API long long tfs_bad_param_count(const tfs_ctx* ctx);
 
-/* Measurement hooks (bench.py).  With profiling on, every launch of the main kernel (track +
- * gather + tile sums) inside tfs_eval is bracketed by CUDA events on the caller's stream.
- * tfs_get_profile synchronises those events and returns, since the last call of
- * tfs_set_profiling: the summed duration [ms] and number of main-kernel launches, and the number
- * of kernels of this library launched in total (all entry points).  Any output may be NULL. */
+/* Measurement hooks (bench.py).  With profiling on, the two evaluation kernels (track + gather +
+ * piece sums: eval_list_kernel, which gathers from global memory, then eval_slab_kernel, which reads
+ * TMA-staged shared-memory slabs) of every evaluation launch inside tfs_eval are bracketed by CUDA
+ * events on the caller's stream.  tfs_get_profile_kernels synchronises those events and returns, since
+ * the last call of tfs_set_profiling: the summed durations [ms] of the slab and of the list kernel, the
+ * number of evaluation launches (pairs of kernels), and the number of kernels of this library launched
+ * in total (all entry points).  tfs_get_profile returns the sum of the two durations.  Any output may
+ * be NULL. */
 TFS_API int tfs_set_profiling(tfs_ctx* ctx, int on);
 TFS_API int tfs_get_profile(tfs_ctx* ctx, double* main_kernel_ms, long long* main_kernel_launches,
                             long long* kernel_launches);
+TFS_API int tfs_get_profile_kernels(tfs_ctx* ctx, double* slab_kernel_ms, double* list_kernel_ms,
+                                    long long* eval_launches, long long* kernel_launches);
 
 /* Measurement aid for the roofline (bench.py): allocate a zero-filled scratch buffer of `bytes`
  * (choose it well inside the L2, e.g. 32 MiB), read it `iters` times with coalesced 16-byte loads from

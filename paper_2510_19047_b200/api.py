@@ -53,6 +53,8 @@ def load_library():
     lib.tfs_upload_timeseries.restype = ip
     lib.tfs_eval.argtypes = [vp, vp, ll, ip, vp, vp, vp, vp, vp]
     lib.tfs_eval.restype = ip
+    lib.tfs_eval_tf.argtypes = [vp, vp, ll, ip, vp, ip, dp, dp, vp, vp, vp, vp, vp]
+    lib.tfs_eval_tf.restype = ip
     lib.tfs_topk.argtypes = [vp, vp, ll, ip, vp, vp, vp]
     lib.tfs_topk.restype = ip
     lib.tfs_refine.argtypes = [vp, vp, ll, vp, ll, ip, dp, dp, vp, vp]
@@ -67,6 +69,8 @@ def load_library():
     lib.tfs_set_profiling.restype = ip
     lib.tfs_get_profile.argtypes = [vp, C.POINTER(dp), C.POINTER(ll), C.POINTER(ll)]
     lib.tfs_get_profile.restype = ip
+    lib.tfs_get_profile_kernels.argtypes = [vp, C.POINTER(dp), C.POINTER(dp), C.POINTER(ll), C.POINTER(ll)]
+    lib.tfs_get_profile_kernels.restype = ip
     lib.tfs_probe_l2_bandwidth.argtypes = [vp, ll, ip, C.POINTER(dp), vp]
     lib.tfs_probe_l2_bandwidth.restype = ip
     lib.tfs_destroy.argtypes = [vp]
@@ -151,6 +155,17 @@ class Tfs:
                                        _ptr(seg_dh, np.float32, 2 * n * N_seg),
                                        _ptr(seg_hh, np.float32, n * N_seg), _stream(stream)))
 
+    def eval_tf(self, params, N_seg, transfer, n_knots, f_knot0, f_knot_step, upsilon, seg_power=None, seg_dh=None,
+                seg_hh=None, n=None, stream=None):
+        if n is None:
+            n = (params.size if isinstance(params, np.ndarray) else params.numel()) // PARAM_COLS
+        self._check(self._lib.tfs_eval_tf(self._h, _ptr(params, np.float64, n * PARAM_COLS), n, N_seg,
+                                          _ptr(transfer, np.float32, 2 * n * self.C * n_knots), n_knots,
+                                          float(f_knot0), float(f_knot_step),
+                                          _ptr(upsilon, np.float32, n), _ptr(seg_power, np.float32, n * N_seg),
+                                          _ptr(seg_dh, np.float32, 2 * n * N_seg),
+                                          _ptr(seg_hh, np.float32, n * N_seg), _stream(stream)))
+
     def topk(self, upsilon, k, idx, val, n=None, stream=None):
         if n is None:
             n = upsilon.size if isinstance(upsilon, np.ndarray) else upsilon.numel()
@@ -186,6 +201,11 @@ class Tfs:
         self._check(self._lib.tfs_get_profile(self._h, C.byref(ms), C.byref(nk), C.byref(nl)))
         return dict(main_kernel_ms=ms.value, main_kernel_launches=nk.value, kernel_launches=nl.value)
 
+    def get_profile_kernels(self):
+        a, b, nk, nl = C.c_double(), C.c_double(), C.c_longlong(), C.c_longlong()
+        self._check(self._lib.tfs_get_profile_kernels(self._h, C.byref(a), C.byref(b), C.byref(nk), C.byref(nl)))
+        return dict(slab_kernel_ms=a.value, list_kernel_ms=b.value, eval_launches=nk.value, kernel_launches=nl.value)
+
     def probe_l2_bandwidth(self, nbytes=32 << 20, iters=200, stream=None):
         g = C.c_double()
         self._check(self._lib.tfs_probe_l2_bandwidth(self._h, nbytes, iters, C.byref(g), _stream(stream)))
@@ -207,18 +227,29 @@ class Tfs:
 
 
 # ---- convenience wrappers on host numpy buffers (used by tests, smoke and the e2e bench leg) ----
-def eval_host(ctx: Tfs, params: np.ndarray, N_seg: int, segments: bool = True):
-    """tfs_eval with HOST buffers in and out (the library does the copies)."""
+def eval_host(ctx: Tfs, params: np.ndarray, N_seg: int, segments: bool = True, transfer=None, f_knot0=0.0,
+              f_knot_step=1.0):
+    """tfs_eval (or tfs_eval_tf when a transfer table [n][C][K][2] is given) with HOST buffers in and out
+    (the library does the copies)."""
     params = np.ascontiguousarray(params, dtype=np.float64)
     n = params.shape[0]
     ups = np.empty(n, dtype=np.float32)
+    if transfer is not None:
+        transfer = np.ascontiguousarray(transfer, dtype=np.float32)
+        K = transfer.shape[2]
+
+        def run(*out):
+            ctx.eval_tf(params, N_seg, transfer, K, f_knot0, f_knot_step, *out)
+    else:
+        def run(*out):
+            ctx.eval(params, N_seg, *out)
     if not segments:
-        ctx.eval(params, N_seg, ups)
+        run(ups)
         return dict(upsilon=ups)
     P = np.empty((n, N_seg), dtype=np.float32)
     z = np.empty((n, N_seg, 2), dtype=np.float32)
     hh = np.empty((n, N_seg), dtype=np.float32)
-    ctx.eval(params, N_seg, ups, P, z, hh)
+    run(ups, P, z, hh)
     return dict(upsilon=ups, seg_power=P, seg_dh=z[..., 0] + 1j * z[..., 1], seg_hh=hh)
 
 

@@ -30,16 +30,23 @@ struct tfs_ctx {
   int device = 0, sm_count = 0;
   bool uploaded = false;
 
-  float4* grid = nullptr;
-  float2* wgt = nullptr;
-  float2* wa = nullptr;                    // [Nt] separable weights: a[m]
-  float2* wb = nullptr;                    // [Nf + kPadRows] separable weights: b[k]
+  // channel pairs: pair 0 = channels (0, 1), pair 1 = channel 2 (n_channels = 3); a missing half is zeros
+  struct Pair {
+    float4* grid = nullptr;                // [Nf + kPadRows][ncol_cap]
+    float2* wgt = nullptr;
+    float2* wa = nullptr;                  // [ncol_cap] separable weights: a[i] by valid-tranche index
+    float2* wb = nullptr;                  // [Nf + kPadRows + kSlabRowsMax] separable weights: b[k]
+    int c0 = 0, c1 = -1;                   // channels packed in the pair (-1: empty half)
+    CUtensorMap map_y, map_w;              // TMA descriptors of grid / wgt for the slab kernel (set at upload)
+  } pair[2];
+  int n_pairs = 1;
+  int ncol_cap = 0, ncol = 0;              // columns allocated per row (Nt rounded up to kTS), columns in use
   float2* colmax = nullptr;                // [Nf] scratch of the weight analysis
   unsigned long long* wcounts = nullptr;   // [2] {pixels violating W = a b, columns with b != 1}
   int wmode = -1;                          // kWGeneral / kWSeparable / kWTimeOnly; -1 before the first upload
   int n_valid = 0;                         // valid (non-gap) tranches of the data uploaded last
   // piece tables (tile x segment cuts of the valid-tranche list), cached per N_seg until the next upload
-  struct PieceTable { int N_seg; int n_tiles; int* tile_first; int* piece_end; int* piece_seg; cudaEvent_t ready; };
+  struct PieceTable { int N_seg; int n_tiles; int* tile_first; int* piece_end; int* piece_seg; int* piece_tile; cudaEvent_t ready; };
   std::vector<PieceTable> piece_tables;
   uint8_t* gap = nullptr;
   int* vprefix = nullptr;                  // [Nt+1] valid tranches before m
@@ -47,12 +54,14 @@ struct tfs_ctx {
   float4* lut = nullptr;
   FarCoef far{};
   unsigned long long* bad = nullptr;       // device counter
-  unsigned long long* work = nullptr;      // device work-item counter of the main kernel
+  unsigned long long* work = nullptr;      // [2] device unit counters of the slab and the list kernel
   long long bad_host = 0;
 
   // growable device scratch
   void* buf_params = nullptr;   size_t cap_params = 0;
   void* buf_partials = nullptr; size_t cap_partials = 0;
+  void* buf_prep = nullptr;     size_t cap_prep = 0;      // per-batch pre-pass: constants, keys, bucket tables, lists, units
+  void* buf_ttab = nullptr;     size_t cap_ttab = 0;      // staged transfer table (tfs_eval_tf with a host table)
   void* buf_out[4] = {nullptr, nullptr, nullptr, nullptr}; size_t cap_out[4] = {0, 0, 0, 0};
   void* buf_keys = nullptr;     size_t cap_keys = 0;
   void* buf_tk_in = nullptr;    size_t cap_tk_in = 0;
@@ -65,7 +74,7 @@ struct tfs_ctx {
 
   // measurement hooks
   bool profiling = false;
-  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pool;   // reused event pairs
+  std::vector<cudaEvent_t> ev_pool;        // reused events, three per evaluation launch: start, list kernel done, slab kernel done
   size_t ev_used = 0;
   long long launches = 0;
 
@@ -260,7 +269,7 @@ double fit_far(FarCoef& out) {
 
 void free_piece_tables(tfs_ctx* ctx) {
   for (auto& t : ctx->piece_tables) {
-    cudaFree(t.tile_first); cudaFree(t.piece_end); cudaFree(t.piece_seg);
+    cudaFree(t.tile_first); cudaFree(t.piece_end); cudaFree(t.piece_seg); cudaFree(t.piece_tile);
     if (t.ready) cudaEventDestroy(t.ready);
   }
   ctx->piece_tables.clear();
@@ -277,19 +286,20 @@ int get_piece_table(tfs_ctx* ctx, int N_seg, cudaStream_t st, const tfs_ctx::Pie
   if (ctx->piece_tables.size() >= 64) free_piece_tables(ctx);         // a sweep over many N_seg: start over
   tfs_ctx::PieceTable t{};
   t.N_seg = N_seg;
-  t.n_tiles = std::max(1, (ctx->n_valid + kTileMax - 1) / kTileMax);
+  t.n_tiles = std::max(1, (ctx->n_valid + kTS - 1) / kTS);
   const size_t max_pieces = (size_t)t.n_tiles + (size_t)N_seg;
   cudaError_t e;
   if ((e = cudaMalloc((void**)&t.tile_first, (t.n_tiles + 1) * sizeof(int))) != cudaSuccess ||
       (e = cudaMalloc((void**)&t.piece_end, max_pieces * sizeof(int))) != cudaSuccess ||
       (e = cudaMalloc((void**)&t.piece_seg, max_pieces * sizeof(int))) != cudaSuccess ||
+      (e = cudaMalloc((void**)&t.piece_tile, max_pieces * sizeof(int))) != cudaSuccess ||
       (e = cudaEventCreateWithFlags(&t.ready, cudaEventDisableTiming)) != cudaSuccess) {
     cudaGetLastError();
-    cudaFree(t.tile_first); cudaFree(t.piece_end); cudaFree(t.piece_seg);
+    cudaFree(t.tile_first); cudaFree(t.piece_end); cudaFree(t.piece_seg); cudaFree(t.piece_tile);
     return fail(ctx, TFS_ENOMEM, "piece table allocation failed: %s", cudaGetErrorString(e));
   }
   piece_table_kernel<<<1, 1, 0, st>>>(ctx->vprefix, ctx->valid_m, ctx->Nt, N_seg, ctx->n_valid, t.n_tiles,
-                                      t.tile_first, t.piece_end, t.piece_seg);
+                                      t.tile_first, t.piece_end, t.piece_seg, t.piece_tile);
   ctx->launches += 1;
   e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaEventRecord(t.ready, st);
@@ -299,20 +309,58 @@ int get_piece_table(tfs_ctx* ctx, int N_seg, cudaStream_t st, const tfs_ctx::Pie
   return TFS_OK;
 }
 
-EvalArgs base_args(const tfs_ctx* ctx) {
+EvalArgs base_args(const tfs_ctx* ctx, int pr = 0) {
   EvalArgs a{};
-  a.grid = ctx->grid; a.wgt = ctx->wgt; a.wa = ctx->wa; a.wb = ctx->wb; a.gap = ctx->gap; a.lut = ctx->lut;
+  const tfs_ctx::Pair& P = ctx->pair[pr];
+  a.grid = P.grid; a.wgt = P.wgt; a.wa = P.wa; a.wb = P.wb; a.gap = ctx->gap; a.lut = ctx->lut;
   a.vprefix = ctx->vprefix; a.valid_m = ctx->valid_m;
   a.bad_count = ctx->bad;
   a.work_counter = ctx->work;
-  a.Nt = ctx->Nt; a.Nf = ctx->Nf;
+  a.Nt = ctx->Nt; a.Nf = ctx->Nf; a.ncol = ctx->ncol;
   a.H = ctx->opts.half_width; a.adaptive = ctx->opts.adaptive_width;
   a.DT = ctx->DT;
   a.x_lo = ctx->f_lo * ctx->DT; a.x_hi = ctx->f_hi * ctx->DT;
   a.c_max = ctx->opts.c_max;
   a.far = ctx->far;
-  a.n_valid = ctx->n_valid; a.n_tiles = 1;
+  a.n_valid = ctx->n_valid; a.n_tiles = 1; a.n_keys = 2;
+  a.wmode = ctx->wmode;
+  a.t_col = 3; a.n_ch_pair = P.c1 >= 0 ? 2 : 1;
   return a;
+}
+
+// the context's device must be current (a caller that switched devices would launch on the wrong GPU)
+int check_device(tfs_ctx* ctx, const char* who) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return fail(ctx, TFS_ECUDA, "%s: cudaGetDevice failed", who); }
+  if (dev != ctx->device)
+    return fail(ctx, TFS_ESTATE, "%s: the context was created on device %d but device %d is current", who, ctx->device, dev);
+  return TFS_OK;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// 2-D TMA descriptor over a [rows][ncol] array of `floats_per_pixel` floats per pixel; box = kTS columns x box_rows rows
+int encode_map(tfs_ctx* ctx, CUtensorMap* map, void* base, int floats_per_pixel, int ncol, int rows, int box_rows) {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || !p) {
+      cudaGetLastError();
+      return fail(ctx, TFS_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
+    }
+    fn = (EncodeTiledFn)p;
+  }
+  const cuuint64_t dims[2] = {(cuuint64_t)ncol * floats_per_pixel, (cuuint64_t)rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)ncol * floats_per_pixel * sizeof(float)};
+  const cuuint32_t box[2] = {(cuuint32_t)(kTS * floats_per_pixel), (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(ctx, TFS_ECUDA, "cuTensorMapEncodeTiled failed with code %d", (int)r);
+  return TFS_OK;
 }
 
 // params on host -> staged copy in ctx scratch; on device -> used in place
@@ -366,10 +414,13 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   *out = nullptr;
   if (Nt < 1 || Nf < 2 || !(dt > 0.0) || !std::isfinite(dt))
     return fail(nullptr, TFS_EINVAL, "tfs_create: need Nt >= 1, Nf >= 2, dt > 0 (got %d, %d, %g)", Nt, Nf, dt);
-  if ((long long)Nt * (Nf + kPadRows) >= (1ll << 31))
+  if (Nt > 2000000)        // launch grids carry Nt/32 (pack) and Nt/kTS (pre-pass) on gridDim.y (<= 65535)
+    return fail(nullptr, TFS_EINVAL, "tfs_create: Nt must be <= 2000000 (got %d)", Nt);
+  const int ncol_cap = (Nt + kTS - 1) / kTS * kTS;
+  if ((long long)ncol_cap * (Nf + kPadRows) >= (1ll << 31))
     return fail(nullptr, TFS_EINVAL, "tfs_create: Nt*(Nf+%d) must be < 2^31", kPadRows);
-  if (n_channels != 2)
-    return fail(nullptr, TFS_EINVAL, "tfs_create: this build supports n_channels == 2 (A, E); got %d", n_channels);
+  if (n_channels < 1 || n_channels > 3)
+    return fail(nullptr, TFS_EINVAL, "tfs_create: n_channels must be 1, 2 or 3 (P:76-79 Eq. 3: A, E, T); got %d", n_channels);
   tfs_opts o;
   tfs_default_opts(&o);
   if (opts) o = *opts;
@@ -385,6 +436,11 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   ctx->opts = o;
   ctx->f_lo = o.f_lo > 0.0 ? o.f_lo : ctx->df;
   ctx->f_hi = o.f_hi > 0.0 ? o.f_hi : (Nf - 1) * ctx->df;
+  ctx->ncol_cap = ncol_cap;
+  ctx->ncol = kTS;
+  ctx->n_pairs = n_channels == 3 ? 2 : 1;
+  ctx->pair[0].c0 = 0; ctx->pair[0].c1 = n_channels >= 2 ? 1 : -1;
+  ctx->pair[1].c0 = 2; ctx->pair[1].c1 = -1;
 
   auto bail = [&](int code, const char* what, cudaError_t e) {
     fail(nullptr, code, "tfs_create: %s: %s", what, cudaGetErrorString(e));
@@ -395,28 +451,34 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   if (e != cudaSuccess) return bail(TFS_ECUDA, "cudaGetDevice (no CUDA device: libtfs has no CPU fallback)", e);
   e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
   if (e != cudaSuccess) return bail(TFS_ECUDA, "cudaDeviceGetAttribute", e);
-  // kPadRows zeroed rows behind row Nf-1: the gather may read up to kPrefetch pixels past a window (pixel_loop)
-  const size_t npix = (size_t)Nt * (Nf + kPadRows);
-  if ((e = cudaMalloc((void**)&ctx->grid, npix * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc grid", e);
-  if ((e = cudaMalloc((void**)&ctx->wgt, npix * sizeof(float2))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc weights", e);
-  if ((e = cudaMalloc((void**)&ctx->wa, (size_t)Nt * sizeof(float2))) != cudaSuccess ||
-      (e = cudaMalloc((void**)&ctx->wb, (size_t)(Nf + kPadRows) * sizeof(float2))) != cudaSuccess ||
-      (e = cudaMalloc((void**)&ctx->colmax, (size_t)Nf * sizeof(float2))) != cudaSuccess ||
+  // kPadRows zeroed rows behind row Nf-1: the global gather may read a few pixels past a window (pixel_loop_global)
+  const size_t npix = (size_t)ncol_cap * (Nf + kPadRows);
+  const size_t nwb = (size_t)Nf + kPadRows + kSlabRowsMax;
+  for (int pr = 0; pr < ctx->n_pairs; ++pr) {
+    tfs_ctx::Pair& P = ctx->pair[pr];
+    if ((e = cudaMalloc((void**)&P.grid, npix * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc grid", e);
+    if ((e = cudaMalloc((void**)&P.wgt, npix * sizeof(float2))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc weights", e);
+    if ((e = cudaMalloc((void**)&P.wa, (size_t)ncol_cap * sizeof(float2))) != cudaSuccess ||
+        (e = cudaMalloc((void**)&P.wb, nwb * sizeof(float2))) != cudaSuccess)
+      return bail(TFS_ENOMEM, "cudaMalloc weight factors", e);
+    if ((e = cudaMemset(P.wb, 0, nwb * sizeof(float2))) != cudaSuccess) return bail(TFS_ECUDA, "cudaMemset wb", e);
+  }
+  if ((e = cudaMalloc((void**)&ctx->colmax, (size_t)Nf * sizeof(float2))) != cudaSuccess ||
       (e = cudaMalloc((void**)&ctx->wcounts, 2 * sizeof(unsigned long long))) != cudaSuccess)
-    return bail(TFS_ENOMEM, "cudaMalloc weight factors", e);
-  if ((e = cudaMemset(ctx->wb, 0, (size_t)(Nf + kPadRows) * sizeof(float2))) != cudaSuccess) return bail(TFS_ECUDA, "cudaMemset wb", e);
-  if ((e = cudaMemset(ctx->grid, 0, npix * sizeof(float4))) != cudaSuccess ||
-      (e = cudaMemset(ctx->wgt, 0, npix * sizeof(float2))) != cudaSuccess) return bail(TFS_ECUDA, "cudaMemset grid", e);
+    return bail(TFS_ENOMEM, "cudaMalloc weight analysis", e);
   if ((e = cudaMalloc((void**)&ctx->gap, (size_t)Nt)) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc gap", e);
   if ((e = cudaMalloc((void**)&ctx->vprefix, ((size_t)Nt + 1) * sizeof(int))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc vprefix", e);
-  if ((e = cudaMalloc((void**)&ctx->valid_m, (size_t)Nt * sizeof(int))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc valid_m", e);
+  if ((e = cudaMalloc((void**)&ctx->valid_m, (size_t)ncol_cap * sizeof(int))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc valid_m", e);
   if ((e = cudaMalloc((void**)&ctx->lut, (kLutN + 1) * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc lut", e);
   if ((e = cudaMalloc((void**)&ctx->bad, sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
-  if ((e = cudaMalloc((void**)&ctx->work, sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
-  if ((e = cudaFuncSetAttribute(eval_tiles_kernel<0, kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess ||
-      (e = cudaFuncSetAttribute(eval_tiles_kernel<0, kWSeparable>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess ||
-      (e = cudaFuncSetAttribute(eval_tiles_kernel<0, kWTimeOnly>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess ||
-      (e = cudaFuncSetAttribute(eval_tiles_kernel<1, kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, kEvalSmemBytes)) != cudaSuccess)
+  if ((e = cudaMalloc((void**)&ctx->work, 2 * sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
+  if ((e = cudaFuncSetAttribute(eval_list_kernel<0, kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_list_kernel<0, kWSeparable>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_list_kernel<0, kWTimeOnly>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_list_kernel<1, kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_slab_kernel<kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWGeneral))) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_slab_kernel<kWSeparable>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWSeparable))) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_slab_kernel<kWTimeOnly>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWTimeOnly))) != cudaSuccess)
     return bail(TFS_ECUDA, "cudaFuncSetAttribute(max dynamic shared memory)", e);
   if ((e = cudaMalloc((void**)&ctx->sel, sizeof(SelectState))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc select state", e);
   std::vector<float4> lut;
@@ -436,25 +498,38 @@ int tfs_set_profiling(tfs_ctx* ctx, int on) {
   return TFS_OK;
 }
 
-int tfs_get_profile(tfs_ctx* ctx, double* main_kernel_ms, long long* main_kernel_launches, long long* kernel_launches) {
-  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_get_profile: ctx is NULL");
-  double ms = 0.0;
-  for (size_t i = 0; i < ctx->ev_used; ++i) {
+int tfs_get_profile_kernels(tfs_ctx* ctx, double* slab_kernel_ms, double* list_kernel_ms, long long* eval_launches,
+                            long long* kernel_launches) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_get_profile_kernels: ctx is NULL");
+  double ms_list = 0.0, ms_slab = 0.0;
+  for (size_t i = 0; i + 3 <= ctx->ev_used; i += 3) {
     float t = 0.f;
-    TFS_CUDA(ctx, cudaEventSynchronize(ctx->ev_pool[i].second));
-    TFS_CUDA(ctx, cudaEventElapsedTime(&t, ctx->ev_pool[i].first, ctx->ev_pool[i].second));
-    ms += t;
+    TFS_CUDA(ctx, cudaEventSynchronize(ctx->ev_pool[i + 2]));
+    TFS_CUDA(ctx, cudaEventElapsedTime(&t, ctx->ev_pool[i], ctx->ev_pool[i + 1]));
+    ms_list += t;
+    TFS_CUDA(ctx, cudaEventElapsedTime(&t, ctx->ev_pool[i + 1], ctx->ev_pool[i + 2]));
+    ms_slab += t;
   }
-  if (main_kernel_ms) *main_kernel_ms = ms;
-  if (main_kernel_launches) *main_kernel_launches = (long long)ctx->ev_used;
+  if (slab_kernel_ms) *slab_kernel_ms = ms_slab;
+  if (list_kernel_ms) *list_kernel_ms = ms_list;
+  if (eval_launches) *eval_launches = (long long)(ctx->ev_used / 3);
   if (kernel_launches) *kernel_launches = ctx->launches;
   return TFS_OK;
 }
 
+int tfs_get_profile(tfs_ctx* ctx, double* main_kernel_ms, long long* main_kernel_launches, long long* kernel_launches) {
+  double a = 0.0, b = 0.0;
+  const int rc = tfs_get_profile_kernels(ctx, &a, &b, main_kernel_launches, kernel_launches);
+  if (rc == TFS_OK && main_kernel_ms) *main_kernel_ms = a + b;
+  return rc;
+}
+
 void tfs_destroy(tfs_ctx* ctx) {
   if (!ctx) return;
-  for (auto& p : ctx->ev_pool) { cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
-  void* bufs[] = {ctx->grid, ctx->wgt, ctx->wa, ctx->wb, ctx->colmax, ctx->wcounts, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut, ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials,
+  for (auto& ev : ctx->ev_pool) cudaEventDestroy(ev);
+  void* bufs[] = {ctx->pair[0].grid, ctx->pair[0].wgt, ctx->pair[0].wa, ctx->pair[0].wb, ctx->pair[1].grid, ctx->pair[1].wgt,
+                  ctx->pair[1].wa, ctx->pair[1].wb, ctx->colmax, ctx->wcounts, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut,
+                  ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials, ctx->buf_prep, ctx->buf_ttab,
                   ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
                   ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children, ctx->buf_fe};
   for (void* b : bufs) if (b) cudaFree(b);
@@ -465,26 +540,28 @@ void tfs_destroy(tfs_ctx* ctx) {
 int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const uint8_t* gap_mask, void* stream) {
   if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_upload_data: ctx is NULL");
   if (!coeff) return fail(ctx, TFS_EINVAL, "tfs_upload_data: coeff is NULL");
+  int rc = check_device(ctx, "tfs_upload_data");
+  if (rc) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   const size_t npix = (size_t)ctx->Nt * ctx->Nf;
+  const int C = ctx->C;
   const float* d_coeff = coeff;
   const float* d_weight = weight;
   void* tmp_c = nullptr;
   void* tmp_w = nullptr;
-  int rc = TFS_OK;
   auto cleanup = [&]() { if (tmp_c) cudaFree(tmp_c); if (tmp_w) cudaFree(tmp_w); };
 #define UP_CUDA(expr)                                                                      \
   do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { cleanup();                       \
        return fail(ctx, e_ == cudaErrorMemoryAllocation ? TFS_ENOMEM : TFS_ECUDA,          \
                    "%s failed: %s", #expr, cudaGetErrorString(e_)); } } while (0)
   if (!is_device_ptr(coeff)) {
-    UP_CUDA(cudaMalloc(&tmp_c, npix * 2 * 2 * sizeof(float)));
-    UP_CUDA(cudaMemcpyAsync(tmp_c, coeff, npix * 2 * 2 * sizeof(float), cudaMemcpyHostToDevice, st));
+    UP_CUDA(cudaMalloc(&tmp_c, npix * C * 2 * sizeof(float)));
+    UP_CUDA(cudaMemcpyAsync(tmp_c, coeff, npix * C * 2 * sizeof(float), cudaMemcpyHostToDevice, st));
     d_coeff = (const float*)tmp_c;
   }
   if (weight && !is_device_ptr(weight)) {
-    UP_CUDA(cudaMalloc(&tmp_w, npix * 2 * sizeof(float)));
-    UP_CUDA(cudaMemcpyAsync(tmp_w, weight, npix * 2 * sizeof(float), cudaMemcpyHostToDevice, st));
+    UP_CUDA(cudaMalloc(&tmp_w, npix * C * sizeof(float)));
+    UP_CUDA(cudaMemcpyAsync(tmp_w, weight, npix * C * sizeof(float), cudaMemcpyHostToDevice, st));
     d_weight = (const float*)tmp_w;
   }
   if (gap_mask) {
@@ -493,35 +570,59 @@ int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const
   } else {
     UP_CUDA(cudaMemsetAsync(ctx->gap, 1, (size_t)ctx->Nt, st));
   }
-  const dim3 blocks((unsigned)((ctx->Nf + 31) / 32), (unsigned)((ctx->Nt + 31) / 32));
-  pack_kernel<<<blocks, 256, 0, st>>>((const float2*)d_coeff, d_weight, ctx->Nt, ctx->Nf, ctx->grid, ctx->wgt);
+  // the compacted list of valid tranches comes first: the grid is stored over it (gap tranches are not kept)
+  valid_list_kernel<<<1, 1024, 0, st>>>(ctx->gap, ctx->Nt, ctx->ncol_cap, ctx->vprefix, ctx->valid_m);
   UP_CUDA(cudaGetLastError());
-  valid_list_kernel<<<1, 1024, 0, st>>>(ctx->gap, ctx->Nt, ctx->vprefix, ctx->valid_m);
-  UP_CUDA(cudaGetLastError());
-  ctx->launches += 2;
-  // weight structure (C11): W = a[m] b[k] on every pixel?  then the hot loop reads no per-pixel weight
-  unsigned long long wc[2] = {1, 1};
-  if (ctx->opts.weight_mode == 0) {
-    UP_CUDA(cudaMemsetAsync(ctx->wcounts, 0, 2 * sizeof(unsigned long long), st));
-    weight_colmax_kernel<<<(unsigned)ctx->Nf, 256, 0, st>>>(ctx->wgt, ctx->Nt, ctx->colmax);
-    UP_CUDA(cudaMemsetAsync(ctx->wa, 0, (size_t)ctx->Nt * sizeof(float2), st));
-    weight_rowmax_kernel<<<dim3((unsigned)((ctx->Nt + 127) / 128), 32), 128, 0, st>>>(ctx->wgt, ctx->Nt, ctx->Nf, ctx->wa);
-    weight_factor_kernel<<<1, 1024, 0, st>>>(ctx->colmax, ctx->Nf, ctx->wb, ctx->wcounts);
-    weight_check_kernel<<<(unsigned)((npix + 255) / 256), 256, 0, st>>>(ctx->wgt, ctx->wa, ctx->wb, ctx->Nt, ctx->Nf, ctx->wcounts);
-    UP_CUDA(cudaGetLastError());
-    ctx->launches += 4;
-    UP_CUDA(cudaMemcpyAsync(wc, ctx->wcounts, sizeof(wc), cudaMemcpyDeviceToHost, st));
-  }
   int n_valid = 0;
   UP_CUDA(cudaMemcpyAsync(&n_valid, ctx->vprefix + ctx->Nt, sizeof(int), cudaMemcpyDeviceToHost, st));
   UP_CUDA(cudaStreamSynchronize(st));
   ctx->n_valid = n_valid;
+  ctx->ncol = std::max(1, (n_valid + kTS - 1) / kTS) * kTS;
   free_piece_tables(ctx);                  // cut for the previous gap mask
-  ctx->wmode = wc[0] != 0 ? kWGeneral : (wc[1] != 0 ? kWSeparable : kWTimeOnly);
+  const size_t nrow = (size_t)ctx->Nf + kPadRows;
+  const dim3 blocks((unsigned)((ctx->Nf + 31) / 32), (unsigned)((ctx->Nt + 31) / 32));
+  int wmode = kWTimeOnly;
+  for (int pr = 0; pr < ctx->n_pairs; ++pr) {
+    tfs_ctx::Pair& P = ctx->pair[pr];
+    UP_CUDA(cudaMemsetAsync(P.grid, 0, nrow * ctx->ncol * sizeof(float4), st));
+    UP_CUDA(cudaMemsetAsync(P.wgt, 0, nrow * ctx->ncol * sizeof(float2), st));
+    pack_kernel<<<blocks, 256, 0, st>>>((const float2*)d_coeff, d_weight, ctx->Nt, ctx->Nf, P.c0, P.c1, ctx->gap, ctx->vprefix,
+                                        ctx->ncol, P.grid, P.wgt);
+    UP_CUDA(cudaGetLastError());
+    ctx->launches += 1;
+    // weight structure (C11): W = a[i] b[k] on every pixel?  then the hot loop reads no per-pixel weight
+    unsigned long long wc[2] = {1, 1};
+    if (ctx->opts.weight_mode == 0) {
+      UP_CUDA(cudaMemsetAsync(ctx->wcounts, 0, 2 * sizeof(unsigned long long), st));
+      weight_colmax_kernel<<<(unsigned)ctx->Nf, 256, 0, st>>>(P.wgt, ctx->ncol, n_valid, ctx->colmax);
+      UP_CUDA(cudaMemsetAsync(P.wa, 0, (size_t)ctx->ncol_cap * sizeof(float2), st));
+      weight_rowmax_kernel<<<dim3((unsigned)((std::max(n_valid, 1) + 127) / 128), 32), 128, 0, st>>>(P.wgt, ctx->ncol, n_valid, ctx->Nf, P.wa);
+      weight_factor_kernel<<<1, 1024, 0, st>>>(ctx->colmax, ctx->Nf, P.wb, ctx->wcounts);
+      weight_check_kernel<<<(unsigned)(((size_t)ctx->ncol * ctx->Nf + 255) / 256), 256, 0, st>>>(P.wgt, P.wa, P.wb, ctx->ncol, n_valid,
+                                                                                              ctx->Nf, ctx->wcounts);
+      UP_CUDA(cudaGetLastError());
+      ctx->launches += 4;
+      UP_CUDA(cudaMemcpyAsync(wc, ctx->wcounts, sizeof(wc), cudaMemcpyDeviceToHost, st));
+      UP_CUDA(cudaStreamSynchronize(st));
+    }
+    const int wm = wc[0] != 0 ? kWGeneral : (wc[1] != 0 ? kWSeparable : kWTimeOnly);
+    wmode = std::min(wmode, wm);           // the most general structure among the pairs decides the kernel
+  }
+  ctx->launches += 1;
+  UP_CUDA(cudaStreamSynchronize(st));
+  ctx->wmode = wmode;
   cleanup();
 #undef UP_CUDA
+  // TMA descriptors of the slab kernel (the box height depends on the weight structure)
+  for (int pr = 0; pr < ctx->n_pairs; ++pr) {
+    tfs_ctx::Pair& P = ctx->pair[pr];
+    rc = encode_map(ctx, &P.map_y, P.grid, 4, ctx->ncol, (int)nrow, slab_rows(wmode));
+    if (rc) return rc;
+    rc = encode_map(ctx, &P.map_w, P.wgt, 2, ctx->ncol, (int)nrow, slab_rows(wmode));
+    if (rc) return rc;
+  }
   ctx->uploaded = true;
-  return rc;
+  return TFS_OK;
 }
 
 int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_mask, const float* psd,
@@ -530,6 +631,8 @@ int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_ma
   if (!x) return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: x is NULL");
   if (!(tukey_alpha >= 0.0 && tukey_alpha <= 1.0))
     return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: tukey_alpha must be in [0, 1] (got %g)", tukey_alpha);
+  if (int rcd = check_device(ctx, "tfs_upload_timeseries")) return rcd;
+  if (ctx->Nt > 65535) return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: Nt must be <= 65535 (got %d)", ctx->Nt);
   cudaStream_t st = (cudaStream_t)stream;
   const int C = ctx->C, Nt = ctx->Nt, Nf = ctx->Nf, N = 2 * ctx->Nf;
   // radices of the length-Nf complex FFT behind the packed real transform
@@ -602,20 +705,44 @@ int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_ma
   return tfs_upload_data(ctx, (const float*)d_coeff, d_weight, d_gap, stream);
 }
 
-int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* upsilon, float* seg_power,
-             float* seg_dh, float* seg_hh, void* stream) {
-  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_eval: ctx is NULL");
-  if (n < 0) return fail(ctx, TFS_EINVAL, "tfs_eval: n < 0");
-  if (N_seg < 1 || N_seg > ctx->Nt) return fail(ctx, TFS_EINVAL, "tfs_eval: need 1 <= N_seg <= Nt (got %d, Nt %d)", N_seg, ctx->Nt);
-  if (!ctx->uploaded) return fail(ctx, TFS_ESTATE, "tfs_eval: no data uploaded (call tfs_upload_data first)");
+}  // extern "C"
+
+namespace {
+
+template <int WMODE>
+void launch_slab(const EvalArgs& a, const tfs_ctx::Pair& P, unsigned blocks, cudaStream_t st) {
+  eval_slab_kernel<WMODE><<<blocks, kWarpsPerCta * 32, slab_smem_bytes(WMODE), st>>>(a, P.map_y, P.map_w);
+}
+
+// the evaluation proper (rows a1-a8) for one batch; `transfer` = per-template table [n][C][n_knots] complex or NULL
+int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const float* transfer, int n_knots,
+              double f_knot0, double f_knot_step, float* upsilon, float* seg_power, float* seg_dh, float* seg_hh,
+              void* stream, const char* who) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "%s: ctx is NULL", who);
+  if (n < 0) return fail(ctx, TFS_EINVAL, "%s: n < 0", who);
+  if (N_seg < 1 || N_seg > ctx->Nt) return fail(ctx, TFS_EINVAL, "%s: need 1 <= N_seg <= Nt (got %d, Nt %d)", who, N_seg, ctx->Nt);
+  if (!ctx->uploaded) return fail(ctx, TFS_ESTATE, "%s: no data uploaded (call tfs_upload_data first)", who);
+  if (transfer && (n_knots < 1 || n_knots > 65536 || !std::isfinite(f_knot0) || (n_knots > 1 && !(f_knot_step > 0.0))))
+    return fail(ctx, TFS_EINVAL, "%s: transfer table needs 1 <= n_knots <= 65536, finite f_knot0 and f_knot_step > 0", who);
+  int rc = check_device(ctx, who);
+  if (rc) return rc;
   if (n == 0) { ctx->bad_host = 0; return TFS_OK; }
-  if (!params || !upsilon) return fail(ctx, TFS_EINVAL, "tfs_eval: params and upsilon are required");
-  if (n >= (1ll << 32)) return fail(ctx, TFS_EINVAL, "tfs_eval: n must be < 2^32");
+  if (!params || !upsilon) return fail(ctx, TFS_EINVAL, "%s: params and upsilon are required", who);
+  if (n >= (1ll << 32)) return fail(ctx, TFS_EINVAL, "%s: n must be < 2^32", who);
   cudaStream_t st = (cudaStream_t)stream;
+  const int C = ctx->C;
 
   const double* d_params = nullptr;
-  int rc = stage_params(ctx, params, n, st, &d_params);
+  rc = stage_params(ctx, params, n, st, &d_params);
   if (rc) return rc;
+  const float2* d_ttab = (const float2*)transfer;
+  if (transfer && !is_device_ptr(transfer)) {
+    const size_t bytes = (size_t)n * C * n_knots * sizeof(float2);
+    rc = ensure(ctx, &ctx->buf_ttab, &ctx->cap_ttab, bytes);
+    if (rc) return rc;
+    TFS_CUDA(ctx, cudaMemcpyAsync(ctx->buf_ttab, transfer, bytes, cudaMemcpyHostToDevice, st));
+    d_ttab = (const float2*)ctx->buf_ttab;
+  }
 
   // outputs: device pointers are written in place, host pointers via ctx scratch + D2H
   float* user[4] = {upsilon, seg_power, seg_dh, seg_hh};
@@ -632,7 +759,7 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
     dev[i] = (float*)ctx->buf_out[i];
   }
 
-  // tiling: tiles of kTileMax valid tranches, cut by the segment boundaries into pieces (one partial each)
+  // tiling: tiles of kTS valid tranches, cut by the segment boundaries into pieces (one partial each)
   const tfs_ctx::PieceTable* pt = nullptr;
   rc = get_piece_table(ctx, N_seg, st, &pt);
   if (rc) return rc;
@@ -644,51 +771,100 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
   rc = ensure(ctx, &ctx->buf_partials, &ctx->cap_partials, (size_t)sub * max_pieces * sizeof(float4));
   if (rc) return rc;
 
+  // pre-pass scratch (one pooled allocation): constants, keys, bucket tables, item list, unit tables
+  const int n_bands = (ctx->Nf - 1) / kBandStride + 1;
+  const bool slab_ok = ctx->opts.fresnel_mode == 0 && n_bands + 2 <= 8192;
+  const int n_keys = slab_ok ? n_bands + 2 : 2;
+  const size_t n_buckets = (size_t)n_tiles * n_keys;
+  const size_t n_items = (size_t)sub * n_tiles;
+  const size_t max_us = n_items / kUnitItems + n_buckets + 1, max_ul = n_items / kListUnitItems + (size_t)n_tiles + 1;
+  auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
+  const size_t sz[8] = {al((size_t)sub * sizeof(TplConst)), al(n_items * sizeof(uint16_t)), al(n_buckets * sizeof(unsigned)),
+                        al(n_buckets * sizeof(unsigned)), al(n_items * sizeof(unsigned)), al(max_us * sizeof(Unit)),
+                        al(max_ul * sizeof(Unit)), al(2 * sizeof(int))};
+  size_t total = 0;
+  for (size_t b : sz) total += b;
+  rc = ensure(ctx, &ctx->buf_prep, &ctx->cap_prep, total);
+  if (rc) return rc;
+  char* part[8];
+  { char* q = (char*)ctx->buf_prep; for (int i = 0; i < 8; ++i) { part[i] = q; q += sz[i]; } }
+
   TFS_CUDA(ctx, cudaMemsetAsync(ctx->bad, 0, sizeof(unsigned long long), st));
-  EvalArgs a = base_args(ctx);
-  a.n_tiles = n_tiles;
-  a.tile_first = pt->tile_first;
-  a.piece_end = pt->piece_end;
-  a.partials = (float4*)ctx->buf_partials;
+  const int wm = ctx->opts.fresnel_mode != 0 ? kWGeneral : ctx->wmode;
+  // channel pairs to run: the pair of channel 2 only when a table can give it a transfer factor (T_T = 0 otherwise)
+  const int n_pass = (ctx->n_pairs == 2 && d_ttab) ? 2 : 1;
   for (long long off = 0; off < n; off += sub) {
     const long long nb = std::min(sub, n - off);
-    a.params = d_params + off * TFS_PARAM_COLS;
-    a.n = nb;
-    const long long n_work = nb * n_tiles;
-    const int wm = ctx->opts.fresnel_mode != 0 ? kWGeneral : ctx->wmode;
-    const int warps = warps_per_cta(wm);
-    const long long want = (n_work + warps - 1) / warps;
-    const unsigned blocks = (unsigned)std::min<long long>(want, (long long)ctx->sm_count);   // persistent, 1 CTA/SM
-    TFS_CUDA(ctx, cudaMemsetAsync(ctx->work, 0, sizeof(unsigned long long), st));
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
-    if (ctx->profiling) {
-      if (ctx->ev_used == ctx->ev_pool.size()) {
-        cudaEvent_t e0, e1;
-        TFS_CUDA(ctx, cudaEventCreate(&e0));
-        TFS_CUDA(ctx, cudaEventCreate(&e1));
-        ctx->ev_pool.emplace_back(e0, e1);
+    for (int pass = 0; pass < n_pass; ++pass) {
+      EvalArgs a = base_args(ctx, pass);
+      a.n_tiles = n_tiles; a.n_keys = n_keys; a.slab_ok = slab_ok ? 1 : 0; a.wmode = wm;
+      a.tile_first = pt->tile_first;
+      a.piece_end = pt->piece_end;
+      a.partials = (float4*)ctx->buf_partials;
+      a.params = d_params + off * TFS_PARAM_COLS;
+      a.n = nb;
+      a.tconst = (TplConst*)part[0]; a.keys = (uint16_t*)part[1]; a.counts = (unsigned*)part[2];
+      a.bucket_off = (unsigned*)part[3]; a.list = (unsigned*)part[4]; a.units_slab = (Unit*)part[5];
+      a.units_list = (Unit*)part[6]; a.n_units = (int*)part[7];
+      a.accumulate = pass;
+      a.t_col = pass == 0 ? 3 : -1;
+      if (pass > 0) a.bad_count = nullptr;
+      if (d_ttab) {
+        a.ttab = d_ttab + (size_t)off * C * n_knots;
+        a.tt_K = n_knots; a.tt_C = C; a.tt_ch0 = ctx->pair[pass].c0;
+        const double step = n_knots > 1 ? f_knot_step : 1.0;
+        a.tt_scale = (float)(1.0 / (ctx->DT * step));        // knot position of bin x: (x/DT - f0)/step
+        a.tt_off = (float)(f_knot0 / step);
       }
-      ev0 = ctx->ev_pool[ctx->ev_used].first;
-      ev1 = ctx->ev_pool[ctx->ev_used].second;
-      ++ctx->ev_used;
-      TFS_CUDA(ctx, cudaEventRecord(ev0, st));
+      const unsigned tb = (unsigned)((nb + 255) / 256);
+      prep_consts_kernel<<<tb, 256, 0, st>>>(a);
+      ctx->launches += 1;
+      if (pass == 0) {
+        TFS_CUDA(ctx, cudaMemsetAsync(a.counts, 0, n_buckets * sizeof(unsigned), st));
+        prep_keys_kernel<<<dim3(tb, (unsigned)n_tiles), 256, n_keys * sizeof(unsigned), st>>>(a);
+        prep_scan_kernel<<<1, 1024, 0, st>>>(a);
+        prep_scatter_kernel<<<dim3(tb, (unsigned)n_tiles), 256, 2 * n_keys * sizeof(unsigned), st>>>(a);
+        ctx->launches += 3;
+      }
+      TFS_CUDA(ctx, cudaGetLastError());
+      TFS_CUDA(ctx, cudaMemsetAsync(ctx->work, 0, 2 * sizeof(unsigned long long), st));
+      cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+      if (ctx->profiling) {
+        while (ctx->ev_pool.size() < ctx->ev_used + 3) {
+          cudaEvent_t e0;
+          TFS_CUDA(ctx, cudaEventCreate(&e0));
+          ctx->ev_pool.push_back(e0);
+        }
+        for (int i = 0; i < 3; ++i) ev[i] = ctx->ev_pool[ctx->ev_used + i];
+        ctx->ev_used += 3;
+        TFS_CUDA(ctx, cudaEventRecord(ev[0], st));
+      }
+      const unsigned blocks = (unsigned)ctx->sm_count;       // persistent, 1 CTA per SM
+      // the items that gather from global memory (and every item with the paper's approximants) ...
+      if (ctx->opts.fresnel_mode != 0) eval_list_kernel<1, kWGeneral><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
+      else if (wm == kWTimeOnly) eval_list_kernel<0, kWTimeOnly><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
+      else if (wm == kWSeparable) eval_list_kernel<0, kWSeparable><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
+      else eval_list_kernel<0, kWGeneral><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
+      TFS_CUDA(ctx, cudaGetLastError());
+      if (ev[1]) TFS_CUDA(ctx, cudaEventRecord(ev[1], st));
+      ctx->launches += 1;
+      // ... and the band buckets from shared-memory slabs
+      if (slab_ok) {
+        if (wm == kWTimeOnly) launch_slab<kWTimeOnly>(a, ctx->pair[pass], blocks, st);
+        else if (wm == kWSeparable) launch_slab<kWSeparable>(a, ctx->pair[pass], blocks, st);
+        else launch_slab<kWGeneral>(a, ctx->pair[pass], blocks, st);
+        TFS_CUDA(ctx, cudaGetLastError());
+        ctx->launches += 1;
+      }
+      if (ev[2]) TFS_CUDA(ctx, cudaEventRecord(ev[2], st));
     }
-    if (ctx->opts.fresnel_mode != 0)          // the paper's approximants: one variant, general weights
-      eval_tiles_kernel<1, kWGeneral><<<blocks, warps * 32, kEvalSmemBytes, st>>>(a);
-    else if (ctx->wmode == kWTimeOnly)
-      eval_tiles_kernel<0, kWTimeOnly><<<blocks, warps * 32, kEvalSmemBytes, st>>>(a);
-    else if (ctx->wmode == kWSeparable)
-      eval_tiles_kernel<0, kWSeparable><<<blocks, warps * 32, kEvalSmemBytes, st>>>(a);
-    else
-      eval_tiles_kernel<0, kWGeneral><<<blocks, warps * 32, kEvalSmemBytes, st>>>(a);
-    TFS_CUDA(ctx, cudaGetLastError());
-    if (ev1) TFS_CUDA(ctx, cudaEventRecord(ev1, st));
-    ctx->launches += 2;     // main kernel + combine
     const int threads = 128;
     combine_kernel<<<(unsigned)((nb + threads - 1) / threads), threads, 0, st>>>(
-        a.partials, nb, N_seg, pt->tile_first, n_tiles, pt->piece_seg, dev[0] + off, dev[1] ? dev[1] + off * per[1] : nullptr,
+        (const float4*)ctx->buf_partials, (const uint16_t*)part[1], nb, N_seg, pt->tile_first, n_tiles, pt->piece_seg,
+        pt->piece_tile, dev[0] + off, dev[1] ? dev[1] + off * per[1] : nullptr,
         dev[2] ? dev[2] + off * per[2] : nullptr, dev[3] ? dev[3] + off * per[3] : nullptr);
     TFS_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 1;
   }
   if (any_host) {
     for (int i = 0; i < 4; ++i)
@@ -700,15 +876,34 @@ int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* 
     ctx->bad_host = (long long)bad;
   } else {
     ctx->bad_host = -1;     // not known yet: tfs_bad_param_count synchronises and reads it on demand
-    if (!is_device_ptr(params)) TFS_CUDA(ctx, cudaStreamSynchronize(st));   // host params buffer may be reused
+    if (!is_device_ptr(params) || (transfer && !is_device_ptr(transfer)))
+      TFS_CUDA(ctx, cudaStreamSynchronize(st));            // host input buffers may be reused
   }
   return TFS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg, float* upsilon, float* seg_power,
+             float* seg_dh, float* seg_hh, void* stream) {
+  return eval_impl(ctx, params, n, N_seg, nullptr, 0, 0.0, 0.0, upsilon, seg_power, seg_dh, seg_hh, stream, "tfs_eval");
+}
+
+int tfs_eval_tf(tfs_ctx* ctx, const double* params, long long n, int N_seg, const float* transfer, int n_knots,
+                double f_knot0, double f_knot_step, float* upsilon, float* seg_power, float* seg_dh, float* seg_hh,
+                void* stream) {
+  if (ctx && !transfer) return fail(ctx, TFS_EINVAL, "tfs_eval_tf: transfer is NULL (use tfs_eval for constant factors)");
+  return eval_impl(ctx, params, n, N_seg, transfer, n_knots, f_knot0, f_knot_step, upsilon, seg_power, seg_dh, seg_hh, stream,
+                   "tfs_eval_tf");
 }
 
 int tfs_count_pixels(tfs_ctx* ctx, const double* params, long long n, long long* counts, void* stream) {
   if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_count_pixels: ctx is NULL");
   if (n < 0) return fail(ctx, TFS_EINVAL, "tfs_count_pixels: n < 0");
   if (!ctx->uploaded) return fail(ctx, TFS_ESTATE, "tfs_count_pixels: no data uploaded (the gap mask is part of the data)");
+  if (int rcd = check_device(ctx, "tfs_count_pixels")) return rcd;
   if (n == 0) return TFS_OK;
   if (!params || !counts) return fail(ctx, TFS_EINVAL, "tfs_count_pixels: params and counts are required");
   cudaStream_t st = (cudaStream_t)stream;
@@ -745,6 +940,7 @@ int tfs_refine(tfs_ctx* ctx, const double* params, long long n, const long long*
   if (n < 0 || k < 0) return fail(ctx, TFS_EINVAL, "tfs_refine: n < 0 or k < 0");
   if (r < 1 || r > 64) return fail(ctx, TFS_EINVAL, "tfs_refine: need 1 <= r <= 64 (got %d)", r);
   if (!std::isfinite(d_mc_rel) || !std::isfinite(d_tc)) return fail(ctx, TFS_EINVAL, "tfs_refine: steps must be finite");
+  if (int rcd = check_device(ctx, "tfs_refine")) return rcd;
   if (k == 0) return TFS_OK;
   if (!params || !idx || !children) return fail(ctx, TFS_EINVAL, "tfs_refine: params, idx and children are required");
   if (k * (long long)r * r >= (1ll << 32)) return fail(ctx, TFS_EINVAL, "tfs_refine: k*r*r must be < 2^32");
@@ -819,7 +1015,8 @@ int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k, long long* 
   if (n < 1 || n >= (1ll << 32)) return fail(ctx, TFS_EINVAL, "tfs_topk: need 1 <= n < 2^32");
   if (k < 1 || k > n) return fail(ctx, TFS_EINVAL, "tfs_topk: need 1 <= k <= n (got k %d, n %lld)", k, n);
   cudaStream_t st = (cudaStream_t)stream;
-  int rc;
+  int rc = check_device(ctx, "tfs_topk");
+  if (rc) return rc;
   const float* d_in = upsilon;
   if (!is_device_ptr(upsilon)) {
     rc = ensure(ctx, &ctx->buf_tk_in, &ctx->cap_tk_in, (size_t)n * sizeof(float));

@@ -1,83 +1,132 @@
 // tfs_kernels.cuh -- device code of libtfs (sm_100a).  See include/tfs.h for the operation and
 // DESIGN.md section 6 for the kernel design.  Citations: P:<line> of PAPER.md, C<n> = DESIGN.md.
 //
-// Work decomposition: one WARP evaluates one (template, time tile) pair.  A time tile is a run
-// of kTileMax consecutive VALID (non-gap) tranches, whatever N_seg is; work items are ordered
-// tile-major so that all templates sweep the same slab of the grid together and the slab stays
-// L2-resident.  Segment boundaries cut a tile into PIECES; the warp writes one partial per piece.
-// Inside a tile lanes are tranches (32 at a time): fp64 0PN track per lane, then each lane walks
-// its own window; the grid is stored time-contiguous so those loads coalesce across lanes.
+// Work decomposition (v10).  A WORK ITEM is one (template, time tile) pair; a time tile is a run of kTS
+// consecutive VALID (non-gap) tranches, whatever N_seg is.  The grid is stored time-contiguous over the
+// COMPACTED list of valid tranches ([k][i], i = index in that list), so a tile is a contiguous block of
+// columns.  Segment boundaries cut a tile into PIECES; one warp evaluates one item and writes one partial
+// per piece.  Inside an item lanes are tranches (32 at a time): fp64 0PN track per lane, then each lane
+// walks its own frequency window.
+//
+// A pre-pass (prep_*_kernel) sorts the items of a batch into BUCKETS: per tile, by the frequency band
+// (kBandStride rows) that holds the bottom of the template's track in that tile.  Items whose whole
+// window fits a slab of kSlabRows rows go through eval_slab_kernel: a persistent CTA per SM claims a
+// UNIT (<= kUnitItems items of one bucket), TMA (cp.async.bulk.tensor) stages the band's data slab
+// [rows][kTS columns] in shared memory behind an mbarrier (two stages), and its 32 warps take the unit's
+// items one by one, reading pixels with conflict-free LDS.128.  The other items (tracks that sweep many
+// rows in one tile, templates that merge inside the tile) go through eval_list_kernel, which gathers
+// from global memory (L2) with software-pipelined LDG.128 -- the v9 pixel loop.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace tfs {
 
-// Warps of the one persistent CTA per SM.  The kernel is short of warps to hide its dependent chains, so
-// it runs the most a CTA can hold: 32 warps at 64 registers per thread (measured against 20, 24, 26, 28
-// for both the separable- and the general-weights variants).
-#ifndef TFS_WARPS_SEPARABLE
-#define TFS_WARPS_SEPARABLE 32
+#ifndef TFS_TS
+#define TFS_TS 64
 #endif
-#ifndef TFS_WARPS_GENERAL
-#define TFS_WARPS_GENERAL 32
+constexpr int kTS = TFS_TS;               // valid tranches per time tile (= columns of a slab); multiple of 32
+static_assert(kTS % 32 == 0 && kTS >= 32 && kTS <= 64, "kTS must be 32 or 64 (TMA box <= 256 floats wide)");
+#ifndef TFS_SLAB_ROWS
+#define TFS_SLAB_ROWS 96
 #endif
-constexpr int kMaxWarpsPerCta = TFS_WARPS_SEPARABLE > TFS_WARPS_GENERAL ? TFS_WARPS_SEPARABLE : TFS_WARPS_GENERAL;
-#ifndef TFS_TILE
-#define TFS_TILE 512
+#ifndef TFS_SLAB_ROWS_GENERAL
+#define TFS_SLAB_ROWS_GENERAL 64
 #endif
-constexpr int kTileMax = TFS_TILE;       // valid tranches per time tile (16 chunks of 32 lanes)
-constexpr int kLutN = 512;          // LUT intervals in t = 1/(1+v)
-constexpr double kMtsun = 4.925490947e-6;   // G Msun / c^3 [s]
+constexpr int kBandStride = 32;           // rows between the bottoms of consecutive bands
+constexpr int kUnitItems = 1024;          // items per unit of the slab kernel (32 per warp)
+constexpr int kListUnitItems = 32;        // items per (warp-claimed) unit of the list kernel
+constexpr int kWarpsPerCta = 32;          // both evaluation kernels: one persistent CTA of 32 warps per SM (64 registers)
+constexpr int kLutN = 512;                // LUT intervals in t = 1/(1+v)
+constexpr double kMtsun = 4.925490947e-6; // G Msun / c^3 [s]
 constexpr double kPi = 3.14159265358979323846;
+constexpr int kPadRows = 16;              // rows of zero padding behind the grid and the weights
+
+// Weight modes (chosen by tfs_upload_data, DESIGN.md C11):
+//   kWGeneral    per-pixel weights W[alpha,m,k], read next to every data pixel
+//   kWSeparable  W[alpha,m,k] = a_alpha[m] b_alpha[k]: b from a small [Nf] table, a applied once per tranche
+//   kWTimeOnly   b = 1: no weight is read in the pixel loop, q' = sum |h'|^2 for both channels
+constexpr int kWGeneral = 0, kWSeparable = 1, kWTimeOnly = 2;
+__host__ __device__ constexpr int slab_rows(int wmode) { return wmode == kWGeneral ? TFS_SLAB_ROWS_GENERAL : TFS_SLAB_ROWS; }
+constexpr int kSlabRowsMax = TFS_SLAB_ROWS > TFS_SLAB_ROWS_GENERAL ? TFS_SLAB_ROWS : TFS_SLAB_ROWS_GENERAL;
+static_assert(TFS_SLAB_ROWS <= 256 && TFS_SLAB_ROWS_GENERAL <= 256, "TMA box <= 256 rows");
+static_assert(TFS_SLAB_ROWS > kBandStride && TFS_SLAB_ROWS_GENERAL > kBandStride, "a slab must overlap the next band");
 
 // f(v) = w (F0 + F1 w^4 + F2 w^8), g(v) = w^3 (G0 + G1 w^4 + G2 w^8), w = 1/v, valid for |v| >= kVFar
 struct FarCoef { float F0, F1, F2, G0, G1, G2; };
 
+// Per-template constants, written once per batch by prep_consts_kernel (a1).
+struct __align__(16) TplConst {
+  double tc, phic_turns, inv5M;
+  double xcoefDT;        // DT / (8 pi M):           x = f DT = X^{-3/8} xcoefDT
+  double ccoef;          // (3/8) DT / (5M):         c = fdot DT^2 = x ccoef / X
+  float acoef;           // amp (8 pi M)^{-2/3}:     A_m = acoef X^{-1/4}
+  int ok;
+  float T0r, T0i, T1r, T1i;   // constant transfer factors of the two channels of the pair (Eq. 29, C5)
+};
+static_assert(sizeof(TplConst) == 64, "TplConst layout");
+
+struct Unit { int tile; int row0; unsigned off; int cnt; };   // items list[off .. off+cnt) of one bucket; cnt < 0: end marker
+
 struct EvalArgs {
-  const float4* __restrict__ grid;     // [Nf][Nt] (time-contiguous) {Y_A.re, Y_E.re, Y_A.im, Y_E.im}, Y = W*D
-  const float2* __restrict__ wgt;      // [Nf][Nt] {W_A, W_E}
-  const float2* __restrict__ wa;       // [Nt] {a_A, a_E}  (separable weights: W = a[m] b[k])
-  const float2* __restrict__ wb;       // [Nf + kPadRows] {b_A, b_E}
+  const float4* __restrict__ grid;     // [Nf+pad][ncol] (time-contiguous over valid tranches) {Y_0.re, Y_1.re, Y_0.im, Y_1.im}, Y = W*D
+  const float2* __restrict__ wgt;      // [Nf+pad][ncol] {W_0, W_1}
+  const float2* __restrict__ wa;       // [ncol] {a_0, a_1} by valid-tranche index (separable weights: W = a[i] b[k])
+  const float2* __restrict__ wb;       // [Nf + kPadRows + kSlabRowsMax] {b_0, b_1}
   const uint8_t* __restrict__ gap;     // [Nt] 1 = valid
   const int* __restrict__ vprefix;     // [Nt+1] number of valid tranches before m
-  const int* __restrict__ valid_m;     // [vprefix[Nt]] the valid tranche indices, ascending (padded to >= 1 entry)
+  const int* __restrict__ valid_m;     // [ncol] the valid tranche indices, ascending (padded with the last one)
   const int* __restrict__ tile_first;  // [n_tiles+1] first piece of each tile (pieces are numbered in time order)
   const int* __restrict__ piece_end;   // [n_pieces] entry of valid_m where the piece ends (exclusive)
   const float4* __restrict__ lut;      // [kLutN+1] {a_G, a_F, b_G, b_F} (see fresnel_aux)
-  const double* __restrict__ params;   // [n][8]
+  const double* __restrict__ params;   // [n][8] (prep only)
+  TplConst* __restrict__ tconst;       // [n]
+  uint16_t* __restrict__ keys;         // [n_tiles][n] bucket of every item: 0 = no active tranche, 1 = list kernel, 2+b = band b
+  unsigned* __restrict__ counts;       // [n_tiles][n_keys] items per bucket; then (scatter) the cursor of each bucket
+  unsigned* __restrict__ bucket_off;   // [n_tiles][n_keys] start of each bucket in `list`
+  unsigned* __restrict__ list;         // template indices, bucket by bucket (tile-major)
+  Unit* __restrict__ units_slab;       // units of the slab kernel
+  Unit* __restrict__ units_list;       // units of the list kernel
+  int* __restrict__ n_units;           // [2] {slab, list}
   float4* __restrict__ partials;       // [n_pieces][n] {z.re, z.im, hh, 0}
-  unsigned long long* bad_count;       // templates rejected (counted on tile 0 only)
-  unsigned long long* work_counter;    // next unclaimed work item (zeroed before each launch)
+  unsigned long long* bad_count;       // templates rejected
+  unsigned long long* work_counter;    // [2] next unclaimed unit of {slab kernel, list kernel} (zeroed before each launch)
+  // optional per-template transfer table (Eq. 29, "computed once per tranche"): T_alpha(f) at n_knots
+  // knots f_knot0 + j f_knot_step, linear in between, clamped outside; [n][tt_C][tt_K] complex
+  const float2* __restrict__ ttab;
+  int tt_K, tt_C, tt_ch0;              // knots, channels in the table, first channel of this pair
+  float tt_scale, tt_off;              // knot position of bin x: x * tt_scale - tt_off
+  int accumulate;                      // 1: add to the partials instead of overwriting them (second channel pair)
+  int t_col;                           // params columns of the pair's first transfer factor (3: T_A, T_E)
+  int n_ch_pair;                       // channels in this pair (1 or 2)
   long long n;                         // templates in this launch
-  int Nt, Nf;
-  int n_valid, n_tiles;                // valid tranches, ceil(n_valid / kTileMax) (>= 1)
+  int Nt, Nf, ncol;
+  int n_valid, n_tiles, n_keys;        // valid tranches, ceil(n_valid / kTS) (>= 1), bands + 2
   int H, adaptive;
+  int slab_ok;                         // 0: every active item goes to the list kernel (fresnel_mode 1, absurd shapes)
+  int wmode;
   double DT;
   double x_lo, x_hi;                   // band in bins: f_lo*DT, f_hi*DT
   double c_max;
   FarCoef far;                         // far-zone polynomials of f, g (fitted at tfs_create)
 };
 
-// Per-template constants derived from the parameter row.
-struct TemplateConst {
-  double tc, phic_turns, inv5M;
-  double xcoefDT;        // DT / (8 pi M):           x = f DT = X^{-3/8} xcoefDT
-  double ccoef;          // (3/8) DT / (5M):         c = fdot DT^2 = x ccoef / X
-  float acoef;           // amp (8 pi M)^{-2/3}:     A_m = acoef X^{-1/4}
-  double TAr, TAi, TEr, TEi;
-  bool ok;
-};
-
-__device__ __forceinline__ TemplateConst load_template(const double* __restrict__ p, double DT) {
-  TemplateConst t;
+// a1: per-template constants from the parameter row (fp64)
+__device__ __forceinline__ TplConst load_template(const double* __restrict__ p, double DT, int t_col, int n_ch) {
+  TplConst t;
   const double Mc = p[0];
   t.tc = p[1];
   const double phic = p[2];
-  t.TAr = p[3]; t.TAi = p[4]; t.TEr = p[5]; t.TEi = p[6];
   const double amp = p[7];
-  bool ok = isfinite(Mc) && isfinite(t.tc) && isfinite(phic) && isfinite(t.TAr) && isfinite(t.TAi) &&
-            isfinite(t.TEr) && isfinite(t.TEi) && isfinite(amp) && (Mc > 0.0);
+  double T[4] = {0.0, 0.0, 0.0, 0.0};
+  bool ok = isfinite(Mc) && isfinite(t.tc) && isfinite(phic) && isfinite(amp) && (Mc > 0.0);
+#pragma unroll
+  for (int c = 3; c < 7; ++c) ok = ok && isfinite(p[c]);          // a bad row is bad for every channel pair
+  if (t_col >= 0) {
+    T[0] = p[t_col]; T[1] = p[t_col + 1];
+    if (n_ch > 1) { T[2] = p[t_col + 2]; T[3] = p[t_col + 3]; }
+  }
   const double M = (ok ? Mc : 1.0) * kMtsun;
   t.inv5M = 1.0 / (5.0 * M);
   const double xcoef = 1.0 / (8.0 * kPi * M);                // f = X^{-3/8} xcoef
@@ -87,7 +136,10 @@ __device__ __forceinline__ TemplateConst load_template(const double* __restrict_
   const float cx = cbrtf((float)xcoef);
   t.acoef = (float)(ok ? amp : 0.0) * cx * cx;
   t.phic_turns = (ok ? phic : 0.0) * (0.5 / kPi);
-  t.ok = ok;
+  t.ok = ok ? 1 : 0;
+  t.T0r = ok ? (float)T[0] : 0.f; t.T0i = ok ? (float)T[1] : 0.f;
+  t.T1r = ok ? (float)T[2] : 0.f; t.T1i = ok ? (float)T[3] : 0.f;
+  if (!ok) t.tc = 0.0;
   return t;
 }
 
@@ -103,7 +155,8 @@ struct TrackPoint {
 // All fractional powers of X come from y = X^{-1/8}: an fp32 seed y0 = 2^{-log2(X)/8} (two MUFU ops,
 // relative error d ~ 4e-7) corrected in fp64 by the binomial series of (1 - e)^{-1/8}, e = 1 - X y0^8
 // ~ 8 d, to third order: the remainder is ~0.04 e^4 < 1e-20, i.e. y is exact to fp64 rounding.
-__device__ __forceinline__ TrackPoint track_point(const TemplateConst& t, int m, double DT,
+// `pre` = the tranche may be active at all (valid lane, tau > DT); the band tests are applied here.
+__device__ __forceinline__ TrackPoint track_point(const TplConst& t, int m, double DT,
                                                   double x_lo, double x_hi, double c_max, bool valid) {
   TrackPoint r;
   const double tau = t.tc - (double)m * DT;
@@ -143,10 +196,10 @@ __device__ __forceinline__ void window(const TrackPoint& tp, int H, int adaptive
 //     f(v) = t (a_F + b_F t),  g(v) = t (a_G + b_G t)
 //   (the linear interpolant of F = f/t, G = g/t around node i with central-difference slope,
 //    rewritten as intercept + slope*t so the fractional index is never formed).
-// In shared memory it is stored kLutCopies times, copy r of entry i at 16-byte slot
-// (i*kLutCopies + r), and lane l reads copy l & 7: the 8 lanes of a quarter-warp always hit 8
-// different bank groups, so an LDS.128 is conflict-free whatever the indices are.
-constexpr int kLutCopies = 8;
+// In shared memory it is stored LC times, copy r of entry i at 16-byte slot (i*LC + r), and lane l reads
+// copy l & (LC-1): with LC = 8 the 8 lanes of a quarter-warp always hit 8 different bank groups, so an
+// LDS.128 is conflict-free whatever the indices are (the slab kernel keeps 4 copies to leave room for
+// its data slabs: at most 2-way conflicts).
 constexpr float kMagic = 12582912.0f;          // 1.5 * 2^23: (p + kMagic) rounds p to an integer in the mantissa
 constexpr unsigned kMagicBits = 0x4B400000u;
 
@@ -157,6 +210,17 @@ __device__ __forceinline__ float rcp_approx(float x) {
 }
 
 __device__ __forceinline__ float4 lds128(unsigned addr) {
+  float4 r;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "r"(addr));
+  return r;
+}
+__device__ __forceinline__ float2 lds64(unsigned addr) {
+  float2 r;
+  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "r"(addr));
+  return r;
+}
+// LUT read: the table is written once before any read, so this one need not be volatile
+__device__ __forceinline__ float4 lds128_const(unsigned addr) {
   float4 r;
   asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "r"(addr));
   return r;
@@ -191,14 +255,14 @@ __device__ __forceinline__ f2_t fadd2(f2_t a, f2_t b) {
 }
 
 // Returns GF = {g(|v|)/t, f(|v|)/t} and ts = sign(v) t, so that Godd(v) = ts GF as a complex {re, im} pair.
-// lut_lane = shared address of this lane's LUT copy minus kMagicBits * (16 * kLutCopies)  (mod 2^32).
-template <int MODE>
+// lut_lane = shared address of this lane's LUT copy minus kMagicBits * (16 * LC)  (mod 2^32).
+template <int MODE, int LC>
 __device__ __forceinline__ void fresnel_aux(float v, unsigned lut_lane, f2_t& GF, float& ts) {
   const float a = fabsf(v);
   if (MODE == 0) {
     const float t = rcp_approx(1.0f + a);         // MUFU.RCP
     const float q = fmaf(t, (float)kLutN, kMagic);
-    const float4 e = lds128(__float_as_uint(q) * (16u * kLutCopies) + lut_lane);   // {a_G, a_F, b_G, b_F}
+    const float4 e = lds128_const(__float_as_uint(q) * (16u * LC) + lut_lane);   // {a_G, a_F, b_G, b_F}
     ts = copysignf(t, v);
     GF = ffma2(pk(t, t), pk(e.z, e.w), pk(e.x, e.y));
   } else {
@@ -216,16 +280,6 @@ __device__ __forceinline__ void fresnel_aux(float v, unsigned lut_lane, f2_t& GF
   }
 }
 
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
-}
-
-// dynamic shared memory of kernel A: [LUT copies][per-lane tile sums: 3 packed pairs per thread, stored [3][threads]]
-constexpr int kLutSmemBytes = (kLutN + 1) * kLutCopies * (int)sizeof(float4);
-constexpr int kEvalSmemBytes = kLutSmemBytes + 3 * kMaxWarpsPerCta * 32 * (int)sizeof(f2_t);
-
 // One pixel of one tranche (a3-a5).  The template coefficient is h = P h', P = A/sqrt(2c) exp(i phi_m)
 // constant over the tranche, and (auxiliary-function form of Eq. 16)
 //   h' = Godd(v0) - Godd(v1) E  [+ (1+i) exp(-i pi u^2/c) inside the swept band],
@@ -233,15 +287,20 @@ constexpr int kEvalSmemBytes = kLutSmemBytes + 3 * kMaxWarpsPerCta * 32 * (int)s
 // The loop accumulates z'_alpha += conj(Y_alpha) h', q'_alpha += W_alpha |h'|^2 and the factor P
 // (|P|^2 for q) is applied once per tranche.
 //
-// Two evaluations of Godd:
+// Three evaluations of Godd:
 //   FAR  (|v0|, |v1| >= kVFar):  f(v) = w Pf(w^4), g(v) = w^3 Pg(w^4), w = 1/v, Pf and Pg quadratics
 //         fitted at tfs_create (they are the asymptotic series of A&S 7.3.27-28 re-fitted on the
 //         interval; odd in v, so the sign comes for free).  No table read: 2 MUFU.RCP + 10 packed ops.
+//   FAR2 (|v0|, |v1| >= kVFar2): the leading terms alone, f = w/pi, g = w^3/pi^2: the next terms are
+//         3/(pi^2 v^4) (< 1e-6 for v >= 24) of f and 15/(pi^2 v^4) of g (itself < 6e-4 f).  4 packed ops.
 //   NEAR (anything else): the shared-memory LUT in t = 1/(1+|v|) (fresnel_aux).
-// The far zone covers all but the ~2 pixels next to the track for the slow chirps that make up the
-// bulk of every bank (|v| = sqrt(2/c) |u|).
+// For the slow chirps that make up the bulk of every bank (|v| = sqrt(2/c) |u|) the far zones cover all
+// but the ~2 pixels next to the track, and FAR2 more than half of the window.
 constexpr float kVFar = 3.0f;
-
+#ifndef TFS_VFAR2
+#define TFS_VFAR2 24.0f
+#endif
+constexpr float kVFar2 = TFS_VFAR2;
 
 struct LaneTrack {      // per-lane (= per-tranche) constants of the pixel loop
   float sc;             // sqrt(2/c)
@@ -251,15 +310,9 @@ struct LaneTrack {      // per-lane (= per-tranche) constants of the pixel loop
   float Er, Ei;         // exp(i psi)
 };
 
-struct LaneSums { f2_t zr, zi, q; };     // {A, E} pairs: Re z', Im z', q'
+struct LaneSums { f2_t zr, zi, q; };     // {channel 0, channel 1} pairs: Re z', Im z', q'
 
-// Weight modes (chosen by tfs_upload_data, DESIGN.md C11):
-//   kWGeneral    per-pixel weights W[alpha,m,k], read next to every data pixel
-//   kWSeparable  W[alpha,m,k] = a_alpha[m] b_alpha[k]: b from a small [Nf] table, a applied once per tranche
-//   kWTimeOnly   b = 1: no weight is read in the pixel loop, q' = sum |h'|^2 for both channels
-constexpr int kWGeneral = 0, kWSeparable = 1, kWTimeOnly = 2;
-
-// grid pixel Y = {Y_A.re, Y_E.re, Y_A.im, Y_E.im}, weights Wt = {W_A, W_E} (or {b_A, b_E})
+// grid pixel Y = {Y_0.re, Y_1.re, Y_0.im, Y_1.im}, weights Wt = {W_0, W_1} (or {b_0, b_1})
 template <int WMODE>
 __device__ __forceinline__ void mac(LaneSums& s, const float4 Y, const float2 Wt, float hr, float hi) {
   const f2_t Yre = pk(Y.x, Y.y), Yim = pk(Y.z, Y.w);
@@ -297,15 +350,30 @@ __device__ __forceinline__ void pixel_far(const LaneTrack& L, const FarCoef& C, 
   hi = fmaf(-L.Er, f1, fmaf(-L.Ei, g1, f0));
 }
 
-template <int MODE, int MASKED>
+// FAR2: f = F0 w, g = G0 w^3 = (G0 / F0^3) f^3
+constexpr float kG0overF03 = 3.14159265358979f;      // (1/pi^2) / (1/pi)^3 = pi
+template <int MASKED>
+__device__ __forceinline__ void pixel_far2(const LaneTrack& L, float u, float msk, float& hr, float& hi) {
+  const f2_t r = pk(rcp_approx(u), rcp_approx(u + L.c));
+  const float kf = (MASKED ? L.kap * msk : L.kap) * 0.318309886183790672f;
+  const f2_t fv = fmul2(r, pk(kf, kf));                          // {f(v0), f(v1)}
+  const f2_t gv = fmul2(fmul2(fv, pk(kG0overF03, kG0overF03)), fmul2(fv, fv));
+  float f0, f1, g0, g1;
+  upk(fv, f0, f1);
+  upk(gv, g0, g1);
+  hr = fmaf(-L.Er, g1, fmaf(L.Ei, f1, g0));
+  hi = fmaf(-L.Er, f1, fmaf(-L.Ei, g1, f0));
+}
+
+template <int MODE, int MASKED, int LC>
 __device__ __forceinline__ void pixel_near(const LaneTrack& L, float u, float msk, unsigned lut_lane,
                                            float& hr, float& hi) {
   const float v0 = L.sc * u;
   const float v1 = fmaf(L.sc, L.c, v0);
   f2_t GF0, GF1;
   float t0, t1;
-  fresnel_aux<MODE>(v0, lut_lane, GF0, t0);
-  fresnel_aux<MODE>(v1, lut_lane, GF1, t1);
+  fresnel_aux<MODE, LC>(v0, lut_lane, GF0, t0);
+  fresnel_aux<MODE, LC>(v1, lut_lane, GF1, t1);
   if (MASKED) { t0 *= msk; t1 *= msk; }
   const f2_t Z0 = fmul2(pk(t0, t0), GF0);                        // Godd(v0) = {re, im}
   const f2_t Z1 = fmul2(pk(t1, t1), GF1);
@@ -326,7 +394,22 @@ __device__ __forceinline__ void pixel_near(const LaneTrack& L, float u, float ms
   }
 }
 
-// Pixel loop of one chunk (32 tranches, one per lane): every lane walks its own window, offsets
+constexpr int kZNear = 0, kZFar = 1, kZFar2 = 2;
+
+// one pixel of kind KIND at offset jj (u = x - k of that pixel, stepped by the caller)
+template <int KIND, int MODE, int WMODE, int MASKED, int LC>
+__device__ __forceinline__ void pixel_kind(const LaneTrack& L, const FarCoef& C, int jj, int Wm, const float4 Yc,
+                                           const float2 Wc, float u, unsigned lut_lane, LaneSums& s) {
+  const float msk = (MASKED && jj >= Wm) ? 0.0f : 1.0f;
+  float hr, hi;
+  if (KIND == kZNear) pixel_near<MODE, MASKED, LC>(L, u, msk, lut_lane, hr, hi);
+  else if (KIND == kZFar) pixel_far<MASKED>(L, C, u, msk, hr, hi);
+  else pixel_far2<MASKED>(L, u, msk, hr, hi);
+  mac<WMODE>(s, Yc, Wc, hr, hi);
+}
+
+// ------------------------------------------------------------------------------------------
+// Pixel loop of the LIST kernel (global-memory gather).  Every lane walks its own window, offsets
 // j = 0 ... Wm-1 from its k_lo, in groups of kGroup offsets.  The gather is software-pipelined through
 // two register buffers: the loads of group g+1 are issued before the arithmetic of group g.  It is never
 // predicated: the grid is allocated with kPadRows zeroed rows past Nf-1, so reading a few pixels past the
@@ -337,24 +420,22 @@ __device__ __forceinline__ void pixel_near(const LaneTrack& L, float u, float ms
 // straight-line far-zone code.  Groups that lie below Wmin (the shortest active window) need no per-lane
 // test at all; the groups that reach past it multiply the contribution of lanes past their own window
 // by zero.  Chunks whose windows differ by more than kRagMax pixels also clamp every load offset.
+// ------------------------------------------------------------------------------------------
 #ifndef TFS_GROUP
 #define TFS_GROUP 2
 #endif
 constexpr int kGroup = TFS_GROUP;
-constexpr int kPadRows = 16;                 // rows of zero padding behind the grid and the weights
 constexpr int kRagMax = kPadRows - 2 * kGroup;   // largest Wmax - Wmin handled without clamping the loads
 static_assert(kRagMax >= 1, "kPadRows too small for kGroup");
+constexpr int kLutCopiesList = 8;
 
 // ZONES: 1 = test the offset against the near zone, 0 = the offset is known to be far
 template <int MODE, int WMODE, int MASKED, int ZONES>
 __device__ __forceinline__ void pixel_step(const LaneTrack& L, const FarCoef& C, int jj, int Wm, int JA, int JB,
                                            const float4 Yc, const float2 Wc, float& u, unsigned lut_lane,
                                            LaneSums& s) {
-  const float msk = (MASKED && jj >= Wm) ? 0.0f : 1.0f;
-  float hr, hi;
-  if (ZONES && jj >= JA && jj < JB) pixel_near<MODE, MASKED>(L, u, msk, lut_lane, hr, hi);
-  else pixel_far<MASKED>(L, C, u, msk, hr, hi);
-  mac<WMODE>(s, Yc, Wc, hr, hi);
+  if (ZONES && jj >= JA && jj < JB) pixel_kind<kZNear, MODE, WMODE, MASKED, kLutCopiesList>(L, C, jj, Wm, Yc, Wc, u, lut_lane, s);
+  else pixel_kind<kZFar, MODE, WMODE, MASKED, kLutCopiesList>(L, C, jj, Wm, Yc, Wc, u, lut_lane, s);
   u -= 1.0f;
 }
 
@@ -374,7 +455,7 @@ __device__ __forceinline__ void load_group(const EvalArgs& a, PixelBuf& B, int i
 #define TFS_BOUNDS_PAD kPadRows   // (a smaller value makes the check fail on purpose: tests the checker)
 #endif
     // debug builds only: the gather is unpredicated, so prove it stays inside the padded arrays
-    if (i < 0 || i >= (a.Nf + TFS_BOUNDS_PAD) * a.Nt || kb + jj * kstp < 0 || kb + jj * kstp >= a.Nf + TFS_BOUNDS_PAD) __trap();
+    if (i < 0 || i >= (a.Nf + TFS_BOUNDS_PAD) * a.ncol || kb + jj * kstp < 0 || kb + jj * kstp >= a.Nf + TFS_BOUNDS_PAD) __trap();
 #endif
     B.Y[p] = __ldg(a.grid + i);
     if (WMODE == kWGeneral) B.W[p] = __ldg(a.wgt + i);
@@ -407,12 +488,12 @@ __device__ __forceinline__ void compute_group_auto(const LaneTrack& L, const Far
   else compute_group<MODE, WMODE, 1>(L, C, B, j0, Wm, Wmax, JA, JB, u, lut_lane, s);
 }
 
-// idx = pixel index of offset 0, stp = Nt for an active lane and 0 otherwise, Wm = window length (>= 1
+// idx = pixel index of offset 0, stp = ncol for an active lane and 0 otherwise, Wm = window length (>= 1
 // for active lanes, 0 otherwise)
 template <int MODE, int WMODE>
-__device__ __forceinline__ void pixel_loop(const EvalArgs& a, const LaneTrack& L, const FarCoef& C, int Wm, int Wmin,
-                                           int Wmax, int JA, int JB, int idx, int stp, int kb, int kstp, float u,
-                                           unsigned lut_lane, LaneSums& s) {
+__device__ __forceinline__ void pixel_loop_global(const EvalArgs& a, const LaneTrack& L, const FarCoef& C, int Wm, int Wmin,
+                                                  int Wmax, int JA, int JB, int idx, int stp, int kb, int kstp, float u,
+                                                  unsigned lut_lane, LaneSums& s) {
   PixelBuf A, B;
 #pragma unroll
   for (int p = 0; p < kGroup; ++p) { A.W[p] = make_float2(0.f, 0.f); B.W[p] = make_float2(0.f, 0.f); }
@@ -443,39 +524,571 @@ __device__ __forceinline__ void pixel_loop(const EvalArgs& a, const LaneTrack& L
 }
 
 // ------------------------------------------------------------------------------------------
-// Kernel A: track + gather + per-tile sums.  Persistent: one CTA per SM, warps claim work items
-// (template, tile) in tile-major order from a global counter, kClaim at a time.
-// Inside a work item LANES ARE TRANCHES: lane l owns the l-th valid (non-gap) tranche of the
-// current chunk of 32, computes its track point in fp64 and then walks its own window pixel by
-// pixel.  The grid is stored time-contiguous ([k][m]), so the 32 lanes' loads of pixel offset j
-// fall on consecutive addresses wherever neighbouring tranches share k_lo (slow chirps: runs of
-// 1/c tranches).  Per chunk the window offsets are split (warp-uniformly) into the NEAR zone around
-// the track, evaluated from the shared-memory LUT, and the FAR zone, evaluated from the fitted
-// asymptotic polynomials in packed fp32 (pixel_loop).
+// Pixel loop of the SLAB kernel.  The band's data slab sits in shared memory as [row][kTS columns] float4
+// (plus [row][kTS] float2 weights, or the band's rows of the b table); lane l of chunk h reads column
+// 32 h + l, so the 8 lanes of a quarter-warp always fall in 8 different 16-byte bank groups: an LDS.128
+// is conflict-free whatever rows the lanes are on.  The window offsets are cut, warp-uniformly, into
+//   [0, J2A) FAR2 | [J2A, JA) FAR | [JA, JB) NEAR | [JB, J2B) FAR | [J2B, Wmax) FAR2
+// and each run into its unmasked part (below Wmin, the shortest active window) and its masked rest.
+// An inactive lane walks rows row0, row0+1, ... of its own column (always inside the slab).
 // ------------------------------------------------------------------------------------------
-constexpr int kClaim = 4;
+constexpr int kLutCopiesSlab = 4;
+
+template <int WMODE>
+struct SlabLane {
+  unsigned y_addr;      // shared address of this lane's pixel of offset 0
+  unsigned w_addr;      // kWGeneral: same in the weight slab; kWSeparable: row of the b table; else unused
+#ifdef TFS_BOUNDS_CHECK
+  int row_rel, rows;    // slab row of offset 0, rows in the slab
+#endif
+  __device__ __forceinline__ void load(int j, float4& Y, float2& W) const {
+#ifdef TFS_BOUNDS_CHECK
+    if (row_rel + j < 0 || row_rel + j >= rows) __trap();
+#endif
+    Y = lds128(y_addr + (unsigned)j * (kTS * 16u));
+    if (WMODE == kWGeneral) W = lds64(w_addr + (unsigned)j * (kTS * 8u));
+    else if (WMODE == kWSeparable) W = lds64(w_addr + (unsigned)j * 8u);
+    else W = make_float2(0.f, 0.f);
+  }
+};
+
+template <int KIND, int MASKED, int WMODE>
+__device__ __forceinline__ void zone_run(const SlabLane<WMODE>& sl, const LaneTrack& L, const FarCoef& C, int jb, int je,
+                                         int Wm, float& u, unsigned lut_lane, LaneSums& s) {
+  int j = jb;
+  for (; j + 1 < je; j += 2) {
+    float4 Y0, Y1;
+    float2 W0, W1;
+    sl.load(j, Y0, W0);
+    sl.load(j + 1, Y1, W1);
+    pixel_kind<KIND, 0, WMODE, MASKED, kLutCopiesSlab>(L, C, j, Wm, Y0, W0, u, lut_lane, s);
+    pixel_kind<KIND, 0, WMODE, MASKED, kLutCopiesSlab>(L, C, j + 1, Wm, Y1, W1, u - 1.0f, lut_lane, s);
+    u -= 2.0f;
+  }
+  if (j < je) {
+    float4 Y0;
+    float2 W0;
+    sl.load(j, Y0, W0);
+    pixel_kind<KIND, 0, WMODE, MASKED, kLutCopiesSlab>(L, C, j, Wm, Y0, W0, u, lut_lane, s);
+    u -= 1.0f;
+  }
+}
+
+template <int KIND, int WMODE>
+__device__ __forceinline__ void zone_auto(const SlabLane<WMODE>& sl, const LaneTrack& L, const FarCoef& C, int jb, int je,
+                                          int Wm, int Wmin, float& u, unsigned lut_lane, LaneSums& s) {
+  const int jm = min(max(jb, Wmin), je);       // [jb, jm) unmasked, [jm, je) masked
+  if (jb < jm) zone_run<KIND, 0, WMODE>(sl, L, C, jb, jm, Wm, u, lut_lane, s);
+  if (jm < je) zone_run<KIND, 1, WMODE>(sl, L, C, jm, je, Wm, u, lut_lane, s);
+}
+
+template <int WMODE>
+__device__ __forceinline__ void pixel_loop_slab(const SlabLane<WMODE>& sl, const LaneTrack& L, const FarCoef& C, int Wm,
+                                                int Wmin, int Wmax, int J2A, int JA, int JB, int J2B, float u,
+                                                unsigned lut_lane, LaneSums& s) {
+  zone_auto<kZFar2, WMODE>(sl, L, C, 0, J2A, Wm, Wmin, u, lut_lane, s);
+  zone_auto<kZFar, WMODE>(sl, L, C, J2A, JA, Wm, Wmin, u, lut_lane, s);
+  zone_auto<kZNear, WMODE>(sl, L, C, JA, JB, Wm, Wmin, u, lut_lane, s);
+  zone_auto<kZFar, WMODE>(sl, L, C, JB, J2B, Wm, Wmin, u, lut_lane, s);
+  zone_auto<kZFar2, WMODE>(sl, L, C, J2B, Wmax, Wm, Wmin, u, lut_lane, s);
+}
+
+// ------------------------------------------------------------------------------------------
+// One work item: template `it` on time tile `tile` (rows a2-a7).  LANES ARE TRANCHES: lane l owns the
+// l-th valid (non-gap) tranche of the current chunk of 32, computes its track point in fp64 and then
+// walks its own window pixel by pixel.  Per chunk the window offsets are split (warp-uniformly) into the
+// NEAR zone around the track, evaluated from the shared-memory LUT, and the FAR zones, evaluated from
+// asymptotic polynomials in packed fp32.  The tranche's sums are multiplied by P, combined over the two
+// channels with the transfer factors (a6: constant per template, or interpolated at f_m from the
+// template's table, Eq. 29) and added to the lane's running sums of the current piece; when a piece
+// ends -- inside a chunk at a segment boundary, or at the end of the tile -- the lanes are summed with a
+// shuffle butterfly and the piece's partial {z, hh} is stored.
+// SLAB: pixels come from the shared-memory slab whose first row is row0 (eval_slab_kernel);
+// otherwise from global memory (eval_list_kernel).
+// ------------------------------------------------------------------------------------------
+template <int MODE, int WMODE, bool SLAB>
+__device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it, const int tile, const int lane,
+                                          const unsigned lut_lane, const unsigned slab_y, const unsigned slab_w,
+                                          const int row0) {
+  const TplConst T = a.tconst[it];
+  // valid (non-gap) tranches of the tile: entries [i0, i1) of the compacted list (C10), cut by the
+  // segment boundaries into pieces [p, p_stop)
+  const int i0 = tile * kTS, i1 = min(i0 + kTS, a.n_valid);
+  int p = a.tile_first[tile];
+  const int p_stop = a.tile_first[tile + 1];
+  int pend = p < p_stop ? a.piece_end[p] : i1;
+  float accr = 0.f, acci = 0.f, acch = 0.f;      // this lane's running sums of the current piece
+
+  // close piece p: sum the lanes (fp32 butterfly: 32 terms), store, reset
+  auto flush = [&]() {
+    float r0 = accr, r1 = acci, r2 = acch;
+    accr = 0.f; acci = 0.f; acch = 0.f;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      r0 += __shfl_xor_sync(0xffffffffu, r0, o);
+      r1 += __shfl_xor_sync(0xffffffffu, r1, o);
+      r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+    }
+    if (lane == 0) {
+      float4* dst = a.partials + (long long)p * a.n + it;
+      float4 v = make_float4(r0, r1, r2, 0.f);
+      if (a.accumulate) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; }
+      *dst = v;
+    }
+  };
+
+  for (int ic = i0; ic < i1; ic += 32) {
+    // ---------------- track point of this lane's tranche (a2) ----------------
+    const int i = ic + lane;
+    const bool valid = i < i1;
+    const int m = a.valid_m[valid ? i : i0];
+    const TrackPoint tp = track_point(T, m, a.DT, a.x_lo, a.x_hi, a.c_max, valid);
+    const unsigned act_mask = __ballot_sync(0xffffffffu, tp.active);
+    const int cend = min(ic + 32, i1);
+    const bool closes = p < p_stop && pend <= cend;   // a piece ends inside this chunk (warp-uniform)
+    float vr = 0.f, vi = 0.f, vq = 0.f;               // this tranche's contribution to z and hh
+    if (act_mask != 0u) {
+      int Wm = 0, k_lo = SLAB ? row0 : 0, ja = 0x7fffffff, jb = 0, j2a = 0x7fffffff, j2b = 0;
+      float u = -1.f, Pr = 0.f, Pi = 0.f;
+      LaneTrack L;        // inactive lanes: u_j = -1 - j, u_j + c = -0.5 - j (finite h' on finite data)
+      L.sc = 1.f; L.kap = 1.f; L.c = 0.5f; L.hc = 0.f; L.Er = 0.f; L.Ei = 0.f;
+      if (tp.active) {
+        int k_hi;
+        window(tp, a.H, a.adaptive, a.Nf, k_lo, k_hi);
+        Wm = k_hi - k_lo + 1;
+        const double flx = floor(tp.x);
+        const float fracx = (float)(tp.x - flx);
+        u = fracx - (float)(k_lo - (int)flx);          // cancellation-safe x - k_lo
+        // phases in turns, reduced in fp64 (phi reaches ~1e8 rad), then to [-1/2, 1/2)
+        double tphi = T.phic_turns - tp.X58 * (1.0 / kPi);
+        tphi -= floor(tphi);
+        double tpsi = 0.5 * tp.c + (tp.x - flx);
+        tpsi -= floor(tpsi);
+        float sphi, cphi, spsi, cpsi;
+        __sincosf(6.283185307179586f * ((float)tphi - 0.5f), &sphi, &cphi);     // = -(sin, cos)(2 pi tphi)
+        __sincosf(6.283185307179586f * ((float)tpsi - 0.5f), &spsi, &cpsi);
+        const float cf = (float)tp.c;
+        L.sc = rsqrtf(0.5f * cf);
+        L.kap = 0.5f * cf * L.sc;                                               // sqrt(c/2)
+        L.c = cf;
+        L.hc = __fdividef(0.5f, cf);
+        const float pre = -(T.acoef * tp.Xm14) * (0.5f * L.sc);               // -A_m / sqrt(2c)
+        Pr = pre * cphi;
+        Pi = pre * sphi;
+        L.Er = -cpsi;
+        L.Ei = -spsi;
+        // near zone of this lane: offsets j with |v0| < kVFar or |v1| < kVFar, i.e. -(c + d) < u - j < d
+        const float d = fmaf(kVFar, L.kap, 1e-3f);
+        ja = max((int)floorf(u - d) + 1, 0);
+        jb = (int)ceilf(u + cf + d);
+        if (SLAB) {
+          const float d2 = fmaf(kVFar2, L.kap, 1e-3f);   // offsets outside (j2a, j2b) have |v0|, |v1| >= kVFar2
+          j2a = max((int)floorf(u - d2) + 1, 0);
+          j2b = (int)ceilf(u + cf + d2);
+        }
+      }
+      const int Wmax = __reduce_max_sync(0xffffffffu, Wm);
+      const int Wmin = __reduce_min_sync(0xffffffffu, tp.active ? Wm : 0x7fffffff);
+      int JA = __reduce_min_sync(0xffffffffu, ja);
+      int JB = min(__reduce_max_sync(0xffffffffu, jb), Wmax);
+      if (MODE != 0) { JA = 0; JB = Wmax; }          // the paper's approximants are used for every pixel
+      JA = min(JA, JB);
+
+      // ---------------- pixel loop (a3-a5): lane walks its own window ----------------
+      LaneSums s;
+      s.zr = pk(0.f, 0.f); s.zi = pk(0.f, 0.f); s.q = pk(0.f, 0.f);
+      if (SLAB) {
+        const int J2A = min(__reduce_min_sync(0xffffffffu, j2a), JA);
+        const int J2B = max(min(__reduce_max_sync(0xffffffffu, j2b), Wmax), JB);
+        SlabLane<WMODE> sl;
+        const int rr = k_lo - row0;
+        const unsigned col = (unsigned)(ic - i0 + lane);
+        sl.y_addr = slab_y + ((unsigned)rr * kTS + col) * 16u;
+        sl.w_addr = WMODE == kWGeneral ? slab_w + ((unsigned)rr * kTS + col) * 8u : slab_w + (unsigned)rr * 8u;
+#ifdef TFS_BOUNDS_CHECK
+        sl.row_rel = rr; sl.rows = slab_rows(WMODE);
+        if (rr < 0 || rr + Wmax > slab_rows(WMODE)) __trap();
+#endif
+        pixel_loop_slab<WMODE>(sl, L, a.far, Wm, Wmin, Wmax, J2A, JA, JB, J2B, u, lut_lane, s);
+      } else {
+        const int stp = tp.active ? a.ncol : 0;
+        const int idx = tp.active ? k_lo * a.ncol + i : (valid ? i : i0);
+        pixel_loop_global<MODE, WMODE>(a, L, a.far, Wm, Wmin, Wmax, JA, JB, idx, stp, tp.active ? k_lo : 0,
+                                       tp.active ? 1 : 0, u, lut_lane, s);
+      }
+      // ---------------- a6: transfer factors, the tranche's factor P, weights a[i] ----------------
+      float T0r = T.T0r, T0i = T.T0i, T1r = T.T1r, T1i = T.T1i;
+      if (a.ttab != nullptr) {
+        // T_alpha(f_m) from the template's table: linear between knots, clamped outside (Eq. 29)
+        const int K = a.tt_K;
+        float sx = fmaf((float)tp.x, a.tt_scale, -a.tt_off);
+        sx = fminf(fmaxf(sx, 0.f), (float)(K - 1));
+        int kn = min((int)sx, max(K - 2, 0));
+        const float tf = K > 1 ? sx - (float)kn : 0.f;
+        const int kn1 = min(kn + 1, K - 1);
+        const float2* tb = a.ttab + ((size_t)it * a.tt_C + a.tt_ch0) * K;
+        const float2 A0 = __ldg(tb + kn), A1 = __ldg(tb + kn1);
+        T0r = fmaf(tf, A1.x - A0.x, A0.x); T0i = fmaf(tf, A1.y - A0.y, A0.y);
+        T1r = 0.f; T1i = 0.f;
+        if (a.tt_ch0 + 1 < a.tt_C && a.n_ch_pair > 1) {
+          const float2 B0 = __ldg(tb + K + kn), B1 = __ldg(tb + K + kn1);
+          T1r = fmaf(tf, B1.x - B0.x, B0.x); T1i = fmaf(tf, B1.y - B0.y, B0.y);
+        }
+      }
+      float zr0, zr1, zi0, zi1, q0, q1;
+      upk(s.zr, zr0, zr1); upk(s.zi, zi0, zi1); upk(s.q, q0, q1);
+      if (WMODE == kWTimeOnly) { q0 = q0 + q1; q1 = q0; }      // the loop summed {hr^2, hi^2}
+      // z' = T_0 z'_0 + T_1 z'_1 ;  q' = |T_0|^2 a_0 q'_0 + |T_1|^2 a_1 q'_1   (Eq. 29, Eq. 31)
+      const float zcr = fmaf(T0r, zr0, fmaf(-T0i, zi0, fmaf(T1r, zr1, -T1i * zi1)));
+      const float zci = fmaf(T0r, zi0, fmaf(T0i, zr0, fmaf(T1r, zi1, T1i * zr1)));
+      float w0 = fmaf(T0r, T0r, T0i * T0i), w1 = fmaf(T1r, T1r, T1i * T1i);
+      if (WMODE != kWGeneral) {
+        const float2 am = __ldg(a.wa + (valid ? i : i0));
+        w0 *= am.x; w1 *= am.y;
+      }
+      const float P2 = fmaf(Pr, Pr, Pi * Pi);
+      vr = fmaf(Pr, zcr, -Pi * zci);                  // Re (P z')
+      vi = fmaf(Pr, zci, Pi * zcr);                   // Im (P z')
+      vq = P2 * fmaf(w0, q0, w1 * q1);
+      if (!closes) { accr += vr; acci += vi; acch += vq; }    // the usual case: the whole chunk belongs to the current piece
+    }
+    if (closes) {
+      // every piece that ends inside this chunk (a segment boundary, or the end of the tile) takes the
+      // lanes before its end and is closed; the lanes behind the last such end open the next piece
+      int lo = 0;
+      for (;;) {
+        const bool ends = p < p_stop && pend <= cend;
+        const int hi = ends ? pend - ic : 32;
+        if (lane >= lo && lane < hi) { accr += vr; acci += vi; acch += vq; }
+        if (!ends) break;
+        flush();
+        ++p;
+        if (p < p_stop) pend = a.piece_end[p];
+        lo = hi;
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// mbarrier / TMA primitives (PTX ISA: mbarrier, cp.async.bulk, cp.async.bulk.tensor)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" :: "r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap* map, int c0, int c1, unsigned bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+               :: "r"(dst), "l"((unsigned long long)map), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_load_1d(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               :: "r"(dst), "l"((unsigned long long)src), "r"(bytes), "r"(bar) : "memory");
+}
+
+// dynamic shared memory of the slab kernel
+//   [LUT: (kLutN+1) * kLutCopiesSlab float4][stage 0][stage 1][control]
+//   stage = data slab [rows][kTS] float4, then (kWGeneral) weight slab [rows][kTS] float2
+//           or (kWSeparable) rows of the b table [rows] float2
+constexpr int kLutSlabBytes = ((kLutN + 1) * kLutCopiesSlab * (int)sizeof(float4) + 127) / 128 * 128;   // slabs start 128-byte aligned
+__host__ __device__ constexpr int slab_y_bytes(int wmode) { return slab_rows(wmode) * kTS * 16; }
+__host__ __device__ constexpr int slab_w_bytes(int wmode) {
+  return wmode == kWGeneral ? slab_rows(wmode) * kTS * 8 : (wmode == kWSeparable ? slab_rows(wmode) * 8 : 0);
+}
+__host__ __device__ constexpr int slab_stage_bytes(int wmode) { return (slab_y_bytes(wmode) + slab_w_bytes(wmode) + 127) / 128 * 128; }
+constexpr int kSlabCtlBytes = 128;        // full[2], empty[2] mbarriers, 2 unit descriptors, 2 item counters
+__host__ __device__ constexpr int slab_smem_bytes(int wmode) { return kLutSlabBytes + 2 * slab_stage_bytes(wmode) + kSlabCtlBytes; }
+static_assert(slab_smem_bytes(kWGeneral) <= 232448 && slab_smem_bytes(kWSeparable) <= 232448, "slab kernel exceeds 227 KB of shared memory");
+
+struct SlabCtl {
+  unsigned long long full[2], empty[2];
+  Unit unit[2];
+  unsigned next_item[2];
+};
+static_assert(sizeof(SlabCtl) <= kSlabCtlBytes, "SlabCtl");
+
+// ------------------------------------------------------------------------------------------
+// eval_slab_kernel: persistent, one CTA of 32 warps per SM.  Thread 0 is also the producer: it claims the
+// next unit from the global counter, posts its descriptor and issues the TMA copies of the band's slab
+// into the stage's buffer; the stage's `full` mbarrier completes when the bytes have landed.  Every warp
+// then takes items of the unit from the stage's counter until it is exhausted, arrives on the stage's
+// `empty` mbarrier and moves on to the other stage; the producer refills a stage once all 32 warps have
+// left it.  Units come in tile-major, band-major order, so consecutive units mostly reload the same slab
+// from the L2.
+// ------------------------------------------------------------------------------------------
+template <int WMODE>
+__global__ void __launch_bounds__(kWarpsPerCta * 32, 1)
+eval_slab_kernel(const EvalArgs a, const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_w) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float4* s_lut = reinterpret_cast<float4*>(smem_raw);
+  SlabCtl* ctl = reinterpret_cast<SlabCtl*>(smem_raw + kLutSlabBytes + 2 * slab_stage_bytes(WMODE));
+  const unsigned smem_base = (unsigned)__cvta_generic_to_shared(smem_raw);
+  const unsigned stage_base = smem_base + kLutSlabBytes;
+  const unsigned ctl_base = stage_base + 2 * slab_stage_bytes(WMODE);
+  const unsigned bar_full = ctl_base + (unsigned)offsetof(SlabCtl, full);
+  const unsigned bar_empty = ctl_base + (unsigned)offsetof(SlabCtl, empty);
+  constexpr int R = slab_rows(WMODE);
+
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int i = threadIdx.x; i < (kLutN + 1) * kLutCopiesSlab; i += blockDim.x) s_lut[i] = a.lut[i / kLutCopiesSlab];
+  if (threadIdx.x == 0) {
+    mbar_init(bar_full, 1); mbar_init(bar_full + 8, 1);
+    mbar_init(bar_empty, kWarpsPerCta); mbar_init(bar_empty + 8, kWarpsPerCta);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const unsigned lut_lane = smem_base + 16u * (unsigned)(lane & (kLutCopiesSlab - 1)) - kMagicBits * (16u * kLutCopiesSlab);
+  const int n_units = a.n_units[0];
+
+  // producer: claim the next unit and fill stage s with it
+  auto produce = [&](int s) {
+    const unsigned long long uid = atomicAdd(a.work_counter, 1ULL);
+    Unit d;
+    if (uid < (unsigned long long)n_units) d = a.units_slab[uid];
+    else { d.tile = 0; d.row0 = 0; d.off = 0; d.cnt = -1; }
+    ctl->unit[s] = d;
+    ctl->next_item[s] = 0;
+    const unsigned bar = bar_full + 8u * s;
+    if (d.cnt < 0) { mbar_arrive(bar); return; }
+    const unsigned dst = stage_base + (unsigned)s * slab_stage_bytes(WMODE);
+    mbar_arrive_expect_tx(bar, (unsigned)(slab_y_bytes(WMODE) + slab_w_bytes(WMODE)));
+    tma_load_2d(dst, &map_y, d.tile * kTS * 4, d.row0, bar);
+    if (WMODE == kWGeneral) tma_load_2d(dst + slab_y_bytes(WMODE), &map_w, d.tile * kTS * 2, d.row0, bar);
+    if (WMODE == kWSeparable) bulk_load_1d(dst + slab_y_bytes(WMODE), a.wb + d.row0, R * 8, bar);
+  };
+  if (threadIdx.x == 0) { produce(0); produce(1); }
+
+  int stage = 0;
+  unsigned phase = 0;
+  for (;;) {
+    mbar_wait(bar_full + 8u * stage, phase);
+    const Unit d = ctl->unit[stage];
+    if (d.cnt < 0) break;
+    const unsigned slab_y = stage_base + (unsigned)stage * slab_stage_bytes(WMODE);
+    const unsigned slab_w = slab_y + slab_y_bytes(WMODE);
+    for (;;) {
+      int k = 0;
+      if (lane == 0) k = (int)atomicAdd(&ctl->next_item[stage], 1u);
+      k = __shfl_sync(0xffffffffu, k, 0);
+      if (k >= d.cnt) break;
+      const long long it = (long long)a.list[d.off + (unsigned)k];
+      eval_item<0, WMODE, true>(a, it, d.tile, lane, lut_lane, slab_y, slab_w, d.row0);
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_empty + 8u * stage);
+    if (warp == 0) {
+      if (lane == 0) {
+        mbar_wait(bar_empty + 8u * stage, phase);       // all 32 warps have left the stage
+        produce(stage);
+      }
+      __syncwarp();
+    }
+    stage ^= 1;
+    if (stage == 0) phase ^= 1u;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// eval_list_kernel: the items the slab kernel cannot take (and every item when fresnel_mode = 1).
+// Persistent: one CTA per SM, warps claim units of <= kListUnitItems items of one tile, in tile-major
+// order so that the tile's columns stay L2-resident, and gather from global memory.
+// ------------------------------------------------------------------------------------------
+constexpr int kLutListBytes = (kLutN + 1) * kLutCopiesList * (int)sizeof(float4);
+
+template <int MODE, int WMODE>
+__global__ void __launch_bounds__(kWarpsPerCta * 32, 1)
+eval_list_kernel(const EvalArgs a) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float4* s_lut = reinterpret_cast<float4*>(smem_raw);
+  const int lane = threadIdx.x & 31;
+  if (MODE == 0) {
+    for (int i = threadIdx.x; i < (kLutN + 1) * kLutCopiesList; i += blockDim.x) s_lut[i] = a.lut[i / kLutCopiesList];
+    __syncthreads();
+  }
+  const unsigned lut_lane = (unsigned)__cvta_generic_to_shared(s_lut) + 16u * (unsigned)(lane & (kLutCopiesList - 1)) -
+                            kMagicBits * (16u * kLutCopiesList);
+  const int n_units = a.n_units[1];
+  for (;;) {
+    unsigned long long uid = 0;
+    if (lane == 0) uid = atomicAdd(a.work_counter + 1, 1ULL);
+    uid = __shfl_sync(0xffffffffu, uid, 0);
+    if (uid >= (unsigned long long)n_units) break;
+    const Unit d = a.units_list[uid];
+    for (int k = 0; k < d.cnt; ++k) {
+      const long long it = (long long)a.list[d.off + (unsigned)k];
+      eval_item<MODE, WMODE, false>(a, it, d.tile, lane, lut_lane, 0u, 0u, 0);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Pre-pass (per batch).
+// ------------------------------------------------------------------------------------------
+__global__ void prep_consts_kernel(const EvalArgs a) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= a.n) return;
+  const TplConst t = load_template(a.params + i * 8, a.DT, a.t_col, a.n_ch_pair);
+  a.tconst[i] = t;
+  if (a.bad_count != nullptr && !t.ok) atomicAdd(a.bad_count, 1ULL);
+}
+
+// Bucket of item (template i, tile t), from the track at the tile's first and last valid tranche (x and c
+// grow with time, so they bound every tranche in between):
+//   0  no tranche of the tile can be active (merged before the tile, above the band or too fast at its
+//      start, below the band at its end, bad row): the item is skipped and its partials are never read;
+//   1  list kernel: the template merges inside the tile, or the rows its lanes can touch
+//      [k_lo(first), ceil(x_last) + floor(c_last) + H + 3] do not fit the slab of its band (a lane reads
+//      Wmax <= floor(c_last) + 2H + 2 rows from its own k_lo <= ceil(x_last) - H, the longest window of its
+//      chunk; rows past Nf + kPadRows do not exist and the TMA copy fills them with zeros);
+//   2+b  slab kernel, band b = k_lo(first) / kBandStride.
+// The skip tests carry a relative slack of 1e-9, so an item is never dropped on a rounding difference
+// against the per-lane tests (an item kept needlessly just yields zeros).
+__device__ __forceinline__ int item_key(const EvalArgs& a, const TplConst& T, int tile) {
+  if (!T.ok) return 0;
+  const int i0 = tile * kTS, i1 = min(i0 + kTS, a.n_valid);
+  if (i0 >= i1) return 0;
+  const int m0 = a.valid_m[i0], m1 = a.valid_m[i1 - 1];
+  const TrackPoint t0 = track_point(T, m0, a.DT, -1.0, 1e300, 1e300, true);
+  if (!t0.active) return 0;                                        // tau <= DT at the tile's start
+  const double slack = 1.0 + 1e-9;
+  if (t0.x + t0.c > a.x_hi * slack || t0.c > a.c_max * slack) return 0;
+  const TrackPoint t1 = track_point(T, m1, a.DT, -1.0, 1e300, 1e300, true);
+  if (!t1.active) return 1;                                        // merges inside the tile
+  if (t1.x * slack < a.x_lo) return 0;
+  if (!a.slab_ok) return 1;
+  if (!(t1.c <= 1e6) || !(t1.x <= 2.0e9)) return 1;
+  const int klo = min(max((int)ceil(t0.x) - a.H, 1), a.Nf - 1);
+  int ktop = (int)ceil(t1.x) + (a.adaptive ? (int)floor(t1.c) : 0) + a.H + 3;
+  const int b = klo / kBandStride;
+  if (ktop >= b * kBandStride + slab_rows(a.wmode) || ktop < klo) return 1;
+  return 2 + b;
+}
+
+// grid (ceil(n/256), n_tiles): keys of the tile's items + the tile's bucket counts
+__global__ void __launch_bounds__(256)
+prep_keys_kernel(const EvalArgs a) {
+  extern __shared__ unsigned s_hist[];                              // [n_keys]
+  for (int k = threadIdx.x; k < a.n_keys; k += blockDim.x) s_hist[k] = 0;
+  __syncthreads();
+  const int tile = blockIdx.y;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < a.n) {
+    const int key = item_key(a, a.tconst[i], tile);
+    a.keys[(size_t)tile * a.n + i] = (uint16_t)key;
+    if (key) atomicAdd(&s_hist[key], 1u);
+  }
+  __syncthreads();
+  for (int k = threadIdx.x; k < a.n_keys; k += blockDim.x)
+    if (s_hist[k]) atomicAdd(&a.counts[(size_t)tile * a.n_keys + k], s_hist[k]);
+}
+
+// one CTA: exclusive scan of the bucket counts (tile-major, key-major) -> bucket_off; unit tables; the
+// counts are zeroed (they become the scatter cursors)
+__global__ void __launch_bounds__(1024)
+prep_scan_kernel(const EvalArgs a) {
+  __shared__ unsigned s_items[1024], s_us[1024], s_ul[1024];
+  const int nb = a.n_tiles * a.n_keys;
+  const int per = (nb + 1023) / 1024;
+  const int b0 = min((int)threadIdx.x * per, nb), b1 = min(b0 + per, nb);
+  unsigned items = 0, us = 0, ul = 0;
+  for (int b = b0; b < b1; ++b) {
+    const int key = b % a.n_keys;
+    const unsigned c = key ? a.counts[b] : 0u;
+    items += c;
+    if (key >= 2) us += (c + kUnitItems - 1) / kUnitItems;
+    if (key == 1) ul += (c + kListUnitItems - 1) / kListUnitItems;
+  }
+  s_items[threadIdx.x] = items; s_us[threadIdx.x] = us; s_ul[threadIdx.x] = ul;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {                             // inclusive Hillis-Steele scans
+    unsigned v0 = 0, v1 = 0, v2 = 0;
+    if ((int)threadIdx.x >= o) { v0 = s_items[threadIdx.x - o]; v1 = s_us[threadIdx.x - o]; v2 = s_ul[threadIdx.x - o]; }
+    __syncthreads();
+    s_items[threadIdx.x] += v0; s_us[threadIdx.x] += v1; s_ul[threadIdx.x] += v2;
+    __syncthreads();
+  }
+  unsigned off = s_items[threadIdx.x] - items, iu = s_us[threadIdx.x] - us, il = s_ul[threadIdx.x] - ul;
+  for (int b = b0; b < b1; ++b) {
+    const int key = b % a.n_keys, tile = b / a.n_keys;
+    const unsigned c = key ? a.counts[b] : 0u;
+    a.bucket_off[b] = off;
+    a.counts[b] = 0;
+    if (key >= 2) {
+      for (unsigned o = 0; o < c; o += kUnitItems) {
+        Unit u; u.tile = tile; u.row0 = (key - 2) * kBandStride; u.off = off + o; u.cnt = (int)min(c - o, (unsigned)kUnitItems);
+        a.units_slab[iu++] = u;
+      }
+    } else if (key == 1) {
+      for (unsigned o = 0; o < c; o += kListUnitItems) {
+        Unit u; u.tile = tile; u.row0 = 0; u.off = off + o; u.cnt = (int)min(c - o, (unsigned)kListUnitItems);
+        a.units_list[il++] = u;
+      }
+    }
+    off += c;
+  }
+  if (threadIdx.x == 1023) { a.n_units[0] = (int)s_us[1023]; a.n_units[1] = (int)s_ul[1023]; }
+}
+
+// grid as prep_keys_kernel: template indices into their bucket's range of `list` (order inside a bucket is
+// arbitrary: every item writes its own partials, so the results do not depend on it)
+__global__ void __launch_bounds__(256)
+prep_scatter_kernel(const EvalArgs a) {
+  extern __shared__ unsigned s_hist[];                              // [2][n_keys]: count, then base
+  unsigned* s_cnt = s_hist;
+  unsigned* s_base = s_hist + a.n_keys;
+  for (int k = threadIdx.x; k < a.n_keys; k += blockDim.x) s_cnt[k] = 0;
+  __syncthreads();
+  const int tile = blockIdx.y;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int key = 0;
+  unsigned rank = 0;
+  if (i < a.n) {
+    key = a.keys[(size_t)tile * a.n + i];
+    if (key) rank = atomicAdd(&s_cnt[key], 1u);
+  }
+  __syncthreads();
+  for (int k = threadIdx.x; k < a.n_keys; k += blockDim.x)
+    if (s_cnt[k]) s_base[k] = atomicAdd(&a.counts[(size_t)tile * a.n_keys + k], s_cnt[k]);
+  __syncthreads();
+  if (key) a.list[a.bucket_off[(size_t)tile * a.n_keys + key] + s_base[key] + rank] = (unsigned)i;
+}
 
 // Piece table (C9, C10).  Segment n = tranches [ceil(n Nt/N_seg), ceil((n+1) Nt/N_seg)), i.e. n(m) =
-// floor(m N_seg / Nt).  Tile t = entries [t kTileMax, (t+1) kTileMax) of the compacted valid-tranche list.
+// floor(m N_seg / Nt).  Tile t = entries [t kTS, (t+1) kTS) of the compacted valid-tranche list.
 // A piece is a maximal run of entries inside one tile and one segment; pieces are numbered in time order.
 // One thread walks the list (<= n_tiles + N_seg pieces); the table is cached per N_seg by the host.
 //   tile_first[t] = first piece of tile t, tile_first[n_tiles] = number of pieces
-//   piece_end[p]  = entry where piece p ends (exclusive);  piece_seg[p] = its segment
+//   piece_end[p]  = entry where piece p ends (exclusive);  piece_seg[p] = its segment;  piece_tile[p] = its tile
 __global__ void piece_table_kernel(const int* __restrict__ vprefix, const int* __restrict__ valid_m, int Nt, int N_seg,
                                    int n_valid, int n_tiles, int* __restrict__ tile_first,
-                                   int* __restrict__ piece_end, int* __restrict__ piece_seg) {
+                                   int* __restrict__ piece_end, int* __restrict__ piece_seg, int* __restrict__ piece_tile) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
   int p = 0;
   for (int t = 0; t < n_tiles; ++t) {
     tile_first[t] = p;
-    int i = t * kTileMax;
-    const int iend = min(i + kTileMax, n_valid);
+    int i = t * kTS;
+    const int iend = min(i + kTS, n_valid);
     while (i < iend) {
       const int seg = (int)(((long long)valid_m[i] * N_seg) / Nt);
       const int s1 = (int)(((long long)(seg + 1) * Nt + N_seg - 1) / N_seg);     // first tranche of the next segment
       const int e = min(vprefix[min(s1, Nt)], iend);
       piece_seg[p] = seg;
       piece_end[p] = e;
+      piece_tile[p] = t;
       ++p;
       i = e;
     }
@@ -483,212 +1096,29 @@ __global__ void piece_table_kernel(const int* __restrict__ vprefix, const int* _
   tile_first[n_tiles] = p;
 }
 
-__host__ __device__ constexpr int warps_per_cta(int wmode) {
-  return wmode == 0 ? TFS_WARPS_GENERAL : TFS_WARPS_SEPARABLE;      // 0 = kWGeneral (declared below)
-}
-
-template <int MODE, int WMODE>
-__global__ void __launch_bounds__(warps_per_cta(WMODE) * 32, 1)
-eval_tiles_kernel(const EvalArgs a) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  float4* s_lut = reinterpret_cast<float4*>(smem_raw);
-  f2_t* s_acc = reinterpret_cast<f2_t*>(smem_raw + kLutSmemBytes) + threadIdx.x;       // [3][blockDim]
-  constexpr int kAccStride = warps_per_cta(WMODE) * 32;
-
-  const int lane = threadIdx.x & 31;
-  if (MODE == 0) {
-    for (int i = threadIdx.x; i < (kLutN + 1) * kLutCopies; i += blockDim.x) s_lut[i] = a.lut[i / kLutCopies];
-    __syncthreads();
-  }
-  const unsigned lut_lane = (unsigned)__cvta_generic_to_shared(s_lut) + 16u * (unsigned)(lane & (kLutCopies - 1)) -
-                            kMagicBits * (16u * kLutCopies);
-
-  const long long n_work = a.n * (long long)a.n_tiles;
-  for (;;) {
-    long long w0 = 0;
-    if (lane == 0) w0 = (long long)atomicAdd(a.work_counter, (unsigned long long)kClaim);
-    w0 = __shfl_sync(0xffffffffu, w0, 0);
-    if (w0 >= n_work) break;
-    const int n_claim = (int)min((long long)kClaim, n_work - w0);
-    int tile = (int)(w0 / a.n);
-    long long it = w0 - (long long)tile * a.n;
-    for (int wi = 0; wi < n_claim; ++wi, ++it) {
-      if (it == a.n) { it = 0; ++tile; }
-      // valid (non-gap) tranches of the tile: entries [i0, i1) of the compacted list (C10), cut by the
-      // segment boundaries into pieces [p, p_last]
-      const int i0 = tile * kTileMax, i1 = min(i0 + kTileMax, a.n_valid);
-      int p = a.tile_first[tile];
-      const int p_stop = a.tile_first[tile + 1];
-
-      const TemplateConst T = load_template(a.params + it * 8, a.DT);
-      if (!T.ok) {
-        for (int q = p + lane; q < p_stop; q += 32) a.partials[(long long)q * a.n + it] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (lane == 0 && tile == 0) atomicAdd(a.bad_count, 1ULL);
-        continue;
-      }
-      int pend = p < p_stop ? a.piece_end[p] : i1;
-
-      // per-lane running sums over the current piece ({A, E} pairs of Re z, Im z, q; <= kTileMax/32 chunk sums
-      // each, fp32) live in shared memory; lanes, pieces and segments are then summed in fp64
-#pragma unroll
-      for (int v = 0; v < 3; ++v) s_acc[v * kAccStride] = pk(0.f, 0.f);
-
-      // close piece p: sum its per-lane sums over the warp (packed fp32 butterfly: 32 terms), combine the
-      // channels in fp64, store, reset
-      auto flush = [&]() {
-        f2_t r0 = s_acc[0 * kAccStride], r1 = s_acc[1 * kAccStride], r2 = s_acc[2 * kAccStride];
-#pragma unroll
-        for (int v = 0; v < 3; ++v) s_acc[v * kAccStride] = pk(0.f, 0.f);
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-          r0 = fadd2(r0, __shfl_xor_sync(0xffffffffu, r0, o));
-          r1 = fadd2(r1, __shfl_xor_sync(0xffffffffu, r1, o));
-          r2 = fadd2(r2, __shfl_xor_sync(0xffffffffu, r2, o));
-        }
-        if (lane == 0) {
-          float zAr, zEr, zAi, zEi, qA, qE;
-          upk(r0, zAr, zEr); upk(r1, zAi, zEi); upk(r2, qA, qE);
-          const double dzAr = zAr, dzAi = zAi, dzEr = zEr, dzEi = zEi, dqA = qA, dqE = qE;
-          // z = T_A z_A + T_E z_E ; hh = |T_A|^2 q_A + |T_E|^2 q_E   (Eq. 29, Eq. 31)
-          const double zr = T.TAr * dzAr - T.TAi * dzAi + T.TEr * dzEr - T.TEi * dzEi;
-          const double zi = T.TAr * dzAi + T.TAi * dzAr + T.TEr * dzEi + T.TEi * dzEr;
-          const double hh = (T.TAr * T.TAr + T.TAi * T.TAi) * dqA + (T.TEr * T.TEr + T.TEi * T.TEi) * dqE;
-          a.partials[(long long)p * a.n + it] = make_float4((float)zr, (float)zi, (float)hh, 0.f);
-        }
-      };
-
-      for (int ic = i0; ic < i1; ic += 32) {
-        // ---------------- track point of this lane's tranche (a2) ----------------
-        const int i = ic + lane;
-        const bool valid = i < i1;
-        const int m = a.valid_m[valid ? i : i0];
-        const TrackPoint tp = track_point(T, m, a.DT, a.x_lo, a.x_hi, a.c_max, valid);
-        const unsigned act_mask = __ballot_sync(0xffffffffu, tp.active);
-        const int cend = min(ic + 32, i1);
-        const bool closes = p < p_stop && pend <= cend;   // a piece ends inside this chunk (warp-uniform)
-        f2_t vr = pk(0.f, 0.f), vi = vr, vq = vr;          // this chunk's per-lane contribution (P z', |P|^2 a q')
-        if (act_mask != 0u) {
-        int Wm = 0, idx = m, stp = 0, kb = 0, kstp = 0, ja = 0x7fffffff, jb = 0;
-        float u = -1.f, Pr = 0.f, Pi = 0.f;
-        LaneTrack L;        // inactive lanes: u_j = -1 - j, u_j + c = -0.5 - j (finite h' on zeroed data)
-        L.sc = 1.f; L.kap = 1.f; L.c = 0.5f; L.hc = 0.f; L.Er = 0.f; L.Ei = 0.f;
-        if (tp.active) {
-          int k_lo, k_hi;
-          window(tp, a.H, a.adaptive, a.Nf, k_lo, k_hi);
-          Wm = k_hi - k_lo + 1;
-          idx = k_lo * a.Nt + m;
-          stp = a.Nt;
-          kb = k_lo;
-          kstp = 1;
-          const double flx = floor(tp.x);
-          const float fracx = (float)(tp.x - flx);
-          u = fracx - (float)(k_lo - (int)flx);          // cancellation-safe x - k_lo
-          // phases in turns, reduced in fp64 (phi reaches ~1e8 rad), then to [-1/2, 1/2)
-          double tphi = T.phic_turns - tp.X58 * (1.0 / kPi);
-          tphi -= floor(tphi);
-          double tpsi = 0.5 * tp.c + (tp.x - flx);
-          tpsi -= floor(tpsi);
-          float sphi, cphi, spsi, cpsi;
-          __sincosf(6.283185307179586f * ((float)tphi - 0.5f), &sphi, &cphi);     // = -(sin, cos)(2 pi tphi)
-          __sincosf(6.283185307179586f * ((float)tpsi - 0.5f), &spsi, &cpsi);
-          const float cf = (float)tp.c;
-          L.sc = rsqrtf(0.5f * cf);
-          L.kap = 0.5f * cf * L.sc;                                               // sqrt(c/2)
-          L.c = cf;
-          L.hc = __fdividef(0.5f, cf);
-          const float pre = -(T.acoef * tp.Xm14) * (0.5f * L.sc);               // -A_m / sqrt(2c)
-          Pr = pre * cphi;
-          Pi = pre * sphi;
-          L.Er = -cpsi;
-          L.Ei = -spsi;
-          // near zone of this lane: offsets j with |v0| < kVFar or |v1| < kVFar, i.e. -(c + d) < u - j < d
-          const float d = fmaf(kVFar, L.kap, 1e-3f);
-          ja = max((int)floorf(u - d) + 1, 0);
-          jb = (int)ceilf(u + cf + d);
-        }
-        const int Wmax = __reduce_max_sync(0xffffffffu, Wm);
-        const int Wmin = __reduce_min_sync(0xffffffffu, tp.active ? Wm : 0x7fffffff);
-        int JA = __reduce_min_sync(0xffffffffu, ja);
-        int JB = min(__reduce_max_sync(0xffffffffu, jb), Wmax);
-        if (MODE != 0) { JA = 0; JB = Wmax; }          // the paper's approximants are used for every pixel
-        JA = min(JA, JB);
-
-        // ---------------- pixel loop (a3-a5): lane walks its own window ----------------
-        LaneSums s;
-        s.zr = pk(0.f, 0.f); s.zi = pk(0.f, 0.f); s.q = pk(0.f, 0.f);
-        pixel_loop<MODE, WMODE>(a, L, a.far, Wm, Wmin, Wmax, JA, JB, idx, stp, kb, kstp, u, lut_lane, s);
-        // apply the tranche's factor P to z' and |P|^2 (times a[m] for separable weights) to q'
-        const float P2 = fmaf(Pr, Pr, Pi * Pi);
-        f2_t qs = s.q, qc = pk(P2, P2);
-        if (WMODE != kWGeneral) {
-          // W = a[m] b[k]: the pixel loop summed b |h'|^2 (b = 1: {sum hr^2, sum hi^2})
-          const float2 am = __ldg(a.wa + m);
-          qc = pk(P2 * am.x, P2 * am.y);
-          if (WMODE == kWTimeOnly) {
-            float q0, q1;
-            upk(s.q, q0, q1);
-            qs = pk(q0 + q1, q0 + q1);
-          }
-        }
-        if (!closes) {
-          // the usual case: the whole chunk belongs to the current piece
-          f2_t accr = s_acc[0 * kAccStride], acci = s_acc[1 * kAccStride];
-          accr = ffma2(pk(Pr, Pr), s.zr, accr);          // Re (P z') = Pr zr - Pi zi
-          accr = ffma2(pk(-Pi, -Pi), s.zi, accr);
-          acci = ffma2(pk(Pr, Pr), s.zi, acci);          // Im (P z') = Pr zi + Pi zr
-          acci = ffma2(pk(Pi, Pi), s.zr, acci);
-          s_acc[0 * kAccStride] = accr;
-          s_acc[1 * kAccStride] = acci;
-          s_acc[2 * kAccStride] = ffma2(qc, qs, s_acc[2 * kAccStride]);
-        } else {
-          vr = fmul2(pk(Pr, Pr), s.zr);
-          vr = ffma2(pk(-Pi, -Pi), s.zi, vr);
-          vi = fmul2(pk(Pr, Pr), s.zi);
-          vi = ffma2(pk(Pi, Pi), s.zr, vi);
-          vq = fmul2(qc, qs);
-        }
-        }
-        if (closes) {
-          // every piece that ends inside this chunk (a segment boundary, or the end of the tile) takes the
-          // lanes before its end and is closed; the lanes behind the last such end open the next piece
-          int lo = 0;
-          for (;;) {
-            const bool ends = p < p_stop && pend <= cend;
-            const int hi = ends ? pend - ic : 32;
-            if (lane >= lo && lane < hi) {
-              s_acc[0 * kAccStride] = fadd2(s_acc[0 * kAccStride], vr);
-              s_acc[1 * kAccStride] = fadd2(s_acc[1 * kAccStride], vi);
-              s_acc[2 * kAccStride] = fadd2(s_acc[2 * kAccStride], vq);
-            }
-            if (!ends) break;
-            flush();
-            ++p;
-            if (p < p_stop) pend = a.piece_end[p];
-            lo = hi;
-          }
-        }
-      }
-    }
-  }
-}
-
 // ------------------------------------------------------------------------------------------
-// Kernel B: sum the piece partials of each segment, P_n = |z_n|^2/hh_n, Upsilon = sum_n P_n (Eq. 8, 9).
-// Pieces are in time order, so the pieces of a segment are consecutive; a segment without a valid
-// tranche has no piece and contributes 0.
+// combine_kernel: sum the piece partials of each segment, P_n = |z_n|^2/hh_n, Upsilon = sum_n P_n
+// (Eq. 8, 9), fp64.  Pieces are in time order, so the pieces of a segment are consecutive; a segment
+// without a valid tranche has no piece and contributes 0; the partials of an item whose bucket is 0 were
+// never written and are not read.
 // ------------------------------------------------------------------------------------------
-__global__ void combine_kernel(const float4* __restrict__ partials, long long n, int N_seg,
+__global__ void combine_kernel(const float4* __restrict__ partials, const uint16_t* __restrict__ keys, long long n, int N_seg,
                                const int* __restrict__ tile_first, int n_tiles, const int* __restrict__ piece_seg,
+                               const int* __restrict__ piece_tile,
                                float* __restrict__ upsilon, float* __restrict__ seg_power,
                                float* __restrict__ seg_dh, float* __restrict__ seg_hh) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int n_pieces = tile_first[n_tiles];
   double ups = 0.0;
-  int p = 0;
+  int p = 0, cur_tile = -1;
+  bool live = false;
   for (int s = 0; s < N_seg; ++s) {
     double zr = 0, zi = 0, hh = 0;
     for (; p < n_pieces && piece_seg[p] == s; ++p) {
+      const int t = piece_tile[p];
+      if (t != cur_tile) { cur_tile = t; live = keys[(size_t)t * n + i] != 0; }
+      if (!live) continue;
       const float4 v = partials[(long long)p * n + i];
       zr += v.x; zi += v.y; hh += v.z;
     }
@@ -708,7 +1138,7 @@ __global__ void count_pixels_kernel(const EvalArgs a, long long* __restrict__ co
   const int lane = threadIdx.x & 31;
   const long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= a.n) return;
-  const TemplateConst T = load_template(a.params + w * 8, a.DT);
+  const TplConst T = load_template(a.params + w * 8, a.DT, -1, 0);
   long long cnt = 0;
   if (T.ok) {
     for (int m = lane; m < a.Nt; m += 32) {
@@ -726,11 +1156,15 @@ __global__ void count_pixels_kernel(const EvalArgs a, long long* __restrict__ co
 }
 
 // ------------------------------------------------------------------------------------------
-// Upload (a0): Y = W*D interleaved by channel and W interleaved, transposed to time-contiguous
-// [k][m] through a 32x32 shared-memory tile (reads coalesced along k, writes coalesced along m).
+// Upload (a0): Y = W*D interleaved by channel and W interleaved, transposed to time-contiguous [k][i]
+// over the compacted list of valid tranches (i = vprefix[m]; gap tranches are not stored) through a
+// 32x32 shared-memory tile (reads coalesced along k, writes coalesced along i).  Channel c1 < 0: the
+// second half of the pair is empty (zeros).  The arrays are zeroed before this kernel runs, so pad rows
+// and pad columns stay zero.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, int Nt, int Nf,
+pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, int Nt, int Nf, int c0, int c1,
+            const uint8_t* __restrict__ gap, const int* __restrict__ vprefix, int ncol,
             float4* __restrict__ grid, float2* __restrict__ wgt) {
   __shared__ float4 sY[32][33];
   __shared__ float2 sW[32][33];
@@ -741,11 +1175,11 @@ pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, 
     const int m = m0 + r, k = k0 + tx;
     if (m < Nt && k < Nf) {
       const long long i = (long long)m * Nf + k;
-      float2 dA = coeff[i], dE = coeff[npix + i];
-      float wA = weight ? weight[i] : 1.0f;
-      float wE = weight ? weight[npix + i] : 1.0f;
+      float2 dA = coeff[c0 * npix + i], dE = c1 >= 0 ? coeff[c1 * npix + i] : make_float2(0.f, 0.f);
+      float wA = weight ? weight[c0 * npix + i] : 1.0f;
+      float wE = c1 >= 0 ? (weight ? weight[c1 * npix + i] : 1.0f) : 0.f;
       // a pixel whose product W*D is not finite carries no information: weight 0 (also keeps every
-      // value the gather can read finite, which pixel_loop relies on)
+      // value the gather can read finite, which the pixel loops rely on)
       if (!(isfinite(wA * dA.x) && isfinite(wA * dA.y) && isfinite(wA))) { wA = 0.f; dA = make_float2(0.f, 0.f); }
       if (!(isfinite(wE * dE.x) && isfinite(wE * dE.y) && isfinite(wE))) { wE = 0.f; dE = make_float2(0.f, 0.f); }
       sY[r][tx] = make_float4(wA * dA.x, wE * dE.x, wA * dA.y, wE * dE.y);
@@ -755,8 +1189,8 @@ pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, 
   __syncthreads();
   for (int r = ty; r < 32; r += 8) {
     const int k = k0 + r, m = m0 + tx;
-    if (m < Nt && k < Nf) {
-      const long long o = (long long)k * Nt + m;
+    if (m < Nt && k < Nf && gap[m] != 0) {
+      const long long o = (long long)k * ncol + vprefix[m];
       grid[o] = sY[tx][r];
       wgt[o] = sW[tx][r];
     }
@@ -764,18 +1198,18 @@ pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, 
 }
 
 // ------------------------------------------------------------------------------------------
-// Weight structure (a0, C11).  If W[alpha,m,k] = a_alpha[m] b_alpha[k] then
-//   rowmax[m] = max_k W = a[m] max b,  colmax[k] = max_m W = b[k] max a,  gmax = max a max b,
-// so a'[m] = rowmax[m], b'[k] = colmax[k] / gmax reproduce W = a' b'.  weight_check_kernel counts the
+// Weight structure (a0, C11), over the valid tranches.  If W[alpha,i,k] = a_alpha[i] b_alpha[k] then
+//   rowmax[i] = max_k W = a[i] max b,  colmax[k] = max_i W = b[k] max a,  gmax = max a max b,
+// so a'[i] = rowmax[i], b'[k] = colmax[k] / gmax reproduce W = a' b'.  weight_check_kernel counts the
 // pixels where that fails by more than a few ulps (or W < 0), and the columns with b' != 1.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-weight_colmax_kernel(const float2* __restrict__ wgt, int Nt, float2* __restrict__ colmax) {   // one block per k
+weight_colmax_kernel(const float2* __restrict__ wgt, int ncol, int n_valid, float2* __restrict__ colmax) {   // one block per k
   __shared__ float2 sh[256];
   const int k = blockIdx.x;
   float2 mx = make_float2(0.f, 0.f);
-  for (int m = threadIdx.x; m < Nt; m += 256) {
-    const float2 w = wgt[(size_t)k * Nt + m];
+  for (int m = threadIdx.x; m < n_valid; m += 256) {
+    const float2 w = wgt[(size_t)k * ncol + m];
     mx.x = fmaxf(mx.x, w.x); mx.y = fmaxf(mx.y, w.y);
   }
   sh[threadIdx.x] = mx;
@@ -790,16 +1224,16 @@ weight_colmax_kernel(const float2* __restrict__ wgt, int Nt, float2* __restrict_
   if (threadIdx.x == 0) colmax[k] = sh[0];
 }
 
-// wa must be zeroed first; grid (ceil(Nt/128), k-slices): weights are >= 0 (or zeroed at upload), so their
+// wa must be zeroed first; grid (ceil(n_valid/128), k-slices): weights are >= 0 (or zeroed at upload), so their
 // bit patterns order like integers and atomicMax on them is the float maximum
-__global__ void weight_rowmax_kernel(const float2* __restrict__ wgt, int Nt, int Nf, float2* __restrict__ wa) {
+__global__ void weight_rowmax_kernel(const float2* __restrict__ wgt, int ncol, int n_valid, int Nf, float2* __restrict__ wa) {
   const int m = blockIdx.x * blockDim.x + threadIdx.x;
-  if (m >= Nt) return;
+  if (m >= n_valid) return;
   const int per = (Nf + gridDim.y - 1) / gridDim.y;
   const int k0 = blockIdx.y * per, k1 = min(k0 + per, Nf);
   float2 mx = make_float2(0.f, 0.f);
   for (int k = k0; k < k1; ++k) {
-    const float2 w = wgt[(size_t)k * Nt + m];
+    const float2 w = wgt[(size_t)k * ncol + m];
     mx.x = fmaxf(mx.x, w.x); mx.y = fmaxf(mx.y, w.y);
   }
   int* out = reinterpret_cast<int*>(wa + m);
@@ -833,29 +1267,34 @@ weight_factor_kernel(const float2* __restrict__ colmax, int Nf, float2* __restri
 }
 
 __global__ void weight_check_kernel(const float2* __restrict__ wgt, const float2* __restrict__ wa,
-                                    const float2* __restrict__ wb, int Nt, int Nf, unsigned long long* counts) {
+                                    const float2* __restrict__ wb, int ncol, int n_valid, int Nf, unsigned long long* counts) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   bool bad = false;
-  if (i < (size_t)Nt * Nf) {
-    const int k = (int)(i / Nt), m = (int)(i - (size_t)k * Nt);
-    const float2 w = wgt[i], a = wa[m], b = wb[k];
-    const float pA = a.x * b.x, pE = a.y * b.y;
-    bad = !(fabsf(w.x - pA) <= 1e-6f * pA) || !(fabsf(w.y - pE) <= 1e-6f * pE) || w.x < 0.f || w.y < 0.f;
+  if (i < (size_t)ncol * Nf) {
+    const int k = (int)(i / ncol), m = (int)(i - (size_t)k * ncol);
+    if (m < n_valid) {
+      const float2 w = wgt[i], a = wa[m], b = wb[k];
+      const float pA = a.x * b.x, pE = a.y * b.y;
+      bad = !(fabsf(w.x - pA) <= 1e-6f * pA) || !(fabsf(w.y - pE) <= 1e-6f * pE) || w.x < 0.f || w.y < 0.f;
+    }
   }
   const unsigned n_bad = __popc(__ballot_sync(0xffffffffu, bad));
   if ((threadIdx.x & 31) == 0 && n_bad) atomicAdd(&counts[0], (unsigned long long)n_bad);
 }
 
-// Compacted list of valid (non-gap) tranches and its prefix counts (C10).  One block.
+// Compacted list of valid (non-gap) tranches and its prefix counts (C10).  One block.  valid_m is padded to
+// ncol_cap entries with its last entry (entry 0 = tranche 0 when everything is masked).
 __global__ void __launch_bounds__(1024)
-valid_list_kernel(const uint8_t* __restrict__ gap, int Nt, int* __restrict__ vprefix, int* __restrict__ valid_m) {
+valid_list_kernel(const uint8_t* __restrict__ gap, int Nt, int ncol_cap, int* __restrict__ vprefix, int* __restrict__ valid_m) {
   __shared__ int s_cnt[1024];
+  __shared__ int s_last;
   const int t = threadIdx.x;
   const int per = (Nt + 1023) / 1024;
   const int b = min(t * per, Nt), e = min(b + per, Nt);
   int c = 0;
   for (int m = b; m < e; ++m) c += gap[m] != 0;
   s_cnt[t] = c;
+  if (t == 0) s_last = 0;
   __syncthreads();
   for (int o = 1; o < 1024; o <<= 1) {                           // inclusive Hillis-Steele scan
     const int v = t >= o ? s_cnt[t - o] : 0;
@@ -864,14 +1303,17 @@ valid_list_kernel(const uint8_t* __restrict__ gap, int Nt, int* __restrict__ vpr
     __syncthreads();
   }
   int pos = s_cnt[t] - c;
+  const int total = s_cnt[1023];
   for (int m = b; m < e; ++m) {
     vprefix[m] = pos;
-    if (gap[m] != 0) valid_m[pos++] = m;
+    if (gap[m] != 0) {
+      valid_m[pos++] = m;
+      if (pos == total) s_last = m;
+    }
   }
-  if (t == 1023) {
-    vprefix[Nt] = s_cnt[1023];
-    if (s_cnt[1023] == 0) valid_m[0] = 0;                        // keep entry 0 readable when everything is masked
-  }
+  if (t == 1023) vprefix[Nt] = total;
+  __syncthreads();
+  for (int i = total + t; i < ncol_cap; i += 1024) valid_m[i] = s_last;
 }
 
 // ------------------------------------------------------------------------------------------

@@ -25,7 +25,8 @@ def test_header_declares_the_boundary():
     syms = declared_symbols()
     for s in ["tfs_create", "tfs_upload_data", "tfs_eval", "tfs_topk", "tfs_destroy", "tfs_last_error",
               "tfs_count_pixels", "tfs_default_opts", "tfs_bad_param_count", "tfs_set_profiling",
-              "tfs_get_profile", "tfs_refine", "tfs_probe_l2_bandwidth"]:
+              "tfs_get_profile", "tfs_get_profile_kernels", "tfs_refine", "tfs_probe_l2_bandwidth", "tfs_eval_tf",
+              "tfs_upload_timeseries", "tfs_weight_structure"]:
         assert s in syms
 
 
@@ -48,7 +49,8 @@ def test_defaults_and_create_fails_loudly_without_gpu(lib_path):
         assert ei.value.code in (api.TFS_ECUDA, api.TFS_ENOMEM)
     h = ctypes.c_void_p()
     assert lib.tfs_create(ctypes.byref(h), 0, 64, 5.0, 2, None) == api.TFS_EINVAL
-    assert lib.tfs_create(ctypes.byref(h), 64, 64, 5.0, 3, None) == api.TFS_EINVAL
+    assert lib.tfs_create(ctypes.byref(h), 64, 64, 5.0, 4, None) == api.TFS_EINVAL      # 1, 2 or 3 channels
+    assert lib.tfs_create(ctypes.byref(h), 64, 64, 5.0, 0, None) == api.TFS_EINVAL
     assert b"n_channels" in lib.tfs_last_error(None)
     assert lib.tfs_eval(None, None, 0, 1, None, None, None, None, None) == api.TFS_EINVAL
 
