@@ -27,17 +27,23 @@ namespace tfs {
 #define TFS_TS 64
 #endif
 constexpr int kTS = TFS_TS;               // valid tranches per time tile (= columns of a slab); multiple of 32
-static_assert(kTS % 32 == 0 && kTS >= 32 && kTS <= 64, "kTS must be 32 or 64 (TMA box <= 256 floats wide)");
+static_assert(kTS == 64, "the slab kernel evaluates the two 32-tranche chunks of a tile in the two halves of packed registers");
 #ifndef TFS_SLAB_ROWS
 #define TFS_SLAB_ROWS 96
 #endif
 #ifndef TFS_SLAB_ROWS_GENERAL
 #define TFS_SLAB_ROWS_GENERAL 64
 #endif
-constexpr int kBandStride = 32;           // rows between the bottoms of consecutive bands
+#ifndef TFS_BAND_STRIDE
+#define TFS_BAND_STRIDE 16
+#endif
+constexpr int kBandStride = TFS_BAND_STRIDE;   // rows between the bottoms of consecutive bands (even: the b table is copied from row0)
 constexpr int kUnitItems = 1024;          // items per unit of the slab kernel (32 per warp)
 constexpr int kListUnitItems = 32;        // items per (warp-claimed) unit of the list kernel
-constexpr int kWarpsPerCta = 32;          // both evaluation kernels: one persistent CTA of 32 warps per SM (64 registers)
+#ifndef TFS_WARPS
+#define TFS_WARPS 32
+#endif
+constexpr int kWarpsPerCta = TFS_WARPS;   // both evaluation kernels: one persistent CTA of 32 warps per SM (64 registers)
 constexpr int kLutN = 512;                // LUT intervals in t = 1/(1+v)
 constexpr double kMtsun = 4.925490947e-6; // G Msun / c^3 [s]
 constexpr double kPi = 3.14159265358979323846;
@@ -51,7 +57,7 @@ constexpr int kWGeneral = 0, kWSeparable = 1, kWTimeOnly = 2;
 __host__ __device__ constexpr int slab_rows(int wmode) { return wmode == kWGeneral ? TFS_SLAB_ROWS_GENERAL : TFS_SLAB_ROWS; }
 constexpr int kSlabRowsMax = TFS_SLAB_ROWS > TFS_SLAB_ROWS_GENERAL ? TFS_SLAB_ROWS : TFS_SLAB_ROWS_GENERAL;
 static_assert(TFS_SLAB_ROWS <= 256 && TFS_SLAB_ROWS_GENERAL <= 256, "TMA box <= 256 rows");
-static_assert(TFS_SLAB_ROWS > kBandStride && TFS_SLAB_ROWS_GENERAL > kBandStride, "a slab must overlap the next band");
+static_assert(kBandStride % 2 == 0 && TFS_SLAB_ROWS > kBandStride && TFS_SLAB_ROWS_GENERAL > kBandStride, "a slab must overlap the next band");
 
 // f(v) = w (F0 + F1 w^4 + F2 w^8), g(v) = w^3 (G0 + G1 w^4 + G2 w^8), w = 1/v, valid for |v| >= kVFar
 struct FarCoef { float F0, F1, F2, G0, G1, G2; };
@@ -143,6 +149,23 @@ __device__ __forceinline__ TplConst load_template(const double* __restrict__ p, 
   return t;
 }
 
+// MUFU approximations without the denormal fix-up code (inputs here are never subnormal)
+__device__ __forceinline__ float rsqrt_approx(float x) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float lg2_approx(float x) {
+  float r;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float ex2_approx(float x) {
+  float r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
 // Track point of one tranche (Eqs. 12-15 at the tranche start, C6; 0PN, C5).
 struct TrackPoint {
   double x;        // f_m * DT  (position in bins)
@@ -162,7 +185,7 @@ __device__ __forceinline__ TrackPoint track_point(const TplConst& t, int m, doub
   const double tau = t.tc - (double)m * DT;
   bool act = valid && (tau > DT);
   const double X = act ? tau * t.inv5M : 1.0;
-  double y0 = (double)exp2f(-0.125f * __log2f((float)X));
+  double y0 = (double)ex2_approx(-0.125f * lg2_approx((float)X));
   // X outside the fp32 range (absurd masses): fall back to the seed 1/sqrt(sqrt(sqrt(X)))
   if (!(X > 1e-30 && X < 1e30)) y0 = rsqrt(sqrt(sqrt(X)));
   const double p2 = y0 * y0, p4 = p2 * p2;
@@ -552,45 +575,75 @@ struct SlabLane {
   }
 };
 
-template <int KIND, int MASKED, int WMODE>
+// offsets [jb, je) of kind KIND, unmasked (every lane's window reaches je): four pixels per iteration, then singles
+template <int KIND, int WMODE>
 __device__ __forceinline__ void zone_run(const SlabLane<WMODE>& sl, const LaneTrack& L, const FarCoef& C, int jb, int je,
-                                         int Wm, float& u, unsigned lut_lane, LaneSums& s) {
+                                         float u0, unsigned lut_lane, LaneSums& s) {
   int j = jb;
-  for (; j + 1 < je; j += 2) {
-    float4 Y0, Y1;
-    float2 W0, W1;
-    sl.load(j, Y0, W0);
-    sl.load(j + 1, Y1, W1);
-    pixel_kind<KIND, 0, WMODE, MASKED, kLutCopiesSlab>(L, C, j, Wm, Y0, W0, u, lut_lane, s);
-    pixel_kind<KIND, 0, WMODE, MASKED, kLutCopiesSlab>(L, C, j + 1, Wm, Y1, W1, u - 1.0f, lut_lane, s);
-    u -= 2.0f;
+  float u = u0 - (float)jb;                     // exact: small integers
+  for (; j + 3 < je; j += 4) {
+    float4 Y[4];
+    float2 W[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) sl.load(j + q, Y[q], W[q]);
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      pixel_kind<KIND, 0, WMODE, 0, kLutCopiesSlab>(L, C, j + q, 0, Y[q], W[q], u - (float)q, lut_lane, s);
+    u -= 4.0f;
   }
-  if (j < je) {
+#pragma unroll 1
+  for (; j < je; ++j) {
     float4 Y0;
     float2 W0;
     sl.load(j, Y0, W0);
-    pixel_kind<KIND, 0, WMODE, MASKED, kLutCopiesSlab>(L, C, j, Wm, Y0, W0, u, lut_lane, s);
+    pixel_kind<KIND, 0, WMODE, 0, kLutCopiesSlab>(L, C, j, 0, Y0, W0, u, lut_lane, s);
     u -= 1.0f;
   }
 }
 
-template <int KIND, int WMODE>
-__device__ __forceinline__ void zone_auto(const SlabLane<WMODE>& sl, const LaneTrack& L, const FarCoef& C, int jb, int je,
-                                          int Wm, int Wmin, float& u, unsigned lut_lane, LaneSums& s) {
-  const int jm = min(max(jb, Wmin), je);       // [jb, jm) unmasked, [jm, je) masked
-  if (jb < jm) zone_run<KIND, 0, WMODE>(sl, L, C, jb, jm, Wm, u, lut_lane, s);
-  if (jm < je) zone_run<KIND, 1, WMODE>(sl, L, C, jm, je, Wm, u, lut_lane, s);
-}
-
+// The zones may run in any order (u is re-derived from the offset), so the two FAR2 runs and the two FAR
+// runs share their code; everything below Wmin (the shortest active window) is unmasked, and the few
+// offsets in [Wmin, Wmax) go through one generic masked loop.
 template <int WMODE>
 __device__ __forceinline__ void pixel_loop_slab(const SlabLane<WMODE>& sl, const LaneTrack& L, const FarCoef& C, int Wm,
-                                                int Wmin, int Wmax, int J2A, int JA, int JB, int J2B, float u,
+                                                int Wmin, int Wmax, int J2A, int JA, int JB, int J2B, float u0,
                                                 unsigned lut_lane, LaneSums& s) {
-  zone_auto<kZFar2, WMODE>(sl, L, C, 0, J2A, Wm, Wmin, u, lut_lane, s);
-  zone_auto<kZFar, WMODE>(sl, L, C, J2A, JA, Wm, Wmin, u, lut_lane, s);
-  zone_auto<kZNear, WMODE>(sl, L, C, JA, JB, Wm, Wmin, u, lut_lane, s);
-  zone_auto<kZFar, WMODE>(sl, L, C, JB, J2B, Wm, Wmin, u, lut_lane, s);
-  zone_auto<kZFar2, WMODE>(sl, L, C, J2B, Wmax, Wm, Wmin, u, lut_lane, s);
+  const int Z2A = min(J2A, Wmin), ZA = min(JA, Wmin), ZB = min(JB, Wmin), Z2B = min(J2B, Wmin);
+#pragma unroll 1
+  for (int r = 0; r < 2; ++r) zone_run<kZFar2, WMODE>(sl, L, C, r ? Z2B : 0, r ? Wmin : Z2A, u0, lut_lane, s);
+#pragma unroll 1
+  for (int r = 0; r < 2; ++r) zone_run<kZFar, WMODE>(sl, L, C, r ? ZB : Z2A, r ? Z2B : ZA, u0, lut_lane, s);
+  {
+    int j = ZA;
+    float u = u0 - (float)ZA;
+    for (; j + 1 < ZB; j += 2) {
+      float4 Y0, Y1;
+      float2 W0, W1;
+      sl.load(j, Y0, W0);
+      sl.load(j + 1, Y1, W1);
+      pixel_kind<kZNear, 0, WMODE, 0, kLutCopiesSlab>(L, C, j, 0, Y0, W0, u, lut_lane, s);
+      pixel_kind<kZNear, 0, WMODE, 0, kLutCopiesSlab>(L, C, j + 1, 0, Y1, W1, u - 1.0f, lut_lane, s);
+      u -= 2.0f;
+    }
+    if (j < ZB) {
+      float4 Y0;
+      float2 W0;
+      sl.load(j, Y0, W0);
+      pixel_kind<kZNear, 0, WMODE, 0, kLutCopiesSlab>(L, C, j, 0, Y0, W0, u, lut_lane, s);
+    }
+  }
+  // masked tail: lanes whose window ended contribute zero
+  float u = u0 - (float)Wmin;
+#pragma unroll 1
+  for (int j = Wmin; j < Wmax; ++j) {
+    float4 Y0;
+    float2 W0;
+    sl.load(j, Y0, W0);
+    if (j >= JA && j < JB) pixel_kind<kZNear, 0, WMODE, 1, kLutCopiesSlab>(L, C, j, Wm, Y0, W0, u, lut_lane, s);
+    else if (j < J2A || j >= J2B) pixel_kind<kZFar2, 0, WMODE, 1, kLutCopiesSlab>(L, C, j, Wm, Y0, W0, u, lut_lane, s);
+    else pixel_kind<kZFar, 0, WMODE, 1, kLutCopiesSlab>(L, C, j, Wm, Y0, W0, u, lut_lane, s);
+    u -= 1.0f;
+  }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -668,10 +721,10 @@ __device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it,
         __sincosf(6.283185307179586f * ((float)tphi - 0.5f), &sphi, &cphi);     // = -(sin, cos)(2 pi tphi)
         __sincosf(6.283185307179586f * ((float)tpsi - 0.5f), &spsi, &cpsi);
         const float cf = (float)tp.c;
-        L.sc = rsqrtf(0.5f * cf);
+        L.sc = rsqrt_approx(0.5f * cf);
         L.kap = 0.5f * cf * L.sc;                                               // sqrt(c/2)
         L.c = cf;
-        L.hc = __fdividef(0.5f, cf);
+        L.hc = 0.5f * rcp_approx(cf);
         const float pre = -(T.acoef * tp.Xm14) * (0.5f * L.sc);               // -A_m / sqrt(2c)
         Pr = pre * cphi;
         Pi = pre * sphi;
@@ -679,12 +732,12 @@ __device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it,
         L.Ei = -spsi;
         // near zone of this lane: offsets j with |v0| < kVFar or |v1| < kVFar, i.e. -(c + d) < u - j < d
         const float d = fmaf(kVFar, L.kap, 1e-3f);
-        ja = max((int)floorf(u - d) + 1, 0);
-        jb = (int)ceilf(u + cf + d);
+        ja = max(__float2int_rd(u - d) + 1, 0);
+        jb = __float2int_ru(u + cf + d);
         if (SLAB) {
           const float d2 = fmaf(kVFar2, L.kap, 1e-3f);   // offsets outside (j2a, j2b) have |v0|, |v1| >= kVFar2
-          j2a = max((int)floorf(u - d2) + 1, 0);
-          j2b = (int)ceilf(u + cf + d2);
+          j2a = max(__float2int_rd(u - d2) + 1, 0);
+          j2b = __float2int_ru(u + cf + d2);
         }
       }
       const int Wmax = __reduce_max_sync(0xffffffffu, Wm);
@@ -762,6 +815,357 @@ __device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it,
         if (lane >= lo && lane < hi) { accr += vr; acci += vi; acch += vq; }
         if (!ends) break;
         flush();
+        ++p;
+        if (p < p_stop) pend = a.piece_end[p];
+        lo = hi;
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// One work item of the SLAB kernel.  A tile is kTS = 64 valid tranches = two chunks of 32, and every lane
+// evaluates TWO tranches at once -- entry i0 + lane of the valid-tranche list (half 0) and entry
+// i0 + 32 + lane (half 1) -- with the two tranches in the two halves of packed fp32 registers: every
+// per-pixel instruction outside the polynomials (which were already packed over v0, v1) then serves two
+// pixels, the loop and zone overheads are paid once for both, and the window-offset zones are taken over
+// all 64 tranches.  Offsets are relative to each tranche's own k_lo, so the zones line up.
+//   [0, J2A) FAR2 | [J2A, JA) FAR | [JA, JB) NEAR | [JB, J2B) FAR | [J2B, Wmin) FAR2 | [Wmin, Wmax) masked
+// The data sit in shared memory as [row][kTS columns] float4 (plus [row][kTS] float2 weights, or the band's
+// rows of the b table); lane l of half h reads column 32 h + l, so the 8 lanes of a quarter-warp always
+// fall in 8 different 16-byte bank groups: an LDS.128 is conflict-free whatever rows the lanes are on.
+// An inactive tranche walks rows row0, row0+1, ... of its own column (always inside the slab).
+// ------------------------------------------------------------------------------------------
+struct PairTrack {        // per-lane constants of the pixel loop, {half 0, half 1}
+  f2_t kap;               // sqrt(c/2)
+  f2_t kapf;              // sqrt(c/2) / pi
+  f2_t c;                 // fdot DT^2
+  f2_t Er, Ei;            // exp(i psi)
+  f2_t sc, hc;            // near zone only: sqrt(2/c), 1/(2c)
+};
+
+struct PairSums { f2_t zr[2], zi[2], q[2]; };   // [half] {channel 0, channel 1}; kWTimeOnly: q[0] = sum hr^2, q[1] = sum hi^2 as {half 0, half 1}
+
+template <int WMODE>
+struct SlabPair {
+  unsigned y[2];          // shared address of the pixel of offset 0, per half
+  unsigned w[2];          // kWGeneral: same in the weight slab; kWSeparable: row of the b table
+#ifdef TFS_BOUNDS_CHECK
+  int row_rel[2], rows;
+#endif
+  __device__ __forceinline__ void load(int h, int j, float4& Y, float2& W) const {
+#ifdef TFS_BOUNDS_CHECK
+    if (row_rel[h] + j < 0 || row_rel[h] + j >= rows) __trap();
+#endif
+    Y = lds128(y[h] + (unsigned)j * (kTS * 16u));
+    if (WMODE == kWGeneral) W = lds64(w[h] + (unsigned)j * (kTS * 8u));
+    else if (WMODE == kWSeparable) W = lds64(w[h] + (unsigned)j * 8u);
+    else W = make_float2(0.f, 0.f);
+  }
+};
+
+// template coefficient h' of the pixel of offset j for both halves: hr = {hr_0, hr_1}, hi = {hi_0, hi_1}
+template <int KIND, int MASKED>
+__device__ __forceinline__ void pair_h(const PairTrack& L, const FarCoef& C, f2_t u, f2_t msk, unsigned lut_lane, f2_t& hr, f2_t& hi) {
+  if (KIND == kZNear) {
+    float u0, u1, m0 = 1.f, m1 = 1.f, hr0, hr1, hi0, hi1;
+    upk(u, u0, u1);
+    if (MASKED) upk(msk, m0, m1);
+    LaneTrack A, B;
+    upk(L.sc, A.sc, B.sc); upk(L.kap, A.kap, B.kap); upk(L.c, A.c, B.c); upk(L.hc, A.hc, B.hc);
+    upk(L.Er, A.Er, B.Er); upk(L.Ei, A.Ei, B.Ei);
+    pixel_near<0, MASKED, kLutCopiesSlab>(A, u0, m0, lut_lane, hr0, hi0);
+    pixel_near<0, MASKED, kLutCopiesSlab>(B, u1, m1, lut_lane, hr1, hi1);
+    hr = pk(hr0, hr1);
+    hi = pk(hi0, hi1);
+    return;
+  }
+  float u0, u1, c0, c1;
+  const f2_t uc = fadd2(u, L.c);          // u + c, rounded at the magnitude of u
+  upk(u, u0, u1);
+  upk(uc, c0, c1);
+  const f2_t r0 = pk(rcp_approx(u0), rcp_approx(u1));      // 1/u of both halves
+  const f2_t r1 = pk(rcp_approx(c0), rcp_approx(c1));      // 1/(u + c)
+  f2_t f0, f1, g0, g1;
+  if (KIND == kZFar) {
+    const f2_t kap = MASKED ? fmul2(L.kap, msk) : L.kap;
+    const f2_t w0 = fmul2(r0, kap), w1 = fmul2(r1, kap);   // 1/v0, 1/v1
+    const f2_t a0 = fmul2(w0, w0), a1 = fmul2(w1, w1);
+    const f2_t b0 = fmul2(a0, a0), b1 = fmul2(a1, a1);
+    const f2_t F2 = pk(C.F2, C.F2), F1 = pk(C.F1, C.F1), F0 = pk(C.F0, C.F0);
+    const f2_t G2 = pk(C.G2, C.G2), G1 = pk(C.G1, C.G1), G0 = pk(C.G0, C.G0);
+    f0 = fmul2(w0, ffma2(b0, ffma2(b0, F2, F1), F0));
+    f1 = fmul2(w1, ffma2(b1, ffma2(b1, F2, F1), F0));
+    g0 = fmul2(fmul2(w0, a0), ffma2(b0, ffma2(b0, G2, G1), G0));
+    g1 = fmul2(fmul2(w1, a1), ffma2(b1, ffma2(b1, G2, G1), G0));
+  } else {
+    const f2_t kf = MASKED ? fmul2(L.kapf, msk) : L.kapf;
+    const f2_t pi2 = pk(kG0overF03, kG0overF03);
+    f0 = fmul2(r0, kf);
+    f1 = fmul2(r1, kf);
+    g0 = fmul2(fmul2(f0, pi2), fmul2(f0, f0));
+    g1 = fmul2(fmul2(f1, pi2), fmul2(f1, f1));
+  }
+  const f2_t nEr = L.Er ^ 0x8000000080000000ULL, nEi = L.Ei ^ 0x8000000080000000ULL;
+  hr = ffma2(nEr, g1, ffma2(L.Ei, f1, g0));            // Godd(v0) - E Godd(v1)
+  hi = ffma2(nEr, f1, ffma2(nEi, g1, f0));
+}
+
+// z', q' of both halves for the pixel of offset j
+template <int KIND, int WMODE, int MASKED>
+__device__ __forceinline__ void pair_pixel(const SlabPair<WMODE>& sl, const PairTrack& L, const FarCoef& C, int j, f2_t u,
+                                           int Wm0, int Wm1, unsigned lut_lane, PairSums& s) {
+  float4 Y0, Y1;
+  float2 W0, W1;
+  sl.load(0, j, Y0, W0);
+  sl.load(1, j, Y1, W1);
+  f2_t msk = 0;
+  if (MASKED) msk = pk(j < Wm0 ? 1.f : 0.f, j < Wm1 ? 1.f : 0.f);
+  f2_t hr, hi;
+  pair_h<KIND, MASKED>(L, C, u, msk, lut_lane, hr, hi);
+  float hr0, hr1, hi0, hi1;
+  upk(hr, hr0, hr1);
+  upk(hi, hi0, hi1);
+  {
+    const f2_t Yre = pk(Y0.x, Y0.y), Yim = pk(Y0.z, Y0.w);
+    s.zr[0] = ffma2(Yre, pk(hr0, hr0), s.zr[0]);
+    s.zr[0] = ffma2(Yim, pk(hi0, hi0), s.zr[0]);
+    s.zi[0] = ffma2(Yre, pk(hi0, hi0), s.zi[0]);
+    s.zi[0] = ffma2(Yim, pk(-hr0, -hr0), s.zi[0]);
+  }
+  {
+    const f2_t Yre = pk(Y1.x, Y1.y), Yim = pk(Y1.z, Y1.w);
+    s.zr[1] = ffma2(Yre, pk(hr1, hr1), s.zr[1]);
+    s.zr[1] = ffma2(Yim, pk(hi1, hi1), s.zr[1]);
+    s.zi[1] = ffma2(Yre, pk(hi1, hi1), s.zi[1]);
+    s.zi[1] = ffma2(Yim, pk(-hr1, -hr1), s.zi[1]);
+  }
+  if (WMODE == kWTimeOnly) {
+    s.q[0] = ffma2(hr, hr, s.q[0]);
+    s.q[1] = ffma2(hi, hi, s.q[1]);
+  } else {
+    float h20, h21;
+    upk(ffma2(hr, hr, fmul2(hi, hi)), h20, h21);
+    s.q[0] = ffma2(pk(W0.x, W0.y), pk(h20, h20), s.q[0]);
+    s.q[1] = ffma2(pk(W1.x, W1.y), pk(h21, h21), s.q[1]);
+  }
+}
+
+#ifndef TFS_PAIR_UNROLL
+#define TFS_PAIR_UNROLL 1
+#endif
+constexpr int kPairUnroll = TFS_PAIR_UNROLL;
+
+template <int KIND, int WMODE>
+__device__ __forceinline__ void pair_zone(const SlabPair<WMODE>& sl, const PairTrack& L, const FarCoef& C, int jb, int je,
+                                          f2_t u0, unsigned lut_lane, PairSums& s) {
+  const float fj = (float)jb;
+  f2_t u = fadd2(u0, pk(-fj, -fj));              // exact: small integers
+  const f2_t m1 = pk(-1.f, -1.f);
+#pragma unroll(kPairUnroll)
+  for (int j = jb; j < je; ++j) {
+    pair_pixel<KIND, WMODE, 0>(sl, L, C, j, u, 0, 0, lut_lane, s);
+    u = fadd2(u, m1);
+  }
+}
+
+template <int WMODE>
+__device__ __forceinline__ void eval_item_pair(const EvalArgs& a, const long long it, const int tile, const int lane,
+                                               const unsigned lut_lane, const unsigned slab_y, const unsigned slab_w,
+                                               const int row0) {
+  const int i0 = tile * kTS, i1 = min(i0 + kTS, a.n_valid);
+  int p = a.tile_first[tile];
+  const int p_stop = a.tile_first[tile + 1];
+  int pend = p < p_stop ? a.piece_end[p] : i1;
+  float accr = 0.f, acci = 0.f, acch = 0.f;      // this lane's running sums of the current piece
+
+  // ---------------- track points of this lane's two tranches (a2) ----------------
+  float uu[2], Pr[2], Pi[2], kap[2], cc[2], Er[2], Ei[2], sc[2], hc[2], xf[2];
+  int Wm[2], krel[2], idxv[2];
+  int ja = 0x7fffffff, jb = 0, j2a = 0x7fffffff, j2b = 0, wmin = 0x7fffffff;
+  bool any = false;
+  {
+    const TplConst T = a.tconst[it];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int i = i0 + 32 * h + lane;
+      const bool valid = i < i1;
+      idxv[h] = valid ? i : i0;
+      const int m = a.valid_m[idxv[h]];
+      const TrackPoint tp = track_point(T, m, a.DT, a.x_lo, a.x_hi, a.c_max, valid);
+      // an inactive tranche: u_j = -1 - j, u_j + c = -0.5 - j (finite h' on finite data), P = 0
+      Wm[h] = 0; krel[h] = 0; uu[h] = -1.f; Pr[h] = 0.f; Pi[h] = 0.f; kap[h] = 1.f; cc[h] = 0.5f; Er[h] = 0.f; Ei[h] = 0.f;
+      sc[h] = 1.f; hc[h] = 0.f; xf[h] = 0.f;
+      if (tp.active) {
+        any = true;
+        int k_lo, k_hi;
+        window(tp, a.H, a.adaptive, a.Nf, k_lo, k_hi);
+        Wm[h] = k_hi - k_lo + 1;
+        krel[h] = k_lo - row0;
+        wmin = min(wmin, Wm[h]);
+        const int kfl = __double2int_rd(tp.x);
+        const double fr = tp.x - (double)kfl;
+        uu[h] = (float)fr - (float)(k_lo - kfl);          // cancellation-safe x - k_lo
+        xf[h] = (float)tp.x;
+        // phases in turns, reduced in fp64 (phi reaches ~1e8 rad), then to [-1/2, 1/2)
+        double tphi = T.phic_turns - tp.X58 * (1.0 / kPi);
+        tphi -= floor(tphi);
+        double tpsi = 0.5 * tp.c + fr;
+        tpsi -= floor(tpsi);
+        float sphi, cphi, spsi, cpsi;
+        __sincosf(6.283185307179586f * ((float)tphi - 0.5f), &sphi, &cphi);     // = -(sin, cos)(2 pi tphi)
+        __sincosf(6.283185307179586f * ((float)tpsi - 0.5f), &spsi, &cpsi);
+        const float cf = (float)tp.c;
+        sc[h] = rsqrt_approx(0.5f * cf);
+        kap[h] = 0.5f * cf * sc[h];                                             // sqrt(c/2)
+        cc[h] = cf;
+        hc[h] = 0.5f * rcp_approx(cf);
+        const float pre = -(T.acoef * tp.Xm14) * (0.5f * sc[h]);              // -A_m / sqrt(2c)
+        Pr[h] = pre * cphi;
+        Pi[h] = pre * sphi;
+        Er[h] = -cpsi;
+        Ei[h] = -spsi;
+        // near zone: offsets j with |v0| < kVFar or |v1| < kVFar, i.e. -(c + d) < u - j < d; FAR2 outside (j2a, j2b)
+        const float d = fmaf(kVFar, kap[h], 1e-3f), d2 = fmaf(kVFar2, kap[h], 1e-3f);
+        ja = min(ja, max(__float2int_rd(uu[h] - d) + 1, 0));
+        jb = max(jb, __float2int_ru(uu[h] + cf + d));
+        j2a = min(j2a, max(__float2int_rd(uu[h] - d2) + 1, 0));
+        j2b = max(j2b, __float2int_ru(uu[h] + cf + d2));
+      }
+    }
+    // transfer factors of the two channels (a6): constant per template, or from the template's table at f_m
+    float vr[2] = {0.f, 0.f}, vi[2] = {0.f, 0.f}, vq[2] = {0.f, 0.f};
+    if (__any_sync(0xffffffffu, any)) {
+      const int Wmax = __reduce_max_sync(0xffffffffu, max(Wm[0], Wm[1]));
+      const int Wmin = __reduce_min_sync(0xffffffffu, wmin);
+      int JB = min(__reduce_max_sync(0xffffffffu, jb), Wmax);
+      int JA = min(__reduce_min_sync(0xffffffffu, ja), JB);
+      const int J2A = min(__reduce_min_sync(0xffffffffu, j2a), JA);
+      const int J2B = max(min(__reduce_max_sync(0xffffffffu, j2b), Wmax), JB);
+
+      // ---------------- pixel loop (a3-a5) ----------------
+      PairTrack L;
+      L.kap = pk(kap[0], kap[1]);
+      L.kapf = pk(kap[0] * 0.318309886183790672f, kap[1] * 0.318309886183790672f);
+      L.c = pk(cc[0], cc[1]);
+      L.Er = pk(Er[0], Er[1]); L.Ei = pk(Ei[0], Ei[1]);
+      L.sc = pk(sc[0], sc[1]); L.hc = pk(hc[0], hc[1]);
+      SlabPair<WMODE> sl;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const unsigned col = (unsigned)(32 * h + lane);
+        sl.y[h] = slab_y + ((unsigned)krel[h] * kTS + col) * 16u;
+        sl.w[h] = WMODE == kWGeneral ? slab_w + ((unsigned)krel[h] * kTS + col) * 8u : slab_w + (unsigned)krel[h] * 8u;
+#ifdef TFS_BOUNDS_CHECK
+        sl.row_rel[h] = krel[h]; sl.rows = slab_rows(WMODE);
+        if (krel[h] < 0 || krel[h] + Wmax > slab_rows(WMODE)) __trap();
+#endif
+      }
+      PairSums s;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) { s.zr[h] = pk(0.f, 0.f); s.zi[h] = pk(0.f, 0.f); s.q[h] = pk(0.f, 0.f); }
+      const f2_t u0 = pk(uu[0], uu[1]);
+      const int Z2A = min(J2A, Wmin), ZA = min(JA, Wmin), ZB = min(JB, Wmin), Z2B = min(J2B, Wmin);
+      // the zones may run in any order (u is re-derived from the offset), so the two FAR2 runs and the two
+      // FAR runs share their code
+#pragma unroll 1
+      for (int r = 0; r < 2; ++r) pair_zone<kZFar2, WMODE>(sl, L, a.far, r ? Z2B : 0, r ? Wmin : Z2A, u0, lut_lane, s);
+#pragma unroll 1
+      for (int r = 0; r < 2; ++r) pair_zone<kZFar, WMODE>(sl, L, a.far, r ? ZB : Z2A, r ? Z2B : ZA, u0, lut_lane, s);
+      pair_zone<kZNear, WMODE>(sl, L, a.far, ZA, ZB, u0, lut_lane, s);
+      {
+        // masked tail: a tranche whose window has ended contributes zero
+        const float fw = (float)Wmin;
+        f2_t u = fadd2(u0, pk(-fw, -fw));
+#pragma unroll 1
+        for (int j = Wmin; j < Wmax; ++j) {
+          if (j >= JA && j < JB) pair_pixel<kZNear, WMODE, 1>(sl, L, a.far, j, u, Wm[0], Wm[1], lut_lane, s);
+          else if (j < J2A || j >= J2B) pair_pixel<kZFar2, WMODE, 1>(sl, L, a.far, j, u, Wm[0], Wm[1], lut_lane, s);
+          else pair_pixel<kZFar, WMODE, 1>(sl, L, a.far, j, u, Wm[0], Wm[1], lut_lane, s);
+          u = fadd2(u, pk(-1.f, -1.f));
+        }
+      }
+      // ---------------- a6: transfer factors, the tranche's factor P, weights a[i] ----------------
+      float q0[2], q1[2];
+      if (WMODE == kWTimeOnly) {
+        float r0, r1, s0, s1;
+        upk(s.q[0], r0, r1); upk(s.q[1], s0, s1);              // {sum hr^2, sum hi^2} per half
+        q0[0] = q1[0] = r0 + s0;
+        q0[1] = q1[1] = r1 + s1;
+      } else {
+        upk(s.q[0], q0[0], q1[0]);
+        upk(s.q[1], q0[1], q1[1]);
+      }
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        float T0r = T.T0r, T0i = T.T0i, T1r = T.T1r, T1i = T.T1i;
+        if (a.ttab != nullptr) {
+          // T_alpha(f_m) from the template's table: linear between knots, clamped outside (Eq. 29)
+          const int K = a.tt_K;
+          float sx = fmaf(xf[h], a.tt_scale, -a.tt_off);
+          sx = fminf(fmaxf(sx, 0.f), (float)(K - 1));
+          const int kn = min((int)sx, max(K - 2, 0));
+          const float tf = K > 1 ? sx - (float)kn : 0.f;
+          const int kn1 = min(kn + 1, K - 1);
+          const float2* tb = a.ttab + ((size_t)it * a.tt_C + a.tt_ch0) * K;
+          const float2 A0 = __ldg(tb + kn), A1 = __ldg(tb + kn1);
+          T0r = fmaf(tf, A1.x - A0.x, A0.x); T0i = fmaf(tf, A1.y - A0.y, A0.y);
+          T1r = 0.f; T1i = 0.f;
+          if (a.tt_ch0 + 1 < a.tt_C && a.n_ch_pair > 1) {
+            const float2 B0 = __ldg(tb + K + kn), B1 = __ldg(tb + K + kn1);
+            T1r = fmaf(tf, B1.x - B0.x, B0.x); T1i = fmaf(tf, B1.y - B0.y, B0.y);
+          }
+        }
+        // z' = T_0 z'_0 + T_1 z'_1 ;  q' = |T_0|^2 a_0 q'_0 + |T_1|^2 a_1 q'_1   (Eq. 29, Eq. 31)
+        const f2_t Tr = pk(T0r, T1r), Ti = pk(T0i, T1i);
+        float ar, br, ai, bi;
+        upk(ffma2(Ti ^ 0x8000000080000000ULL, s.zi[h], fmul2(Tr, s.zr[h])), ar, br);     // T.re z.re - T.im z.im per channel
+        upk(ffma2(Ti, s.zr[h], fmul2(Tr, s.zi[h])), ai, bi);                             // T.re z.im + T.im z.re
+        const float zcr = ar + br, zci = ai + bi;
+        f2_t w2 = ffma2(Tr, Tr, fmul2(Ti, Ti));                                           // |T|^2 per channel
+        if (WMODE != kWGeneral) {
+          const float2 am = __ldg(a.wa + idxv[h]);
+          w2 = fmul2(w2, pk(am.x, am.y));
+        }
+        float w0, w1;
+        upk(w2, w0, w1);
+        const float P2 = fmaf(Pr[h], Pr[h], Pi[h] * Pi[h]);
+        vr[h] = fmaf(Pr[h], zcr, -Pi[h] * zci);                  // Re (P z')
+        vi[h] = fmaf(Pr[h], zci, Pi[h] * zcr);                   // Im (P z')
+        vq[h] = P2 * fmaf(w0, q0[h], w1 * q1[h]);
+      }
+    }
+
+    // ---------------- a7: pieces.  Chunk h covers entries [i0 + 32 h, ...): add its lanes to the current piece;
+    // every piece that ends inside the chunk (a segment boundary, or the end of the tile) takes the lanes
+    // before its end and is closed; the lanes behind the last such end open the next piece ----------------
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int ic = i0 + 32 * h;
+      if (ic >= i1) break;
+      const int cend = min(ic + 32, i1);
+      if (!(p < p_stop && pend <= cend)) { accr += vr[h]; acci += vi[h]; acch += vq[h]; continue; }
+      int lo = 0;
+      for (;;) {
+        const bool ends = p < p_stop && pend <= cend;
+        const int hi = ends ? pend - ic : 32;
+        if (lane >= lo && lane < hi) { accr += vr[h]; acci += vi[h]; acch += vq[h]; }
+        if (!ends) break;
+        // close piece p: sum the lanes (fp32 butterfly: 32 terms), store, reset
+        float r0 = accr, r1 = acci, r2 = acch;
+        accr = 0.f; acci = 0.f; acch = 0.f;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          r0 += __shfl_xor_sync(0xffffffffu, r0, o);
+          r1 += __shfl_xor_sync(0xffffffffu, r1, o);
+          r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+        }
+        if (lane == 0) {
+          float4* dst = a.partials + (long long)p * a.n + it;
+          float4 v = make_float4(r0, r1, r2, 0.f);
+          if (a.accumulate) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; }
+          *dst = v;
+        }
         ++p;
         if (p < p_stop) pend = a.piece_end[p];
         lo = hi;
@@ -886,7 +1290,7 @@ eval_slab_kernel(const EvalArgs a, const __grid_constant__ CUtensorMap map_y, co
       k = __shfl_sync(0xffffffffu, k, 0);
       if (k >= d.cnt) break;
       const long long it = (long long)a.list[d.off + (unsigned)k];
-      eval_item<0, WMODE, true>(a, it, d.tile, lane, lut_lane, slab_y, slab_w, d.row0);
+      eval_item_pair<WMODE>(a, it, d.tile, lane, lut_lane, slab_y, slab_w, d.row0);
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(bar_empty + 8u * stage);
