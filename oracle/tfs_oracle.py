@@ -263,8 +263,9 @@ def segment_products(Hd, T, D, W, gap_mask, N_seg: int):
     """z_n and hh_n by dense sums over EVERY pixel of every channel (Eq. 31, Eq. 30).
 
     Hd [Nt][Nf] complex128; T [C] complex (transfer factors, Eq. 29, constant per
-    template under C5/A12); D [C][Nt][Nf] complex; W [C][Nt][Nf] real >= 0 (or None => 1);
-    gap_mask [Nt] (or None).  W stands for 4 df / S so that
+    template under C5/A12) or [C][Nt] complex (one factor per tranche: T_alpha(f_nm), "computed
+    once per tranche for all frequency bins"); D [C][Nt][Nf] complex; W [C][Nt][Nf] real >= 0
+    (or None => 1); gap_mask [Nt] (or None).  W stands for 4 df / S so that
     Upsilon = |sum W conj(D) y|^2 / sum W |y|^2.
     """
     Cn, Nt, Nf = D.shape
@@ -278,9 +279,16 @@ def segment_products(Hd, T, D, W, gap_mask, N_seg: int):
         Wa = np.ones((Nt, Nf)) if W is None else W[a].astype(np.float64)
         zm = np.sum(Wa * np.conj(Da) * Hd, axis=1) * g          # per-tranche (d_nm | h_nm)
         qm = np.sum(Wa * H2, axis=1) * g
-        z += T[a] * np.bincount(seg, weights=zm.real, minlength=N_seg)
-        z += T[a] * 1j * np.bincount(seg, weights=zm.imag, minlength=N_seg)
-        hh += abs(T[a]) ** 2 * np.bincount(seg, weights=qm, minlength=N_seg)
+        if np.ndim(T[a]) == 0:
+            z += T[a] * np.bincount(seg, weights=zm.real, minlength=N_seg)
+            z += T[a] * 1j * np.bincount(seg, weights=zm.imag, minlength=N_seg)
+            hh += abs(T[a]) ** 2 * np.bincount(seg, weights=qm, minlength=N_seg)
+        else:
+            Ta = np.asarray(T[a], dtype=np.complex128)           # [Nt]: the factor of each tranche
+            tz = Ta * zm
+            z += np.bincount(seg, weights=tz.real, minlength=N_seg)
+            z += 1j * np.bincount(seg, weights=tz.imag, minlength=N_seg)
+            hh += np.bincount(seg, weights=np.abs(Ta) ** 2 * qm, minlength=N_seg)
     return z, hh
 
 
@@ -308,11 +316,67 @@ def evaluate(params, D, W, gap_mask, grid: Grid, N_seg: int, opts: Opts = Opts()
         if not np.all(np.isfinite(p)) or p[0] <= 0:
             continue
         Hd = dense_template(p[0], p[1], p[2], p[7], grid, opts, gap_mask, truncate=True)
-        T = np.array([p[3] + 1j * p[4], p[5] + 1j * p[6]])
+        T = np.array([p[3] + 1j * p[4], p[5] + 1j * p[6], 0.0])   # a third channel has no column: T_T = 0
         z, hh = segment_products(Hd, T[: D.shape[0]], D, W, gap_mask, N_seg)
         P, U = combine(z, hh)
         ups[i], segP[i], segz[i], segh[i] = U, P, z, hh
     return dict(upsilon=ups, seg_power=segP, seg_dh=segz, seg_hh=segh)
+
+
+# ----------------------------------------------------------------------------------------------
+# Frequency-dependent transfer factor per tranche (Eq. 7, Eq. 29)
+# ----------------------------------------------------------------------------------------------
+def transfer_at(table, f_knot0: float, f_knot_step: float, f):
+    """T(f) from a table of K complex values at the knots f_knot0 + j f_knot_step: linear between knots,
+    held at the end values outside them (include/tfs.h, tfs_eval_tf); K = 1 is a constant."""
+    table = np.asarray(table, dtype=np.complex128)
+    f = np.asarray(f, dtype=np.float64)
+    K = table.shape[-1]
+    if K == 1:
+        return np.broadcast_to(table[..., 0], f.shape).astype(np.complex128)
+    s = np.clip((f - f_knot0) / f_knot_step, 0.0, K - 1.0)
+    j = np.minimum(np.floor(s).astype(np.int64), K - 2)
+    t = s - j
+    return table[..., j] * (1.0 - t) + table[..., j + 1] * t
+
+
+def evaluate_tf(params, tables, f_knot0, f_knot_step, D, W, gap_mask, grid: Grid, N_seg: int, opts: Opts = Opts()):
+    """As evaluate, with the transfer factor of channel alpha in tranche m read from the template's table
+    at the tranche-start frequency f_m (C6): T_alpha,m = transfer_at(tables[i, alpha], ..., f_m).
+    tables [n][C][K] complex.  The T columns of params are ignored."""
+    params = np.atleast_2d(np.asarray(params, dtype=np.float64))
+    tables = np.asarray(tables, dtype=np.complex128)
+    n = params.shape[0]
+    Cn = D.shape[0]
+    ups = np.zeros(n)
+    segP = np.zeros((n, N_seg))
+    segz = np.zeros((n, N_seg), dtype=np.complex128)
+    segh = np.zeros((n, N_seg))
+    for i in range(n):
+        p = params[i]
+        if not np.all(np.isfinite(p)) or p[0] <= 0:
+            continue
+        Hd = dense_template(p[0], p[1], p[2], p[7], grid, opts, gap_mask, truncate=True)
+        tr = track(p[0], p[1], p[2], p[7], grid, opts, gap_mask)
+        T = [transfer_at(tables[i, a], f_knot0, f_knot_step, tr["f"]) for a in range(Cn)]
+        z, hh = segment_products(Hd, T, D, W, gap_mask, N_seg)
+        P, U = combine(z, hh)
+        ups[i], segP[i], segz[i], segh[i] = U, P, z, hh
+    return dict(upsilon=ups, seg_power=segP, seg_dh=segz, seg_hh=segh)
+
+
+def injection_tf(p, table, f_knot0, f_knot_step, rho: float, W, gap_mask, grid: Grid, opts: Opts = Opts(),
+                 truncate=False):
+    """As injection, for a source whose channel alpha carries T_alpha(f_m) from `table` [C][K] in tranche m."""
+    Hd = dense_template(p[0], p[1], p[2], p[7], grid, opts, None, truncate=truncate)
+    tr = track(p[0], p[1], p[2], p[7], grid, opts, None)
+    table = np.asarray(table, dtype=np.complex128)
+    S = np.stack([transfer_at(table[a], f_knot0, f_knot_step, tr["f"])[:, None] * Hd for a in range(table.shape[0])])
+    g = np.ones(grid.Nt) if gap_mask is None else (np.asarray(gap_mask) != 0).astype(np.float64)
+    Wd = np.ones_like(S.real) if W is None else W.astype(np.float64)
+    norm2 = float(np.sum(Wd * (S.real ** 2 + S.imag ** 2) * g[None, :, None]))
+    S *= rho / math.sqrt(norm2)
+    return S * g[None, :, None]
 
 
 def topk(upsilon, k: int):
@@ -330,7 +394,7 @@ def injection(p, rho: float, W, gap_mask, grid: Grid, opts: Opts = Opts(), trunc
     sum_alpha |T_alpha|^2 sum W |H|^2 = rho^2 over non-gap tranches.  Returns S [C][Nt][Nf]
     complex128 to be ADDED to the data (signal present inside gaps is removed with the data)."""
     Hd = dense_template(p[0], p[1], p[2], p[7], grid, opts, None, truncate=truncate)
-    T = np.array([p[3] + 1j * p[4], p[5] + 1j * p[6]])
+    T = np.array([p[3] + 1j * p[4], p[5] + 1j * p[6], 0.0])          # a third channel has no column: T_T = 0
     Cn = 2 if W is None else W.shape[0]
     S = np.stack([T[a] * Hd for a in range(Cn)])
     g = np.ones(grid.Nt) if gap_mask is None else (np.asarray(gap_mask) != 0).astype(np.float64)

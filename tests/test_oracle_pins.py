@@ -544,3 +544,111 @@ def test_p13_ladder_recovers_a_noiseless_injection():
     # without refinement the stage-0 lattice is far too coarse for the coherent statistic
     u1 = O.evaluate(bank, S, None, None, g, 1)["upsilon"]
     assert u1.max() < 0.5 * 400.0 < 0.9 * 400.0 < st[-1]["top_val"][0]
+
+
+# ------------------------------------------------------------------------------------------
+# P14 channels (1, 2, 3) and the per-tranche transfer factor T_alpha(f_nm) (Eq. 3, Eq. 7,
+#     P:213 Eq. 29, "computed once per tranche for all frequency bins")
+# ------------------------------------------------------------------------------------------
+def test_p14_transfer_table_interpolation():
+    tab = np.array([1 + 1j, 3 - 1j, 2 + 5j])
+    f0, df = 0.01, 0.005
+    # at the knots, half-way between them, and held outside
+    f = np.array([0.01, 0.015, 0.02, 0.0125, 0.0175, 0.0, 0.5])
+    want = np.array([tab[0], tab[1], tab[2], 0.5 * (tab[0] + tab[1]), 0.5 * (tab[1] + tab[2]), tab[0], tab[2]])
+    assert np.allclose(O.transfer_at(tab, f0, df, f), want, rtol=0, atol=1e-14)
+    # a table sampled from a straight line reproduces the line between its ends
+    a, b = 0.3 - 0.2j, 40.0 + 10.0j
+    knots = f0 + df * np.arange(7)
+    f = np.linspace(knots[0], knots[-1], 1001)
+    assert np.allclose(O.transfer_at(a + b * knots, f0, df, f), a + b * f, rtol=0, atol=1e-13)
+    assert np.allclose(O.transfer_at(np.array([2 - 3j]), 0.0, 1.0, f), 2 - 3j)          # one knot: a constant
+
+
+def _p14_data(C, seed=14):
+    g = O.Grid(64, 128, 40.0)                                            # DT = 10240 s
+    rng = np.random.default_rng(seed)
+    D = rng.standard_normal((C, g.Nt, g.Nf)) + 1j * rng.standard_normal((C, g.Nt, g.Nf))
+    W = rng.uniform(0.5, 2.0, (C, g.Nt, g.Nf))
+    gap = np.ones(g.Nt, dtype=np.uint8)
+    gap[20:24] = 0
+    # heavy systems so that the track crosses a good part of the band of this small grid
+    P = np.array([[1500.0, 1.2e6, 0.4, 0.6, -0.2, 0.3, 0.5, 1.2], [1500.0, 2.0e6, 1.9, -0.4, 0.1, 0.7, 0.2, 0.8]])
+    return g, D, W, gap, P
+
+
+def test_p14_constant_table_is_the_constant_factor():
+    g, D, W, gap, P = _p14_data(2)
+    ref = O.evaluate(P, D, W, gap, g, 4)
+    tabs = np.stack([[[p[3] + 1j * p[4]], [p[5] + 1j * p[6]]] for p in P])            # [n][2][1]
+    one = O.evaluate_tf(P, tabs, 0.0, 1.0, D, W, gap, g, 4)
+    many = O.evaluate_tf(P, np.repeat(tabs, 5, axis=2), 1e-4, 2e-3, D, W, gap, g, 4)   # five equal knots
+    for r in (one, many):
+        assert np.allclose(r["seg_dh"], ref["seg_dh"], rtol=1e-12, atol=1e-12)
+        assert np.allclose(r["seg_hh"], ref["seg_hh"], rtol=1e-12)
+        assert np.allclose(r["upsilon"], ref["upsilon"], rtol=1e-12)
+
+
+def test_p14_channel_counts():
+    g, D, W, gap, P = _p14_data(3)
+    two = O.evaluate(P, D[:2], W[:2], gap, g, 4)
+    # a third channel without a transfer factor (T_T = 0) changes nothing, exactly
+    three = O.evaluate(P, D, W, gap, g, 4)
+    for k in ("upsilon", "seg_dh", "seg_hh"):
+        assert np.array_equal(two[k], three[k])
+    # ... and the same through a table whose third row is zero
+    tabs = np.stack([[[p[3] + 1j * p[4]], [p[5] + 1j * p[6]], [0.0]] for p in P])
+    t3 = O.evaluate_tf(P, tabs, 0.0, 1.0, D, W, gap, g, 4)
+    assert np.allclose(t3["upsilon"], two["upsilon"], rtol=1e-12)
+    # one channel = two channels with T_E = 0
+    Q = P.copy()
+    Q[:, 5:7] = 0.0
+    one = O.evaluate(P, D[:1], W[:1], gap, g, 4)
+    assert np.allclose(one["upsilon"], O.evaluate(Q, D[:2], W[:2], gap, g, 4)["upsilon"], rtol=1e-13)
+    # three channels with three factors: the sum over alpha of Eq. 3, term by term
+    tabs3 = np.stack([[[0.5 + 0.1j], [-0.2 + 0.6j], [0.3 - 0.3j]]] * len(P))
+    full = O.evaluate_tf(P, tabs3, 0.0, 1.0, D, W, gap, g, 1)
+    zsum, hsum = 0j, 0.0
+    for a in range(3):
+        ta = np.zeros((len(P), 1, 1), dtype=complex) + tabs3[:, a:a + 1]
+        ra = O.evaluate_tf(P[:1], ta[:1], 0.0, 1.0, D[a:a + 1], W[a:a + 1], gap, g, 1)
+        zsum += ra["seg_dh"][0, 0]
+        hsum += ra["seg_hh"][0, 0]
+    assert abs(full["seg_dh"][0, 0] - zsum) < 1e-10 * abs(zsum) and abs(full["seg_hh"][0, 0] - hsum) < 1e-12 * hsum
+
+
+def test_p14_varying_transfer_noiseless_injection_and_loop():
+    g, D, W, gap, P = _p14_data(3)
+    p = P[0]
+    f0, dfk, K = 7.5e-3, 0.6e-3, 6
+    rng = np.random.default_rng(3)
+    tab = rng.standard_normal((3, K)) + 1j * rng.standard_normal((3, K))
+    tr = O.track(p[0], p[1], p[2], p[7], g, O.Opts(), gap)
+    fa = tr["f"][tr["active"]]
+    assert fa.min() < f0 + 2 * dfk and fa.max() > f0 + 5 * dfk            # the track crosses several knots and leaves the table
+    # (i) noiseless injection carrying the same T_alpha(f_m): Upsilon_N = rho^2 for every N
+    S = O.injection_tf(p, tab, f0, dfk, 17.0, W, gap, g, truncate=True)
+    for N in (1, 4, 16):
+        r = O.evaluate_tf(p[None], tab[None], f0, dfk, S, W, gap, g, N)
+        assert abs(r["upsilon"][0] - 289.0) < 1e-8
+    # ... while the factor frozen at its first-knot value loses power
+    frozen = O.evaluate_tf(p[None], tab[None, :, :1], f0, dfk, S, W, gap, g, 1)
+    assert frozen["upsilon"][0] < 0.9 * 289.0
+    # (ii) the per-tranche factor against plain loops: z_n = sum_alpha sum_m T_alpha(f_m) sum_k W conj(D) H
+    N = 4
+    r = O.evaluate_tf(p[None], tab[None], f0, dfk, D, W, gap, g, N)
+    Hd = O.dense_template(p[0], p[1], p[2], p[7], g, O.Opts(), gap)
+    z = [0j] * N
+    hh = [0.0] * N
+    for m in range(g.Nt):
+        if not tr["active"][m]:
+            continue
+        s = min(max((tr["f"][m] - f0) / dfk, 0.0), K - 1.0)
+        j = min(int(math.floor(s)), K - 2)
+        for a in range(3):
+            T = tab[a, j] + (tab[a, j + 1] - tab[a, j]) * (s - j)
+            n = (m * N) // g.Nt
+            for k in range(int(tr["k_lo"][m]), int(tr["k_hi"][m]) + 1):
+                z[n] += T * W[a, m, k] * np.conj(D[a, m, k]) * Hd[m, k]
+                hh[n] += abs(T) ** 2 * W[a, m, k] * abs(Hd[m, k]) ** 2
+    assert np.allclose(r["seg_dh"][0], z, rtol=1e-10, atol=1e-12) and np.allclose(r["seg_hh"][0], hh, rtol=1e-10)
