@@ -66,6 +66,16 @@ typedef struct {
   int    weight_mode;    /* 0 (default): tfs_upload_data looks for separable weights W[a,m,k] = a[m] b[k]
                             (PSD per tranche x PSD shape; C11) and then reads no per-pixel
                             weight in the hot loop; 1: always treat W as a general per-pixel array            */
+  int    basis;          /* 0 (default): the paper's grid, complex short-time Fourier tranches with the
+                            Fresnel-kernel template (Eq. 16).  1: real-coefficient orthonormal WDM wavelet pixels
+                            (BASELINE.json north_star's wording; the paper only cites wavelet methods):
+                            Nt time pixels of duration Nf*dt x Nf layers of width 1/(2 Nf dt), `coeff` is then
+                            [C][Nt][Nf] REAL floats, C <= 2, the track is expanded about the pixel centre and the
+                            template pixel is the Meyer window's chirp response (readings W1-W7);
+                            per segment the statistic is maximised over amplitude and phase with the 2x2 Gram matrix
+                            of the two template quadratures; seg_dh = (a, b), seg_hh = (hcc + hss)/2                  */
+  int    wdm_half_width; /* basis 1: layers kept on either side of the two the track sits between; default 2 (W5)    */
+  double wdm_kappa_max;  /* basis 1: pixels with 4 fdot (Nf dt)^2 above this are skipped; default 8 (W7)              */
 } tfs_opts;
 
 TFS_API void tfs_default_opts(tfs_opts* opts);

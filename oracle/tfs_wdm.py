@@ -176,13 +176,37 @@ def transform(x, g: WdmGrid):
 # ----------------------------------------------------------------------------------------------
 # W4: response of the window to a linear chirp
 # ----------------------------------------------------------------------------------------------
+def chirp_response_closed(x, kappa):
+    """K(x, kappa) in closed form: completing the square in the exponent of each half of cos(pi y/2) turns the
+    defining integral (W4) into Fresnel integrals F = C + i S (oracle/tfs_oracle.py's own routine),
+        K = exp(i pi/4)/(2 sqrt2) sum_{s=+-1} exp(i pi kappa/16 - s i pi x/2) conj[F(v_hi) - F(v_lo)],
+        v_hi,lo = sqrt(2/kappa) (x +- 1 - s kappa/4).
+    Pinned against the quadrature below where both are affordable (tests/test_wdm_pins.py)."""
+    from oracle.tfs_oracle import fresnel_cs
+    x = np.atleast_1d(np.asarray(x, dtype=np.float64))
+    tot = np.zeros(x.shape, dtype=np.complex128)
+    for s in (+1.0, -1.0):
+        vhi = math.sqrt(2.0 / kappa) * (x + 1.0 - s * kappa / 4.0)
+        vlo = math.sqrt(2.0 / kappa) * (x - 1.0 - s * kappa / 4.0)
+        Ch, Sh = fresnel_cs(vhi)
+        Cl, Sl = fresnel_cs(vlo)
+        tot += np.exp(1j * (math.pi * kappa / 16.0 - s * 0.5 * math.pi * x)) * np.conj((Ch - Cl) + 1j * (Sh - Sl))
+    return tot * np.exp(0.25j * math.pi) / (2.0 * math.sqrt(2.0))
+
+
+KAPPA_QUADRATURE_MIN = 0.02      # below this the quadrature needs > 1e4 panels per pixel: the closed form takes over
+
+
 def chirp_response(x, kappa, panels_per_cycle: int = 6):
-    """K(x, kappa) by Gauss-Legendre quadrature of its defining integral (W4); kappa <= 1e-9: the limit."""
+    """K(x, kappa): Gauss-Legendre quadrature of its defining integral (W4) for kappa >= KAPPA_QUADRATURE_MIN, the
+    closed form (pinned against the quadrature) for slower chirps; kappa <= 1e-9: the limit cos(pi x/2)."""
     x = np.atleast_1d(np.asarray(x, dtype=np.float64))
     out = np.empty(x.shape, dtype=np.complex128)
     if kappa <= 1e-9:
         out[:] = np.where(np.abs(x) < 1.0, np.cos(0.5 * math.pi * x), 0.0)
         return out
+    if kappa < KAPPA_QUADRATURE_MIN:
+        return chirp_response_closed(x, kappa)
     xs, ws = np.polynomial.legendre.leggauss(16)
     for i, xv in enumerate(x.ravel()):
         # the phase pi (y + x)^2 / kappa turns at most 2 (|x| + 1) / kappa times per unit y

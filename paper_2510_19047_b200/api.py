@@ -21,7 +21,8 @@ PARAM_COLS = 8
 class tfs_opts(C.Structure):
     _fields_ = [("half_width", C.c_int), ("adaptive_width", C.c_int), ("c_max", C.c_double),
                 ("f_lo", C.c_double), ("f_hi", C.c_double), ("fresnel_mode", C.c_int),
-                ("weight_mode", C.c_int)]
+                ("weight_mode", C.c_int), ("basis", C.c_int), ("wdm_half_width", C.c_int),
+                ("wdm_kappa_max", C.c_double)]
 
 
 class TfsError(RuntimeError):
@@ -127,6 +128,7 @@ class Tfs:
             raise TfsError(rc, self._lib.tfs_last_error(None).decode())
         self._h = h
         self.Nt, self.Nf, self.dt, self.C = Nt, Nf, dt, n_channels
+        self.basis = int(o.basis)
 
     def _check(self, rc):
         if rc != TFS_OK:
@@ -134,7 +136,7 @@ class Tfs:
 
     def upload_data(self, coeff, weight=None, gap_mask=None, stream=None):
         npix = self.C * self.Nt * self.Nf
-        self._check(self._lib.tfs_upload_data(self._h, _ptr(coeff, np.float32, 2 * npix),
+        self._check(self._lib.tfs_upload_data(self._h, _ptr(coeff, np.float32, (1 if self.basis == 1 else 2) * npix),
                                               _ptr(weight, np.float32, npix),
                                               _ptr(gap_mask, np.uint8, self.Nt), _stream(stream)))
 

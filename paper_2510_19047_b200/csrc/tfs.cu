@@ -3,6 +3,7 @@
 #include "../../include/tfs.h"
 #include "tfs_kernels.cuh"
 #include "tfs_frontend.cuh"
+#include "tfs_wdm.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -320,7 +321,8 @@ EvalArgs base_args(const tfs_ctx* ctx, int pr = 0) {
   a.H = ctx->opts.half_width; a.adaptive = ctx->opts.adaptive_width;
   a.DT = ctx->DT;
   a.x_lo = ctx->f_lo * ctx->DT; a.x_hi = ctx->f_hi * ctx->DT;
-  a.c_max = ctx->opts.c_max;
+  a.c_max = ctx->opts.basis == 1 ? ctx->opts.wdm_kappa_max : ctx->opts.c_max;
+  a.basis = ctx->opts.basis; a.wdm_Hw = ctx->opts.wdm_half_width; a.wdm_DTpix = 0.5 * ctx->DT;
   a.far = ctx->far;
   a.n_valid = ctx->n_valid; a.n_tiles = 1; a.n_keys = 2;
   a.wmode = ctx->wmode;
@@ -388,6 +390,9 @@ void tfs_default_opts(tfs_opts* o) {
   o->f_hi = 0.0;
   o->fresnel_mode = 0;
   o->weight_mode = 0;
+  o->basis = 0;
+  o->wdm_half_width = 2;
+  o->wdm_kappa_max = 8.0;
 }
 
 const char* tfs_last_error(const tfs_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
@@ -425,9 +430,14 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   tfs_default_opts(&o);
   if (opts) o = *opts;
   if (o.half_width < 0 || o.half_width > 4096 || !(o.c_max >= 0.0) || o.c_max > 1e6 ||
-      (o.fresnel_mode != 0 && o.fresnel_mode != 1) || (o.weight_mode != 0 && o.weight_mode != 1))
-    return fail(nullptr, TFS_EINVAL, "tfs_create: bad options (half_width %d, c_max %g, fresnel_mode %d, weight_mode %d)",
-                o.half_width, o.c_max, o.fresnel_mode, o.weight_mode);
+      (o.fresnel_mode != 0 && o.fresnel_mode != 1) || (o.weight_mode != 0 && o.weight_mode != 1) ||
+      (o.basis != 0 && o.basis != 1) || o.wdm_half_width < 0 || o.wdm_half_width > 64 || !(o.wdm_kappa_max > 0.0) ||
+      o.wdm_kappa_max > 1e4)
+    return fail(nullptr, TFS_EINVAL, "tfs_create: bad options (half_width %d, c_max %g, fresnel_mode %d, weight_mode %d, basis %d, "
+                "wdm_half_width %d, wdm_kappa_max %g)", o.half_width, o.c_max, o.fresnel_mode, o.weight_mode, o.basis,
+                o.wdm_half_width, o.wdm_kappa_max);
+  if (o.basis == 1 && (n_channels > 2 || o.fresnel_mode != 0))
+    return fail(nullptr, TFS_EINVAL, "tfs_create: the WDM basis takes 1 or 2 channels and fresnel_mode 0");
   tfs_ctx* ctx = new (std::nothrow) tfs_ctx();
   if (!ctx) return fail(nullptr, TFS_ENOMEM, "tfs_create: host allocation failed");
   ctx->Nt = Nt; ctx->Nf = Nf; ctx->C = n_channels; ctx->dt = dt;
@@ -476,6 +486,7 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
       (e = cudaFuncSetAttribute(eval_list_kernel<0, kWSeparable>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_list_kernel<0, kWTimeOnly>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_list_kernel<1, kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_wdm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_slab_kernel<kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWGeneral))) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_slab_kernel<kWSeparable>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWSeparable))) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_slab_kernel<kWTimeOnly>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWTimeOnly))) != cudaSuccess)
@@ -554,9 +565,10 @@ int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const
   do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { cleanup();                       \
        return fail(ctx, e_ == cudaErrorMemoryAllocation ? TFS_ENOMEM : TFS_ECUDA,          \
                    "%s failed: %s", #expr, cudaGetErrorString(e_)); } } while (0)
+  const size_t cfl = ctx->opts.basis == 1 ? 1 : 2;          // floats per coefficient: real WDM pixels / complex tranche bins
   if (!is_device_ptr(coeff)) {
-    UP_CUDA(cudaMalloc(&tmp_c, npix * C * 2 * sizeof(float)));
-    UP_CUDA(cudaMemcpyAsync(tmp_c, coeff, npix * C * 2 * sizeof(float), cudaMemcpyHostToDevice, st));
+    UP_CUDA(cudaMalloc(&tmp_c, npix * C * cfl * sizeof(float)));
+    UP_CUDA(cudaMemcpyAsync(tmp_c, coeff, npix * C * cfl * sizeof(float), cudaMemcpyHostToDevice, st));
     d_coeff = (const float*)tmp_c;
   }
   if (weight && !is_device_ptr(weight)) {
@@ -581,6 +593,21 @@ int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const
   free_piece_tables(ctx);                  // cut for the previous gap mask
   const size_t nrow = (size_t)ctx->Nf + kPadRows;
   const dim3 blocks((unsigned)((ctx->Nf + 31) / 32), (unsigned)((ctx->Nt + 31) / 32));
+  if (ctx->opts.basis == 1) {
+    // WDM pixels: real coefficients [C][Nt][Nf]; y = W d and W as float2 planes in the pair's buffers
+    tfs_ctx::Pair& P = ctx->pair[0];
+    UP_CUDA(cudaMemsetAsync(P.grid, 0, nrow * ctx->ncol * sizeof(float2), st));
+    UP_CUDA(cudaMemsetAsync(P.wgt, 0, nrow * ctx->ncol * sizeof(float2), st));
+    pack_wdm_kernel<<<blocks, 256, 0, st>>>(d_coeff, d_weight, ctx->Nt, ctx->Nf, C, ctx->gap, ctx->vprefix, ctx->ncol,
+                                            (float2*)P.grid, P.wgt);
+    UP_CUDA(cudaGetLastError());
+    ctx->launches += 2;
+    UP_CUDA(cudaStreamSynchronize(st));
+    ctx->wmode = kWGeneral;
+    cleanup();
+    ctx->uploaded = true;
+    return TFS_OK;
+  }
   int wmode = kWTimeOnly;
   for (int pr = 0; pr < ctx->n_pairs; ++pr) {
     tfs_ctx::Pair& P = ctx->pair[pr];
@@ -722,6 +749,7 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
   if (n < 0) return fail(ctx, TFS_EINVAL, "%s: n < 0", who);
   if (N_seg < 1 || N_seg > ctx->Nt) return fail(ctx, TFS_EINVAL, "%s: need 1 <= N_seg <= Nt (got %d, Nt %d)", who, N_seg, ctx->Nt);
   if (!ctx->uploaded) return fail(ctx, TFS_ESTATE, "%s: no data uploaded (call tfs_upload_data first)", who);
+  if (transfer && ctx->opts.basis == 1) return fail(ctx, TFS_EINVAL, "%s: transfer tables are not available in the WDM basis", who);
   if (transfer && (n_knots < 1 || n_knots > 65536 || !std::isfinite(f_knot0) || (n_knots > 1 && !(f_knot_step > 0.0))))
     return fail(ctx, TFS_EINVAL, "%s: transfer table needs 1 <= n_knots <= 65536, finite f_knot0 and f_knot_step > 0", who);
   int rc = check_device(ctx, who);
@@ -765,15 +793,17 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
   if (rc) return rc;
   const int n_tiles = pt->n_tiles;
   const size_t max_pieces = (size_t)n_tiles + (size_t)N_seg;
-  long long sub = (long long)(kScratchBytes / (max_pieces * sizeof(float4)));
+  const bool wdm = ctx->opts.basis == 1;
+  const size_t part_bytes = (wdm ? 2 : 1) * sizeof(float4);          // per (piece, template)
+  long long sub = (long long)(kScratchBytes / (max_pieces * part_bytes));
   sub = std::max<long long>(sub, 1024);
   sub = std::min<long long>(sub, n);
-  rc = ensure(ctx, &ctx->buf_partials, &ctx->cap_partials, (size_t)sub * max_pieces * sizeof(float4));
+  rc = ensure(ctx, &ctx->buf_partials, &ctx->cap_partials, (size_t)sub * max_pieces * part_bytes);
   if (rc) return rc;
 
   // pre-pass scratch (one pooled allocation): constants, keys, bucket tables, item list, unit tables
   const int n_bands = (ctx->Nf - 1) / kBandStride + 1;
-  const bool slab_ok = ctx->opts.fresnel_mode == 0 && n_bands + 2 <= 8192;
+  const bool slab_ok = ctx->opts.fresnel_mode == 0 && n_bands + 2 <= 8192 && !wdm;
   const int n_keys = slab_ok ? n_bands + 2 : 2;
   const size_t n_buckets = (size_t)n_tiles * n_keys;
   const size_t n_items = (size_t)sub * n_tiles;
@@ -841,7 +871,8 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
       }
       const unsigned blocks = (unsigned)ctx->sm_count;       // persistent, 1 CTA per SM
       // the items that gather from global memory (and every item with the paper's approximants) ...
-      if (ctx->opts.fresnel_mode != 0) eval_list_kernel<1, kWGeneral><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
+      if (wdm) eval_wdm_kernel<<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
+      else if (ctx->opts.fresnel_mode != 0) eval_list_kernel<1, kWGeneral><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
       else if (wm == kWTimeOnly) eval_list_kernel<0, kWTimeOnly><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
       else if (wm == kWSeparable) eval_list_kernel<0, kWSeparable><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
       else eval_list_kernel<0, kWGeneral><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
@@ -859,6 +890,12 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
       if (ev[2]) TFS_CUDA(ctx, cudaEventRecord(ev[2], st));
     }
     const int threads = 128;
+    if (wdm)
+      combine_wdm_kernel<<<(unsigned)((nb + threads - 1) / threads), threads, 0, st>>>(
+          (const float4*)ctx->buf_partials, (const uint16_t*)part[1], nb, N_seg, pt->tile_first, n_tiles, pt->piece_seg,
+          pt->piece_tile, dev[0] + off, dev[1] ? dev[1] + off * per[1] : nullptr,
+          dev[2] ? dev[2] + off * per[2] : nullptr, dev[3] ? dev[3] + off * per[3] : nullptr);
+    else
     combine_kernel<<<(unsigned)((nb + threads - 1) / threads), threads, 0, st>>>(
         (const float4*)ctx->buf_partials, (const uint16_t*)part[1], nb, N_seg, pt->tile_first, n_tiles, pt->piece_seg,
         pt->piece_tile, dev[0] + off, dev[1] ? dev[1] + off * per[1] : nullptr,
@@ -922,7 +959,8 @@ int tfs_count_pixels(tfs_ctx* ctx, const double* params, long long n, long long*
   a.n = n;
   const int threads = 256;
   const long long blocks = (n * 32 + threads - 1) / threads;
-  count_pixels_kernel<<<(unsigned)blocks, threads, 0, st>>>(a, d_counts);
+  if (ctx->opts.basis == 1) count_pixels_wdm_kernel<<<(unsigned)blocks, threads, 0, st>>>(a, d_counts);
+  else count_pixels_kernel<<<(unsigned)blocks, threads, 0, st>>>(a, d_counts);
   TFS_CUDA(ctx, cudaGetLastError());
   ctx->launches += 1;
   if (host) {

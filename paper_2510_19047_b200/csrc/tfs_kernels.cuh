@@ -103,6 +103,9 @@ struct EvalArgs {
   const float2* __restrict__ ttab;
   int tt_K, tt_C, tt_ch0;              // knots, channels in the table, first channel of this pair
   float tt_scale, tt_off;              // knot position of bin x: x * tt_scale - tt_off
+  int basis;                           // 0: complex short-time Fourier tranches (the paper); 1: real WDM wavelet pixels (tfs_wdm.cuh)
+  int wdm_Hw;                          // WDM layer window half width
+  double wdm_DTpix;                    // WDM pixel duration Nf dt (DT above is then 2 Nf dt = 1/DF)
   int accumulate;                      // 1: add to the partials instead of overwriting them (second channel pair)
   int t_col;                           // params columns of the pair's first transfer factor (3: T_A, T_E)
   int n_ch_pair;                       // channels in this pair (1 or 2)
@@ -179,11 +182,13 @@ struct TrackPoint {
 // relative error d ~ 4e-7) corrected in fp64 by the binomial series of (1 - e)^{-1/8}, e = 1 - X y0^8
 // ~ 8 d, to third order: the remainder is ~0.04 e^4 < 1e-20, i.e. y is exact to fp64 rounding.
 // `pre` = the tranche may be active at all (valid lane, tau > DT); the band tests are applied here.
-__device__ __forceinline__ TrackPoint track_point(const TplConst& t, int m, double DT,
-                                                  double x_lo, double x_hi, double c_max, bool valid) {
+// tnow = time of the expansion point; the point can be active when tau = tc - tnow > tau_min; band test
+// x >= x_lo, x + band_c c <= x_hi, c <= c_max
+__device__ __forceinline__ TrackPoint track_point_at(const TplConst& t, double tnow, double tau_min,
+                                                     double x_lo, double x_hi, double c_max, double band_c, bool valid) {
   TrackPoint r;
-  const double tau = t.tc - (double)m * DT;
-  bool act = valid && (tau > DT);
+  const double tau = t.tc - tnow;
+  bool act = valid && (tau > tau_min);
   const double X = act ? tau * t.inv5M : 1.0;
   double y0 = (double)ex2_approx(-0.125f * lg2_approx((float)X));
   // X outside the fp32 range (absurd masses): fall back to the seed 1/sqrt(sqrt(sqrt(X)))
@@ -198,9 +203,14 @@ __device__ __forceinline__ TrackPoint track_point(const TplConst& t, int m, doub
   r.Xm14 = (float)y2;
   r.x = y3 * t.xcoefDT;
   r.c = r.x * t.ccoef * (y4 * y4);         // 3 f DT^2 / (8 tau), 1/tau = y^8 / (5M)
-  act = act && (r.x >= x_lo) && (r.x + r.c <= x_hi) && (r.c <= c_max);
+  act = act && (r.x >= x_lo) && (r.x + band_c * r.c <= x_hi) && (r.c <= c_max);
   r.active = act;
   return r;
+}
+
+__device__ __forceinline__ TrackPoint track_point(const TplConst& t, int m, double DT,
+                                                  double x_lo, double x_hi, double c_max, bool valid) {
+  return track_point_at(t, (double)m * DT, DT, x_lo, x_hi, c_max, 1.0, valid);
 }
 
 __device__ __forceinline__ void window(const TrackPoint& tp, int H, int adaptive, int Nf,
@@ -1366,6 +1376,16 @@ __device__ __forceinline__ int item_key(const EvalArgs& a, const TplConst& T, in
   const int i0 = tile * kTS, i1 = min(i0 + kTS, a.n_valid);
   if (i0 >= i1) return 0;
   const int m0 = a.valid_m[i0], m1 = a.valid_m[i1 - 1];
+  if (a.basis == 1) {
+    // WDM pixels (tfs_wdm.cuh): the same monotone bounds with the WDM activity rule; always the list path
+    const double sl = 1.0 + 1e-9;
+    const TrackPoint w0 = track_point_at(T, (double)m0 * a.wdm_DTpix, a.DT, -1.0, 1e300, 1e300, 0.0, true);
+    if (!w0.active) return 0;
+    if (w0.x + 0.5 * w0.c > a.x_hi * sl || w0.c > a.c_max * sl) return 0;
+    const TrackPoint w1 = track_point_at(T, (double)m1 * a.wdm_DTpix, a.DT, -1.0, 1e300, 1e300, 0.0, true);
+    if (w1.active && w1.x * sl < a.x_lo) return 0;
+    return 1;
+  }
   const TrackPoint t0 = track_point(T, m0, a.DT, -1.0, 1e300, 1e300, true);
   if (!t0.active) return 0;                                        // tau <= DT at the tile's start
   const double slack = 1.0 + 1e-9;

@@ -66,19 +66,22 @@ def test_w_response_limits_and_symmetry():
 
 
 def test_w_response_closed_form_in_fresnel_integrals():
-    """K has a closed form in Fresnel integrals (complete the square in the exponent of each half of the cosine):
-       K = exp(i pi/4) / (2 sqrt2) sum_{s=+-1} exp(i pi kappa/16 - s i pi x/2) conj[F(v_hi) - F(v_lo)],
-       v = sqrt(2/kappa) (x +- 1 - s kappa/4),  F = C + i S.   (What the CUDA path evaluates.)"""
-    for kap in (1e-3, 0.05, 0.5, 3.0):
-        x = np.linspace(-3, 3, 25)
-        tot = 0
-        for s in (+1, -1):
-            vhi = math.sqrt(2 / kap) * (x + 1 - s * kap / 4)
-            vlo = math.sqrt(2 / kap) * (x - 1 - s * kap / 4)
-            Ch, Sh = O.fresnel_cs(vhi)
-            Cl, Sl = O.fresnel_cs(vlo)
-            tot = tot + np.exp(1j * math.pi * kap / 16 - s * 1j * math.pi * x / 2) * np.conj((Ch - Cl) + 1j * (Sh - Sl))
-        assert np.abs(tot * np.exp(0.25j * math.pi) / (2 * math.sqrt(2)) - Wd.chirp_response(x, kap)).max() < 1e-11
+    """The closed form the oracle switches to for slow chirps (and the CUDA path evaluates) against the quadrature
+    of the defining integral, on both sides of the switch, and its continuity across it."""
+    x = np.linspace(-3, 3, 25)
+    for kap in (1e-3, 0.01, 0.05, 0.5, 3.0):
+        quad = Wd.chirp_response(x, max(kap, Wd.KAPPA_QUADRATURE_MIN)) if kap >= Wd.KAPPA_QUADRATURE_MIN else None
+        if quad is None:
+            # force the quadrature below the switch (slow: only here)
+            saved = Wd.KAPPA_QUADRATURE_MIN
+            Wd.KAPPA_QUADRATURE_MIN = 0.0
+            try:
+                quad = Wd.chirp_response(x, kap)
+            finally:
+                Wd.KAPPA_QUADRATURE_MIN = saved
+        assert np.abs(Wd.chirp_response_closed(x, kap) - quad).max() < 1e-11
+    k0 = Wd.KAPPA_QUADRATURE_MIN
+    assert np.abs(Wd.chirp_response(x, k0 * (1 - 1e-9)) - Wd.chirp_response(x, k0)).max() < 1e-8
 
 
 @pytest.mark.parametrize("kappa", [1e-3, 0.05, 0.5])
