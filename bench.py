@@ -237,6 +237,113 @@ def roofline_terms(leg, steps, pixels, wstruct, l2_gbs, peaks, peak_src, sm_coun
     return terms, kern_ms, bytes_per_launch
 
 
+def _wdm_oracle_one(i):
+    from oracle import tfs_wdm as Wd
+    d = _ORA
+    r = Wd.evaluate(d["params"][i:i + 1], d["D"], d["W"], d["gap"], d["grid"], d["N_seg"])
+    return float(r["upsilon"][0]), int((r["seg_gram"][0, :, 0] > 0).sum())
+
+
+def main_wdm(args, info, w, n, N_seg, k_top, cfg):
+    """The same step in the WDM wavelet pixel basis (tfs_opts.basis = 1): real coefficients on the same Nt x Nf
+    grid (pixel duration Nf dt), general per-pixel weights.  One timed leg + the oracle (oracle/tfs_wdm.py) on a
+    bounded sample; algorithmic bytes per pixel-eval: 4 B datum + 4 B weight."""
+    import multiprocessing as mp
+    rank, world = info.rank, info.world
+    cfg = dict(cfg, workload=cfg["workload"].replace("x 2 channels (A,E)", "x 2 channels (A,E), real WDM wavelet pixels (basis = 1)"))
+    coeff_c, weight, gap = synth.make_data(w)
+    coeff = np.ascontiguousarray(coeff_c[..., 0])                        # real pixels with the same noise model
+    del coeff_c
+    params = synth.make_templates(w, n, seed=replicas.bank_seed(w.seed, rank))
+    if args.impl == "reference" or (rank == 0 and world == 1 and not args.no_cpu_baseline):
+        from oracle import tfs_wdm as Wd
+        cores = host_cores()
+        procs = max(1, min(cores, 16))
+        ns = args.cpu_sample or 4 * procs
+        _ORA.update(params=params, D=coeff.astype(np.float64), W=weight.astype(np.float64), gap=gap,
+                    grid=Wd.WdmGrid(w.Nt, w.Nf, w.dt), N_seg=N_seg)
+        t0 = time.perf_counter()
+        with mp.get_context("fork").Pool(procs) as pool:
+            ora = pool.map(_wdm_oracle_one, list(range(ns)), chunksize=1)
+        dt = time.perf_counter() - t0
+        _ORA.clear()
+        cpu_baseline = {"value": ns / dt, "unit": "templates/s", "cores": procs, "kind": "oracle",
+                        "sample": f"first {ns} templates of the bank, {dt:.1f} s wall (oracle/tfs_wdm.py, {procs} processes)"}
+        if args.impl == "reference":
+            if rank == 0:
+                print(json.dumps({"impl": "reference", "metric": "templates/sec", "value": ns / dt, "unit": "templates/s",
+                                  "n_gpus": args.gpus, "steps": 1, "warmup": 0, "ms_per_step": 1e3 * dt,
+                                  "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                                  "data": "synthetic", "config": cfg, "cpu_baseline": cpu_baseline,
+                                  "e2e": {"value": ns / dt, "unit": "templates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                                  "gpu_launches": 0}))
+            return 0
+    else:
+        cpu_baseline, ora = None, None
+    import torch
+    from paper_2510_19047_b200 import api, build
+    torch.cuda.set_device(info.local_rank)
+    dev = torch.device("cuda", info.local_rank)
+    replicas.init(info, "nccl", dev)
+    if rank == 0:
+        build.build()
+    replicas.barrier(info)
+    ctx = api.Tfs(w.Nt, w.Nf, w.dt, basis=1)
+    ctx.upload_data(coeff, weight, gap)
+    d_params = torch.from_numpy(params).to(dev)
+    counts = torch.empty(n, dtype=torch.int64, device=dev)
+    ctx.count_pixels(d_params, counts)
+    torch.cuda.synchronize()
+    pixels = int(counts.sum().item())
+    l2_gbs = ctx.probe_l2_bandwidth(32 << 20, 200)
+    warm = max(args.warmup, 3)
+    leg = time_leg(api, torch, ctx, w, d_params, n, N_seg, k_top, args.steps, warm, info, dev, rank == 0)
+    parity = None
+    if ora is not None:
+        uo = np.array([u for u, _ in ora]); neff = np.maximum(np.array([e for _, e in ora]), 1)
+        err = np.abs(leg["d_ups"][:len(uo)].cpu().numpy().astype(np.float64) - uo) / np.maximum(uo, 2.0 * neff)
+        parity = {"n": int(len(uo)), "max_norm_err": float(err.max()), "tolerance": 1e-4, "ok": bool(err.max() <= 1e-4),
+                  "criterion": "|dUpsilon| <= 1e-4 max(Upsilon, 2 N_eff), GPU output of the timed run vs oracle/tfs_wdm.py"}
+    h_params = torch.from_numpy(params).pin_memory()
+    h_ups = torch.empty(n, dtype=torch.float32).pin_memory()
+    h_idx = torch.empty(k_top, dtype=torch.int64).pin_memory()
+    h_val = torch.empty(k_top, dtype=torch.float32).pin_memory()
+    ctx.eval(h_params.numpy(), N_seg, h_ups.numpy())
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ctx.eval(h_params.numpy(), N_seg, h_ups.numpy())
+        ctx.topk(h_ups.numpy(), k_top, h_idx.numpy(), h_val.numpy())
+    torch.cuda.synchronize()
+    ms_e2e = replicas.max_over_ranks(1e3 * (time.perf_counter() - t0) / args.steps, info, dev)
+    if rank != 0:
+        replicas.finish(info)
+        return 0
+    prof = leg["prof"]
+    n_launch = max(prof["eval_launches"], 1)
+    kern_ms = (prof["slab_kernel_ms"] + prof["list_kernel_ms"]) / n_launch
+    bytes_per_launch = 8.0 * 2 * pixels / (n_launch / args.steps)
+    achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
+    line = {"metric": "templates/sec", "value": world * n / (leg["ms_step"] * 1e-3), "unit": "templates/s", "n_gpus": world,
+            "steps": args.steps, "warmup": warm, "ms_per_step": leg["ms_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
+            "pixel_evals_per_sec": world * 2 * pixels / (leg["ms_step"] * 1e-3), "pixel_evals_per_template": 2 * pixels / n,
+            "roofline": {"bound": "l2", "kernel": "eval_wdm_kernel", "achieved": achieved, "peak": l2_gbs, "unit": "GB/s",
+                         "frac": achieved / l2_gbs, "traffic": None,
+                         "peak_source": "tfs_probe_l2_bandwidth, 32 MiB buffer, this run",
+                         "algorithmic_bytes_per_pixel_eval": 8.0, "algorithmic_bytes_per_launch": bytes_per_launch,
+                         "kernel_ms_per_launch": kern_ms,
+                         "note": "a first kernel for this basis: four table look-ups and two fp64 phase reductions per pixel; "
+                                 "it is instruction-bound, far from the byte roof"},
+            "cpu_baseline": cpu_baseline, "parity": parity,
+            "e2e": {"value": world * n / (ms_e2e * 1e-3), "unit": "templates/s", "h2d_bytes_per_step": int(params.nbytes),
+                    "d2h_bytes_per_step": int(4 * n + 12 * k_top), "ms_per_step": ms_e2e},
+            "gpu_launches": int(prof["kernel_launches"]), "clocks": leg["clocks"]}
+    print(json.dumps(line))
+    replicas.finish(info)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -250,6 +357,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-general-leg", action="store_true",
                     help="skip the second timed leg with general per-pixel weights (weight_mode = 1)")
+    ap.add_argument("--basis", default="sft", choices=["sft", "wdm"],
+                    help="sft: the paper's complex short-time Fourier tranches (headline); wdm: real WDM wavelet pixels "
+                         "(tfs_opts.basis = 1, SURVEY.md 8(f) NEXT-1) on the same grid shape")
     ap.add_argument("--weight-mode", type=int, default=0, choices=[0, 1],
                     help="tfs_opts.weight_mode of the headline leg: 0 = exploit separable weights (default), 1 = general per-pixel path")
     args = ap.parse_args()
@@ -270,6 +380,9 @@ def main():
                   f"inputs fit the L2 (grid {grid_bytes / 1e6:.0f} MB): the step's own scratch (partials, item lists) is rewritten "
                   "every step"),
            "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no collective), one seeded bank per rank"}
+
+    if args.basis == "wdm":
+        return main_wdm(args, info, w, n, N_seg, k_top, cfg)
 
     # ---------------- reference arm: the CPU oracle, rank 0 only ----------------
     if args.impl == "reference":
