@@ -334,6 +334,7 @@ constexpr float kVFar = 3.0f;
 #define TFS_VFAR2 24.0f
 #endif
 constexpr float kVFar2 = TFS_VFAR2;
+constexpr float kNearSeries = 0.3f;    // pixel_near: midpoint expansion of F(v1) - F(v0) when pi |vm| (v1 - v0)/2 is below this
 
 struct LaneTrack {      // per-lane (= per-tranche) constants of the pixel loop
   float sc;             // sqrt(2/c)
@@ -425,6 +426,23 @@ __device__ __forceinline__ void pixel_near(const LaneTrack& L, float u, float ms
     hr -= m * (ct + st);
     hi -= m * (ct - st);
   }
+  const float hs = 0.5f * L.sc * L.c;                 // (v1 - v0)/2 = sqrt(c/2)
+  const float al = 3.14159265358979f * (v0 + hs);     // pi * midpoint
+  if (MODE == 0 && fabsf(al) * hs < kNearSeries && hs < 0.1f) {
+    // slow chirp next to the track: h' = exp(-i pi u^2/c) [F(v1) - F(v0)] is O(sqrt(2c)) while the terms above are
+    // O(1) (table error 2e-7 absolute, i.e. 2e-7/sqrt(2c) relative).  Expand the integral about the midpoint vm:
+    //   F(v1) - F(v0) = exp(i pi vm^2/2) int_{-h}^{h} exp(i (alpha t + beta t^2)) dt,  alpha = pi vm, beta = pi/2,
+    // the prefactor's phase cancels against -pi u^2/c up to pi (u + c/4), and the integral is, to O((alpha h)^6),
+    //   2h [1 + (i beta - alpha^2/2) h^2/3 + (alpha^4/24 - beta^2/2 - i alpha^2 beta/2) h^4/5]
+    const float A2 = al * al, h2 = hs * hs;
+    const float R = fmaf(h2 * h2, 0.2f * fmaf(A2 * A2, 1.0f / 24.0f, -1.2337006f), fmaf(A2 * h2, -1.0f / 6.0f, 1.0f));
+    const float I = h2 * fmaf(h2, -0.15707963f * A2, 0.52359878f);
+    float st, ct;
+    __sincosf(3.14159265358979f * fmaf(0.25f, L.c, u), &st, &ct);
+    const float m = 2.0f * hs * (MASKED ? msk : 1.0f);
+    hr = m * fmaf(R, ct, -I * st);
+    hi = m * fmaf(R, st, I * ct);
+  }
 }
 
 constexpr int kZNear = 0, kZFar = 1, kZFar2 = 2;
@@ -462,14 +480,19 @@ constexpr int kRagMax = kPadRows - 2 * kGroup;   // largest Wmax - Wmin handled 
 static_assert(kRagMax >= 1, "kPadRows too small for kGroup");
 constexpr int kLutCopiesList = 8;
 
-// ZONES: 1 = test the offset against the near zone, 0 = the offset is known to be far
+// ZONES: 1 = test the offset against the near zone, 0 = the offset is known to be far.
+// The bin offset u = x - k is formed per pixel as fr + n with fr = x - round(x) in [-1/2, 1/2] (from the fp64 x)
+// and n = round(x) - k an exact small integer: for the bin nearest the track (n = 0) u = fr exactly, elsewhere
+// |u| >= 1/2 and the rounding is relative.  A value stepped down from u(k_lo) ~ H would carry 1 ulp of H against
+// u ~ 1e-5 when the track sits on a bin (found by tests/test_gpu_parity.py::test_precision_worst_case_hunt).
 template <int MODE, int WMODE, int MASKED, int ZONES>
 __device__ __forceinline__ void pixel_step(const LaneTrack& L, const FarCoef& C, int jj, int Wm, int JA, int JB,
-                                           const float4 Yc, const float2 Wc, float& u, unsigned lut_lane,
+                                           const float4 Yc, const float2 Wc, float fr, float& nn, unsigned lut_lane,
                                            LaneSums& s) {
+  const float u = fr + nn;
   if (ZONES && jj >= JA && jj < JB) pixel_kind<kZNear, MODE, WMODE, MASKED, kLutCopiesList>(L, C, jj, Wm, Yc, Wc, u, lut_lane, s);
   else pixel_kind<kZFar, MODE, WMODE, MASKED, kLutCopiesList>(L, C, jj, Wm, Yc, Wc, u, lut_lane, s);
-  u -= 1.0f;
+  nn -= 1.0f;
 }
 
 struct PixelBuf { float4 Y[kGroup]; float2 W[kGroup]; };
@@ -498,35 +521,35 @@ __device__ __forceinline__ void load_group(const EvalArgs& a, PixelBuf& B, int i
 
 template <int MODE, int WMODE, int MASKED>
 __device__ __forceinline__ void compute_group(const LaneTrack& L, const FarCoef& C, const PixelBuf& B, int j0, int Wm,
-                                              int Wmax, int JA, int JB, float& u, unsigned lut_lane, LaneSums& s) {
+                                              int Wmax, int JA, int JB, float fr, float& nn, unsigned lut_lane, LaneSums& s) {
   if (j0 < JB && j0 + kGroup > JA) {
 #pragma unroll
     for (int p = 0; p < kGroup; ++p)
       if (!MASKED || j0 + p < Wmax)
-        pixel_step<MODE, WMODE, MASKED, 1>(L, C, j0 + p, Wm, JA, JB, B.Y[p], B.W[p], u, lut_lane, s);
+        pixel_step<MODE, WMODE, MASKED, 1>(L, C, j0 + p, Wm, JA, JB, B.Y[p], B.W[p], fr, nn, lut_lane, s);
   } else {
 #pragma unroll
     for (int p = 0; p < kGroup; ++p)
       if (!MASKED || j0 + p < Wmax)
-        pixel_step<MODE, WMODE, MASKED, 0>(L, C, j0 + p, Wm, JA, JB, B.Y[p], B.W[p], u, lut_lane, s);
+        pixel_step<MODE, WMODE, MASKED, 0>(L, C, j0 + p, Wm, JA, JB, B.Y[p], B.W[p], fr, nn, lut_lane, s);
   }
 }
 
 // one group from buffer B: unmasked while the whole group lies below Wmin
 template <int MODE, int WMODE>
 __device__ __forceinline__ void compute_group_auto(const LaneTrack& L, const FarCoef& C, const PixelBuf& B, int j0,
-                                                   int Wm, int Wmin, int Wmax, int JA, int JB, float& u,
+                                                   int Wm, int Wmin, int Wmax, int JA, int JB, float fr, float& nn,
                                                    unsigned lut_lane, LaneSums& s) {
-  if (j0 + kGroup <= Wmin) compute_group<MODE, WMODE, 0>(L, C, B, j0, Wm, Wmax, JA, JB, u, lut_lane, s);
-  else compute_group<MODE, WMODE, 1>(L, C, B, j0, Wm, Wmax, JA, JB, u, lut_lane, s);
+  if (j0 + kGroup <= Wmin) compute_group<MODE, WMODE, 0>(L, C, B, j0, Wm, Wmax, JA, JB, fr, nn, lut_lane, s);
+  else compute_group<MODE, WMODE, 1>(L, C, B, j0, Wm, Wmax, JA, JB, fr, nn, lut_lane, s);
 }
 
 // idx = pixel index of offset 0, stp = ncol for an active lane and 0 otherwise, Wm = window length (>= 1
 // for active lanes, 0 otherwise)
 template <int MODE, int WMODE>
 __device__ __forceinline__ void pixel_loop_global(const EvalArgs& a, const LaneTrack& L, const FarCoef& C, int Wm, int Wmin,
-                                                  int Wmax, int JA, int JB, int idx, int stp, int kb, int kstp, float u,
-                                                  unsigned lut_lane, LaneSums& s) {
+                                                  int Wmax, int JA, int JB, int idx, int stp, int kb, int kstp, float fr,
+                                                  float nn, unsigned lut_lane, LaneSums& s) {
   PixelBuf A, B;
 #pragma unroll
   for (int p = 0; p < kGroup; ++p) { A.W[p] = make_float2(0.f, 0.f); B.W[p] = make_float2(0.f, 0.f); }
@@ -538,123 +561,25 @@ __device__ __forceinline__ void pixel_loop_global(const EvalArgs& a, const LaneT
     load_group<0, WMODE>(a, A, idx, stp, kb, kstp, 0, jlast);
     for (int j = 0; j < Wmax; j += 2 * kGroup) {
       if (j + kGroup < Wmax) load_group<0, WMODE>(a, B, idx, stp, kb, kstp, j + kGroup, jlast);
-      compute_group_auto<MODE, WMODE>(L, C, A, j, Wm, Wmin, Wmax, JA, JB, u, lut_lane, s);
+      compute_group_auto<MODE, WMODE>(L, C, A, j, Wm, Wmin, Wmax, JA, JB, fr, nn, lut_lane, s);
       if (j + kGroup >= Wmax) break;
       if (j + 2 * kGroup < Wmax) load_group<0, WMODE>(a, A, idx, stp, kb, kstp, j + 2 * kGroup, jlast);
-      compute_group_auto<MODE, WMODE>(L, C, B, j + kGroup, Wm, Wmin, Wmax, JA, JB, u, lut_lane, s);
+      compute_group_auto<MODE, WMODE>(L, C, B, j + kGroup, Wm, Wmin, Wmax, JA, JB, fr, nn, lut_lane, s);
     }
   } else {
     // very ragged chunk (wide tracks next to narrow ones): every load clamped, every step masked
     load_group<1, WMODE>(a, A, idx, stp, kb, kstp, 0, jlast);
     for (int j = 0; j < Wmax; j += 2 * kGroup) {
       load_group<1, WMODE>(a, B, idx, stp, kb, kstp, j + kGroup, jlast);
-      compute_group<MODE, WMODE, 1>(L, C, A, j, Wm, Wmax, JA, JB, u, lut_lane, s);
+      compute_group<MODE, WMODE, 1>(L, C, A, j, Wm, Wmax, JA, JB, fr, nn, lut_lane, s);
       if (j + kGroup >= Wmax) break;
       load_group<1, WMODE>(a, A, idx, stp, kb, kstp, j + 2 * kGroup, jlast);
-      compute_group<MODE, WMODE, 1>(L, C, B, j + kGroup, Wm, Wmax, JA, JB, u, lut_lane, s);
+      compute_group<MODE, WMODE, 1>(L, C, B, j + kGroup, Wm, Wmax, JA, JB, fr, nn, lut_lane, s);
     }
   }
 }
 
-// ------------------------------------------------------------------------------------------
-// Pixel loop of the SLAB kernel.  The band's data slab sits in shared memory as [row][kTS columns] float4
-// (plus [row][kTS] float2 weights, or the band's rows of the b table); lane l of chunk h reads column
-// 32 h + l, so the 8 lanes of a quarter-warp always fall in 8 different 16-byte bank groups: an LDS.128
-// is conflict-free whatever rows the lanes are on.  The window offsets are cut, warp-uniformly, into
-//   [0, J2A) FAR2 | [J2A, JA) FAR | [JA, JB) NEAR | [JB, J2B) FAR | [J2B, Wmax) FAR2
-// and each run into its unmasked part (below Wmin, the shortest active window) and its masked rest.
-// An inactive lane walks rows row0, row0+1, ... of its own column (always inside the slab).
-// ------------------------------------------------------------------------------------------
 constexpr int kLutCopiesSlab = 4;
-
-template <int WMODE>
-struct SlabLane {
-  unsigned y_addr;      // shared address of this lane's pixel of offset 0
-  unsigned w_addr;      // kWGeneral: same in the weight slab; kWSeparable: row of the b table; else unused
-#ifdef TFS_BOUNDS_CHECK
-  int row_rel, rows;    // slab row of offset 0, rows in the slab
-#endif
-  __device__ __forceinline__ void load(int j, float4& Y, float2& W) const {
-#ifdef TFS_BOUNDS_CHECK
-    if (row_rel + j < 0 || row_rel + j >= rows) __trap();
-#endif
-    Y = lds128(y_addr + (unsigned)j * (kTS * 16u));
-    if (WMODE == kWGeneral) W = lds64(w_addr + (unsigned)j * (kTS * 8u));
-    else if (WMODE == kWSeparable) W = lds64(w_addr + (unsigned)j * 8u);
-    else W = make_float2(0.f, 0.f);
-  }
-};
-
-// offsets [jb, je) of kind KIND, unmasked (every lane's window reaches je): four pixels per iteration, then singles
-template <int KIND, int WMODE>
-__device__ __forceinline__ void zone_run(const SlabLane<WMODE>& sl, const LaneTrack& L, const FarCoef& C, int jb, int je,
-                                         float u0, unsigned lut_lane, LaneSums& s) {
-  int j = jb;
-  float u = u0 - (float)jb;                     // exact: small integers
-  for (; j + 3 < je; j += 4) {
-    float4 Y[4];
-    float2 W[4];
-#pragma unroll
-    for (int q = 0; q < 4; ++q) sl.load(j + q, Y[q], W[q]);
-#pragma unroll
-    for (int q = 0; q < 4; ++q)
-      pixel_kind<KIND, 0, WMODE, 0, kLutCopiesSlab>(L, C, j + q, 0, Y[q], W[q], u - (float)q, lut_lane, s);
-    u -= 4.0f;
-  }
-#pragma unroll 1
-  for (; j < je; ++j) {
-    float4 Y0;
-    float2 W0;
-    sl.load(j, Y0, W0);
-    pixel_kind<KIND, 0, WMODE, 0, kLutCopiesSlab>(L, C, j, 0, Y0, W0, u, lut_lane, s);
-    u -= 1.0f;
-  }
-}
-
-// The zones may run in any order (u is re-derived from the offset), so the two FAR2 runs and the two FAR
-// runs share their code; everything below Wmin (the shortest active window) is unmasked, and the few
-// offsets in [Wmin, Wmax) go through one generic masked loop.
-template <int WMODE>
-__device__ __forceinline__ void pixel_loop_slab(const SlabLane<WMODE>& sl, const LaneTrack& L, const FarCoef& C, int Wm,
-                                                int Wmin, int Wmax, int J2A, int JA, int JB, int J2B, float u0,
-                                                unsigned lut_lane, LaneSums& s) {
-  const int Z2A = min(J2A, Wmin), ZA = min(JA, Wmin), ZB = min(JB, Wmin), Z2B = min(J2B, Wmin);
-#pragma unroll 1
-  for (int r = 0; r < 2; ++r) zone_run<kZFar2, WMODE>(sl, L, C, r ? Z2B : 0, r ? Wmin : Z2A, u0, lut_lane, s);
-#pragma unroll 1
-  for (int r = 0; r < 2; ++r) zone_run<kZFar, WMODE>(sl, L, C, r ? ZB : Z2A, r ? Z2B : ZA, u0, lut_lane, s);
-  {
-    int j = ZA;
-    float u = u0 - (float)ZA;
-    for (; j + 1 < ZB; j += 2) {
-      float4 Y0, Y1;
-      float2 W0, W1;
-      sl.load(j, Y0, W0);
-      sl.load(j + 1, Y1, W1);
-      pixel_kind<kZNear, 0, WMODE, 0, kLutCopiesSlab>(L, C, j, 0, Y0, W0, u, lut_lane, s);
-      pixel_kind<kZNear, 0, WMODE, 0, kLutCopiesSlab>(L, C, j + 1, 0, Y1, W1, u - 1.0f, lut_lane, s);
-      u -= 2.0f;
-    }
-    if (j < ZB) {
-      float4 Y0;
-      float2 W0;
-      sl.load(j, Y0, W0);
-      pixel_kind<kZNear, 0, WMODE, 0, kLutCopiesSlab>(L, C, j, 0, Y0, W0, u, lut_lane, s);
-    }
-  }
-  // masked tail: lanes whose window ended contribute zero
-  float u = u0 - (float)Wmin;
-#pragma unroll 1
-  for (int j = Wmin; j < Wmax; ++j) {
-    float4 Y0;
-    float2 W0;
-    sl.load(j, Y0, W0);
-    if (j >= JA && j < JB) pixel_kind<kZNear, 0, WMODE, 1, kLutCopiesSlab>(L, C, j, Wm, Y0, W0, u, lut_lane, s);
-    else if (j < J2A || j >= J2B) pixel_kind<kZFar2, 0, WMODE, 1, kLutCopiesSlab>(L, C, j, Wm, Y0, W0, u, lut_lane, s);
-    else pixel_kind<kZFar, 0, WMODE, 1, kLutCopiesSlab>(L, C, j, Wm, Y0, W0, u, lut_lane, s);
-    u -= 1.0f;
-  }
-}
 
 // ------------------------------------------------------------------------------------------
 // One work item: template `it` on time tile `tile` (rows a2-a7).  LANES ARE TRANCHES: lane l owns the
@@ -666,13 +591,12 @@ __device__ __forceinline__ void pixel_loop_slab(const SlabLane<WMODE>& sl, const
 // template's table, Eq. 29) and added to the lane's running sums of the current piece; when a piece
 // ends -- inside a chunk at a segment boundary, or at the end of the tile -- the lanes are summed with a
 // shuffle butterfly and the piece's partial {z, hh} is stored.
-// SLAB: pixels come from the shared-memory slab whose first row is row0 (eval_slab_kernel);
-// otherwise from global memory (eval_list_kernel).
+// This is the item evaluator of eval_list_kernel (pixels gathered from global memory); eval_slab_kernel uses
+// eval_item_pair below.
 // ------------------------------------------------------------------------------------------
-template <int MODE, int WMODE, bool SLAB>
+template <int MODE, int WMODE>
 __device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it, const int tile, const int lane,
-                                          const unsigned lut_lane, const unsigned slab_y, const unsigned slab_w,
-                                          const int row0) {
+                                          const unsigned lut_lane) {
   const TplConst T = a.tconst[it];
   // valid (non-gap) tranches of the tile: entries [i0, i1) of the compacted list (C10), cut by the
   // segment boundaries into pieces [p, p_stop)
@@ -711,8 +635,8 @@ __device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it,
     const bool closes = p < p_stop && pend <= cend;   // a piece ends inside this chunk (warp-uniform)
     float vr = 0.f, vi = 0.f, vq = 0.f;               // this tranche's contribution to z and hh
     if (act_mask != 0u) {
-      int Wm = 0, k_lo = SLAB ? row0 : 0, ja = 0x7fffffff, jb = 0, j2a = 0x7fffffff, j2b = 0;
-      float u = -1.f, Pr = 0.f, Pi = 0.f;
+      int Wm = 0, k_lo = 0, ja = 0x7fffffff, jb = 0;
+      float fr = 0.f, n0 = -1.f, Pr = 0.f, Pi = 0.f;       // u_j = fr + (n0 - j)
       LaneTrack L;        // inactive lanes: u_j = -1 - j, u_j + c = -0.5 - j (finite h' on finite data)
       L.sc = 1.f; L.kap = 1.f; L.c = 0.5f; L.hc = 0.f; L.Er = 0.f; L.Ei = 0.f;
       if (tp.active) {
@@ -720,8 +644,10 @@ __device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it,
         window(tp, a.H, a.adaptive, a.Nf, k_lo, k_hi);
         Wm = k_hi - k_lo + 1;
         const double flx = floor(tp.x);
-        const float fracx = (float)(tp.x - flx);
-        u = fracx - (float)(k_lo - (int)flx);          // cancellation-safe x - k_lo
+        const int kr = __double2int_rn(tp.x);
+        fr = (float)(tp.x - (double)kr);               // x - k = (x - round(x)) + (round(x) - k): see pixel_step
+        n0 = (float)(kr - k_lo);
+        const float u = fr + n0;
         // phases in turns, reduced in fp64 (phi reaches ~1e8 rad), then to [-1/2, 1/2)
         double tphi = T.phic_turns - tp.X58 * (1.0 / kPi);
         tphi -= floor(tphi);
@@ -744,11 +670,6 @@ __device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it,
         const float d = fmaf(kVFar, L.kap, 1e-3f);
         ja = max(__float2int_rd(u - d) + 1, 0);
         jb = __float2int_ru(u + cf + d);
-        if (SLAB) {
-          const float d2 = fmaf(kVFar2, L.kap, 1e-3f);   // offsets outside (j2a, j2b) have |v0|, |v1| >= kVFar2
-          j2a = max(__float2int_rd(u - d2) + 1, 0);
-          j2b = __float2int_ru(u + cf + d2);
-        }
       }
       const int Wmax = __reduce_max_sync(0xffffffffu, Wm);
       const int Wmin = __reduce_min_sync(0xffffffffu, tp.active ? Wm : 0x7fffffff);
@@ -760,24 +681,11 @@ __device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it,
       // ---------------- pixel loop (a3-a5): lane walks its own window ----------------
       LaneSums s;
       s.zr = pk(0.f, 0.f); s.zi = pk(0.f, 0.f); s.q = pk(0.f, 0.f);
-      if (SLAB) {
-        const int J2A = min(__reduce_min_sync(0xffffffffu, j2a), JA);
-        const int J2B = max(min(__reduce_max_sync(0xffffffffu, j2b), Wmax), JB);
-        SlabLane<WMODE> sl;
-        const int rr = k_lo - row0;
-        const unsigned col = (unsigned)(ic - i0 + lane);
-        sl.y_addr = slab_y + ((unsigned)rr * kTS + col) * 16u;
-        sl.w_addr = WMODE == kWGeneral ? slab_w + ((unsigned)rr * kTS + col) * 8u : slab_w + (unsigned)rr * 8u;
-#ifdef TFS_BOUNDS_CHECK
-        sl.row_rel = rr; sl.rows = slab_rows(WMODE);
-        if (rr < 0 || rr + Wmax > slab_rows(WMODE)) __trap();
-#endif
-        pixel_loop_slab<WMODE>(sl, L, a.far, Wm, Wmin, Wmax, J2A, JA, JB, J2B, u, lut_lane, s);
-      } else {
+      {
         const int stp = tp.active ? a.ncol : 0;
         const int idx = tp.active ? k_lo * a.ncol + i : (valid ? i : i0);
         pixel_loop_global<MODE, WMODE>(a, L, a.far, Wm, Wmin, Wmax, JA, JB, idx, stp, tp.active ? k_lo : 0,
-                                       tp.active ? 1 : 0, u, lut_lane, s);
+                                       tp.active ? 1 : 0, fr, n0, lut_lane, s);
       }
       // ---------------- a6: transfer factors, the tranche's factor P, weights a[i] ----------------
       float T0r = T.T0r, T0i = T.T0i, T1r = T.T1r, T1i = T.T1i;
@@ -966,16 +874,18 @@ __device__ __forceinline__ void pair_pixel(const SlabPair<WMODE>& sl, const Pair
 #endif
 constexpr int kPairUnroll = TFS_PAIR_UNROLL;
 
+// offsets [jb, je) of kind KIND.  u = x - k is formed per pixel as fr + n, fr = x - round(x), n = round(x) - k an
+// exact small integer (n0 at offset 0): the bin nearest the track gets u = fr exactly (see pixel_step).
 template <int KIND, int WMODE>
 __device__ __forceinline__ void pair_zone(const SlabPair<WMODE>& sl, const PairTrack& L, const FarCoef& C, int jb, int je,
-                                          f2_t u0, unsigned lut_lane, PairSums& s) {
+                                          f2_t fr, f2_t n0, unsigned lut_lane, PairSums& s) {
   const float fj = (float)jb;
-  f2_t u = fadd2(u0, pk(-fj, -fj));              // exact: small integers
+  f2_t nn = fadd2(n0, pk(-fj, -fj));             // exact: small integers
   const f2_t m1 = pk(-1.f, -1.f);
 #pragma unroll(kPairUnroll)
   for (int j = jb; j < je; ++j) {
-    pair_pixel<KIND, WMODE, 0>(sl, L, C, j, u, 0, 0, lut_lane, s);
-    u = fadd2(u, m1);
+    pair_pixel<KIND, WMODE, 0>(sl, L, C, j, fadd2(fr, nn), 0, 0, lut_lane, s);
+    nn = fadd2(nn, m1);
   }
 }
 
@@ -990,7 +900,7 @@ __device__ __forceinline__ void eval_item_pair(const EvalArgs& a, const long lon
   float accr = 0.f, acci = 0.f, acch = 0.f;      // this lane's running sums of the current piece
 
   // ---------------- track points of this lane's two tranches (a2) ----------------
-  float uu[2], Pr[2], Pi[2], kap[2], cc[2], Er[2], Ei[2], sc[2], hc[2], xf[2];
+  float frx[2], nn0[2], Pr[2], Pi[2], kap[2], cc[2], Er[2], Ei[2], sc[2], hc[2], xf[2];
   int Wm[2], krel[2], idxv[2];
   int ja = 0x7fffffff, jb = 0, j2a = 0x7fffffff, j2b = 0, wmin = 0x7fffffff;
   bool any = false;
@@ -1004,7 +914,7 @@ __device__ __forceinline__ void eval_item_pair(const EvalArgs& a, const long lon
       const int m = a.valid_m[idxv[h]];
       const TrackPoint tp = track_point(T, m, a.DT, a.x_lo, a.x_hi, a.c_max, valid);
       // an inactive tranche: u_j = -1 - j, u_j + c = -0.5 - j (finite h' on finite data), P = 0
-      Wm[h] = 0; krel[h] = 0; uu[h] = -1.f; Pr[h] = 0.f; Pi[h] = 0.f; kap[h] = 1.f; cc[h] = 0.5f; Er[h] = 0.f; Ei[h] = 0.f;
+      Wm[h] = 0; krel[h] = 0; frx[h] = 0.f; nn0[h] = -1.f; Pr[h] = 0.f; Pi[h] = 0.f; kap[h] = 1.f; cc[h] = 0.5f; Er[h] = 0.f; Ei[h] = 0.f;
       sc[h] = 1.f; hc[h] = 0.f; xf[h] = 0.f;
       if (tp.active) {
         any = true;
@@ -1013,9 +923,11 @@ __device__ __forceinline__ void eval_item_pair(const EvalArgs& a, const long lon
         Wm[h] = k_hi - k_lo + 1;
         krel[h] = k_lo - row0;
         wmin = min(wmin, Wm[h]);
-        const int kfl = __double2int_rd(tp.x);
+        const int kfl = __double2int_rd(tp.x), kr = __double2int_rn(tp.x);
         const double fr = tp.x - (double)kfl;
-        uu[h] = (float)fr - (float)(k_lo - kfl);          // cancellation-safe x - k_lo
+        frx[h] = (float)(tp.x - (double)kr);               // x - k = (x - round(x)) + (round(x) - k)
+        nn0[h] = (float)(kr - k_lo);
+        const float u0h = frx[h] + nn0[h];
         xf[h] = (float)tp.x;
         // phases in turns, reduced in fp64 (phi reaches ~1e8 rad), then to [-1/2, 1/2)
         double tphi = T.phic_turns - tp.X58 * (1.0 / kPi);
@@ -1037,10 +949,10 @@ __device__ __forceinline__ void eval_item_pair(const EvalArgs& a, const long lon
         Ei[h] = -spsi;
         // near zone: offsets j with |v0| < kVFar or |v1| < kVFar, i.e. -(c + d) < u - j < d; FAR2 outside (j2a, j2b)
         const float d = fmaf(kVFar, kap[h], 1e-3f), d2 = fmaf(kVFar2, kap[h], 1e-3f);
-        ja = min(ja, max(__float2int_rd(uu[h] - d) + 1, 0));
-        jb = max(jb, __float2int_ru(uu[h] + cf + d));
-        j2a = min(j2a, max(__float2int_rd(uu[h] - d2) + 1, 0));
-        j2b = max(j2b, __float2int_ru(uu[h] + cf + d2));
+        ja = min(ja, max(__float2int_rd(u0h - d) + 1, 0));
+        jb = max(jb, __float2int_ru(u0h + cf + d));
+        j2a = min(j2a, max(__float2int_rd(u0h - d2) + 1, 0));
+        j2b = max(j2b, __float2int_ru(u0h + cf + d2));
       }
     }
     // transfer factors of the two channels (a6): constant per template, or from the template's table at f_m
@@ -1074,25 +986,26 @@ __device__ __forceinline__ void eval_item_pair(const EvalArgs& a, const long lon
       PairSums s;
 #pragma unroll
       for (int h = 0; h < 2; ++h) { s.zr[h] = pk(0.f, 0.f); s.zi[h] = pk(0.f, 0.f); s.q[h] = pk(0.f, 0.f); }
-      const f2_t u0 = pk(uu[0], uu[1]);
+      const f2_t fr2 = pk(frx[0], frx[1]), n02 = pk(nn0[0], nn0[1]);
       const int Z2A = min(J2A, Wmin), ZA = min(JA, Wmin), ZB = min(JB, Wmin), Z2B = min(J2B, Wmin);
       // the zones may run in any order (u is re-derived from the offset), so the two FAR2 runs and the two
       // FAR runs share their code
 #pragma unroll 1
-      for (int r = 0; r < 2; ++r) pair_zone<kZFar2, WMODE>(sl, L, a.far, r ? Z2B : 0, r ? Wmin : Z2A, u0, lut_lane, s);
+      for (int r = 0; r < 2; ++r) pair_zone<kZFar2, WMODE>(sl, L, a.far, r ? Z2B : 0, r ? Wmin : Z2A, fr2, n02, lut_lane, s);
 #pragma unroll 1
-      for (int r = 0; r < 2; ++r) pair_zone<kZFar, WMODE>(sl, L, a.far, r ? ZB : Z2A, r ? Z2B : ZA, u0, lut_lane, s);
-      pair_zone<kZNear, WMODE>(sl, L, a.far, ZA, ZB, u0, lut_lane, s);
+      for (int r = 0; r < 2; ++r) pair_zone<kZFar, WMODE>(sl, L, a.far, r ? ZB : Z2A, r ? Z2B : ZA, fr2, n02, lut_lane, s);
+      pair_zone<kZNear, WMODE>(sl, L, a.far, ZA, ZB, fr2, n02, lut_lane, s);
       {
         // masked tail: a tranche whose window has ended contributes zero
         const float fw = (float)Wmin;
-        f2_t u = fadd2(u0, pk(-fw, -fw));
+        f2_t nn = fadd2(n02, pk(-fw, -fw));
 #pragma unroll 1
         for (int j = Wmin; j < Wmax; ++j) {
+          const f2_t u = fadd2(fr2, nn);
           if (j >= JA && j < JB) pair_pixel<kZNear, WMODE, 1>(sl, L, a.far, j, u, Wm[0], Wm[1], lut_lane, s);
           else if (j < J2A || j >= J2B) pair_pixel<kZFar2, WMODE, 1>(sl, L, a.far, j, u, Wm[0], Wm[1], lut_lane, s);
           else pair_pixel<kZFar, WMODE, 1>(sl, L, a.far, j, u, Wm[0], Wm[1], lut_lane, s);
-          u = fadd2(u, pk(-1.f, -1.f));
+          nn = fadd2(nn, pk(-1.f, -1.f));
         }
       }
       // ---------------- a6: transfer factors, the tranche's factor P, weights a[i] ----------------
@@ -1344,7 +1257,7 @@ eval_list_kernel(const EvalArgs a) {
     const Unit d = a.units_list[uid];
     for (int k = 0; k < d.cnt; ++k) {
       const long long it = (long long)a.list[d.off + (unsigned)k];
-      eval_item<MODE, WMODE, false>(a, it, d.tile, lane, lut_lane, 0u, 0u, 0);
+      eval_item<MODE, WMODE>(a, it, d.tile, lane, lut_lane);
     }
   }
 }

@@ -1,6 +1,7 @@
 """Throughput tables for the secondary BASELINE.json configurations (markdown on stdout).
 
     python -m paper_2510_19047_b200.report track-width     # configs[3]: throughput vs track width
+    python -m paper_2510_19047_b200.report stress          # configs[3] at its stated size: 10^7 templates, batches of 2^20
     python -m paper_2510_19047_b200.report nseg            # configs[2]: N_seg swept over {1, 4, 16, 64}
     python -m paper_2510_19047_b200.report ladder          # configs[4]: the 64 -> 16 -> 4 -> 1 ladder at full size
     python -m paper_2510_19047_b200.report frontend        # NEXT-2: time series -> TF grid at the 2-year-shaped size
@@ -95,6 +96,46 @@ def track_width():
     ctx.destroy()
 
 
+def stress():
+    """configs[3] at its stated size: 10 batches of 2^20 templates (1.05 x 10^7) back to back, N_seg = 32, each batch its
+    own seeded bank, resident on the device; sustained rate with the SM clock sampled during the run."""
+    import subprocess
+    import threading
+    torch, api, synth, w, ctx, data = _setup("cfg4")
+    dev = torch.device("cuda:0")
+    banks = [torch.from_numpy(synth.make_templates(w, seed=w.seed + 100 * b)).to(dev) for b in range(10)]
+    n = sum(b.shape[0] for b in banks)
+    ups = torch.empty(banks[0].shape[0], dtype=torch.float32, device=dev)
+    idx = torch.empty(banks[0].shape[0] // 100, dtype=torch.int64, device=dev)
+    val = torch.empty(banks[0].shape[0] // 100, dtype=torch.float32, device=dev)
+    for b in banks[:2]:
+        ctx.eval(b, w.N_seg, ups)
+    torch.cuda.synchronize()
+    clocks = []
+    proc = subprocess.Popen(["nvidia-smi", "-i", "0", "--query-gpu=clocks.sm,clocks_event_reasons.sw_power_cap,"
+                             "clocks_event_reasons.hw_slowdown", "--format=csv,noheader,nounits", "-lms", "100"],
+                            stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+    th = threading.Thread(target=lambda: clocks.extend(proc.stdout), daemon=True)
+    th.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for rep in range(3):
+        for b in banks:
+            ctx.eval(b, w.N_seg, ups)
+            ctx.topk(ups, idx.shape[0], idx, val)
+    e1.record()
+    torch.cuda.synchronize()
+    proc.terminate()
+    ms = e0.elapsed_time(e1) / 3
+    mhz = [float(c.split(",")[0]) for c in clocks if c.strip()]
+    flags = sorted({f.strip() for c in clocks for f in c.split(",")[1:] if "Active" in f and "Not" not in f})
+    print(f"# configs[3] (cfg4) at its stated size: 10 batches of 2^20 = {n} templates, N_seg = {w.N_seg}, grid {w.Nt} x {w.Nf}\n")
+    print(f"{ms:.1f} ms for the 10 batches (tfs_eval + tfs_topk of the top 1 % each; mean of 3 passes) = "
+          f"{n / ms * 1e3:.3e} templates/s sustained; SM clock median {np.median(mhz) if mhz else float('nan'):.0f} MHz "
+          f"over {len(mhz)} samples, throttle flags active: {flags or 'none'}")
+    ctx.destroy()
+
+
 def nseg():
     torch, api, synth, w, ctx, data = _setup("cfg3")
     dev = torch.device("cuda:0")
@@ -103,8 +144,8 @@ def nseg():
     d = torch.from_numpy(params).to(dev)
     pix = _counts(ctx, torch, d)
     print(f"# configs[2] (cfg3): N_seg sweep, {len(params)} templates, grid {w.Nt} x {w.Nf}, "
-          f"weight structure {ctx.weight_structure()}, {n_valid} valid tranches = {-(-n_valid // 512)} time tiles "
-          f"of 512 for every N_seg\n")
+          f"weight structure {ctx.weight_structure()}, {n_valid} valid tranches = {-(-n_valid // 64)} time tiles "
+          f"of 64 for every N_seg\n")
     print("| N_seg | ms per tfs_eval | templates/s | pixel-evals/s |")
     print("|---:|---:|---:|---:|")
     for N in (1, 4, 16, 64):
@@ -178,6 +219,8 @@ if __name__ == "__main__":
     what = sys.argv[1] if len(sys.argv) > 1 else ""
     if what == "track-width":
         track_width()
+    elif what == "stress":
+        stress()
     elif what == "nseg":
         nseg()
     elif what == "ladder":

@@ -590,3 +590,36 @@ def test_seeded_shape_sweep(api, case):
         ora = oracle_eval(coeff, weight, gap, params, Nt, Nf, w.dt, N_seg, **opts)
         assert_parity(gpu, ora, N_seg, label=f"sweep case {case} Nt={Nt} Nf={Nf} N_seg={N_seg} {opts}")
     ctx.destroy()
+
+
+# --------------------------------------------------------------------------------------------
+# Precision hunt: where the fp32 pixel arithmetic has the least margin -- very slow chirps
+# (c = fdot DT^2 in [1e-4, 1e-2]: every pixel is a small difference of O(1) auxiliary-function values), one tranche per
+# segment (nothing averages), an 81-bin window, general per-pixel weights -- over 10^4 templates against the oracle.
+# The bar is 1e-4; the measured worst case is asserted with a margin so that a regression shows up.
+# --------------------------------------------------------------------------------------------
+def test_precision_worst_case_hunt(api):
+    w = synth.scaled(synth.WORKLOADS["cfg2"], Nt=64, Nf=512, n_templates=10_000)
+    coeff, _, gap = synth.make_data(w)
+    rng = np.random.default_rng(99)
+    weight = rng.uniform(0.2, 3.0, (2, w.Nt, w.Nf)).astype(np.float32)
+    params = synth.make_templates(w)
+    params[:, 0] = np.exp(rng.uniform(np.log(5.0), np.log(100.0), len(params)))
+    params[:, 1] = rng.uniform(2.0, 30.0, len(params)) * O.YEAR_S
+    g = O.Grid(w.Nt, w.Nf, w.dt)
+    cs = []
+    for p in params[:200]:
+        tr = O.track(p[0], p[1], 0, 1, g, O.Opts(half_width=40))
+        if tr["active"].any():
+            cs.append(tr["c"][tr["active"]].max())
+    assert len(cs) > 100 and 1e-5 < np.median(cs) < 1e-2
+    ctx = _mk(api, w, coeff, weight, gap, half_width=40)
+    assert ctx.weight_structure() == 0
+    N_seg = w.Nt
+    gpu = api.eval_host(ctx, params, N_seg)
+    ora = oracle_eval(coeff, weight, gap, params, w.Nt, w.Nf, w.dt, N_seg, half_width=40)
+    r = parity_report(gpu, ora, N_seg)
+    print("precision hunt:", r)
+    assert r["n_active"] > 5000
+    assert max(r["hh"], r["z"], r["P"], r["ups"]) <= 2e-5, r       # measured 1.1e-5 (P), 8e-6 (hh), 7e-6 (z)
+    ctx.destroy()
