@@ -156,6 +156,7 @@ class Opts:
     f_lo: float | None = None
     f_hi: float | None = None
     fresnel_mode: int = 0         # 0 exact C,S ; 1 the paper's Eqs. 23-28 verbatim
+    tukey_alpha: float = 0.0      # > 0: window-aware template for Tukey(alpha)-windowed tranches (C2/C24)
 
     def band(self, grid: Grid):
         lo = grid.df if self.f_lo is None else self.f_lo
@@ -228,6 +229,95 @@ def kernel_pixels(x, c, phi, A, k, fresnel_mode: int = 0):
     return (A / np.sqrt(2.0 * c)) * (np.cos(ph) + 1j * np.sin(ph)) * F     # Eq. 16
 
 
+# ----------------------------------------------------------------------------------------------
+# Window-aware template pixels: the tranche is Tukey-windowed before its Fourier transform
+# ----------------------------------------------------------------------------------------------
+def tukey_profile(s, alpha: float):
+    """Tukey (tapered-cosine) window as a function of the position s in [0, 1] inside the tranche, shape
+    parameter alpha = fraction of the tranche inside the two cosine tapers ("Tukey-windowed with a shape
+    parameter of 0.1"; reading C24: the continuous profile, the O(1/N) difference to a sampled window is dropped)."""
+    s = np.asarray(s, dtype=np.float64)
+    if alpha <= 0.0:
+        return np.ones_like(s)
+    ell = 0.5 * min(alpha, 1.0)
+    w = np.ones_like(s)
+    lo = s < ell
+    hi = s > 1.0 - ell
+    w[lo] = 0.5 * (1.0 - np.cos(math.pi * s[lo] / ell))
+    w[hi] = 0.5 * (1.0 - np.cos(math.pi * (1.0 - s[hi]) / ell))
+    return w
+
+
+_GL_NODES, _GL_WEIGHTS = np.polynomial.legendre.leggauss(16)
+
+
+def kernel_pixels_windowed_quad(x, c, phi, A, k, alpha: float):
+    """THE DEFINITION: h~_nm(f_k)/DT for a tranche multiplied by the Tukey(alpha) window before its Fourier
+    transform, by direct quadrature of
+
+        A exp(i phi) int_0^1 w(s) exp{i (2 pi u s + pi c s^2)} ds,    u = x - k,
+
+    i.e. Eq. 16's integrand (phase Taylor-expanded about the tranche start, Eqs. 12-15, in units s = t/DT)
+    times w(s).  Composite 16-point Gauss-Legendre on [0, l], [l, 1-l], [1-l, 1] (l = alpha/2), panels short enough
+    that the phase advances by less than ~2 rad per panel.  Slow: for pins and small cases."""
+    x, c, phi, A, k = np.broadcast_arrays(*(np.asarray(v, dtype=np.float64) for v in (x, c, phi, A, k)))
+    shape = k.shape
+    u = (x - k).ravel()[:, None]
+    cc = c.ravel()[:, None]
+    ell = 0.5 * min(max(alpha, 0.0), 1.0)
+    cuts = [0.0, 1.0] if ell == 0.0 else sorted({0.0, ell, 1.0 - ell, 1.0})
+    total = np.zeros(u.shape[0], dtype=np.complex128)
+    rate = float(np.max(2.0 * math.pi * (np.abs(u) + cc)))             # max |d phase / ds| of the chirp
+    for s0, s1 in zip(cuts[:-1], cuts[1:]):
+        taper = ell > 0.0 and (s1 <= ell or s0 >= 1.0 - ell)           # the cosine adds pi of argument over a taper
+        npan = 1 + int(math.ceil((rate * (s1 - s0) + (math.pi if taper else 0.0)) / 2.0))
+        edges = np.linspace(s0, s1, npan + 1)
+        h = 0.5 * (edges[1:] - edges[:-1])[:, None]
+        mid = 0.5 * (edges[1:] + edges[:-1])[:, None]
+        s = (mid + h * _GL_NODES[None, :]).ravel()[None, :]                 # [1][nodes]
+        wq = (h * _GL_WEIGHTS[None, :]).ravel()[None, :]
+        for i0 in range(0, u.shape[0], 64):                                 # pixels in blocks (memory)
+            ub, cb = u[i0:i0 + 64], cc[i0:i0 + 64]
+            f = tukey_profile(s, alpha) * np.exp(1j * (2.0 * math.pi * ub * s + math.pi * cb * s * s))
+            total[i0:i0 + 64] += np.sum(wq * f, axis=1)
+    out = A.ravel() * (np.cos(phi.ravel()) + 1j * np.sin(phi.ravel())) * total
+    return out.reshape(shape)
+
+
+def _chirp_integral(u, c, s0: float, s1: float):
+    """I(u; s0, s1) = int_{s0}^{s1} exp{i (2 pi u s + pi c s^2)} ds in Fresnel integrals: completing the square,
+    2 pi u s + pi c s^2 = pi v^2/2 - pi u^2/c with v = sqrt(2/c) (u + c s) (Eq. 22 at a general time), so
+    I = exp(-i pi u^2/c) [F(v(s1)) - F(v(s0))] / sqrt(2c),  F = C + iS  (Eqs. 16-21 with other end points)."""
+    sq = np.sqrt(2.0 / c)
+    C1, S1 = fresnel_cs(sq * (u + c * s1))
+    C0, S0 = fresnel_cs(sq * (u + c * s0))
+    ph = -math.pi * np.mod(u * u / c, 2.0)
+    return (np.cos(ph) + 1j * np.sin(ph)) * ((C1 - C0) + 1j * (S1 - S0)) / np.sqrt(2.0 * c)
+
+
+def kernel_pixels_windowed(x, c, phi, A, k, alpha: float):
+    """The same quantity in closed form (pinned against kernel_pixels_windowed_quad).  With l = alpha/2, b = 1/alpha,
+    the window is 1 minus the two taper deficits [1 + cos(2 pi b s)]/2 on [0, l] and [1 + cos(2 pi b (1-s))]/2 on
+    [1-l, 1]; a cosine shifts u by +-b, so
+
+        K_w(u) = I(u;0,1) - [ I(u;0,l)/2 + I(u+b;0,l)/4 + I(u-b;0,l)/4 ]
+                          - [ I(u;1-l,1)/2 + e^{-2 pi i b} I(u+b;1-l,1)/4 + e^{+2 pi i b} I(u-b;1-l,1)/4 ]."""
+    k = np.asarray(k, dtype=np.float64)
+    x = np.asarray(x, dtype=np.float64)
+    c = np.asarray(c, dtype=np.float64)
+    u = x - k
+    K = _chirp_integral(u, c, 0.0, 1.0)
+    if alpha > 0.0:
+        a = min(alpha, 1.0)
+        ell, b = 0.5 * a, 1.0 / a
+        eb = complex(math.cos(2.0 * math.pi * b), math.sin(2.0 * math.pi * b))
+        K = K - (0.5 * _chirp_integral(u, c, 0.0, ell) + 0.25 * _chirp_integral(u + b, c, 0.0, ell)
+                 + 0.25 * _chirp_integral(u - b, c, 0.0, ell))
+        K = K - (0.5 * _chirp_integral(u, c, 1.0 - ell, 1.0) + 0.25 * np.conj(eb) * _chirp_integral(u + b, c, 1.0 - ell, 1.0)
+                 + 0.25 * eb * _chirp_integral(u - b, c, 1.0 - ell, 1.0))
+    return np.asarray(A) * (np.cos(phi) + 1j * np.sin(phi)) * K
+
+
 def dense_template(Mc_msun, tc, phic, amp, grid: Grid, opts: Opts, gap_mask=None, truncate=True):
     """Dense [Nt][Nf] complex128 template (without T_alpha), zero outside each tranche's window.
 
@@ -244,8 +334,12 @@ def dense_template(Mc_msun, tc, phic, amp, grid: Grid, opts: Opts, gap_mask=None
     # all window pixels of all active tranches, flattened: (mm[i], kk[i])
     mm = np.repeat(ms, hi - lo + 1)
     kk = np.concatenate([np.arange(l, h + 1) for l, h in zip(lo, hi)])
-    Hd[mm, kk] = kernel_pixels(tr["x"][mm], tr["c"][mm], tr["phi"][mm], tr["A"][mm], kk,
-                               opts.fresnel_mode)
+    if opts.tukey_alpha > 0.0:
+        Hd[mm, kk] = kernel_pixels_windowed(tr["x"][mm], tr["c"][mm], tr["phi"][mm], tr["A"][mm], kk,
+                                            opts.tukey_alpha)
+    else:
+        Hd[mm, kk] = kernel_pixels(tr["x"][mm], tr["c"][mm], tr["phi"][mm], tr["A"][mm], kk,
+                                   opts.fresnel_mode)
     return Hd
 
 
