@@ -76,6 +76,15 @@ typedef struct {
                             of the two template quadratures; seg_dh = (a, b), seg_hh = (hcc + hss)/2                  */
   int    wdm_half_width; /* basis 1: layers kept on either side of the two the track sits between; default 2 (W5)    */
   double wdm_kappa_max;  /* basis 1: pixels with 4 fdot (Nf dt)^2 above this are skipped; default 8 (W7)              */
+  double tukey_alpha;    /* 0 (default): the template pixel is Eq. 16 as printed, the transform of the un-windowed
+                            tranche.  alpha in [1e-3, 1]: window-aware template for data whose tranches were multiplied by a
+                            Tukey window of shape parameter alpha before their FFT ("Tukey-windowed with a shape
+                            parameter of 0.1"; tfs_upload_timeseries): Eq. 16's integrand times the continuous window
+                            w(s), s = t/DT in [0, 1] (cosine tapers of length alpha/2 at both ends; readings C2, C24):
+                                h~_w(f_k)/DT = A e^{i phi} int_0^1 w(s) exp{i (2 pi u s + pi c s^2)} ds,  u = x - k,
+                            evaluated in closed form (Fresnel auxiliary functions at the taper ends and at u +- 1/alpha).
+                            Window, activity and segment rules are unchanged.  Basis 0 and fresnel_mode 0 only; every
+                            item then takes the global-memory gather kernel (about 4x the cost of the default)            */
 } tfs_opts;
 
 TFS_API void tfs_default_opts(tfs_opts* opts);

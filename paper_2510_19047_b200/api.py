@@ -22,7 +22,7 @@ class tfs_opts(C.Structure):
     _fields_ = [("half_width", C.c_int), ("adaptive_width", C.c_int), ("c_max", C.c_double),
                 ("f_lo", C.c_double), ("f_hi", C.c_double), ("fresnel_mode", C.c_int),
                 ("weight_mode", C.c_int), ("basis", C.c_int), ("wdm_half_width", C.c_int),
-                ("wdm_kappa_max", C.c_double)]
+                ("wdm_kappa_max", C.c_double), ("tukey_alpha", C.c_double)]
 
 
 class TfsError(RuntimeError):

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtfs.so")
 SOURCES = [os.path.join(CSRC, "tfs.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "tfs_kernels.cuh"), os.path.join(CSRC, "tfs_frontend.cuh"),
+DEPS = SOURCES + [os.path.join(CSRC, "tfs_kernels.cuh"), os.path.join(CSRC, "tfs_frontend.cuh"), os.path.join(CSRC, "tfs_wdm.cuh"),
                   os.path.join(os.path.dirname(HERE), "include", "tfs.h")]
 
 

@@ -324,6 +324,7 @@ EvalArgs base_args(const tfs_ctx* ctx, int pr = 0) {
   a.c_max = ctx->opts.basis == 1 ? ctx->opts.wdm_kappa_max : ctx->opts.c_max;
   a.basis = ctx->opts.basis; a.wdm_Hw = ctx->opts.wdm_half_width; a.wdm_DTpix = 0.5 * ctx->DT;
   a.far = ctx->far;
+  if (ctx->opts.tukey_alpha > 0.0) { a.far.win_ell = (float)(0.5 * ctx->opts.tukey_alpha); a.far.win_b = (float)(1.0 / ctx->opts.tukey_alpha); }
   a.n_valid = ctx->n_valid; a.n_tiles = 1; a.n_keys = 2;
   a.wmode = ctx->wmode;
   a.t_col = 3; a.n_ch_pair = P.c1 >= 0 ? 2 : 1;
@@ -393,6 +394,7 @@ void tfs_default_opts(tfs_opts* o) {
   o->basis = 0;
   o->wdm_half_width = 2;
   o->wdm_kappa_max = 8.0;
+  o->tukey_alpha = 0.0;
 }
 
 const char* tfs_last_error(const tfs_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
@@ -438,6 +440,10 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
                 o.wdm_half_width, o.wdm_kappa_max);
   if (o.basis == 1 && (n_channels > 2 || o.fresnel_mode != 0))
     return fail(nullptr, TFS_EINVAL, "tfs_create: the WDM basis takes 1 or 2 channels and fresnel_mode 0");
+  if (!(o.tukey_alpha >= 0.0) || o.tukey_alpha > 1.0 || (o.tukey_alpha > 0.0 && o.tukey_alpha < 1e-3) ||
+      (o.tukey_alpha > 0.0 && (o.basis != 0 || o.fresnel_mode != 0)))
+    return fail(nullptr, TFS_EINVAL, "tfs_create: tukey_alpha must be 0 or in [1e-3, 1], with basis 0 and fresnel_mode 0 (got %g)",
+                o.tukey_alpha);
   tfs_ctx* ctx = new (std::nothrow) tfs_ctx();
   if (!ctx) return fail(nullptr, TFS_ENOMEM, "tfs_create: host allocation failed");
   ctx->Nt = Nt; ctx->Nf = Nf; ctx->C = n_channels; ctx->dt = dt;
@@ -486,6 +492,9 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
       (e = cudaFuncSetAttribute(eval_list_kernel<0, kWSeparable>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_list_kernel<0, kWTimeOnly>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_list_kernel<1, kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_list_kernel<2, kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_list_kernel<2, kWSeparable>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_list_kernel<2, kWTimeOnly>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_wdm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_slab_kernel<kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWGeneral))) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_slab_kernel<kWSeparable>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWSeparable))) != cudaSuccess ||
@@ -803,7 +812,8 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
 
   // pre-pass scratch (one pooled allocation): constants, keys, bucket tables, item list, unit tables
   const int n_bands = (ctx->Nf - 1) / kBandStride + 1;
-  const bool slab_ok = ctx->opts.fresnel_mode == 0 && n_bands + 2 <= 8192 && !wdm;
+  const bool windowed = ctx->opts.tukey_alpha > 0.0;          // window-aware template: every item through the list kernel (MODE 2)
+  const bool slab_ok = ctx->opts.fresnel_mode == 0 && n_bands + 2 <= 8192 && !wdm && !windowed;
   const int n_keys = slab_ok ? n_bands + 2 : 2;
   const size_t n_buckets = (size_t)n_tiles * n_keys;
   const size_t n_items = (size_t)sub * n_tiles;
@@ -873,6 +883,9 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
       // the items that gather from global memory (and every item with the paper's approximants) ...
       if (wdm) eval_wdm_kernel<<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
       else if (ctx->opts.fresnel_mode != 0) eval_list_kernel<1, kWGeneral><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
+      else if (windowed && wm == kWTimeOnly) eval_list_kernel<2, kWTimeOnly><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
+      else if (windowed && wm == kWSeparable) eval_list_kernel<2, kWSeparable><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
+      else if (windowed) eval_list_kernel<2, kWGeneral><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
       else if (wm == kWTimeOnly) eval_list_kernel<0, kWTimeOnly><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
       else if (wm == kWSeparable) eval_list_kernel<0, kWSeparable><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
       else eval_list_kernel<0, kWGeneral><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);

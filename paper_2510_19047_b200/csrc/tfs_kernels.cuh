@@ -60,7 +60,10 @@ static_assert(TFS_SLAB_ROWS <= 256 && TFS_SLAB_ROWS_GENERAL <= 256, "TMA box <= 
 static_assert(kBandStride % 2 == 0 && TFS_SLAB_ROWS > kBandStride && TFS_SLAB_ROWS_GENERAL > kBandStride, "a slab must overlap the next band");
 
 // f(v) = w (F0 + F1 w^4 + F2 w^8), g(v) = w^3 (G0 + G1 w^4 + G2 w^8), w = 1/v, valid for |v| >= kVFar
-struct FarCoef { float F0, F1, F2, G0, G1, G2; };
+struct FarCoef {
+  float F0, F1, F2, G0, G1, G2;
+  float win_ell, win_b;     // window-aware template (MODE 2): taper length l = alpha/2 and shift b = 1/alpha (tfs_opts.tukey_alpha)
+};
 
 // Per-template constants, written once per batch by prep_consts_kernel (a1).
 struct __align__(16) TplConst {
@@ -292,7 +295,7 @@ __device__ __forceinline__ f2_t fadd2(f2_t a, f2_t b) {
 template <int MODE, int LC>
 __device__ __forceinline__ void fresnel_aux(float v, unsigned lut_lane, f2_t& GF, float& ts) {
   const float a = fabsf(v);
-  if (MODE == 0) {
+  if (MODE != 1) {
     const float t = rcp_approx(1.0f + a);         // MUFU.RCP
     const float q = fmaf(t, (float)kLutN, kMagic);
     const float4 e = lds128_const(__float_as_uint(q) * (16u * LC) + lut_lane);   // {a_G, a_F, b_G, b_F}
@@ -428,7 +431,7 @@ __device__ __forceinline__ void pixel_near(const LaneTrack& L, float u, float ms
   }
   const float hs = 0.5f * L.sc * L.c;                 // (v1 - v0)/2 = sqrt(c/2)
   const float al = 3.14159265358979f * (v0 + hs);     // pi * midpoint
-  if (MODE == 0 && fabsf(al) * hs < kNearSeries && hs < 0.1f) {
+  if (MODE != 1 && fabsf(al) * hs < kNearSeries && hs < 0.1f) {
     // slow chirp next to the track: h' = exp(-i pi u^2/c) [F(v1) - F(v0)] is O(sqrt(2c)) while the terms above are
     // O(1) (table error 2e-7 absolute, i.e. 2e-7/sqrt(2c) relative).  Expand the integral about the midpoint vm:
     //   F(v1) - F(v0) = exp(i pi vm^2/2) int_{-h}^{h} exp(i (alpha t + beta t^2)) dt,  alpha = pi vm, beta = pi/2,
@@ -445,6 +448,72 @@ __device__ __forceinline__ void pixel_near(const LaneTrack& L, float u, float ms
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Window-aware template (MODE 2; tfs_opts.tukey_alpha > 0).  The data tranche was multiplied
+// by a Tukey window before its Fourier transform, so the template pixel is Eq. 16's integrand
+// times the window w(s) = 1 - [taper deficits]: with l = alpha/2, b = 1/alpha the deficits are
+// [1 + cos(2 pi b s)]/2 on [0, l] and its mirror image on [1 - l, 1], and a cosine shifts u by +-b.  In the
+// normalisation of h' (h = P h'):
+//     h'_w = h' - Lam(u) - E Lam(-(u + c)),        Lam(w) = J(w)/2 + J(w + b)/4 + J(w - b)/4,
+//     J(w) = sqrt(2c) int_0^l exp{i (2 pi w s + pi c s^2)} ds
+//          = Godd(sc w) - Godd(sc (w + c l)) rho(w)  [+ (1+i) exp(-i pi w^2/c) if -c l < w < 0],
+//     rho(w) = exp{i (2 pi w l + pi c l^2)},  rho(w +- b) = -rho(w)  (2 b l = 1),  sc = sqrt(2/c),
+// the right taper being the left one seen from the tranche's end (s -> 1 - s turns u into -(u + c) and brings
+// out the factor E = exp{i (2 pi u + pi c)}).  The taper terms are <= alpha/4 of the main pixel, so the LUT
+// (absolute error 2e-7) serves every Godd here whatever |v| is.
+// ------------------------------------------------------------------------------------------
+template <int LC>
+__device__ __forceinline__ void godd_lut(float v, unsigned lut_lane, float& gr, float& gi) {
+  f2_t GF;
+  float ts;
+  fresnel_aux<0, LC>(v, lut_lane, GF, ts);
+  upk(fmul2(pk(ts, ts), GF), gr, gi);
+}
+
+template <int LC>
+__device__ __forceinline__ void taper_J(const LaneTrack& L, float w, float cl, float rr, float ri, unsigned lut_lane,
+                                        float& jr, float& ji) {
+  float a0r, a0i, a1r, a1i;
+  godd_lut<LC>(L.sc * w, lut_lane, a0r, a0i);
+  godd_lut<LC>(L.sc * (w + cl), lut_lane, a1r, a1i);
+  jr = a0r - fmaf(a1r, rr, -a1i * ri);
+  ji = a0i - fmaf(a1r, ri, a1i * rr);
+  if (w < 0.0f && w + cl > 0.0f) {
+    // the stationary point lies inside the taper: + (1+i) exp(-i pi w^2/c), pi w^2/c < pi c l^2
+    float st, ct;
+    __sincosf(6.283185307179586f * (w * w * L.hc), &st, &ct);
+    jr += ct + st;
+    ji += ct - st;
+  }
+}
+
+template <int LC>
+__device__ __forceinline__ void taper_lambda(const LaneTrack& L, float w, float ell, float b, unsigned lut_lane,
+                                             float& lr, float& li) {
+  const float cl = L.c * ell;
+  float turns = fmaf(w, ell, 0.5f * cl * ell);         // (2 pi w l + pi c l^2) / 2 pi
+  turns -= floorf(turns);
+  float sr, cr;
+  __sincosf(6.283185307179586f * (turns - 0.5f), &sr, &cr);     // = -(sin, cos)(2 pi turns)
+  float j0r, j0i, jpr, jpi, jmr, jmi;
+  taper_J<LC>(L, w, cl, -cr, -sr, lut_lane, j0r, j0i);
+  taper_J<LC>(L, w + b, cl, cr, sr, lut_lane, jpr, jpi);        // rho(w +- b) = -rho(w)
+  taper_J<LC>(L, w - b, cl, cr, sr, lut_lane, jmr, jmi);
+  lr = fmaf(0.25f, jpr + jmr, 0.5f * j0r);
+  li = fmaf(0.25f, jpi + jmi, 0.5f * j0i);
+}
+
+// h' -> h'_w for the pixel at u (msk = 0 for a lane past its window)
+template <int LC>
+__device__ __forceinline__ void taper_terms(const LaneTrack& L, const FarCoef& C, float u, float msk, unsigned lut_lane,
+                                            float& hr, float& hi) {
+  float l0r, l0i, l1r, l1i;
+  taper_lambda<LC>(L, u, C.win_ell, C.win_b, lut_lane, l0r, l0i);
+  taper_lambda<LC>(L, -(u + L.c), C.win_ell, C.win_b, lut_lane, l1r, l1i);
+  hr -= msk * (l0r + fmaf(L.Er, l1r, -L.Ei * l1i));
+  hi -= msk * (l0i + fmaf(L.Er, l1i, L.Ei * l1r));
+}
+
 constexpr int kZNear = 0, kZFar = 1, kZFar2 = 2;
 
 // one pixel of kind KIND at offset jj (u = x - k of that pixel, stepped by the caller)
@@ -456,6 +525,7 @@ __device__ __forceinline__ void pixel_kind(const LaneTrack& L, const FarCoef& C,
   if (KIND == kZNear) pixel_near<MODE, MASKED, LC>(L, u, msk, lut_lane, hr, hi);
   else if (KIND == kZFar) pixel_far<MASKED>(L, C, u, msk, hr, hi);
   else pixel_far2<MASKED>(L, u, msk, hr, hi);
+  if (MODE == 2) taper_terms<LC>(L, C, u, msk, lut_lane, hr, hi);
   mac<WMODE>(s, Yc, Wc, hr, hi);
 }
 
@@ -675,7 +745,7 @@ __device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it,
       const int Wmin = __reduce_min_sync(0xffffffffu, tp.active ? Wm : 0x7fffffff);
       int JA = __reduce_min_sync(0xffffffffu, ja);
       int JB = min(__reduce_max_sync(0xffffffffu, jb), Wmax);
-      if (MODE != 0) { JA = 0; JB = Wmax; }          // the paper's approximants are used for every pixel
+      if (MODE == 1) { JA = 0; JB = Wmax; }          // the paper's approximants are used for every pixel
       JA = min(JA, JB);
 
       // ---------------- pixel loop (a3-a5): lane walks its own window ----------------
@@ -1242,7 +1312,7 @@ eval_list_kernel(const EvalArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float4* s_lut = reinterpret_cast<float4*>(smem_raw);
   const int lane = threadIdx.x & 31;
-  if (MODE == 0) {
+  if (MODE != 1) {
     for (int i = threadIdx.x; i < (kLutN + 1) * kLutCopiesList; i += blockDim.x) s_lut[i] = a.lut[i / kLutCopiesList];
     __syncthreads();
   }
