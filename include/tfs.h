@@ -158,6 +158,19 @@ TFS_API int tfs_eval_tf(tfs_ctx* ctx, const double* params, long long n, int N_s
                 const float* transfer, int n_knots, double f_knot0, double f_knot_step,
                 float* upsilon, float* seg_power, float* seg_dh, float* seg_hh, void* stream);
 
+/* The same evaluation with segments of FIXED DURATION T_seg = seg_tranches * DT laid from the start of the data,
+ * t_n = n T_seg ("the n-th segment covers [t_n, t_n+1], t_n = n T_seg"; P:57 M_tr = T_seg/DT tranches per segment):
+ * n(m) = floor(m / seg_tranches), N_seg = ceil(Nt / seg_tranches) segments, the last one shorter when seg_tranches does
+ * not divide Nt (tfs_eval's equal-index rule, reading C9, is the same thing whenever N_seg divides Nt).
+ *   n_seg_eff [n] int32, nullable: the number of segments in which template i has signal (hh_n > 0).  This is the
+ *             paper's template-dependent "total number of segments" N_seg = tau / T_seg, tau = min(T_obs, t_c),
+ *             counted on the grid: segments past the merger, outside the band or wholly inside gaps do not count.  For
+ *             pure noise E[Upsilon] = 2 n_seg_eff, so it is what a threshold on Upsilon has to be scaled with.
+ *   seg_power [n][N_seg], seg_dh [n][N_seg][2], seg_hh [n][N_seg] with N_seg = ceil(Nt / seg_tranches); nullable.
+ * 1 <= seg_tranches (values >= Nt give one segment).  Everything else as tfs_eval. */
+TFS_API int tfs_eval_tseg(tfs_ctx* ctx, const double* params, long long n, int seg_tranches,
+                          float* upsilon, int* n_seg_eff, float* seg_power, float* seg_dh, float* seg_hh, void* stream);
+
 /* Top-k of a batch (BASELINE.json north_star (3); the optimiser keeps the best parameter sets of each
  * iteration).  Indices and values of the k largest entries of upsilon[0..n), descending; equal values are
  * ordered by lower index first; NaN sorts below everything.  1 <= k <= n.

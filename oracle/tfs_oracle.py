@@ -169,6 +169,12 @@ def segment_of_bin(m, Nt: int, N_seg: int):
     return (np.asarray(m, dtype=np.int64) * N_seg) // Nt
 
 
+def segment_of_bin_tseg(m, seg_tranches: int):
+    """n(m) = floor(m / M_tr): segments of fixed duration T_seg = M_tr DT laid from the start of the data,
+    t_n = n T_seg (M_tr = T_seg/DT tranches per segment).  N_seg = ceil(Nt / M_tr)."""
+    return np.asarray(m, dtype=np.int64) // int(seg_tranches)
+
+
 # ----------------------------------------------------------------------------------------------
 # Step 1-2: 0PN track and window per tranche
 # ----------------------------------------------------------------------------------------------
@@ -353,18 +359,19 @@ def window_pixel_counts(Mc_msun, tc, grid: Grid, opts: Opts, gap_mask=None):
 # ----------------------------------------------------------------------------------------------
 # Steps 4-5: dense inner products, segment combine
 # ----------------------------------------------------------------------------------------------
-def segment_products(Hd, T, D, W, gap_mask, N_seg: int):
+def segment_products(Hd, T, D, W, gap_mask, N_seg: int, seg=None):
     """z_n and hh_n by dense sums over EVERY pixel of every channel (Eq. 31, Eq. 30).
 
     Hd [Nt][Nf] complex128; T [C] complex (transfer factors, Eq. 29, constant per
     template under C5/A12) or [C][Nt] complex (one factor per tranche: T_alpha(f_nm), "computed
     once per tranche for all frequency bins"); D [C][Nt][Nf] complex; W [C][Nt][Nf] real >= 0
     (or None => 1); gap_mask [Nt] (or None).  W stands for 4 df / S so that
-    Upsilon = |sum W conj(D) y|^2 / sum W |y|^2.
+    Upsilon = |sum W conj(D) y|^2 / sum W |y|^2.  seg [Nt] = segment of each tranche (default: segment_of_bin).
     """
     Cn, Nt, Nf = D.shape
     g = np.ones(Nt) if gap_mask is None else (np.asarray(gap_mask) != 0).astype(np.float64)
-    seg = segment_of_bin(np.arange(Nt), Nt, N_seg)
+    if seg is None:
+        seg = segment_of_bin(np.arange(Nt), Nt, N_seg)
     z = np.zeros(N_seg, dtype=np.complex128)
     hh = np.zeros(N_seg, dtype=np.float64)
     H2 = (Hd.real ** 2 + Hd.imag ** 2)
@@ -415,6 +422,31 @@ def evaluate(params, D, W, gap_mask, grid: Grid, N_seg: int, opts: Opts = Opts()
         P, U = combine(z, hh)
         ups[i], segP[i], segz[i], segh[i] = U, P, z, hh
     return dict(upsilon=ups, seg_power=segP, seg_dh=segz, seg_hh=segh)
+
+
+def evaluate_tseg(params, D, W, gap_mask, grid: Grid, seg_tranches: int, opts: Opts = Opts()):
+    """As evaluate, with segments of fixed duration T_seg = seg_tranches * DT (segment_of_bin_tseg; P:93, P:57);
+    N_seg = ceil(Nt / seg_tranches).  Also returns n_seg_eff[n] = number of segments with hh_n > 0: the paper's
+    template-dependent N_seg = tau / T_seg, tau = min(T_obs, t_c), counted on the grid."""
+    params = np.atleast_2d(np.asarray(params, dtype=np.float64))
+    n = params.shape[0]
+    N_seg = -(-grid.Nt // int(seg_tranches))
+    seg = segment_of_bin_tseg(np.arange(grid.Nt), seg_tranches)
+    ups = np.zeros(n)
+    neff = np.zeros(n, dtype=np.int64)
+    segP = np.zeros((n, N_seg))
+    segz = np.zeros((n, N_seg), dtype=np.complex128)
+    segh = np.zeros((n, N_seg))
+    for i in range(n):
+        p = params[i]
+        if not np.all(np.isfinite(p)) or p[0] <= 0:
+            continue
+        Hd = dense_template(p[0], p[1], p[2], p[7], grid, opts, gap_mask, truncate=True)
+        T = np.array([p[3] + 1j * p[4], p[5] + 1j * p[6], 0.0])
+        z, hh = segment_products(Hd, T[: D.shape[0]], D, W, gap_mask, N_seg, seg=seg)
+        P, U = combine(z, hh)
+        ups[i], segP[i], segz[i], segh[i], neff[i] = U, P, z, hh, int(np.sum(hh > 0))
+    return dict(upsilon=ups, n_seg_eff=neff, seg_power=segP, seg_dh=segz, seg_hh=segh)
 
 
 # ----------------------------------------------------------------------------------------------

@@ -56,6 +56,8 @@ def load_library():
     lib.tfs_eval.restype = ip
     lib.tfs_eval_tf.argtypes = [vp, vp, ll, ip, vp, ip, dp, dp, vp, vp, vp, vp, vp]
     lib.tfs_eval_tf.restype = ip
+    lib.tfs_eval_tseg.argtypes = [vp, vp, ll, ip, vp, vp, vp, vp, vp, vp]
+    lib.tfs_eval_tseg.restype = ip
     lib.tfs_topk.argtypes = [vp, vp, ll, ip, vp, vp, vp]
     lib.tfs_topk.restype = ip
     lib.tfs_refine.argtypes = [vp, vp, ll, vp, ll, ip, dp, dp, vp, vp]
@@ -95,7 +97,7 @@ def _ptr(x, dtype, nelem=None):
     import torch
     if isinstance(x, torch.Tensor):
         want = {np.float32: torch.float32, np.float64: torch.float64, np.int64: torch.int64,
-                np.uint8: torch.uint8}[dtype]
+                np.int32: torch.int32, np.uint8: torch.uint8}[dtype]
         if x.dtype != want or not x.is_contiguous():
             raise TypeError(f"expected contiguous {want} tensor, got {x.dtype}")
         if nelem is not None and x.numel() < nelem:
@@ -156,6 +158,16 @@ class Tfs:
                                        _ptr(upsilon, np.float32, n), _ptr(seg_power, np.float32, n * N_seg),
                                        _ptr(seg_dh, np.float32, 2 * n * N_seg),
                                        _ptr(seg_hh, np.float32, n * N_seg), _stream(stream)))
+
+    def eval_tseg(self, params, seg_tranches, upsilon, n_seg_eff=None, seg_power=None, seg_dh=None, seg_hh=None, n=None,
+                  stream=None):
+        if n is None:
+            n = (params.size if isinstance(params, np.ndarray) else params.numel()) // PARAM_COLS
+        N_seg = -(-self.Nt // max(int(seg_tranches), 1))
+        self._check(self._lib.tfs_eval_tseg(self._h, _ptr(params, np.float64, n * PARAM_COLS), n, seg_tranches,
+                                            _ptr(upsilon, np.float32, n), _ptr(n_seg_eff, np.int32, n),
+                                            _ptr(seg_power, np.float32, n * N_seg), _ptr(seg_dh, np.float32, 2 * n * N_seg),
+                                            _ptr(seg_hh, np.float32, n * N_seg), _stream(stream)))
 
     def eval_tf(self, params, N_seg, transfer, n_knots, f_knot0, f_knot_step, upsilon, seg_power=None, seg_dh=None,
                 seg_hh=None, n=None, stream=None):
@@ -261,3 +273,17 @@ def topk_host(ctx: Tfs, upsilon: np.ndarray, k: int):
     val = np.empty(k, dtype=np.float32)
     ctx.topk(upsilon, k, idx, val)
     return idx, val
+
+
+def eval_tseg_host(ctx: Tfs, params: np.ndarray, seg_tranches: int):
+    """tfs_eval_tseg with HOST buffers in and out."""
+    params = np.ascontiguousarray(params, dtype=np.float64)
+    n = params.shape[0]
+    N_seg = -(-ctx.Nt // max(int(seg_tranches), 1))
+    ups = np.empty(n, dtype=np.float32)
+    neff = np.empty(n, dtype=np.int32)
+    P = np.empty((n, N_seg), dtype=np.float32)
+    z = np.empty((n, N_seg, 2), dtype=np.float32)
+    hh = np.empty((n, N_seg), dtype=np.float32)
+    ctx.eval_tseg(params, seg_tranches, ups, neff, P, z, hh)
+    return dict(upsilon=ups, n_seg_eff=neff, seg_power=P, seg_dh=z[..., 0] + 1j * z[..., 1], seg_hh=hh)

@@ -47,7 +47,7 @@ struct tfs_ctx {
   int wmode = -1;                          // kWGeneral / kWSeparable / kWTimeOnly; -1 before the first upload
   int n_valid = 0;                         // valid (non-gap) tranches of the data uploaded last
   // piece tables (tile x segment cuts of the valid-tranche list), cached per N_seg until the next upload
-  struct PieceTable { int N_seg; int n_tiles; int* tile_first; int* piece_end; int* piece_seg; int* piece_tile; cudaEvent_t ready; };
+  struct PieceTable { int N_seg; int M_tr; int n_tiles; int* tile_first; int* piece_end; int* piece_seg; int* piece_tile; cudaEvent_t ready; };
   std::vector<PieceTable> piece_tables;
   uint8_t* gap = nullptr;
   int* vprefix = nullptr;                  // [Nt+1] valid tranches before m
@@ -63,7 +63,7 @@ struct tfs_ctx {
   void* buf_partials = nullptr; size_t cap_partials = 0;
   void* buf_prep = nullptr;     size_t cap_prep = 0;      // per-batch pre-pass: constants, keys, bucket tables, lists, units
   void* buf_ttab = nullptr;     size_t cap_ttab = 0;      // staged transfer table (tfs_eval_tf with a host table)
-  void* buf_out[4] = {nullptr, nullptr, nullptr, nullptr}; size_t cap_out[4] = {0, 0, 0, 0};
+  void* buf_out[5] = {nullptr, nullptr, nullptr, nullptr, nullptr}; size_t cap_out[5] = {0, 0, 0, 0, 0};
   void* buf_keys = nullptr;     size_t cap_keys = 0;
   void* buf_tk_in = nullptr;    size_t cap_tk_in = 0;
   void* buf_tk_idx = nullptr;   size_t cap_tk_idx = 0;
@@ -277,9 +277,9 @@ void free_piece_tables(tfs_ctx* ctx) {
 }
 
 // piece table for N_seg (built on `st` on first use; later users on other streams wait for the build event)
-int get_piece_table(tfs_ctx* ctx, int N_seg, cudaStream_t st, const tfs_ctx::PieceTable** out) {
+int get_piece_table(tfs_ctx* ctx, int N_seg, int M_tr, cudaStream_t st, const tfs_ctx::PieceTable** out) {
   for (auto& t : ctx->piece_tables)
-    if (t.N_seg == N_seg) {
+    if (t.N_seg == N_seg && t.M_tr == M_tr) {
       TFS_CUDA(ctx, cudaStreamWaitEvent(st, t.ready, 0));
       *out = &t;
       return TFS_OK;
@@ -287,6 +287,7 @@ int get_piece_table(tfs_ctx* ctx, int N_seg, cudaStream_t st, const tfs_ctx::Pie
   if (ctx->piece_tables.size() >= 64) free_piece_tables(ctx);         // a sweep over many N_seg: start over
   tfs_ctx::PieceTable t{};
   t.N_seg = N_seg;
+  t.M_tr = M_tr;
   t.n_tiles = std::max(1, (ctx->n_valid + kTS - 1) / kTS);
   const size_t max_pieces = (size_t)t.n_tiles + (size_t)N_seg;
   cudaError_t e;
@@ -299,7 +300,7 @@ int get_piece_table(tfs_ctx* ctx, int N_seg, cudaStream_t st, const tfs_ctx::Pie
     cudaFree(t.tile_first); cudaFree(t.piece_end); cudaFree(t.piece_seg); cudaFree(t.piece_tile);
     return fail(ctx, TFS_ENOMEM, "piece table allocation failed: %s", cudaGetErrorString(e));
   }
-  piece_table_kernel<<<1, 1, 0, st>>>(ctx->vprefix, ctx->valid_m, ctx->Nt, N_seg, ctx->n_valid, t.n_tiles,
+  piece_table_kernel<<<1, 1, 0, st>>>(ctx->vprefix, ctx->valid_m, ctx->Nt, N_seg, M_tr, ctx->n_valid, t.n_tiles,
                                       t.tile_first, t.piece_end, t.piece_seg, t.piece_tile);
   ctx->launches += 1;
   e = cudaGetLastError();
@@ -550,7 +551,7 @@ void tfs_destroy(tfs_ctx* ctx) {
   void* bufs[] = {ctx->pair[0].grid, ctx->pair[0].wgt, ctx->pair[0].wa, ctx->pair[0].wb, ctx->pair[1].grid, ctx->pair[1].wgt,
                   ctx->pair[1].wa, ctx->pair[1].wb, ctx->colmax, ctx->wcounts, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut,
                   ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials, ctx->buf_prep, ctx->buf_ttab,
-                  ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_keys,
+                  ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_out[4], ctx->buf_keys,
                   ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children, ctx->buf_fe};
   for (void* b : bufs) if (b) cudaFree(b);
   free_piece_tables(ctx);
@@ -753,9 +754,12 @@ void launch_slab(const EvalArgs& a, const tfs_ctx::Pair& P, unsigned blocks, cud
 // the evaluation proper (rows a1-a8) for one batch; `transfer` = per-template table [n][C][n_knots] complex or NULL
 int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const float* transfer, int n_knots,
               double f_knot0, double f_knot_step, float* upsilon, float* seg_power, float* seg_dh, float* seg_hh,
-              void* stream, const char* who) {
+              void* stream, const char* who, int M_tr = 0, int* n_seg_eff = nullptr) {
   if (!ctx) return fail(nullptr, TFS_EINVAL, "%s: ctx is NULL", who);
   if (n < 0) return fail(ctx, TFS_EINVAL, "%s: n < 0", who);
+  if (M_tr < 0) return fail(ctx, TFS_EINVAL, "%s: seg_tranches must be >= 1", who);
+  if (M_tr > 0) N_seg = (ctx->Nt + M_tr - 1) / M_tr;
+  if (n_seg_eff && ctx->opts.basis == 1) return fail(ctx, TFS_EINVAL, "%s: n_seg_eff is not available in the WDM basis", who);
   if (N_seg < 1 || N_seg > ctx->Nt) return fail(ctx, TFS_EINVAL, "%s: need 1 <= N_seg <= Nt (got %d, Nt %d)", who, N_seg, ctx->Nt);
   if (!ctx->uploaded) return fail(ctx, TFS_ESTATE, "%s: no data uploaded (call tfs_upload_data first)", who);
   if (transfer && ctx->opts.basis == 1) return fail(ctx, TFS_EINVAL, "%s: transfer tables are not available in the WDM basis", who);
@@ -782,12 +786,12 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
   }
 
   // outputs: device pointers are written in place, host pointers via ctx scratch + D2H
-  float* user[4] = {upsilon, seg_power, seg_dh, seg_hh};
-  const size_t per[4] = {1, (size_t)N_seg, (size_t)N_seg * 2, (size_t)N_seg};
-  float* dev[4] = {nullptr, nullptr, nullptr, nullptr};
-  bool host_out[4] = {false, false, false, false};
+  float* user[5] = {upsilon, seg_power, seg_dh, seg_hh, reinterpret_cast<float*>(n_seg_eff)};   // int32 rides as 4-byte words
+  const size_t per[5] = {1, (size_t)N_seg, (size_t)N_seg * 2, (size_t)N_seg, 1};
+  float* dev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  bool host_out[5] = {false, false, false, false, false};
   bool any_host = false;
-  for (int i = 0; i < 4; ++i) {
+  for (int i = 0; i < 5; ++i) {
     if (!user[i]) continue;
     if (is_device_ptr(user[i])) { dev[i] = user[i]; continue; }
     host_out[i] = true; any_host = true;
@@ -798,7 +802,7 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
 
   // tiling: tiles of kTS valid tranches, cut by the segment boundaries into pieces (one partial each)
   const tfs_ctx::PieceTable* pt = nullptr;
-  rc = get_piece_table(ctx, N_seg, st, &pt);
+  rc = get_piece_table(ctx, N_seg, M_tr, st, &pt);
   if (rc) return rc;
   const int n_tiles = pt->n_tiles;
   const size_t max_pieces = (size_t)n_tiles + (size_t)N_seg;
@@ -828,6 +832,14 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
   if (rc) return rc;
   char* part[8];
   { char* q = (char*)ctx->buf_prep; for (int i = 0; i < 8; ++i) { part[i] = q; q += sz[i]; } }
+#ifdef TFS_POISON
+  // debug builds only (the initcheck substitute, tests/test_gpu_parity.py): every scratch buffer starts as NaN /
+  // 0xFFFF... patterns, so a value read before it was written shows up in the outputs
+  TFS_CUDA(ctx, cudaMemsetAsync(ctx->buf_partials, 0xFF, (size_t)sub * max_pieces * part_bytes, st));
+  TFS_CUDA(ctx, cudaMemsetAsync(ctx->buf_prep, 0xFF, total, st));
+  for (int i = 0; i < 5; ++i)
+    if (host_out[i]) TFS_CUDA(ctx, cudaMemsetAsync(dev[i], 0xFF, (size_t)n * per[i] * sizeof(float), st));
+#endif
 
   TFS_CUDA(ctx, cudaMemsetAsync(ctx->bad, 0, sizeof(unsigned long long), st));
   const int wm = ctx->opts.fresnel_mode != 0 ? kWGeneral : ctx->wmode;
@@ -912,12 +924,13 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
     combine_kernel<<<(unsigned)((nb + threads - 1) / threads), threads, 0, st>>>(
         (const float4*)ctx->buf_partials, (const uint16_t*)part[1], nb, N_seg, pt->tile_first, n_tiles, pt->piece_seg,
         pt->piece_tile, dev[0] + off, dev[1] ? dev[1] + off * per[1] : nullptr,
-        dev[2] ? dev[2] + off * per[2] : nullptr, dev[3] ? dev[3] + off * per[3] : nullptr);
+        dev[2] ? dev[2] + off * per[2] : nullptr, dev[3] ? dev[3] + off * per[3] : nullptr,
+        dev[4] ? reinterpret_cast<int*>(dev[4]) + off : nullptr);
     TFS_CUDA(ctx, cudaGetLastError());
     ctx->launches += 1;
   }
   if (any_host) {
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 5; ++i)
       if (host_out[i])
         TFS_CUDA(ctx, cudaMemcpyAsync(user[i], dev[i], (size_t)n * per[i] * sizeof(float), cudaMemcpyDeviceToHost, st));
     unsigned long long bad = 0;
@@ -947,6 +960,13 @@ int tfs_eval_tf(tfs_ctx* ctx, const double* params, long long n, int N_seg, cons
   if (ctx && !transfer) return fail(ctx, TFS_EINVAL, "tfs_eval_tf: transfer is NULL (use tfs_eval for constant factors)");
   return eval_impl(ctx, params, n, N_seg, transfer, n_knots, f_knot0, f_knot_step, upsilon, seg_power, seg_dh, seg_hh, stream,
                    "tfs_eval_tf");
+}
+
+int tfs_eval_tseg(tfs_ctx* ctx, const double* params, long long n, int seg_tranches, float* upsilon, int* n_seg_eff,
+                  float* seg_power, float* seg_dh, float* seg_hh, void* stream) {
+  if (ctx && seg_tranches < 1) return fail(ctx, TFS_EINVAL, "tfs_eval_tseg: seg_tranches must be >= 1 (got %d)", seg_tranches);
+  return eval_impl(ctx, params, n, 1, nullptr, 0, 0.0, 0.0, upsilon, seg_power, seg_dh, seg_hh, stream, "tfs_eval_tseg",
+                   seg_tranches, n_seg_eff);
 }
 
 int tfs_count_pixels(tfs_ctx* ctx, const double* params, long long n, long long* counts, void* stream) {

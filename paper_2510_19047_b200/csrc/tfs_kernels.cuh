@@ -1475,13 +1475,14 @@ prep_scatter_kernel(const EvalArgs a) {
 }
 
 // Piece table (C9, C10).  Segment n = tranches [ceil(n Nt/N_seg), ceil((n+1) Nt/N_seg)), i.e. n(m) =
-// floor(m N_seg / Nt).  Tile t = entries [t kTS, (t+1) kTS) of the compacted valid-tranche list.
+// floor(m N_seg / Nt); or, with M_tr > 0 (tfs_eval_tseg: segments of fixed duration T_seg = M_tr DT, t_n = n T_seg,
+// P:93), n(m) = floor(m / M_tr) and N_seg = ceil(Nt / M_tr).  Tile t = entries [t kTS, (t+1) kTS) of the compacted valid-tranche list.
 // A piece is a maximal run of entries inside one tile and one segment; pieces are numbered in time order.
 // One thread walks the list (<= n_tiles + N_seg pieces); the table is cached per N_seg by the host.
 //   tile_first[t] = first piece of tile t, tile_first[n_tiles] = number of pieces
 //   piece_end[p]  = entry where piece p ends (exclusive);  piece_seg[p] = its segment;  piece_tile[p] = its tile
 __global__ void piece_table_kernel(const int* __restrict__ vprefix, const int* __restrict__ valid_m, int Nt, int N_seg,
-                                   int n_valid, int n_tiles, int* __restrict__ tile_first,
+                                   int M_tr, int n_valid, int n_tiles, int* __restrict__ tile_first,
                                    int* __restrict__ piece_end, int* __restrict__ piece_seg, int* __restrict__ piece_tile) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
   int p = 0;
@@ -1490,8 +1491,10 @@ __global__ void piece_table_kernel(const int* __restrict__ vprefix, const int* _
     int i = t * kTS;
     const int iend = min(i + kTS, n_valid);
     while (i < iend) {
-      const int seg = (int)(((long long)valid_m[i] * N_seg) / Nt);
-      const int s1 = (int)(((long long)(seg + 1) * Nt + N_seg - 1) / N_seg);     // first tranche of the next segment
+      const int seg = M_tr > 0 ? valid_m[i] / M_tr : (int)(((long long)valid_m[i] * N_seg) / Nt);
+      const long long s1l = M_tr > 0 ? (long long)(seg + 1) * M_tr
+                                     : ((long long)(seg + 1) * Nt + N_seg - 1) / N_seg;   // first tranche of the next segment
+      const int s1 = (int)(s1l < (long long)Nt ? s1l : (long long)Nt);
       const int e = min(vprefix[min(s1, Nt)], iend);
       piece_seg[p] = seg;
       piece_end[p] = e;
@@ -1513,12 +1516,12 @@ __global__ void combine_kernel(const float4* __restrict__ partials, const uint16
                                const int* __restrict__ tile_first, int n_tiles, const int* __restrict__ piece_seg,
                                const int* __restrict__ piece_tile,
                                float* __restrict__ upsilon, float* __restrict__ seg_power,
-                               float* __restrict__ seg_dh, float* __restrict__ seg_hh) {
+                               float* __restrict__ seg_dh, float* __restrict__ seg_hh, int* __restrict__ n_seg_eff) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int n_pieces = tile_first[n_tiles];
   double ups = 0.0;
-  int p = 0, cur_tile = -1;
+  int p = 0, cur_tile = -1, n_eff = 0;
   bool live = false;
   for (int s = 0; s < N_seg; ++s) {
     double zr = 0, zi = 0, hh = 0;
@@ -1531,11 +1534,13 @@ __global__ void combine_kernel(const float4* __restrict__ partials, const uint16
     }
     const double P = hh > 0.0 ? (zr * zr + zi * zi) / hh : 0.0;
     ups += P;
+    n_eff += hh > 0.0 ? 1 : 0;
     if (seg_power) seg_power[i * N_seg + s] = (float)P;
     if (seg_dh) { seg_dh[(i * N_seg + s) * 2] = (float)zr; seg_dh[(i * N_seg + s) * 2 + 1] = (float)zi; }
     if (seg_hh) seg_hh[i * N_seg + s] = (float)hh;
   }
   upsilon[i] = (float)ups;
+  if (n_seg_eff) n_seg_eff[i] = n_eff;      // segments the template occupies: the paper's N_seg = tau / T_seg
 }
 
 // ------------------------------------------------------------------------------------------

@@ -518,6 +518,64 @@ def test_gather_stays_inside_the_padded_grid(api, tmp_path):
     assert r.returncode == 0 and "bounds ok" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
 
 
+_POISON_SCRIPT = r"""
+import sys
+import numpy as np, torch
+from paper_2510_19047_b200 import api, synth
+assert "poison" in api.LIB_PATH
+ref = np.load(sys.argv[1])
+w = synth.scaled(synth.WORKLOADS["cfg3"], Nt=700, Nf=1024, n_templates=4000)
+coeff, weight, gap = synth.make_data(w)
+p = synth.make_templates(w)
+p[:, 1] = np.random.default_rng(8).uniform(0.0, 3.0, len(p)) * w.Nt * w.DT
+p[5] = np.nan
+for wm in (0, 1):
+    ctx = api.Tfs(w.Nt, w.Nf, w.dt, weight_mode=wm)
+    ctx.upload_data(coeff, weight, gap)
+    for N_seg in (1, 16, w.Nt):
+        r = api.eval_host(ctx, p, N_seg)
+        for k in ("upsilon", "seg_power", "seg_dh", "seg_hh"):
+            assert np.isfinite(r[k]).all(), (wm, N_seg, k)
+            assert np.array_equal(r[k], ref[f"{k}_{wm}_{N_seg}"]), (wm, N_seg, k)
+    idx, val = api.topk_host(ctx, r["upsilon"], 40)
+    assert np.array_equal(idx, ref[f"idx_{wm}"])
+    ctx.destroy()
+print("poison ok")
+"""
+
+
+def test_no_scratch_value_is_read_before_it_is_written(api, tmp_path):
+    """The initcheck substitute (compute-sanitizer is closed on this pool): a build that fills the piece partials, the
+    pre-pass scratch and the staged outputs with 0xFF (NaN) before every evaluation must give finite outputs that are
+    bit-identical to the default build's -- items of bucket 0 are never read, bad rows and empty segments included."""
+    import os
+    import subprocess
+    import sys
+    from paper_2510_19047_b200 import build
+    w = synth.scaled(synth.WORKLOADS["cfg3"], Nt=700, Nf=1024, n_templates=4000)
+    coeff, weight, gap = synth.make_data(w)
+    p = synth.make_templates(w)
+    p[:, 1] = np.random.default_rng(8).uniform(0.0, 3.0, len(p)) * w.Nt * w.DT
+    p[5] = np.nan
+    ref = {}
+    for wm in (0, 1):
+        ctx = api.Tfs(w.Nt, w.Nf, w.dt, weight_mode=wm)
+        ctx.upload_data(coeff, weight, gap)
+        for N_seg in (1, 16, w.Nt):
+            r = api.eval_host(ctx, p, N_seg)
+            for k in ("upsilon", "seg_power", "seg_dh", "seg_hh"):
+                ref[f"{k}_{wm}_{N_seg}"] = r[k]
+        ref[f"idx_{wm}"] = api.topk_host(ctx, r["upsilon"], 40)[0]
+        ctx.destroy()
+    np.savez(tmp_path / "ref.npz", **ref)
+    lib = build.build_variant(str(tmp_path / "libtfs_poison.so"), ["TFS_POISON"])
+    env = dict(os.environ, TFS_LIB_PATH=lib)
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", _POISON_SCRIPT, str(tmp_path / "ref.npz")], cwd=root, env=env,
+                       capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0 and "poison ok" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
+
+
 def test_sub_batches_match_separate_calls(api):
     """A bank whose piece partials exceed the scratch cap is cut into sub-batches inside one tfs_eval call;
     the results must be bit-identical to evaluating the same rows in separate, smaller calls."""

@@ -652,3 +652,82 @@ def test_p14_varying_transfer_noiseless_injection_and_loop():
                 z[n] += T * W[a, m, k] * np.conj(D[a, m, k]) * Hd[m, k]
                 hh[n] += abs(T) ** 2 * W[a, m, k] * abs(Hd[m, k]) ** 2
     assert np.allclose(r["seg_dh"][0], z, rtol=1e-10, atol=1e-12) and np.allclose(r["seg_hh"][0], hh, rtol=1e-10)
+
+
+# ----------------------------------------------------------------------------------------------
+# P15  segments of fixed duration T_seg = M_tr DT ("t_n = n T_seg", P:57 N_seg = tau/T_seg, M_tr = T_seg/DT)
+# ----------------------------------------------------------------------------------------------
+def test_p15_fixed_duration_segments():
+    rng = np.random.default_rng(15)
+    g = O.Grid(48, 128, 5.0)
+    D = rng.standard_normal((2, g.Nt, g.Nf)) + 1j * rng.standard_normal((2, g.Nt, g.Nf))
+    W = rng.uniform(0.5, 2.0, (2, g.Nt, g.Nf))
+    gap = (rng.uniform(size=g.Nt) > 0.2).astype(np.uint8)
+    p = np.array([[30.0, 0.9 * g.Tobs, 0.3, 0.7, 0.1, 0.5, -0.2, 1.0],       # merges inside the grid
+                  [22.0, 3.0 * g.Tobs, 1.0, 0.2, 0.0, 0.9, 0.3, 2.0]])
+    # (a) M_tr divides Nt: the same numbers as the equal-index rule with N_seg = Nt / M_tr
+    for M_tr in (1, 4, 12, 48):
+        a = O.evaluate_tseg(p, D, W, gap, g, M_tr)
+        b = O.evaluate(p, D, W, gap, g, g.Nt // M_tr)
+        for k in ("upsilon", "seg_power", "seg_dh", "seg_hh"):
+            assert np.array_equal(a[k], b[k]), (M_tr, k)
+    # (b) ragged last segment, against plain loops over tranches: z_n, hh_n accumulated tranche by tranche
+    M_tr = 10
+    a = O.evaluate_tseg(p, D, W, gap, g, M_tr)
+    assert a["seg_hh"].shape == (2, 5)
+    for i in range(2):
+        Hd = O.dense_template(p[i, 0], p[i, 1], p[i, 2], p[i, 7], g, O.Opts(), gap)
+        T = [p[i, 3] + 1j * p[i, 4], p[i, 5] + 1j * p[i, 6]]
+        z = np.zeros(5, dtype=complex); hh = np.zeros(5)
+        for m in range(g.Nt):
+            if not gap[m]:
+                continue
+            for al in range(2):
+                z[m // M_tr] += T[al] * np.sum(W[al, m] * np.conj(D[al, m]) * Hd[m])
+                hh[m // M_tr] += abs(T[al]) ** 2 * np.sum(W[al, m] * np.abs(Hd[m]) ** 2)
+        assert np.allclose(a["seg_dh"][i], z, rtol=1e-12, atol=1e-12) and np.allclose(a["seg_hh"][i], hh, rtol=1e-12)
+        assert a["n_seg_eff"][i] == int((hh > 0).sum())
+    # (c) M_tr >= Nt: one segment, the coherent statistic
+    assert np.array_equal(O.evaluate_tseg(p, D, W, gap, g, 1000)["upsilon"], O.evaluate(p, D, W, gap, g, 1)["upsilon"])
+
+
+def test_p15_n_seg_eff_is_tau_over_tseg():
+    """Without gaps and inside the band the number of occupied segments is ceil(tau / T_seg) with tau = min(T_obs, t_c - DT)
+    rounded down to whole tranches: the paper's N_seg = tau / T_seg for tau = min(T_obs, t_c) on the tranche grid."""
+    g = O.Grid(64, 512, 5.0)
+    D = np.ones((1, g.Nt, g.Nf), dtype=complex)
+    for frac in (0.13, 0.5, 0.77, 1.0, 4.0):
+        tc = frac * g.Tobs
+        p = np.array([[25.0, tc, 0.0, 1.0, 0.0, 0.0, 0.0, 1.0]])
+        n_active = int(min(g.Nt, math.ceil(tc / g.DT - 1.0)))         # tranches with tau = tc - m DT > DT
+        o = O.Opts(f_lo=0.0, f_hi=1e9, c_max=1e300)                   # no band or sweep limit: only tau > DT cuts
+        tr = O.track(25.0, tc, 0.0, 1.0, g, o)
+        assert int(tr["active"].sum()) == n_active
+        for M_tr in (1, 5, 16):
+            r = O.evaluate_tseg(p, D, None, None, g, M_tr, o)
+            assert r["n_seg_eff"][0] == math.ceil(n_active / M_tr), (frac, M_tr)
+
+
+def test_p15_noise_mean_is_twice_n_seg_eff():
+    """E[Upsilon] = 2 n_seg_eff for pure noise (each occupied segment contributes a chi^2_2), over 4000 noise draws of
+    the window pixels of a template that merges inside the grid."""
+    rng = np.random.default_rng(151)
+    g = O.Grid(40, 256, 5.0)
+    p = np.array([30.0, 0.62 * g.Tobs, 0.3, 0.7, 0.0, 0.5, 0.0, 1.0])
+    M_tr = 6
+    o = O.Opts(f_lo=0.0, f_hi=1e9, c_max=1e300)      # only the merger ends the track (its window is clipped to the top bin)
+    Hd = O.dense_template(p[0], p[1], p[2], p[7], g, o)
+    T = np.array([p[3] + 1j * p[4], p[5] + 1j * p[6]])
+    seg = O.segment_of_bin_tseg(np.arange(g.Nt), M_tr)
+    N_seg = -(-g.Nt // M_tr)
+    ms, ks = np.nonzero(Hd)
+    tot, n_draw = 0.0, 4000
+    for _ in range(n_draw):
+        D = np.zeros((2, g.Nt, g.Nf), dtype=complex)
+        D[:, ms, ks] = rng.standard_normal((2, ms.size)) + 1j * rng.standard_normal((2, ms.size))
+        z, hh = O.segment_products(Hd, T, D, None, None, N_seg, seg=seg)
+        tot += O.combine(z, hh)[1]
+    n_eff = int((hh > 0).sum())
+    assert n_eff == math.ceil(int(O.track(p[0], p[1], 0, 1, g, o)["active"].sum()) / M_tr) and 1 < n_eff < N_seg
+    mean, sig = tot / n_draw, 2.0 * math.sqrt(n_eff / n_draw)
+    assert abs(mean - 2.0 * n_eff) < 4.0 * sig, (mean, n_eff)
