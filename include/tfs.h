@@ -192,6 +192,25 @@ TFS_API int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k,
 TFS_API int tfs_refine(tfs_ctx* ctx, const double* params, long long n, const long long* idx, long long k,
                int r, double d_mc_rel, double d_tc, double* children, void* stream);
 
+/* Tile search (the paper tiles the search volume in (Mc, f_in), f_in = f(t_0 = 0): tiles of 5 Msun x
+ * 1e-4 Hz below and 1e-3 Hz above 10 mHz, and maximises the statistic in each tile).
+ * tfs_tile_lattice writes the cell-centred n_mc x n_fin lattice of the tile [mc_lo, mc_hi] x [fin_lo, fin_hi]:
+ *     row i*n_fin + j:  Mc = mc_lo + (i + 1/2) d_mc,  f_in = fin_lo + (j + 1/2) d_fin,
+ *                       tc = tau(Mc, f_in) = 5 M (8 pi M f_in)^(-8/3),  M = Mc G Msun/c^3   (t_c = remaining lifetime, P:57;
+ *                       the inverse of tfs_eval's 0PN track at t = 0), columns 2..7 copied from row[2..7],
+ *     d_mc = (mc_hi - mc_lo)/n_mc,  d_fin = (fin_hi - fin_lo)/n_fin.
+ *   row [8] double, HOST pointer;  params [n_mc*n_fin][8] double, host or device.  n_mc*n_fin < 2^31.
+ * tfs_refine_fin is tfs_refine carried out in (Mc, f_in): survivor j (row idx[j] of params) is replaced by r*r
+ * children that tile its (d_mc x d_fin) cell,
+ *     f_in = f(tc) = (tc/5M)^(-3/8)/(8 pi M);  child (a, b):  Mc' = Mc + o_a d_mc,  f_in' = f_in + o_b d_fin,
+ *     tc' = tau(Mc', f_in'),  o_i = (2 i + 1 - r)/(2 r),  other columns copied;  row j*r*r + a*r + b of children.
+ * Lattice positions use separately rounded fp64 products and sums; tau and f go through pow (a few ulp).
+ * Arguments otherwise as tfs_refine. */
+TFS_API int tfs_tile_lattice(tfs_ctx* ctx, double mc_lo, double mc_hi, int n_mc, double fin_lo, double fin_hi, int n_fin,
+                             const double* row, double* params, void* stream);
+TFS_API int tfs_refine_fin(tfs_ctx* ctx, const double* params, long long n, const long long* idx, long long k,
+                           int r, double d_mc, double d_fin, double* children, void* stream);
+
 /* Number of window pixels (k_hi-k_lo+1 summed over active tranches) of each template:
  * pixel_evals = n_channels * counts[i].  counts [n] int64, host or device.  Used by the
  * benchmark for the pixel-evals/s metric and by tests for the window logic. */

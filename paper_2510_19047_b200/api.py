@@ -62,6 +62,10 @@ def load_library():
     lib.tfs_topk.restype = ip
     lib.tfs_refine.argtypes = [vp, vp, ll, vp, ll, ip, dp, dp, vp, vp]
     lib.tfs_refine.restype = ip
+    lib.tfs_refine_fin.argtypes = [vp, vp, ll, vp, ll, ip, dp, dp, vp, vp]
+    lib.tfs_refine_fin.restype = ip
+    lib.tfs_tile_lattice.argtypes = [vp, dp, dp, ip, dp, dp, ip, vp, vp, vp]
+    lib.tfs_tile_lattice.restype = ip
     lib.tfs_count_pixels.argtypes = [vp, vp, ll, vp, vp]
     lib.tfs_count_pixels.restype = ip
     lib.tfs_bad_param_count.argtypes = [vp]
@@ -194,6 +198,22 @@ class Tfs:
         self._check(self._lib.tfs_refine(self._h, _ptr(params, np.float64, n * PARAM_COLS), n,
                                          _ptr(idx, np.int64, k), k, r, d_mc_rel, d_tc,
                                          _ptr(children, np.float64, k * r * r * PARAM_COLS), _stream(stream)))
+
+    def refine_fin(self, params, idx, r, d_mc, d_fin, children, n=None, k=None, stream=None):
+        if n is None:
+            n = (params.size if isinstance(params, np.ndarray) else params.numel()) // PARAM_COLS
+        if k is None:
+            k = idx.size if isinstance(idx, np.ndarray) else idx.numel()
+        self._check(self._lib.tfs_refine_fin(self._h, _ptr(params, np.float64, n * PARAM_COLS), n,
+                                             _ptr(idx, np.int64, k), k, r, d_mc, d_fin,
+                                             _ptr(children, np.float64, k * r * r * PARAM_COLS), _stream(stream)))
+
+    def tile_lattice(self, mc_lo, mc_hi, n_mc, fin_lo, fin_hi, n_fin, row, params, stream=None):
+        row = np.ascontiguousarray(row, dtype=np.float64)
+        if row.size != PARAM_COLS:
+            raise ValueError("row must hold 8 doubles")
+        self._check(self._lib.tfs_tile_lattice(self._h, mc_lo, mc_hi, n_mc, fin_lo, fin_hi, n_fin, row.ctypes.data,
+                                               _ptr(params, np.float64, n_mc * n_fin * PARAM_COLS), _stream(stream)))
 
     def count_pixels(self, params, counts, n=None, stream=None):
         if n is None:

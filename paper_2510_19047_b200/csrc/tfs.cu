@@ -1044,6 +1044,76 @@ int tfs_refine(tfs_ctx* ctx, const double* params, long long n, const long long*
   return TFS_OK;
 }
 
+int tfs_tile_lattice(tfs_ctx* ctx, double mc_lo, double mc_hi, int n_mc, double fin_lo, double fin_hi, int n_fin,
+                     const double* row, double* params, void* stream) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_tile_lattice: ctx is NULL");
+  if (n_mc < 1 || n_fin < 1 || (long long)n_mc * n_fin >= (1ll << 31))
+    return fail(ctx, TFS_EINVAL, "tfs_tile_lattice: need n_mc, n_fin >= 1 and n_mc*n_fin < 2^31");
+  if (!(mc_lo > 0.0) || !(mc_hi >= mc_lo) || !(fin_lo > 0.0) || !(fin_hi >= fin_lo) || !std::isfinite(mc_hi) || !std::isfinite(fin_hi))
+    return fail(ctx, TFS_EINVAL, "tfs_tile_lattice: need 0 < mc_lo <= mc_hi and 0 < fin_lo <= fin_hi (finite)");
+  if (!row || !params) return fail(ctx, TFS_EINVAL, "tfs_tile_lattice: row and params are required");
+  if (is_device_ptr(row)) return fail(ctx, TFS_EINVAL, "tfs_tile_lattice: row must be a host pointer (8 doubles)");
+  if (int rcd = check_device(ctx, "tfs_tile_lattice")) return rcd;
+  cudaStream_t st = (cudaStream_t)stream;
+  const long long nc = (long long)n_mc * n_fin;
+  Row8 r8;
+  for (int c = 0; c < 8; ++c) r8.v[c] = row[c];
+  const double d_mc = (mc_hi - mc_lo) / (double)n_mc, d_fin = (fin_hi - fin_lo) / (double)n_fin;
+  const bool host_out = !is_device_ptr(params);
+  double* d_out = params;
+  if (host_out) {
+    int rc = ensure(ctx, &ctx->buf_children, &ctx->cap_children, (size_t)nc * TFS_PARAM_COLS * sizeof(double));
+    if (rc) return rc;
+    d_out = (double*)ctx->buf_children;
+  }
+  tile_lattice_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(mc_lo, d_mc, n_mc, fin_lo, d_fin, n_fin, r8, d_out);
+  TFS_CUDA(ctx, cudaGetLastError());
+  ctx->launches += 1;
+  if (host_out) {
+    TFS_CUDA(ctx, cudaMemcpyAsync(params, d_out, (size_t)nc * TFS_PARAM_COLS * sizeof(double), cudaMemcpyDeviceToHost, st));
+    TFS_CUDA(ctx, cudaStreamSynchronize(st));
+  }
+  return TFS_OK;
+}
+
+int tfs_refine_fin(tfs_ctx* ctx, const double* params, long long n, const long long* idx, long long k, int r,
+                   double d_mc, double d_fin, double* children, void* stream) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_refine_fin: ctx is NULL");
+  if (n < 0 || k < 0) return fail(ctx, TFS_EINVAL, "tfs_refine_fin: n < 0 or k < 0");
+  if (r < 1 || r > 64) return fail(ctx, TFS_EINVAL, "tfs_refine_fin: need 1 <= r <= 64 (got %d)", r);
+  if (!std::isfinite(d_mc) || !std::isfinite(d_fin)) return fail(ctx, TFS_EINVAL, "tfs_refine_fin: steps must be finite");
+  if (int rcd = check_device(ctx, "tfs_refine_fin")) return rcd;
+  if (k == 0) return TFS_OK;
+  if (!params || !idx || !children) return fail(ctx, TFS_EINVAL, "tfs_refine_fin: params, idx and children are required");
+  if (k * (long long)r * r >= (1ll << 32)) return fail(ctx, TFS_EINVAL, "tfs_refine_fin: k*r*r must be < 2^32");
+  cudaStream_t st = (cudaStream_t)stream;
+  const long long nc = k * (long long)r * r;
+  const double* d_params = nullptr;
+  int rc = stage_params(ctx, params, n, st, &d_params);
+  if (rc) return rc;
+  const long long* d_idx = idx;
+  const bool host_idx = !is_device_ptr(idx), host_out = !is_device_ptr(children);
+  if (host_idx) {
+    rc = ensure(ctx, &ctx->buf_tk_idx, &ctx->cap_tk_idx, (size_t)k * sizeof(long long));
+    if (rc) return rc;
+    TFS_CUDA(ctx, cudaMemcpyAsync(ctx->buf_tk_idx, idx, (size_t)k * sizeof(long long), cudaMemcpyHostToDevice, st));
+    d_idx = (const long long*)ctx->buf_tk_idx;
+  }
+  double* d_out = children;
+  if (host_out) {
+    rc = ensure(ctx, &ctx->buf_children, &ctx->cap_children, (size_t)nc * TFS_PARAM_COLS * sizeof(double));
+    if (rc) return rc;
+    d_out = (double*)ctx->buf_children;
+  }
+  refine_fin_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(d_params, n, d_idx, k, r, d_mc, d_fin, d_out);
+  TFS_CUDA(ctx, cudaGetLastError());
+  ctx->launches += 1;
+  if (host_out)
+    TFS_CUDA(ctx, cudaMemcpyAsync(children, d_out, (size_t)nc * TFS_PARAM_COLS * sizeof(double), cudaMemcpyDeviceToHost, st));
+  if (host_out || host_idx || !is_device_ptr(params)) TFS_CUDA(ctx, cudaStreamSynchronize(st));
+  return TFS_OK;
+}
+
 int tfs_probe_l2_bandwidth(tfs_ctx* ctx, long long bytes, int iters, double* gb_per_s, void* stream) {
   if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_probe_l2_bandwidth: ctx is NULL");
   if (bytes < (1 << 20) || bytes > (1ll << 32) || iters < 1 || iters > 100000 || !gb_per_s)

@@ -1783,6 +1783,67 @@ __global__ void refine_kernel(const double* __restrict__ params, long long n, co
 }
 
 // ------------------------------------------------------------------------------------------
+// Tile search (P:275 tiles in (M_c, f_in), P:57 t_c = remaining lifetime at t_0 = 0).
+// tau(f) = 5 M (8 pi M f)^(-8/3), f(tau) = (tau/5M)^(-3/8)/(8 pi M): the 0PN track of load_template/track_point
+// solved for the time to coalescence.  Lattice positions are formed with separately rounded products and sums
+// (bit-identical to the host arithmetic of the oracle); the two powers go through pow().
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double tau_of_f(double Mc, double f) {
+  const double M = __dmul_rn(Mc, kMtsun);
+  const double z = __dmul_rn(__dmul_rn(__dmul_rn(8.0, kPi), M), f);
+  return __dmul_rn(__dmul_rn(5.0, M), pow(z, -8.0 / 3.0));
+}
+__device__ __forceinline__ double f_of_tau(double Mc, double tau) {
+  const double M = __dmul_rn(Mc, kMtsun);
+  return __ddiv_rn(pow(__ddiv_rn(tau, __dmul_rn(5.0, M)), -0.375), __dmul_rn(__dmul_rn(8.0, kPi), M));
+}
+
+struct Row8 { double v[8]; };
+
+// cell-centred lattice over [mc_lo, mc_lo + n_mc d_mc] x [fin_lo, fin_lo + n_fin d_fin]; row i n_fin + j
+__global__ void tile_lattice_kernel(double mc_lo, double d_mc, int n_mc, double fin_lo, double d_fin, int n_fin,
+                                    const Row8 row, double* __restrict__ out) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (long long)n_mc * n_fin) return;
+  const int i = (int)(t / n_fin), j = (int)(t - (long long)i * n_fin);
+  const double mc = __dadd_rn(mc_lo, __dmul_rn(__dadd_rn((double)i, 0.5), d_mc));
+  const double fin = __dadd_rn(fin_lo, __dmul_rn(__dadd_rn((double)j, 0.5), d_fin));
+  double* o = out + t * 8;
+  o[0] = mc;
+  o[1] = tau_of_f(mc, fin);
+#pragma unroll
+  for (int c = 2; c < 8; ++c) o[c] = row.v[c];
+}
+
+// r*r children per survivor in (M_c, f_in): M_c' = M_c + o_a d_mc, f_in' = f_in + o_b d_fin, t_c' = tau(M_c', f_in')
+__global__ void refine_fin_kernel(const double* __restrict__ params, long long n, const long long* __restrict__ idx,
+                                  long long k, int r, double d_mc, double d_fin, double* __restrict__ out) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long rr = (long long)r * r;
+  if (t >= k * rr) return;
+  const long long j = t / rr;
+  const int ab = (int)(t - j * rr);
+  const int ia = ab / r, ib = ab - ia * r;
+  const long long src = idx[j];
+  double* o = out + t * 8;
+  if (src < 0 || src >= n) {
+    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+#pragma unroll
+    for (int c = 0; c < 8; ++c) o[c] = qnan;
+    return;
+  }
+  const double* p = params + src * 8;
+  const double oa = __ddiv_rn((double)(2 * ia + 1 - r), (double)(2 * r));
+  const double ob = __ddiv_rn((double)(2 * ib + 1 - r), (double)(2 * r));
+  const double fin = f_of_tau(p[0], p[1]);
+  const double mc = __dadd_rn(p[0], __dmul_rn(oa, d_mc));
+  o[0] = mc;
+  o[1] = tau_of_f(mc, __dadd_rn(fin, __dmul_rn(ob, d_fin)));
+#pragma unroll
+  for (int c = 2; c < 8; ++c) o[c] = p[c];
+}
+
+// ------------------------------------------------------------------------------------------
 // Top-k: radix select on 64-bit composite keys (value order, then lower index), then bitonic sort.
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned long long topk_key(float v, unsigned idx) {

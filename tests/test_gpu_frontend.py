@@ -95,3 +95,35 @@ def test_chirp_from_time_series_to_upsilon(api):
         assert r["n_active"] >= 30
     assert np.argmax(gpu["upsilon"]) == len(params) - 1 and gpu["upsilon"][-1] > 100.0
     ctx.destroy()
+
+
+def test_two_tranche_lengths_from_one_series(api):
+    """tranches of 6 h for f_in below 10 mHz and 3 h above.  One context has one tranche length, so the split is
+    two contexts over the same series, (Nt, Nf) and (2 Nt, Nf/2); each runs through tfs_upload_timeseries + tfs_eval
+    against the oracle chain, and the fast high-band chirp is recovered at least as well by the short tranches."""
+    Nt, Nf = 96, 2048                                  # DT = 20480 s (5.7 h) and 10240 s (2.8 h) at dt = 5 s
+    w = synth.scaled(synth.WORKLOADS["cfg1"], Nt=Nt, Nf=Nf, n_templates=16)
+    x, mask, psd = synth.make_timeseries(w)
+    inj = np.array([60.0, 0.35 * O.YEAR_S, 0.3, 0.7, 0.0, 0.5, 0.0, 1.0])          # f ~ 27 -> 40 mHz: the high band
+    N = 2 * Nf
+    t = np.arange(Nt * N) * w.dt
+    M = inj[0] * O.MTSUN_S
+    X = (inj[1] - t) / (5 * M)
+    f = X ** (-0.375) / (8 * np.pi * M)
+    h = f ** (2.0 / 3.0) * np.exp(1j * (inj[2] - 2 * X ** 0.625))
+    h *= 0.35 / np.abs(h).max()
+    x = x + np.stack([((inj[3] + 1j * inj[4]) * h).real, ((inj[5] + 1j * inj[6]) * h).real]).astype(np.float32)
+    params = np.vstack([synth.make_templates(w), inj[None]])
+    ups = {}
+    for nt, nf in ((Nt, Nf), (2 * Nt, Nf // 2)):
+        g = O.Grid(nt, nf, w.dt)
+        psd_b = np.ascontiguousarray(psd[:, :: Nf // nf])                           # the same PSD model on the coarser bins
+        ctx = api.Tfs(nt, nf, w.dt)
+        ctx.upload_timeseries(x, mask, psd_b, tukey_alpha=0.0)
+        gpu = api.eval_host(ctx, params, 1)
+        Do, Wo, go = F.frontend(x, nt, nf, w.dt, sample_mask=mask, psd=psd_b, tukey_alpha=0.0)
+        ora = O.evaluate(params, Do, Wo, go, g, 1, O.Opts())
+        assert_parity(gpu, ora, 1, label=f"tranches of {2 * nf * w.dt:.0f} s")
+        ups[nt] = float(gpu["upsilon"][-1])
+        ctx.destroy()
+    assert ups[2 * Nt] > 0.98 * ups[Nt] > 50.0, ups
