@@ -84,7 +84,7 @@ typedef struct {
                                 h~_w(f_k)/DT = A e^{i phi} int_0^1 w(s) exp{i (2 pi u s + pi c s^2)} ds,  u = x - k,
                             evaluated in closed form (Fresnel auxiliary functions at the taper ends and at u +- 1/alpha).
                             Window, activity and segment rules are unchanged.  Basis 0 and fresnel_mode 0 only; every
-                            item then takes the global-memory gather kernel (about 4x the cost of the default)            */
+                            item then takes the global-memory gather kernel (about 10x the cost of the default)            */
 } tfs_opts;
 
 TFS_API void tfs_default_opts(tfs_opts* opts);

@@ -1184,6 +1184,16 @@ int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k, long long* 
     d_val = (float*)ctx->buf_tk_val;
   }
   const int threads = 256;
+  if (n <= (long long)kBitonicBlock) {
+    // small batch: select, sort and emit in one launch (the radix select below is 20+ launches: launch-bound here)
+    topk_small_kernel<<<1, 1024, 0, st>>>(d_in, (int)n, k, d_idx, d_val);
+    ctx->launches += 1;
+    TFS_CUDA(ctx, cudaGetLastError());
+    if (host_idx) TFS_CUDA(ctx, cudaMemcpyAsync(idx, d_idx, (size_t)k * sizeof(long long), cudaMemcpyDeviceToHost, st));
+    if (host_val) TFS_CUDA(ctx, cudaMemcpyAsync(val, d_val, (size_t)k * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (host_idx || host_val || !is_device_ptr(upsilon)) TFS_CUDA(ctx, cudaStreamSynchronize(st));
+    return TFS_OK;
+  }
   const unsigned blocks = (unsigned)std::min<long long>((n + threads - 1) / threads, (long long)ctx->sm_count * 8);
   topk_init_kernel<<<1, 256, 0, st>>>(ctx->sel, (unsigned long long)k);
   ctx->launches += 1 + 16 + 1 + 1;   // init, 8 x (hist, pick), gather, emit

@@ -1972,6 +1972,35 @@ bitonic_block_kernel(unsigned long long* keys, unsigned size_first, unsigned siz
   for (unsigned i = threadIdx.x; i < kBitonicBlock; i += blockDim.x) keys[base + i] = sk[i];
 }
 
+// Small batches (n <= kBitonicBlock, e.g. the 64-template batches of BASELINE.json configs[0]): the whole select in ONE
+// launch -- keys of all n values into shared memory (padding keys are 0: below every real key, whose low word is
+// 0xFFFFFFFF - idx > 0 for idx < 2^32 - 1), bitonic sort descending, emit the first k.  Same order as the general path.
+__global__ void __launch_bounds__(1024)
+topk_small_kernel(const float* __restrict__ v, int n, int k, long long* __restrict__ idx, float* __restrict__ val) {
+  __shared__ unsigned long long sk[kBitonicBlock];
+  unsigned P = 2;
+  while (P < (unsigned)n) P <<= 1;
+  for (unsigned i = threadIdx.x; i < P; i += blockDim.x) sk[i] = i < (unsigned)n ? topk_key(v[i], i) : 0ULL;
+  __syncthreads();
+  for (unsigned size = 2; size <= P; size <<= 1) {
+    for (unsigned stride = size >> 1; stride > 0; stride >>= 1) {
+      for (unsigned t = threadIdx.x; t < P / 2; t += blockDim.x) {
+        const unsigned lo = 2 * stride * (t / stride) + (t % stride);
+        const unsigned hi = lo + stride;
+        const bool desc = ((lo & size) == 0);
+        const unsigned long long a = sk[lo], b = sk[hi];
+        if ((a < b) == desc) { sk[lo] = b; sk[hi] = a; }
+      }
+      __syncthreads();
+    }
+  }
+  for (unsigned i = threadIdx.x; i < (unsigned)k; i += blockDim.x) {
+    const unsigned id = 0xFFFFFFFFu - (unsigned)(sk[i] & 0xFFFFFFFFull);
+    idx[i] = (long long)id;
+    val[i] = v[id];
+  }
+}
+
 __global__ void topk_emit_kernel(const unsigned long long* __restrict__ keys, const float* __restrict__ v,
                                  int k, long long* __restrict__ idx, float* __restrict__ val) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;

@@ -5,6 +5,8 @@
     python -m paper_2510_19047_b200.report nseg            # configs[2]: N_seg swept over {1, 4, 16, 64}
     python -m paper_2510_19047_b200.report ladder          # configs[4]: the 64 -> 16 -> 4 -> 1 ladder at full size
     python -m paper_2510_19047_b200.report frontend        # NEXT-2: time series -> TF grid at the 2-year-shaped size
+    python -m paper_2510_19047_b200.report window          # NEXT-2: window-aware template (tukey_alpha) vs the default
+    python -m paper_2510_19047_b200.report search          # NEXT-4: tfs_eval_tseg and the per-tile lattice search
 
 Uses only the public binding (api.Tfs) and the seeded generators (synth); timing with CUDA events on
 the current stream after warm-up, inputs resident on the device.  bench.py prints the headline line;
@@ -215,6 +217,73 @@ def frontend_report():
     ctx.destroy()
 
 
+def window_report():
+    """The window-aware template (tfs_opts.tukey_alpha = 0.1) against the default on the same cfg3 data: every item
+    goes through the list kernel and every pixel adds the two taper terms (twelve table look-ups)."""
+    import torch
+    from . import api, synth
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda:0")
+    w = synth.WORKLOADS["cfg3"]
+    coeff, weight, gap = synth.make_data(w)
+    d = torch.from_numpy(synth.make_templates(w, 200_000)).to(dev)
+    print(f"# window-aware template on the cfg3 grid, {d.shape[0]} templates, N_seg = {w.N_seg}\n")
+    print("| tukey_alpha | kernels | ms per tfs_eval | templates/s | pixel-evals/s |")
+    print("|---|---|---:|---:|---:|")
+    for alpha in (0.0, 0.1):
+        ctx = api.Tfs(w.Nt, w.Nf, w.dt, tukey_alpha=alpha)
+        ctx.upload_data(coeff, weight, gap)
+        pix = _counts(ctx, torch, d)
+        ms = _time_eval(ctx, torch, d, w.N_seg)
+        print(f"| {alpha} | {'slab + list' if alpha == 0.0 else 'list, MODE 2'} | {ms:.2f} | {d.shape[0] / ms * 1e3:.3e} | "
+              f"{2 * pix.sum() / ms * 1e3:.3e} |")
+        ctx.destroy()
+
+
+def search_report():
+    """tfs_eval_tseg at the cfg3 size, and the tile search over a row of paper-sized tiles (5 Msun x 1e-4 Hz)
+    on the cfg3 data (noise only): lattice 32 x 32 per tile, stages 16 -> 4 -> 1, 16 kept, 4 x 4 children, <= 3 extra levels."""
+    import time
+    torch, api, synth, w, ctx, _ = _setup("cfg3")
+    from . import search
+    dev = torch.device("cuda:0")
+    d = torch.from_numpy(synth.make_templates(w)).to(dev)
+    n = d.shape[0]
+    ups = torch.empty(n, dtype=torch.float32, device=dev)
+    neff = torch.empty(n, dtype=torch.int32, device=dev)
+    print(f"# tfs_eval_tseg on the cfg3 grid ({w.Nt} tranches of {w.DT:.0f} s), {n} templates\n")
+    print("| seg_tranches (T_seg) | N_seg | ms | templates/s | mean n_seg_eff |")
+    print("|---:|---:|---:|---:|---:|")
+    for M_tr in (256, 100, 30):
+        for _ in range(2):
+            ctx.eval_tseg(d, M_tr, ups, neff)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(3):
+            ctx.eval_tseg(d, M_tr, ups, neff)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 3
+        print(f"| {M_tr} ({M_tr * w.DT / 86400:.1f} d) | {-(-w.Nt // M_tr)} | {ms:.2f} | {n / ms * 1e3:.3e} | "
+              f"{neff.float().mean().item():.2f} |")
+    row = np.array([0.0, 0.0, 0.3, 0.7, 0.0, 0.5, 0.0, 1.0])
+    tiles = [(25.0, 30.0, 8.0e-3 + 1e-4 * j, 8.1e-3 + 1e-4 * j) for j in range(16)]
+    kw = dict(stages=(16, 4, 1), keep=16, r=4, max_extra=3, tol=1e-3)
+    search.search_tiles(ctx, tiles[:2], row, 32, 32, **kw)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    res = search.search_tiles(ctx, tiles, row, 32, 32, **kw)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    nev = sum(l[1] for r_ in res for l in r_.levels)
+    print(f"\n# tile search: {len(tiles)} tiles of 5 Msun x 1e-4 Hz at 8.0-9.6 mHz, noise only\n")
+    print(f"{dt * 1e3:.1f} ms wall for {len(tiles)} tiles ({dt / len(tiles) * 1e3:.1f} ms per tile, {nev} template evaluations, "
+          f"{sum(len(r_.levels) for r_ in res)} levels); hat-Upsilon_1 per tile: "
+          + ", ".join(f"{r_.upsilon:.1f}" for r_ in res))
+    ctx.destroy()
+
+
 if __name__ == "__main__":
     what = sys.argv[1] if len(sys.argv) > 1 else ""
     if what == "track-width":
@@ -227,5 +296,9 @@ if __name__ == "__main__":
         ladder_report()
     elif what == "frontend":
         frontend_report()
+    elif what == "window":
+        window_report()
+    elif what == "search":
+        search_report()
     else:
         sys.exit(__doc__)

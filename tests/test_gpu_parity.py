@@ -285,7 +285,7 @@ def test_device_pointer_path_matches_host_path(api, cfg1):
 # --------------------------------------------------------------------------------------------
 # top-k: bit-exact against a CPU stable sort
 # --------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("n,k", [(1, 1), (37, 37), (1000, 10), (5000, 4096), (5000, 4097), (300_000, 3000),
+@pytest.mark.parametrize("n,k", [(1, 1), (2, 2), (37, 37), (64, 1), (1000, 10), (4096, 4096), (4096, 41), (4097, 5), (5000, 4096), (5000, 4097), (300_000, 3000),
                                  (1 << 20, 10486), (100_000, 100_000)])
 def test_topk_exact(api, n, k):
     rng = np.random.default_rng(n + k)
