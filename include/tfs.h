@@ -116,13 +116,16 @@ TFS_API int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weigh
  *                (= dt*DFT/DT: the continuous-FT convention with the common factor DT dropped, C16)
  *     W[a,m,k] = 4*DT / S_a[k]   (0 where S is not positive and finite; 1 everywhere if psd == NULL),
  *                so that E[W |D|^2] = 2 <w^2> for noise of that PSD
- *     g[m]     = 1 iff every sample of tranche m is valid
+ *     g[m]     = 1 iff every sample of tranche m is valid (sample_mask) and finite (a NaN/Inf sample drops its tranche, C20)
  *   x           [C][Nt*2*Nf] float, real TDI series at cadence dt            host or device, required
  *   sample_mask [Nt*2*Nf]    uint8, 1 = valid sample; NULL => all valid        host or device
  *   psd         [C][Nf]      float, one-sided PSD [1/Hz] at f_k = k/DT; NULL => W = 1   host or device
  *   coeff_out [C][Nt][Nf][2], weight_out [C][Nt][Nf], gap_out [Nt]: nullable copies of D, W, g
  *                (host or device), e.g. to draw the whitened spectrogram of Fig. 3
- * Nf must factor into 2, 3 and 5 (shared-memory FFT) and be <= 12800.  Synchronises `stream`. */
+ * These weights are separable by construction (one PSD model per channel), so with weight_mode = 0 the library takes
+ * the per-bin table b_a[k] = 4 DT / S_a[k] directly (tfs_weight_structure 1, or 2 without a PSD): the per-pixel array
+ * W is only materialised when weight_out is given or weight_mode = 1.
+ * Nf must factor into 2, 3 and 5 (shared-memory FFT) and be <= 12800; basis 0 only.  Synchronises `stream`. */
 TFS_API int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_mask, const float* psd,
                                   double tukey_alpha, float* coeff_out, float* weight_out, uint8_t* gap_out,
                                   void* stream);

@@ -558,7 +558,10 @@ void tfs_destroy(tfs_ctx* ctx) {
   delete ctx;
 }
 
-int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const uint8_t* gap_mask, void* stream) {
+// The upload proper.  sep_bk: the caller KNOWS the weights are W[a,m,k] = bk[a][k] (device table [C][Nf], or NULL for
+// W = 1) and passes weight == NULL: no per-pixel weight array is written, read or analysed (the time-series front end).
+static int upload_impl(tfs_ctx* ctx, const float* coeff, const float* weight, const uint8_t* gap_mask, void* stream,
+                       bool sep_known, const float* sep_bk) {
   if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_upload_data: ctx is NULL");
   if (!coeff) return fail(ctx, TFS_EINVAL, "tfs_upload_data: coeff is NULL");
   int rc = check_device(ctx, "tfs_upload_data");
@@ -622,14 +625,22 @@ int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const
   for (int pr = 0; pr < ctx->n_pairs; ++pr) {
     tfs_ctx::Pair& P = ctx->pair[pr];
     UP_CUDA(cudaMemsetAsync(P.grid, 0, nrow * ctx->ncol * sizeof(float4), st));
-    UP_CUDA(cudaMemsetAsync(P.wgt, 0, nrow * ctx->ncol * sizeof(float2), st));
-    pack_kernel<<<blocks, 256, 0, st>>>((const float2*)d_coeff, d_weight, ctx->Nt, ctx->Nf, P.c0, P.c1, ctx->gap, ctx->vprefix,
-                                        ctx->ncol, P.grid, P.wgt);
+    if (!sep_known) UP_CUDA(cudaMemsetAsync(P.wgt, 0, nrow * ctx->ncol * sizeof(float2), st));
+    pack_kernel<<<blocks, 256, 0, st>>>((const float2*)d_coeff, d_weight, sep_known ? sep_bk : nullptr, ctx->Nt, ctx->Nf, P.c0,
+                                        P.c1, ctx->gap, ctx->vprefix, ctx->ncol, P.grid, sep_known ? nullptr : P.wgt);
     UP_CUDA(cudaGetLastError());
     ctx->launches += 1;
     // weight structure (C11): W = a[i] b[k] on every pixel?  then the hot loop reads no per-pixel weight
     unsigned long long wc[2] = {1, 1};
-    if (ctx->opts.weight_mode == 0) {
+    if (sep_known) {
+      UP_CUDA(cudaMemsetAsync(ctx->wcounts, 0, 2 * sizeof(unsigned long long), st));
+      UP_CUDA(cudaMemsetAsync(P.wa, 0, (size_t)ctx->ncol_cap * sizeof(float2), st));
+      weight_sep_set_kernel<<<1, 1024, 0, st>>>(sep_bk, ctx->Nf, P.c0, P.c1, n_valid, P.wa, P.wb, ctx->wcounts);
+      UP_CUDA(cudaGetLastError());
+      ctx->launches += 1;
+      UP_CUDA(cudaMemcpyAsync(wc, ctx->wcounts, sizeof(wc), cudaMemcpyDeviceToHost, st));
+      UP_CUDA(cudaStreamSynchronize(st));
+    } else if (ctx->opts.weight_mode == 0) {
       UP_CUDA(cudaMemsetAsync(ctx->wcounts, 0, 2 * sizeof(unsigned long long), st));
       weight_colmax_kernel<<<(unsigned)ctx->Nf, 256, 0, st>>>(P.wgt, ctx->ncol, n_valid, ctx->colmax);
       UP_CUDA(cudaMemsetAsync(P.wa, 0, (size_t)ctx->ncol_cap * sizeof(float2), st));
@@ -662,6 +673,10 @@ int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const
   return TFS_OK;
 }
 
+int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weight, const uint8_t* gap_mask, void* stream) {
+  return upload_impl(ctx, coeff, weight, gap_mask, stream, false, nullptr);
+}
+
 int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_mask, const float* psd,
                           double tukey_alpha, float* coeff_out, float* weight_out, uint8_t* gap_out, void* stream) {
   if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_upload_timeseries: ctx is NULL");
@@ -669,6 +684,7 @@ int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_ma
   if (!(tukey_alpha >= 0.0 && tukey_alpha <= 1.0))
     return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: tukey_alpha must be in [0, 1] (got %g)", tukey_alpha);
   if (int rcd = check_device(ctx, "tfs_upload_timeseries")) return rcd;
+  if (ctx->opts.basis != 0) return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: the front end builds short-time Fourier tranches (basis 0)");
   if (ctx->Nt > 65535) return fail(ctx, TFS_EINVAL, "tfs_upload_timeseries: Nt must be <= 65535 (got %d)", ctx->Nt);
   cudaStream_t st = (cudaStream_t)stream;
   const int C = ctx->C, Nt = ctx->Nt, Nf = ctx->Nf, N = 2 * ctx->Nf;
@@ -691,10 +707,13 @@ int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_ma
   const bool copy_mask = sample_mask && !is_device_ptr(sample_mask);
   const bool copy_psd = psd && !is_device_ptr(psd);
   auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
+  // the per-pixel weight array is only materialised when the caller wants it back or forces the general path:
+  // W[a,m,k] = b_a[k] is separable by construction, so the upload takes the table b directly
+  const bool need_w = weight_out != nullptr || ctx->opts.weight_mode != 0;
   const size_t sz[7] = {copy_x ? al(C * nsamp * sizeof(float)) : 0, copy_mask ? al(nsamp) : 0,
                         copy_psd ? al((size_t)C * Nf * sizeof(float)) : 0, al((size_t)(rad.total + 2) * sizeof(float2)),
-                        al((size_t)N * sizeof(float)), al(C * npix * sizeof(float2)), al(C * npix * sizeof(float))};
-  size_t total = al((size_t)Nt);
+                        al((size_t)N * sizeof(float)), al(C * npix * sizeof(float2)), need_w ? al(C * npix * sizeof(float)) : 0};
+  size_t total = al((size_t)Nt) + al((size_t)C * Nf * sizeof(float));
   for (size_t b : sz) total += b;
   int rc0 = ensure(ctx, &ctx->buf_fe, &ctx->cap_fe, total);
   if (rc0) return rc0;
@@ -723,23 +742,34 @@ int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_ma
   float2* d_coeff = (float2*)part[5];
   float* d_weight = (float*)part[6];
   uint8_t* d_gap = (uint8_t*)part[7];
+  float* d_bk = (float*)(part[7] + al((size_t)Nt));
 
   fe_tables_kernel<<<(unsigned)((std::max(N, rad.total) + 255) / 256), 256, 0, st>>>(d_tw, rad, d_win, N, tukey_alpha);
   FE_CUDA(cudaGetLastError());
   FE_CUDA(cudaFuncSetAttribute(fe_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  fe_fft_kernel<<<dim3((unsigned)Nt, (unsigned)C), kFeThreads, smem, st>>>(d_x, d_win, d_tw, rad, Nt, Nf, d_coeff);
+  fe_gap_kernel<<<(unsigned)Nt, 256, 0, st>>>(d_mask, N, d_gap);          // before the FFT: it also clears g[m] on non-finite samples
   FE_CUDA(cudaGetLastError());
-  fe_weight_kernel<<<dim3((unsigned)((Nf + 255) / 256), (unsigned)Nt, (unsigned)C), 256, 0, st>>>(d_psd, Nt, Nf, ctx->DT, d_weight);
+  fe_fft_kernel<<<dim3((unsigned)Nt, (unsigned)C), kFeThreads, smem, st>>>(d_x, d_win, d_tw, rad, Nt, Nf, d_coeff, d_gap);
   FE_CUDA(cudaGetLastError());
-  fe_gap_kernel<<<(unsigned)Nt, 256, 0, st>>>(d_mask, N, d_gap);
-  FE_CUDA(cudaGetLastError());
-  ctx->launches += 4;
+  ctx->launches += 3;
+  if (need_w) {
+    fe_weight_kernel<<<dim3((unsigned)((Nf + 255) / 256), (unsigned)Nt, (unsigned)C), 256, 0, st>>>(d_psd, Nt, Nf, ctx->DT, d_weight);
+    FE_CUDA(cudaGetLastError());
+    ctx->launches += 1;
+  }
+  if (d_psd) {
+    fe_bk_kernel<<<(unsigned)((C * Nf + 255) / 256), 256, 0, st>>>(d_psd, C, Nf, ctx->DT, d_bk);
+    FE_CUDA(cudaGetLastError());
+    ctx->launches += 1;
+  }
   if (coeff_out) FE_CUDA(cudaMemcpyAsync(coeff_out, d_coeff, C * npix * sizeof(float2), cudaMemcpyDefault, st));
   if (weight_out) FE_CUDA(cudaMemcpyAsync(weight_out, d_weight, C * npix * sizeof(float), cudaMemcpyDefault, st));
   if (gap_out) FE_CUDA(cudaMemcpyAsync(gap_out, d_gap, (size_t)Nt, cudaMemcpyDefault, st));
 #undef FE_CUDA
-  // the rest is the ordinary upload, from device buffers (it synchronises the stream before returning)
-  return tfs_upload_data(ctx, (const float*)d_coeff, d_weight, d_gap, stream);
+  // the rest is the ordinary upload, from device buffers (it synchronises the stream before returning); with the
+  // default weight_mode the weights go in as the per-bin table (no per-pixel array is read or analysed)
+  if (ctx->opts.weight_mode != 0) return upload_impl(ctx, (const float*)d_coeff, d_weight, d_gap, stream, false, nullptr);
+  return upload_impl(ctx, (const float*)d_coeff, nullptr, d_gap, stream, true, d_psd ? d_bk : nullptr);
 }
 
 }  // extern "C"

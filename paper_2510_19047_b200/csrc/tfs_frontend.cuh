@@ -123,7 +123,7 @@ __device__ __forceinline__ void stockham_stage(const float2* __restrict__ in, fl
 constexpr int kFeThreads = TFS_FE_THREADS;
 __global__ void __launch_bounds__(kFeThreads)
 fe_fft_kernel(const float* __restrict__ x, const float* __restrict__ win, const float2* __restrict__ tw,
-              const FeRadices rad, int Nt, int Nf, float2* __restrict__ coeff_out) {
+              const FeRadices rad, int Nt, int Nf, float2* __restrict__ coeff_out, uint8_t* __restrict__ gap) {
   extern __shared__ float2 fe_smem[];
   const int L = Nf, N = 2 * Nf;
   const int m = blockIdx.x, a = blockIdx.y;
@@ -132,11 +132,14 @@ fe_fft_kernel(const float* __restrict__ x, const float* __restrict__ win, const 
   const float2* xs = reinterpret_cast<const float2*>(x + ((size_t)a * Nt + m) * N);      // N is even: 8-byte aligned
   const float2* ws = reinterpret_cast<const float2*>(win);
   const int smask = (L & 15) == 0 ? 15 : 0;
+  int bad = 0;
   for (int n = threadIdx.x; n < L; n += blockDim.x) {
     const float2 s = __ldg(xs + n), w = __ldg(ws + n);
+    bad |= !(isfinite(s.x) && isfinite(s.y));
     cur[fe_swz(n, smask)] = make_float2(s.x * w.x, s.y * w.y);
   }
-  __syncthreads();
+  // a tranche with a sample that is not finite carries no usable transform: it is dropped like a gap (C20)
+  if (__syncthreads_or(bad) && threadIdx.x == 0 && gap) gap[m] = 0;
   int Ns = 1;
   for (int st = 0; st < rad.n; ++st) {
     const int R = rad.r[st];
@@ -171,6 +174,14 @@ __global__ void fe_weight_kernel(const float* __restrict__ psd, int Nt, int Nf, 
     w = (isfinite(S) && S > 0.0f) ? (float)(4.0 * DT / (double)S) : 0.0f;
   }
   weight_out[((size_t)a * Nt + m) * Nf + k] = w;
+}
+
+// b[alpha][k] = 4 DT / S_alpha[k] (0 where S is not positive and finite): the per-bin weight table of the front end
+__global__ void fe_bk_kernel(const float* __restrict__ psd, int C, int Nf, double DT, float* __restrict__ bk) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= C * Nf) return;
+  const float S = psd[i];
+  bk[i] = (isfinite(S) && S > 0.0f) ? (float)(4.0 * DT / (double)S) : 0.0f;
 }
 
 // g[m] = 1 iff every sample of tranche m is valid; one block per tranche

@@ -1575,8 +1575,8 @@ __global__ void count_pixels_kernel(const EvalArgs a, long long* __restrict__ co
 // and pad columns stay zero.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, int Nt, int Nf, int c0, int c1,
-            const uint8_t* __restrict__ gap, const int* __restrict__ vprefix, int ncol,
+pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, const float* __restrict__ bk, int Nt, int Nf,
+            int c0, int c1, const uint8_t* __restrict__ gap, const int* __restrict__ vprefix, int ncol,
             float4* __restrict__ grid, float2* __restrict__ wgt) {
   __shared__ float4 sY[32][33];
   __shared__ float2 sW[32][33];
@@ -1588,8 +1588,9 @@ pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, 
     if (m < Nt && k < Nf) {
       const long long i = (long long)m * Nf + k;
       float2 dA = coeff[c0 * npix + i], dE = c1 >= 0 ? coeff[c1 * npix + i] : make_float2(0.f, 0.f);
-      float wA = weight ? weight[c0 * npix + i] : 1.0f;
-      float wE = c1 >= 0 ? (weight ? weight[c1 * npix + i] : 1.0f) : 0.f;
+      // W: the per-pixel array; or (front end, weights known to be W[a,m,k] = bk[a][k]) the per-bin table; or 1
+      float wA = weight ? weight[c0 * npix + i] : (bk ? bk[(size_t)c0 * Nf + k] : 1.0f);
+      float wE = c1 >= 0 ? (weight ? weight[c1 * npix + i] : (bk ? bk[(size_t)c1 * Nf + k] : 1.0f)) : 0.f;
       // a pixel whose product W*D is not finite carries no information: weight 0 (also keeps every
       // value the gather can read finite, which the pixel loops rely on)
       if (!(isfinite(wA * dA.x) && isfinite(wA * dA.y) && isfinite(wA))) { wA = 0.f; dA = make_float2(0.f, 0.f); }
@@ -1604,7 +1605,7 @@ pack_kernel(const float2* __restrict__ coeff, const float* __restrict__ weight, 
     if (m < Nt && k < Nf && gap[m] != 0) {
       const long long o = (long long)k * ncol + vprefix[m];
       grid[o] = sY[tx][r];
-      wgt[o] = sW[tx][r];
+      if (wgt) wgt[o] = sW[tx][r];
     }
   }
 }
@@ -1692,6 +1693,41 @@ __global__ void weight_check_kernel(const float2* __restrict__ wgt, const float2
   }
   const unsigned n_bad = __popc(__ballot_sync(0xffffffffu, bad));
   if ((threadIdx.x & 31) == 0 && n_bad) atomicAdd(&counts[0], (unsigned long long)n_bad);
+}
+
+// Separable weights known by construction (tfs_upload_timeseries: W[a,m,k] = bk[a][k], one PSD model per channel,
+// or 1 without a PSD): fill a[i] = g = max_k bk, b[k] = bk[k]/g directly -- no per-pixel weight array is written,
+// read or analysed.  One CTA.  counts[1] = number of bins with b != 1 (-> kWSeparable, else kWTimeOnly).
+__global__ void __launch_bounds__(1024)
+weight_sep_set_kernel(const float* __restrict__ bk, int Nf, int c0, int c1, int n_valid, float2* __restrict__ wa,
+                      float2* __restrict__ wb, unsigned long long* counts) {
+  __shared__ float2 sh[1024];
+  float2 mx = make_float2(0.f, 0.f);
+  for (int k = threadIdx.x; k < Nf; k += 1024) {
+    const float bA = bk ? bk[(size_t)c0 * Nf + k] : 1.0f, bE = c1 >= 0 ? (bk ? bk[(size_t)c1 * Nf + k] : 1.0f) : 0.f;
+    mx.x = fmaxf(mx.x, isfinite(bA) ? bA : 0.f); mx.y = fmaxf(mx.y, isfinite(bE) ? bE : 0.f);
+  }
+  sh[threadIdx.x] = mx;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) {
+    if (threadIdx.x < o) {
+      sh[threadIdx.x].x = fmaxf(sh[threadIdx.x].x, sh[threadIdx.x + o].x);
+      sh[threadIdx.x].y = fmaxf(sh[threadIdx.x].y, sh[threadIdx.x + o].y);
+    }
+    __syncthreads();
+  }
+  const float2 g = sh[0];
+  unsigned long long not_one = 0;
+  for (int k = threadIdx.x; k < Nf; k += 1024) {
+    float bA = bk ? bk[(size_t)c0 * Nf + k] : 1.0f, bE = c1 >= 0 ? (bk ? bk[(size_t)c1 * Nf + k] : 1.0f) : 0.f;
+    if (!isfinite(bA)) bA = 0.f;
+    if (!isfinite(bE)) bE = 0.f;
+    const float2 b = make_float2(g.x > 0.f ? bA / g.x : 0.f, g.y > 0.f ? bE / g.y : 0.f);
+    wb[k] = b;
+    not_one += (g.x > 0.f && b.x != 1.0f) + (g.y > 0.f && b.y != 1.0f);
+  }
+  for (int i = threadIdx.x; i < n_valid; i += 1024) wa[i] = g;
+  if (not_one) atomicAdd(&counts[1], not_one);
 }
 
 // Compacted list of valid (non-gap) tranches and its prefix counts (C10).  One block.  valid_m is padded to

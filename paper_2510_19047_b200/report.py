@@ -187,8 +187,8 @@ def ladder_report():
 def frontend_report():
     """tfs_upload_timeseries at the cfg3 size (2 channels x 4096 tranches x 6144 samples), device-resident input.
     The call = window + FFT + weights + gap mask (4 kernels) followed by the ordinary upload (pack, valid list,
-    weight analysis) and a stream synchronisation.  Bytes that must cross HBM: read x, write and re-read D and W,
-    write the packed grid and weights."""
+    weight classification from the per-bin table) and a stream synchronisation.  Bytes that must cross HBM: read x and the
+    mask, write and re-read D, write the packed grid (no per-pixel weight array exists on this path)."""
     import torch
     from . import api, synth
     torch.cuda.set_device(0)
@@ -208,7 +208,7 @@ def frontend_report():
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / reps
     npix = 2 * w.Nt * w.Nf
-    mandatory = x.nbytes + mask.nbytes + 2 * (npix * 8 + npix * 4) + npix * 8 + npix * 4
+    mandatory = x.nbytes + mask.nbytes + 2 * npix * 8 + npix * 8        # read x and the mask; write and re-read D; write the grid
     print(f"# NEXT-2 front end at the cfg3 size: {w.Nt} tranches x {2 * w.Nf} samples x 2 channels\n")
     print(f"tfs_upload_timeseries (device input, Tukey 0.1, PSD weights, gap mask; includes the ordinary upload and "
           f"its synchronisation): {ms:.2f} ms per call; {mandatory / 1e9:.2f} GB must cross HBM "

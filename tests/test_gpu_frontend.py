@@ -127,3 +127,30 @@ def test_two_tranche_lengths_from_one_series(api):
         ups[nt] = float(gpu["upsilon"][-1])
         ctx.destroy()
     assert ups[2 * Nt] > 0.98 * ups[Nt] > 50.0, ups
+
+
+def test_non_finite_samples_drop_their_tranche(api):
+    """C20 for the front end: a NaN or Inf sample makes its tranche a gap (in any channel); everything else is unchanged."""
+    w = synth.scaled(synth.WORKLOADS["cfg1"], Nt=24, Nf=256, n_templates=12)
+    x, mask, psd = synth.make_timeseries(w)
+    N = 2 * w.Nf
+    ctx = api.Tfs(w.Nt, w.Nf, w.dt)
+    g0 = np.empty(w.Nt, dtype=np.uint8)
+    ctx.upload_timeseries(x, mask, psd, tukey_alpha=0.1, gap_out=g0)
+    ref = api.eval_host(ctx, synth.make_templates(w), 2)
+    good = np.nonzero(g0)[0]
+    xb = x.copy()
+    xb[0, good[1] * N + 7] = np.nan
+    xb[1, good[3] * N + N - 1] = np.inf
+    g1 = np.empty(w.Nt, dtype=np.uint8)
+    ctx.upload_timeseries(xb, mask, psd, tukey_alpha=0.1, gap_out=g1)
+    want = g0.copy(); want[[good[1], good[3]]] = 0
+    assert np.array_equal(g1, want)
+    r = api.eval_host(ctx, synth.make_templates(w), 2)
+    assert all(np.isfinite(r[k]).all() for k in ("upsilon", "seg_power", "seg_hh"))
+    # the same result as masking those two tranches by hand
+    m2 = mask.copy(); m2[good[1] * N] = 0; m2[good[3] * N] = 0
+    ctx.upload_timeseries(x, m2, psd, tukey_alpha=0.1)
+    r2 = api.eval_host(ctx, synth.make_templates(w), 2)
+    assert np.array_equal(r["upsilon"], r2["upsilon"]) and not np.array_equal(r["upsilon"], ref["upsilon"])
+    ctx.destroy()
