@@ -903,9 +903,10 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
       ctx->launches += 1;
       if (pass == 0) {
         TFS_CUDA(ctx, cudaMemsetAsync(a.counts, 0, n_buckets * sizeof(unsigned), st));
-        prep_keys_kernel<<<dim3(tb, (unsigned)n_tiles), 256, n_keys * sizeof(unsigned), st>>>(a);
+        const unsigned tbp = (unsigned)((nb + 256 * kPrepItems - 1) / (256 * kPrepItems));
+        prep_keys_kernel<<<dim3(tbp, (unsigned)n_tiles), 256, n_keys * sizeof(unsigned), st>>>(a);
         prep_scan_kernel<<<1, 1024, 0, st>>>(a);
-        prep_scatter_kernel<<<dim3(tb, (unsigned)n_tiles), 256, 2 * n_keys * sizeof(unsigned), st>>>(a);
+        prep_scatter_kernel<<<dim3(tbp, (unsigned)n_tiles), 256, 2 * n_keys * sizeof(unsigned), st>>>(a);
         ctx->launches += 3;
       }
       TFS_CUDA(ctx, cudaGetLastError());

@@ -1385,18 +1385,24 @@ __device__ __forceinline__ int item_key(const EvalArgs& a, const TplConst& T, in
   return 2 + b;
 }
 
-// grid (ceil(n/256), n_tiles): keys of the tile's items + the tile's bucket counts
+// grid (ceil(n/(256 kPrepItems)), n_tiles): keys of the tile's items + the tile's bucket counts; every thread takes
+// kPrepItems templates (strided by the block size: coalesced) so that the per-block histogram work -- zeroing and
+// flushing n_keys (~200) shared counters -- is paid once per 1024 items
+constexpr int kPrepItems = 4;
 __global__ void __launch_bounds__(256)
 prep_keys_kernel(const EvalArgs a) {
   extern __shared__ unsigned s_hist[];                              // [n_keys]
   for (int k = threadIdx.x; k < a.n_keys; k += blockDim.x) s_hist[k] = 0;
   __syncthreads();
   const int tile = blockIdx.y;
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < a.n) {
-    const int key = item_key(a, a.tconst[i], tile);
-    a.keys[(size_t)tile * a.n + i] = (uint16_t)key;
-    if (key) atomicAdd(&s_hist[key], 1u);
+#pragma unroll 1
+  for (int q = 0; q < kPrepItems; ++q) {
+    const long long i = ((long long)blockIdx.x * kPrepItems + q) * blockDim.x + threadIdx.x;
+    if (i < a.n) {
+      const int key = item_key(a, a.tconst[i], tile);
+      a.keys[(size_t)tile * a.n + i] = (uint16_t)key;
+      if (key) atomicAdd(&s_hist[key], 1u);
+    }
   }
   __syncthreads();
   for (int k = threadIdx.x; k < a.n_keys; k += blockDim.x)
@@ -1460,18 +1466,26 @@ prep_scatter_kernel(const EvalArgs a) {
   for (int k = threadIdx.x; k < a.n_keys; k += blockDim.x) s_cnt[k] = 0;
   __syncthreads();
   const int tile = blockIdx.y;
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  int key = 0;
-  unsigned rank = 0;
-  if (i < a.n) {
-    key = a.keys[(size_t)tile * a.n + i];
-    if (key) rank = atomicAdd(&s_cnt[key], 1u);
+  int key[kPrepItems];
+  unsigned rank[kPrepItems];
+#pragma unroll
+  for (int q = 0; q < kPrepItems; ++q) {
+    const long long i = ((long long)blockIdx.x * kPrepItems + q) * blockDim.x + threadIdx.x;
+    key[q] = 0; rank[q] = 0;
+    if (i < a.n) {
+      key[q] = a.keys[(size_t)tile * a.n + i];
+      if (key[q]) rank[q] = atomicAdd(&s_cnt[key[q]], 1u);
+    }
   }
   __syncthreads();
   for (int k = threadIdx.x; k < a.n_keys; k += blockDim.x)
     if (s_cnt[k]) s_base[k] = atomicAdd(&a.counts[(size_t)tile * a.n_keys + k], s_cnt[k]);
   __syncthreads();
-  if (key) a.list[a.bucket_off[(size_t)tile * a.n_keys + key] + s_base[key] + rank] = (unsigned)i;
+#pragma unroll
+  for (int q = 0; q < kPrepItems; ++q) {
+    const long long i = ((long long)blockIdx.x * kPrepItems + q) * blockDim.x + threadIdx.x;
+    if (key[q]) a.list[a.bucket_off[(size_t)tile * a.n_keys + key[q]] + s_base[key[q]] + rank[q]] = (unsigned)i;
+  }
 }
 
 // Piece table (C9, C10).  Segment n = tranches [ceil(n Nt/N_seg), ceil((n+1) Nt/N_seg)), i.e. n(m) =
