@@ -778,7 +778,7 @@ namespace {
 
 template <int WMODE>
 void launch_slab(const EvalArgs& a, const tfs_ctx::Pair& P, unsigned blocks, cudaStream_t st) {
-  eval_slab_kernel<WMODE><<<blocks, kWarpsPerCta * 32, slab_smem_bytes(WMODE), st>>>(a, P.map_y, P.map_w);
+  eval_slab_kernel<WMODE><<<blocks, kSlabWarps * 32, slab_smem_bytes(WMODE), st>>>(a, P.map_y, P.map_w);
 }
 
 // the evaluation proper (rows a1-a8) for one batch; `transfer` = per-template table [n][C][n_knots] complex or NULL

@@ -43,7 +43,11 @@ constexpr int kListUnitItems = 32;        // items per (warp-claimed) unit of th
 #ifndef TFS_WARPS
 #define TFS_WARPS 32
 #endif
-constexpr int kWarpsPerCta = TFS_WARPS;   // both evaluation kernels: one persistent CTA of 32 warps per SM (64 registers)
+constexpr int kWarpsPerCta = TFS_WARPS;   // list / WDM kernels: one persistent CTA of 32 warps per SM (64 registers)
+#ifndef TFS_SLAB_WARPS
+#define TFS_SLAB_WARPS TFS_WARPS
+#endif
+constexpr int kSlabWarps = TFS_SLAB_WARPS;   // slab kernel: warps of its persistent CTA (registers per thread = 65536 / (32 kSlabWarps))
 constexpr int kLutN = 512;                // LUT intervals in t = 1/(1+v)
 constexpr double kMtsun = 4.925490947e-6; // G Msun / c^3 [s]
 constexpr double kPi = 3.14159265358979323846;
@@ -1228,7 +1232,7 @@ static_assert(sizeof(SlabCtl) <= kSlabCtlBytes, "SlabCtl");
 // from the L2.
 // ------------------------------------------------------------------------------------------
 template <int WMODE>
-__global__ void __launch_bounds__(kWarpsPerCta * 32, 1)
+__global__ void __launch_bounds__(kSlabWarps * 32, 1)
 eval_slab_kernel(const EvalArgs a, const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_w) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float4* s_lut = reinterpret_cast<float4*>(smem_raw);
@@ -1244,7 +1248,7 @@ eval_slab_kernel(const EvalArgs a, const __grid_constant__ CUtensorMap map_y, co
   for (int i = threadIdx.x; i < (kLutN + 1) * kLutCopiesSlab; i += blockDim.x) s_lut[i] = a.lut[i / kLutCopiesSlab];
   if (threadIdx.x == 0) {
     mbar_init(bar_full, 1); mbar_init(bar_full + 8, 1);
-    mbar_init(bar_empty, kWarpsPerCta); mbar_init(bar_empty + 8, kWarpsPerCta);
+    mbar_init(bar_empty, kSlabWarps); mbar_init(bar_empty + 8, kSlabWarps);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
