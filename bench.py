@@ -453,6 +453,10 @@ def main():
     torch.cuda.synchronize()
     pixels = int(counts.sum().item())
     pixel_evals = 2 * pixels
+    # active-pixel histogram of the bank (templates that start above the band or merge at once are empty)
+    cq = counts.cpu().numpy()
+    pix_hist = {"zero_frac": float((cq == 0).mean()),
+                "quantiles_pixels_per_template": {q: int(np.quantile(cq, float(q))) for q in ("0.10", "0.25", "0.50", "0.75", "0.90", "1.00")}}
     l2_gbs = ctx.probe_l2_bandwidth(32 << 20, 200)
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
     warm = max(args.warmup, 3)
@@ -531,6 +535,7 @@ def main():
         "data": "synthetic", "config": cfg,
         "pixel_evals_per_sec": world * pixel_evals / (ms_step * 1e-3),
         "pixel_evals_per_template": pixel_evals / n,
+        "active_pixel_histogram": pix_hist,
         "roofline": {"bound": bound, "kernel": "eval_list_kernel + eval_slab_kernel (one pair per step)",
                      "achieved": terms[bound]["achieved"],
                      "peak": terms[bound]["peak"], "peak_source": terms[bound]["peak_source"],

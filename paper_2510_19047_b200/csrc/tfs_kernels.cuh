@@ -653,7 +653,10 @@ __device__ __forceinline__ void pixel_loop_global(const EvalArgs& a, const LaneT
   }
 }
 
-constexpr int kLutCopiesSlab = 4;
+#ifndef TFS_LUT_COPIES_SLAB
+#define TFS_LUT_COPIES_SLAB 4
+#endif
+constexpr int kLutCopiesSlab = TFS_LUT_COPIES_SLAB;
 
 // ------------------------------------------------------------------------------------------
 // One work item: template `it` on time tile `tile` (rows a2-a7).  LANES ARE TRANCHES: lane l owns the
