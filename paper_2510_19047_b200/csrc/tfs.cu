@@ -78,6 +78,7 @@ struct tfs_ctx {
   std::vector<cudaEvent_t> ev_pool;        // reused events, three per evaluation launch: start, list kernel done, slab kernel done
   size_t ev_used = 0;
   long long launches = 0;
+  long long l2_window_used = 0;            // evaluation launches that ran under an L2 access-policy window (TFS_L2_WINDOW=1)
 
   char err[512] = "";
 };
@@ -547,6 +548,8 @@ int tfs_get_profile(tfs_ctx* ctx, double* main_kernel_ms, long long* main_kernel
 
 void tfs_destroy(tfs_ctx* ctx) {
   if (!ctx) return;
+  if (ctx->l2_window_used)
+    fprintf(stderr, "tfs: TFS_L2_WINDOW=1: %lld evaluation launches ran with the grid declared persisting in L2\n", ctx->l2_window_used);
   for (auto& ev : ctx->ev_pool) cudaEventDestroy(ev);
   void* bufs[] = {ctx->pair[0].grid, ctx->pair[0].wgt, ctx->pair[0].wa, ctx->pair[0].wb, ctx->pair[1].grid, ctx->pair[1].wgt,
                   ctx->pair[1].wa, ctx->pair[1].wb, ctx->colmax, ctx->wcounts, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut,
@@ -923,6 +926,29 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
         TFS_CUDA(ctx, cudaEventRecord(ev[0], st));
       }
       const unsigned blocks = (unsigned)ctx->sm_count;       // persistent, 1 CTA per SM
+      // Measurement aid (BASELINE.json north_star (2): "the grid pinned in L2 through an access-policy window when it
+      // fits"): with TFS_L2_WINDOW=1 in the environment the pair's grid is declared persisting for the two evaluation
+      // launches when it fits the device's persisting-L2 limit.  Off by default: DESIGN.md section 7 has the measurement.
+      bool l2win = false;
+      {
+        static const bool want = [] { const char* e = getenv("TFS_L2_WINDOW"); return e && e[0] == '1'; }();
+        const size_t gbytes = ((size_t)ctx->Nf + kPadRows) * ctx->ncol * sizeof(float4);
+        int max_persist = 0, max_win = 0;
+        if (want && cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, ctx->device) == cudaSuccess &&
+            cudaDeviceGetAttribute(&max_win, cudaDevAttrMaxAccessPolicyWindowSize, ctx->device) == cudaSuccess &&
+            gbytes <= (size_t)max_persist && gbytes <= (size_t)max_win) {
+          cudaStreamAttrValue v{};
+          v.accessPolicyWindow.base_ptr = (void*)ctx->pair[pass].grid;
+          v.accessPolicyWindow.num_bytes = gbytes;
+          v.accessPolicyWindow.hitRatio = 1.0f;
+          v.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+          v.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+          l2win = cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, gbytes) == cudaSuccess &&
+                  cudaStreamSetAttribute(st, cudaStreamAttributeAccessPolicyWindow, &v) == cudaSuccess;
+          cudaGetLastError();
+          ctx->l2_window_used += l2win ? 1 : 0;
+        }
+      }
       // the items that gather from global memory (and every item with the paper's approximants) ...
       if (wdm) eval_wdm_kernel<<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
       else if (ctx->opts.fresnel_mode != 0) eval_list_kernel<1, kWGeneral><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
@@ -944,6 +970,12 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
         ctx->launches += 1;
       }
       if (ev[2]) TFS_CUDA(ctx, cudaEventRecord(ev[2], st));
+      if (l2win) {
+        cudaStreamAttrValue v{};
+        v.accessPolicyWindow.num_bytes = 0;
+        cudaStreamSetAttribute(st, cudaStreamAttributeAccessPolicyWindow, &v);
+        cudaGetLastError();
+      }
     }
     const int threads = 128;
     if (wdm)
