@@ -7,6 +7,7 @@
     python -m paper_2510_19047_b200.report frontend        # NEXT-2: time series -> TF grid at the 2-year-shaped size
     python -m paper_2510_19047_b200.report window          # NEXT-2: window-aware template (tukey_alpha) vs the default
     python -m paper_2510_19047_b200.report search          # NEXT-4: tfs_eval_tseg and the per-tile lattice search
+    python -m paper_2510_19047_b200.report channels        # NEXT-3: 1 / 2 / 3 channels, constant factors vs per-tranche transfer tables
 
 Uses only the public binding (api.Tfs) and the seeded generators (synth); timing with CUDA events on
 the current stream after warm-up, inputs resident on the device.  bench.py prints the headline line;
@@ -284,6 +285,49 @@ def search_report():
     ctx.destroy()
 
 
+def channels_report():
+    """Channels and transfer factors at the cfg3 size (Eq. 3 sums A, E, T; Eq. 29 T_alpha(f_nm) per tranche):
+    the cfg3 bank on 1, 2 and 3 channels of cfg3-like noise, with the constant factors of `params` (tfs_eval) and with a
+    16-knot complex table per template and channel interpolated at every tranche (tfs_eval_tf).  The third channel is a
+    second pass over its own pair."""
+    import torch
+    from . import api, synth
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda:0")
+    w = synth.WORKLOADS["cfg3"]
+    coeff, weight, gap = synth.make_data(w)
+    n, K = 500_000, 16
+    params = synth.make_templates(w, n)
+    d = torch.from_numpy(params).to(dev)
+    rng = np.random.default_rng(33)
+    print(f"# channels and transfer factors on the cfg3 grid, {n} templates, N_seg = {w.N_seg}, {K} knots over 1-100 mHz\n")
+    print("| channels | transfer factor | ms per call | templates/s | pixel-evals/s |")
+    print("|---:|---|---:|---:|---:|")
+    for C in (1, 2, 3):
+        cc = np.ascontiguousarray(np.concatenate([coeff, coeff[:1]])[:C])
+        ww = np.ascontiguousarray(np.concatenate([weight, weight[:1]])[:C])
+        ctx = api.Tfs(w.Nt, w.Nf, w.dt, C)
+        ctx.upload_data(cc, ww, gap)
+        pix = _counts(ctx, torch, d)
+        ups = torch.empty(n, dtype=torch.float32, device=dev)
+        tab = torch.from_numpy(rng.standard_normal((n, C, K, 2)).astype(np.float32)).to(dev)
+        for label, call in (("constant (params)", lambda: ctx.eval(d, w.N_seg, ups)),
+                            ("table, interpolated per tranche", lambda: ctx.eval_tf(d, w.N_seg, tab, K, 1e-3, 6.6e-3, ups))):
+            for _ in range(2):
+                call()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(3):
+                call()
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / 3
+            n_used = min(C, 2) if label.startswith("constant") else C       # tfs_eval gives the third channel T = 0 (skipped)
+            print(f"| {C} | {label} | {ms:.2f} | {n / ms * 1e3:.3e} | {n_used * pix.sum() / ms * 1e3:.3e} |")
+        ctx.destroy()
+
+
 if __name__ == "__main__":
     what = sys.argv[1] if len(sys.argv) > 1 else ""
     if what == "track-width":
@@ -300,5 +344,7 @@ if __name__ == "__main__":
         window_report()
     elif what == "search":
         search_report()
+    elif what == "channels":
+        channels_report()
     else:
         sys.exit(__doc__)
