@@ -27,6 +27,9 @@
  * its calls share scratch buffers: work enqueued on one stream must have completed (or be ordered
  * before) the next call on another stream; tfs_upload_data / tfs_upload_timeseries must not be
  * called while a tfs_eval of the same context is still running.
+ * CUDA graphs: after one warm-up call with the same shapes and N_seg (scratch buffers and the piece table then exist),
+ * tfs_eval / tfs_eval_tf / tfs_eval_tseg / tfs_topk / tfs_refine* with DEVICE buffers only enqueue kernels and memsets --
+ * no allocation, copy or synchronisation -- and can be captured into a CUDA graph (stream capture) and replayed.
  */
 #ifndef TFS_H
 #define TFS_H

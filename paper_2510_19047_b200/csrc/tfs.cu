@@ -281,7 +281,8 @@ void free_piece_tables(tfs_ctx* ctx) {
 int get_piece_table(tfs_ctx* ctx, int N_seg, int M_tr, cudaStream_t st, const tfs_ctx::PieceTable** out) {
   for (auto& t : ctx->piece_tables)
     if (t.N_seg == N_seg && t.M_tr == M_tr) {
-      TFS_CUDA(ctx, cudaStreamWaitEvent(st, t.ready, 0));
+      // the build was synchronised when the table was made: nothing to wait for (and a tfs_eval that is being captured
+      // into a CUDA graph stays free of dependencies on work outside the capture)
       *out = &t;
       return TFS_OK;
     }
@@ -307,6 +308,7 @@ int get_piece_table(tfs_ctx* ctx, int N_seg, int M_tr, cudaStream_t st, const tf
   e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaEventRecord(t.ready, st);
   ctx->piece_tables.push_back(t);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);      // once per (N_seg, upload): later calls on any stream just use it
   if (e != cudaSuccess) return fail(ctx, TFS_ECUDA, "piece_table_kernel failed: %s", cudaGetErrorString(e));
   *out = &ctx->piece_tables.back();
   return TFS_OK;

@@ -681,3 +681,45 @@ def test_precision_worst_case_hunt(api):
     assert r["n_active"] > 5000
     assert max(r["hh"], r["z"], r["P"], r["ups"]) <= 2e-5, r       # measured 1.1e-5 (P), 8e-6 (hh), 7e-6 (z)
     ctx.destroy()
+
+
+def test_eval_and_topk_capture_into_a_cuda_graph(api):
+    """Launch-bound small batches (BASELINE.json configs[0]: 64 templates): after one warm-up call with the same shapes,
+    tfs_eval + tfs_topk with device buffers make no allocation, copy or synchronisation, so they can be captured into a
+    CUDA graph and replayed; the replay gives the same bits."""
+    import torch
+    w = synth.WORKLOADS["cfg1"]
+    coeff, weight, gap = synth.make_data(w)
+    ctx = _mk(api, w, coeff, weight, gap)
+    p = torch.from_numpy(synth.make_templates(w)).cuda()
+    n = p.shape[0]
+    ups = torch.empty(n, dtype=torch.float32, device="cuda")
+    P = torch.empty((n, 4), dtype=torch.float32, device="cuda")
+    idx = torch.empty(5, dtype=torch.int64, device="cuda")
+    val = torch.empty(5, dtype=torch.float32, device="cuda")
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        ctx.eval(p, 4, ups, P)
+        ctx.topk(ups, 5, idx, val)
+    torch.cuda.synchronize()
+    ref = (ups.clone(), P.clone(), idx.clone(), val.clone())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        ctx.eval(p, 4, ups, P)
+        ctx.topk(ups, 5, idx, val)
+    for t in (ups, P, idx, val):
+        t.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert all(torch.equal(a, b) for a, b in zip((ups, P, idx, val), ref))
+    # new parameters in the same buffer, replayed: equal to a plain call
+    p2 = torch.from_numpy(synth.make_templates(w, seed=77)).cuda()
+    p.copy_(p2)
+    g.replay()
+    torch.cuda.synchronize()
+    got = ups.clone()
+    ctx.eval(p2, 4, ups)
+    torch.cuda.synchronize()
+    assert torch.equal(got, ups)
+    ctx.destroy()
+
