@@ -250,6 +250,8 @@ def main_wdm(args, info, w, n, N_seg, k_top, cfg):
     bounded sample; algorithmic bytes per pixel-eval: 4 B datum + 4 B weight."""
     import multiprocessing as mp
     rank, world = info.rank, info.world
+    if args.impl == "reference" and rank != 0:
+        return 0                                   # the reference arm runs on rank 0 alone
     cfg = dict(cfg, workload=cfg["workload"].replace("x 2 channels (A,E)", "x 2 channels (A,E), real WDM wavelet pixels (basis = 1)"))
     coeff_c, weight, gap = synth.make_data(w)
     coeff = np.ascontiguousarray(coeff_c[..., 0])                        # real pixels with the same noise model
