@@ -723,3 +723,26 @@ def test_eval_and_topk_capture_into_a_cuda_graph(api):
     assert torch.equal(got, ups)
     ctx.destroy()
 
+
+def test_high_band_grid_full_size_sampled(api):
+    """The paper's second grid (3 h tranches above 10 mHz): the cfg3 data span cut into twice as many tranches of
+    half the length, 8192 x 1536, with 2 x 10^5 templates; a sample of rows against the oracle and properties on all."""
+    import dataclasses
+    w = dataclasses.replace(synth.WORKLOADS["cfg3"], Nt=8192, Nf=1536, n_templates=200_000)
+    coeff, weight, gap = synth.make_data(w)
+    params = synth.make_templates(w)
+    ctx = _mk(api, w, coeff, weight, gap)
+    r16 = api.eval_host(ctx, params, 16, segments=False)["upsilon"]
+    r1 = api.eval_host(ctx, params, 1, segments=False)["upsilon"]
+    assert np.isfinite(r16).all() and (r16 >= r1 * (1 - 1e-4) - 1e-3).all()          # Cauchy-Schwarz (P8)
+    act = np.nonzero(r16 > 0)[0]
+    assert len(act) > 100_000
+    rng = np.random.default_rng(12)
+    rows = np.concatenate([rng.choice(act, 5, replace=False), [int(np.argmax(r16))]])
+    sub = params[rows]
+    gpu = api.eval_host(ctx, sub, 16)
+    ora = oracle_eval(coeff, weight, gap, sub, w.Nt, w.Nf, w.dt, 16)
+    assert_parity(gpu, ora, 16, label="8192 x 1536")
+    assert np.array_equal(gpu["upsilon"], r16[rows])                                 # rows do not depend on the batch
+    ctx.destroy()
+
