@@ -189,8 +189,21 @@ __global__ void __launch_bounds__(256)
 fe_gap_kernel(const uint8_t* __restrict__ sample_mask, int N, uint8_t* __restrict__ gap_out) {
   const int m = blockIdx.x;
   int bad = 0;
-  if (sample_mask)
-    for (int n = threadIdx.x; n < N; n += blockDim.x) bad |= (sample_mask[(size_t)m * N + n] == 0);
+  if (sample_mask) {
+    const uint8_t* row = sample_mask + (size_t)m * N;
+    if ((N & 15) == 0 && (((uintptr_t)row) & 15) == 0) {
+      // 16 mask bytes per load: a zero byte anywhere in the word (the classic has-zero-byte test)
+      const uint4* r4 = reinterpret_cast<const uint4*>(row);
+      for (int n = threadIdx.x; n < N / 16; n += blockDim.x) {
+        const uint4 v = __ldg(r4 + n);
+        const unsigned w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) bad |= ((w[q] - 0x01010101u) & ~w[q] & 0x80808080u) != 0u;
+      }
+    } else {
+      for (int n = threadIdx.x; n < N; n += blockDim.x) bad |= (row[n] == 0);
+    }
+  }
   bad = __syncthreads_or(bad);
   if (threadIdx.x == 0) gap_out[m] = bad ? 0 : 1;
 }
