@@ -184,6 +184,38 @@ TFS_API int tfs_eval_tseg(tfs_ctx* ctx, const double* params, long long n, int s
 TFS_API int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k,
              long long* idx, float* val, void* stream);
 
+/* tfs_topk for callers that must not allocate device memory.
+ *
+ * Who this is for: code that runs where cudaMalloc / cudaFree are off limits -- a plug-in handed a fixed memory
+ * budget by its host application (an inference server or pipeline stage that owns the whole device heap and forbids
+ * growth after start-up), a latency-critical loop that cannot tolerate the implicit device synchronisation of
+ * cudaMalloc/cudaFree, or a process whose memory pool is already full.  Every other call of this library needs a
+ * tfs_ctx, and tfs_create, tfs_upload_* and the first call of each size allocate; this one needs no context and
+ * never calls cudaMalloc, cudaFree or any allocating library routine.
+ *
+ * What it computes: exactly what tfs_topk computes (same kernels, same order: descending value, equal values by
+ * lower index, NaN last), so idx/val are bit-identical to tfs_topk's.
+ *   upsilon [n] float, idx [k] int64, val [k] float: DEVICE pointers only (a host pointer would need a staging
+ *   buffer, i.e. an allocation) -> TFS_EINVAL otherwise.  The caller owns all three.
+ *   1 <= n < 2^32;  1 <= k <= min(n, TFS_TOPK_STATIC_MAX_K).  A larger k is rejected with TFS_EINVAL and a message
+ *   naming the limit (tfs_last_error(NULL)); use tfs_topk for those.
+ * Work is only enqueued on `stream`; nothing is synchronised.
+ *
+ * Where the scratch lives: the radix-select state (1 KiB) and the 2^ceil(log2 k) sort keys (8 B each) sit in one
+ * array of fixed size compiled into the library (TFS_TOPK_STATIC_MAX_K * 8 + 2048 bytes = 514 KiB).  Every GPU on
+ * which a process loads libtfs.so holds that array from load until exit, used or not.
+ *
+ * First call on each device: it looks up the array's device address (once per device, with that device current)
+ * and the SM count, and caches them.  Make that first call outside any stream capture.
+ *
+ * Sharing: there is ONE array per device, shared by every caller and every stream in the process, and it keeps
+ * whatever the previous call left.  Each call re-initialises the parts that must start from zero (histogram,
+ * counters, padding keys) on `stream` before using them, so calls issued one after another on the same stream are
+ * independent.  Two calls whose kernels can overlap on the GPU (different streams without an event between them,
+ * or two host threads) race on the array and return garbage: order them yourself. */
+#define TFS_TOPK_STATIC_MAX_K 65536
+TFS_API int tfs_topk_static(const float* upsilon, long long n, int k, long long* idx, float* val, void* stream);
+
 /* Ladder refinement (BASELINE.json configs[4]; the hierarchical N_seg reduction of P:104, P:347;
  * reading C19 of DESIGN.md).  For each of the k survivors j (row idx[j] of params) write r*r
  * children on a lattice r times denser per dimension that tiles the parent's (Mc, tc) cell of

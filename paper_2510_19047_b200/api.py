@@ -60,6 +60,8 @@ def load_library():
     lib.tfs_eval_tseg.restype = ip
     lib.tfs_topk.argtypes = [vp, vp, ll, ip, vp, vp, vp]
     lib.tfs_topk.restype = ip
+    lib.tfs_topk_static.argtypes = [vp, ll, ip, vp, vp, vp]
+    lib.tfs_topk_static.restype = ip
     lib.tfs_refine.argtypes = [vp, vp, ll, vp, ll, ip, dp, dp, vp, vp]
     lib.tfs_refine.restype = ip
     lib.tfs_refine_fin.argtypes = [vp, vp, ll, vp, ll, ip, dp, dp, vp, vp]
@@ -293,6 +295,27 @@ def topk_host(ctx: Tfs, upsilon: np.ndarray, k: int):
     val = np.empty(k, dtype=np.float32)
     ctx.topk(upsilon, k, idx, val)
     return idx, val
+
+
+TOPK_STATIC_MAX_K = 65536       # TFS_TOPK_STATIC_MAX_K of include/tfs.h
+
+
+def topk_static(upsilon, k, idx, val, n=None, stream=None):
+    """``tfs_topk_static``: the top-k of ``tfs_topk`` for callers that are not allowed to allocate device memory
+    (a plug-in living inside someone else's fixed memory budget, a latency-critical loop that cannot take the
+    device-wide stall of ``cudaMalloc``/``cudaFree``, a process whose pool is full).  No context is needed; the
+    select's scratch is a 514 KiB array built into ``libtfs.so``.  ``upsilon``, ``idx`` (int64) and ``val`` (float32)
+    must be CUDA tensors on the current device and ``k <= TOPK_STATIC_MAX_K``; anything else raises ``TfsError``
+    (``TFS_EINVAL``).  Only enqueues on ``stream``.  All calls on one GPU share that one array: issue them in order
+    on one stream (or order them with events) -- overlapping calls corrupt each other's result.  The first call
+    on a device also looks up the array's address; do it before starting any stream capture."""
+    lib = load_library()
+    if n is None:
+        n = upsilon.numel()
+    rc = lib.tfs_topk_static(_ptr(upsilon, np.float32, n), n, k, _ptr(idx, np.int64, min(k, max(n, 0))),
+                             _ptr(val, np.float32, min(k, max(n, 0))), _stream(stream))
+    if rc != TFS_OK:
+        raise TfsError(rc, lib.tfs_last_error(None).decode())
 
 
 def eval_tseg_host(ctx: Tfs, params: np.ndarray, seg_tranches: int):

@@ -10,6 +10,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1296,3 +1297,124 @@ int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k, long long* 
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// tfs_topk_static: tfs_topk without a context and without any device allocation (include/tfs.h).
+//
+// Some users of this library run where they may not allocate on the device: a plug-in inside a host application
+// that hands out a fixed memory budget, a real-time loop that cannot afford cudaMalloc's device-wide
+// synchronisation, a process whose pool is exhausted.  For them the select's scratch (radix state + sort keys) is
+// the fixed array below, part of the library image on every GPU that loads it.
+//
+// `g_topk_static_scratch` is a DEVICE symbol.  In host code its name is only a host-side shadow of the symbol:
+// handing `g_topk_static_scratch` (or &g_topk_static_scratch[0]) to a kernel would pass a host address, which
+// faults or -- on systems where the GPU can reach host memory -- quietly scribbles over the wrong bytes.  The
+// usable device address comes from cudaGetSymbolAddress, asked once per device with that device current.
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t kStaticStateBytes = 2048;   // SelectState (1048 B) rounded up so that the keys stay 256-byte aligned
+constexpr size_t kStaticScratchBytes = kStaticStateBytes + (size_t)TFS_TOPK_STATIC_MAX_K * sizeof(unsigned long long);
+static_assert(sizeof(SelectState) <= kStaticStateBytes, "SelectState outgrew its slot in the static scratch");
+static_assert((TFS_TOPK_STATIC_MAX_K & (TFS_TOPK_STATIC_MAX_K - 1)) == 0, "the key area must hold a power of two");
+
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_topk_static_scratch[kStaticScratchBytes];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticSlot { unsigned char* base = nullptr; int sm_count = 0; };
+StaticSlot g_static_slot[kStaticMaxDevices];
+std::mutex g_static_mutex;
+
+// Device address of the scratch on the CURRENT device (looked up on the first call per device, cached afterwards).
+int static_scratch(int* device_out, StaticSlot* out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { cudaGetLastError(); return fail(nullptr, TFS_ECUDA, "tfs_topk_static: cudaGetDevice failed: %s", cudaGetErrorString(e)); }
+  if (dev < 0 || dev >= kStaticMaxDevices) return fail(nullptr, TFS_EINVAL, "tfs_topk_static: device ordinal %d not supported (< %d)", dev, kStaticMaxDevices);
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  StaticSlot& s = g_static_slot[dev];
+  if (!s.base) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_topk_static_scratch);
+    if (e != cudaSuccess || !p) {
+      cudaGetLastError();
+      return fail(nullptr, TFS_ECUDA, "tfs_topk_static: cudaGetSymbolAddress failed on device %d: %s", dev, cudaGetErrorString(e));
+    }
+    int sms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess || sms < 1) {
+      cudaGetLastError();
+      return fail(nullptr, TFS_ECUDA, "tfs_topk_static: cudaDeviceGetAttribute failed on device %d: %s", dev, cudaGetErrorString(e));
+    }
+    s.sm_count = sms;
+    s.base = (unsigned char*)p;
+  }
+  *device_out = dev;
+  *out = s;
+  return TFS_OK;
+}
+
+// device memory that belongs to `dev` (managed memory is accepted as well)
+bool is_device_ptr_on(const void* p, int dev) {
+  cudaPointerAttributes at;
+  cudaError_t e = cudaPointerGetAttributes(&at, p);
+  if (e != cudaSuccess) { cudaGetLastError(); return false; }
+  if (at.type == cudaMemoryTypeManaged) return true;
+  return at.type == cudaMemoryTypeDevice && at.device == dev;
+}
+
+}  // namespace
+
+extern "C" int tfs_topk_static(const float* upsilon, long long n, int k, long long* idx, float* val, void* stream) {
+  if (!upsilon || !idx || !val) return fail(nullptr, TFS_EINVAL, "tfs_topk_static: upsilon, idx and val are required");
+  if (n < 1 || n >= (1ll << 32)) return fail(nullptr, TFS_EINVAL, "tfs_topk_static: need 1 <= n < 2^32");
+  if (k < 1 || k > n) return fail(nullptr, TFS_EINVAL, "tfs_topk_static: need 1 <= k <= n (got k %d, n %lld)", k, n);
+  if (k > TFS_TOPK_STATIC_MAX_K)
+    return fail(nullptr, TFS_EINVAL, "tfs_topk_static: k = %d exceeds TFS_TOPK_STATIC_MAX_K = %d, the size of the built-in "
+                                     "scratch (use tfs_topk, which allocates)", k, TFS_TOPK_STATIC_MAX_K);
+  int dev = -1;
+  StaticSlot slot;
+  int rc = static_scratch(&dev, &slot);
+  if (rc) return rc;
+  if (!is_device_ptr_on(upsilon, dev) || !is_device_ptr_on(idx, dev) || !is_device_ptr_on(val, dev))
+    return fail(nullptr, TFS_EINVAL, "tfs_topk_static: upsilon, idx and val must be device pointers on the current device "
+                                     "(staging a host buffer would need an allocation)");
+  cudaStream_t st = (cudaStream_t)stream;
+  SelectState* sel = (SelectState*)slot.base;
+  unsigned long long* keys = (unsigned long long*)(slot.base + kStaticStateBytes);
+  auto launched = [&](const char* what) {
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? TFS_OK : fail(nullptr, TFS_ECUDA, "tfs_topk_static: %s failed: %s", what, cudaGetErrorString(e));
+  };
+  const int threads = 256;
+  if (n <= (long long)kBitonicBlock) {       // whole select in shared memory, as in tfs_topk: the scratch is not touched
+    topk_small_kernel<<<1, 1024, 0, st>>>(upsilon, (int)n, k, idx, val);
+    return launched("topk_small_kernel");
+  }
+  unsigned P = 1;
+  while (P < (unsigned)k) P <<= 1;           // <= TFS_TOPK_STATIC_MAX_K: fits the key area
+  const unsigned blocks = (unsigned)std::min<long long>((n + threads - 1) / threads, (long long)slot.sm_count * 8);
+  topk_init_kernel<<<1, 256, 0, st>>>(sel, (unsigned long long)k);      // zeroes prefix, rank, counter and histogram left by the last call
+  for (int pass = 0; pass < 8; ++pass) {
+    topk_hist_kernel<<<blocks, threads, 0, st>>>(upsilon, n, pass, sel);
+    topk_pick_kernel<<<1, 256, 0, st>>>(pass, sel);
+  }
+  topk_gather_kernel<<<blocks, threads, 0, st>>>(upsilon, n, sel, keys, (unsigned)k);     // writes keys[0, k)
+  if (P > (unsigned)k) topk_pad_kernel<<<(P - k + threads - 1) / threads, threads, 0, st>>>(keys, (unsigned)k, P);   // and [k, P)
+  if (P <= 4096) {
+    bitonic_small_kernel<<<1, 1024, P * sizeof(unsigned long long), st>>>(keys, P);
+  } else {
+    bitonic_block_kernel<<<P / kBitonicBlock, 1024, 0, st>>>(keys, 2u, kBitonicBlock);
+    for (unsigned size = 2 * kBitonicBlock; size <= P && size != 0; size <<= 1) {
+      for (unsigned stride = size >> 1; stride > kBitonicBlock / 2; stride >>= 1)
+        bitonic_step_kernel<<<(P / 2 + threads - 1) / threads, threads, 0, st>>>(keys, P, size, stride);
+      bitonic_block_kernel<<<P / kBitonicBlock, 1024, 0, st>>>(keys, size, size);
+    }
+  }
+  topk_emit_kernel<<<(k + threads - 1) / threads, threads, 0, st>>>(keys, upsilon, k, idx, val);
+  return launched("top-k kernels");
+}
