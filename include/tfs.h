@@ -30,6 +30,16 @@
  * CUDA graphs: after one warm-up call with the same shapes and N_seg (scratch buffers and the piece table then exist),
  * tfs_eval / tfs_eval_tf / tfs_eval_tseg / tfs_topk / tfs_refine* with DEVICE buffers only enqueue kernels and memsets --
  * no allocation, copy or synchronisation -- and can be captured into a CUDA graph (stream capture) and replayed.
+ * A captured graph holds raw device addresses of context-owned memory (scratch buffers, the cached piece table of its
+ * (N_seg, seg_tranches), the data grid and its TMA descriptors).  They stay valid only while the context is left as the
+ * capture found it.  RE-CAPTURE the graph (after a new warm-up call) whenever one of these happened since:
+ *   - any tfs_upload_data / tfs_upload_timeseries on the context (the grid is rewritten, every piece table is dropped);
+ *   - any call on the context with a larger n, larger N_seg * n, more knots or other outputs than the captured one
+ *     (a scratch buffer may have been freed and re-allocated larger);
+ *   - calls with more than 64 distinct (N_seg, seg_tranches) pairs since the last upload (the piece-table cache is then
+ *     emptied and rebuilt);
+ *   - tfs_destroy.
+ * Replaying a stale graph reads freed or re-laid-out memory; the library cannot detect it.
  */
 #ifndef TFS_H
 #define TFS_H
@@ -127,7 +137,7 @@ TFS_API int tfs_upload_data(tfs_ctx* ctx, const float* coeff, const float* weigh
  *                (host or device), e.g. to draw the whitened spectrogram of Fig. 3
  * These weights are separable by construction (one PSD model per channel), so with weight_mode = 0 the library takes
  * the per-bin table b_a[k] = 4 DT / S_a[k] directly (tfs_weight_structure 1, or 2 without a PSD): the per-pixel array
- * W is only materialised when weight_out is given or weight_mode = 1.
+ * W is only materialised when weight_out is given, weight_mode = 1 or fresnel_mode = 1 (whose kernel reads per-pixel weights).
  * Nf must factor into 2, 3 and 5 (shared-memory FFT) and be <= 12800; basis 0 only.  Synchronises `stream`. */
 TFS_API int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_mask, const float* psd,
                                   double tukey_alpha, float* coeff_out, float* weight_out, uint8_t* gap_out,
@@ -146,17 +156,26 @@ TFS_API int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* s
  * 1 <= N_seg <= Nt.  Rows containing NaN/Inf or Mc <= 0 yield zeros and are counted
  * (tfs_bad_param_count), not fatal.  n == 0 is a no-op.  Arithmetic: fp64 track, fp32 pixels,
  * fp32 sums within a piece (<= 64 tranches of one segment), fp64 across pieces and segments, fp32 stores.
- * On a 1-channel context T_E is ignored; on a 3-channel context T_T = 0 (see tfs_eval_tf). */
+ * On a 1-channel context T_E is ignored.  The row has no column for a third channel: on a 3-channel context tfs_eval
+ * (and tfs_eval_tseg) return TFS_EINVAL until the caller has stated T_T with tfs_set_third_channel_factor, so that the
+ * paper's A, E, T sum (Eq. 3) never silently becomes a two-channel statistic. */
 TFS_API int tfs_eval(tfs_ctx* ctx, const double* params, long long n, int N_seg,
              float* upsilon, float* seg_power, float* seg_dh, float* seg_hh, void* stream);
+
+/* The third channel's transfer factor for tfs_eval / tfs_eval_tseg on a 3-channel context: one complex constant T_T for
+ * every template of the following calls (kept until set again).  (0, 0) is allowed and means "leave channel T out on
+ * purpose": the evaluation then costs what a 2-channel context costs; any other value adds a pass over the third
+ * channel.  Per-template or frequency-dependent factors go through tfs_eval_tf, which ignores this constant.
+ * TFS_EINVAL on a context with fewer than 3 channels or for a non-finite value. */
+TFS_API int tfs_set_third_channel_factor(tfs_ctx* ctx, double re, double im);
 
 /* The same evaluation with a frequency-dependent transfer factor per template (Eq. 7 and P:213 Eq. 29:
  * T_alpha(f_nm), "computed once per tranche for all frequency bins"): template i carries, for each of the
  * context's C channels, a table of n_knots complex values at the frequencies f_knot0 + j*f_knot_step; the factor
  * of tranche m is the table interpolated linearly at f_m (the tranche-start frequency, C6), held at the end
  * values outside the knots; n_knots == 1 means one constant per channel.  The columns T_A, T_E of `params` are
- * then ignored (they must still be finite).  This is also how the third channel gets a transfer factor: tfs_eval
- * on a 3-channel context uses T_A, T_E of `params` and T_T = 0.
+ * then ignored (they must still be finite).  This is also how the third channel gets a per-template transfer factor:
+ * tfs_eval on a 3-channel context uses T_A, T_E of `params` and the one constant of tfs_set_third_channel_factor.
  *   transfer [n][C][n_knots][2] float (re, im)       host or device, required
  *   1 <= n_knots <= 65536; f_knot_step > 0 [Hz] when n_knots > 1.
  * The factors are applied in fp32 once per tranche; everything else is as in tfs_eval. */

@@ -60,6 +60,8 @@ def load_library():
     lib.tfs_eval_tseg.restype = ip
     lib.tfs_topk.argtypes = [vp, vp, ll, ip, vp, vp, vp]
     lib.tfs_topk.restype = ip
+    lib.tfs_set_third_channel_factor.argtypes = [vp, dp, dp]
+    lib.tfs_set_third_channel_factor.restype = ip
     lib.tfs_topk_static.argtypes = [vp, ll, ip, vp, vp, vp]
     lib.tfs_topk_static.restype = ip
     lib.tfs_refine.argtypes = [vp, vp, ll, vp, ll, ip, dp, dp, vp, vp]
@@ -185,6 +187,9 @@ class Tfs:
                                           _ptr(upsilon, np.float32, n), _ptr(seg_power, np.float32, n * N_seg),
                                           _ptr(seg_dh, np.float32, 2 * n * N_seg),
                                           _ptr(seg_hh, np.float32, n * N_seg), _stream(stream)))
+
+    def set_third_channel_factor(self, re, im=0.0):
+        self._check(self._lib.tfs_set_third_channel_factor(self._h, float(re), float(im)))
 
     def topk(self, upsilon, k, idx, val, n=None, stream=None):
         if n is None:

@@ -45,6 +45,8 @@ struct tfs_ctx {
   int ncol_cap = 0, ncol = 0;              // columns allocated per row (Nt rounded up to kTS), columns in use
   float2* colmax = nullptr;                // [Nf] scratch of the weight analysis
   unsigned long long* wcounts = nullptr;   // [2] {pixels violating W = a b, columns with b != 1}
+  bool t3_set = false;                     // tfs_set_third_channel_factor was called (3-channel contexts)
+  double t3[2] = {0.0, 0.0};               // constant T_T of the third channel for tfs_eval / tfs_eval_tseg
   int wmode = -1;                          // kWGeneral / kWSeparable / kWTimeOnly; -1 before the first upload
   int n_valid = 0;                         // valid (non-gap) tranches of the data uploaded last
   // piece tables (tile x segment cuts of the valid-tranche list), cached per N_seg until the next upload
@@ -715,7 +717,9 @@ int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_ma
   auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
   // the per-pixel weight array is only materialised when the caller wants it back or forces the general path:
   // W[a,m,k] = b_a[k] is separable by construction, so the upload takes the table b directly
-  const bool need_w = weight_out != nullptr || ctx->opts.weight_mode != 0;
+  // (fresnel_mode 1 always evaluates with the general-weight kernel, which reads the per-pixel array: it needs it too)
+  const bool per_pixel_w = ctx->opts.weight_mode != 0 || ctx->opts.fresnel_mode != 0;
+  const bool need_w = weight_out != nullptr || per_pixel_w;
   const size_t sz[7] = {copy_x ? al(C * nsamp * sizeof(float)) : 0, copy_mask ? al(nsamp) : 0,
                         copy_psd ? al((size_t)C * Nf * sizeof(float)) : 0, al((size_t)(rad.total + 2) * sizeof(float2)),
                         al((size_t)N * sizeof(float)), al(C * npix * sizeof(float2)), need_w ? al(C * npix * sizeof(float)) : 0};
@@ -774,7 +778,7 @@ int tfs_upload_timeseries(tfs_ctx* ctx, const float* x, const uint8_t* sample_ma
 #undef FE_CUDA
   // the rest is the ordinary upload, from device buffers (it synchronises the stream before returning); with the
   // default weight_mode the weights go in as the per-bin table (no per-pixel array is read or analysed)
-  if (ctx->opts.weight_mode != 0) return upload_impl(ctx, (const float*)d_coeff, d_weight, d_gap, stream, false, nullptr);
+  if (per_pixel_w) return upload_impl(ctx, (const float*)d_coeff, d_weight, d_gap, stream, false, nullptr);
   return upload_impl(ctx, (const float*)d_coeff, nullptr, d_gap, stream, true, d_psd ? d_bk : nullptr);
 }
 
@@ -801,6 +805,9 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
   if (transfer && ctx->opts.basis == 1) return fail(ctx, TFS_EINVAL, "%s: transfer tables are not available in the WDM basis", who);
   if (transfer && (n_knots < 1 || n_knots > 65536 || !std::isfinite(f_knot0) || (n_knots > 1 && !(f_knot_step > 0.0))))
     return fail(ctx, TFS_EINVAL, "%s: transfer table needs 1 <= n_knots <= 65536, finite f_knot0 and f_knot_step > 0", who);
+  if (ctx->C == 3 && !transfer && !ctx->t3_set)
+    return fail(ctx, TFS_EINVAL, "%s: the parameter row has no column for the third channel's transfer factor: declare it with "
+                                 "tfs_set_third_channel_factor (0, 0 drops the channel) or pass a table to tfs_eval_tf", who);
   int rc = check_device(ctx, who);
   if (rc) return rc;
   if (n == 0) { ctx->bad_host = 0; return TFS_OK; }
@@ -879,8 +886,10 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
 
   TFS_CUDA(ctx, cudaMemsetAsync(ctx->bad, 0, sizeof(unsigned long long), st));
   const int wm = ctx->opts.fresnel_mode != 0 ? kWGeneral : ctx->wmode;
-  // channel pairs to run: the pair of channel 2 only when a table can give it a transfer factor (T_T = 0 otherwise)
-  const int n_pass = (ctx->n_pairs == 2 && d_ttab) ? 2 : 1;
+  // channel pairs to run: the pair of channel 2 only when it has a transfer factor -- from the table, or the context's
+  // constant T_T when that is not zero
+  const bool t3_const = !d_ttab && (ctx->t3[0] != 0.0 || ctx->t3[1] != 0.0);
+  const int n_pass = (ctx->n_pairs == 2 && (d_ttab || t3_const)) ? 2 : 1;
   for (long long off = 0; off < n; off += sub) {
     const long long nb = std::min(sub, n - off);
     for (int pass = 0; pass < n_pass; ++pass) {
@@ -896,6 +905,7 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
       a.units_list = (Unit*)part[6]; a.n_units = (int*)part[7];
       a.accumulate = pass;
       a.t_col = pass == 0 ? 3 : -1;
+      a.t3_re = ctx->t3[0]; a.t3_im = ctx->t3[1];
       if (pass > 0) a.bad_count = nullptr;
       if (d_ttab) {
         a.ttab = d_ttab + (size_t)off * C * n_knots;
@@ -1214,6 +1224,14 @@ int tfs_probe_l2_bandwidth(tfs_ctx* ctx, long long bytes, int iters, double* gb_
   if ((e = cudaEventElapsedTime(&ms, e0, e1)) != cudaSuccess) return done(TFS_ECUDA, "cudaEventElapsedTime", e);
   *gb_per_s = (double)n_vec * 16.0 * iters / (ms * 1e-3) / 1e9;
   return done(rc, "", cudaSuccess);
+}
+
+int tfs_set_third_channel_factor(tfs_ctx* ctx, double re, double im) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_set_third_channel_factor: ctx is NULL");
+  if (ctx->C != 3) return fail(ctx, TFS_EINVAL, "tfs_set_third_channel_factor: the context has %d channels, not 3", ctx->C);
+  if (!std::isfinite(re) || !std::isfinite(im)) return fail(ctx, TFS_EINVAL, "tfs_set_third_channel_factor: the factor must be finite");
+  ctx->t3[0] = re; ctx->t3[1] = im; ctx->t3_set = true;
+  return TFS_OK;
 }
 
 int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k, long long* idx, float* val, void* stream) {

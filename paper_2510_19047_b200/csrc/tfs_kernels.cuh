@@ -115,6 +115,7 @@ struct EvalArgs {
   double wdm_DTpix;                    // WDM pixel duration Nf dt (DT above is then 2 Nf dt = 1/DF)
   int accumulate;                      // 1: add to the partials instead of overwriting them (second channel pair)
   int t_col;                           // params columns of the pair's first transfer factor (3: T_A, T_E)
+  double t3_re, t3_im;                 // t_col < 0 (the pair of channel 2, no table): the context's constant T_T (tfs_set_third_channel_factor)
   int n_ch_pair;                       // channels in this pair (1 or 2)
   long long n;                         // templates in this launch
   int Nt, Nf, ncol;
@@ -1345,7 +1346,8 @@ eval_list_kernel(const EvalArgs a) {
 __global__ void prep_consts_kernel(const EvalArgs a) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= a.n) return;
-  const TplConst t = load_template(a.params + i * 8, a.DT, a.t_col, a.n_ch_pair);
+  TplConst t = load_template(a.params + i * 8, a.DT, a.t_col, a.n_ch_pair);
+  if (a.t_col < 0 && t.ok) { t.T0r = (float)a.t3_re; t.T0i = (float)a.t3_im; }
   a.tconst[i] = t;
   if (a.bad_count != nullptr && !t.ok) atomicAdd(a.bad_count, 1ULL);
 }

@@ -25,9 +25,27 @@ class TileResult:
 
 
 def search_tile(ctx: api.Tfs, tile, row, n_mc: int, n_fin: int, stages=(16, 4, 1), keep: int = 8, r: int = 4,
-                max_extra: int = 3, tol: float = 1e-3, stream=None) -> TileResult:
-    """tile = (mc_lo, mc_hi, fin_lo, fin_hi) in Msun and Hz; ``row`` [8] gives the columns the lattice does not span."""
+                max_extra: int = 3, tol: float = 1e-3, stream=None, transfer=None) -> TileResult:
+    """tile = (mc_lo, mc_hi, fin_lo, fin_hi) in Msun and Hz; ``row`` [8] gives the columns the lattice does not span.
+
+    ``transfer`` = (table [C][K][2] float32, f_knot0, f_knot_step): one transfer table shared by every template of the
+    tile (sky position and polarisation are fixed by ``row``), evaluated with ``tfs_eval_tf`` -- the way a 3-channel
+    context gets its T_T(f); without it the search calls ``tfs_eval`` (on a 3-channel context that needs
+    ``set_third_channel_factor`` first).
+
+    ``stream``: a raw CUDA stream handle.  The whole search -- library calls, the tensors allocated here and the two
+    scalars read back per level -- then runs with that stream as torch's current stream, so the caching allocator and
+    the ``.item()`` reads are ordered with the library's kernels."""
+    if stream is not None:
+        with torch.cuda.stream(torch.cuda.ExternalStream(int(stream))):
+            return search_tile(ctx, tile, row, n_mc, n_fin, stages, keep, r, max_extra, tol, None, transfer)
     dev = torch.device("cuda", torch.cuda.current_device())
+    tab = None
+    if transfer is not None:
+        tab, f_knot0, f_knot_step = transfer
+        tab = torch.as_tensor(np.ascontiguousarray(tab, dtype=np.float32) if isinstance(tab, np.ndarray) else tab,
+                              device=dev).to(torch.float32)
+        n_knots = int(tab.shape[1])
     mc_lo, mc_hi, fin_lo, fin_hi = (float(v) for v in tile)
     d_mc, d_fin = (mc_hi - mc_lo) / n_mc, (fin_hi - fin_lo) / n_fin
     cur = torch.empty((n_mc * n_fin, api.PARAM_COLS), dtype=torch.float64, device=dev)
@@ -38,7 +56,11 @@ def search_tile(ctx: api.Tfs, tile, row, n_mc: int, n_fin: int, stages=(16, 4, 1
         N_seg = stages[min(lev, len(stages) - 1)]
         n = cur.shape[0]
         ups = torch.empty(n, dtype=torch.float32, device=dev)
-        ctx.eval(cur, N_seg, ups, stream=stream)
+        if tab is None:
+            ctx.eval(cur, N_seg, ups, stream=stream)
+        else:
+            ctx.eval_tf(cur, N_seg, tab.unsqueeze(0).expand(n, *tab.shape).contiguous(), n_knots, float(f_knot0),
+                        float(f_knot_step), ups, stream=stream)
         k = min(n, keep)
         idx = torch.empty(k, dtype=torch.int64, device=dev)
         val = torch.empty(k, dtype=torch.float32, device=dev)

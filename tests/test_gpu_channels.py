@@ -50,11 +50,52 @@ def test_constant_factors_per_channel_count(api, C, kind):
     ctx = api.Tfs(w.Nt, w.Nf, w.dt, C)
     ctx.upload_data(coeff, weight, gap)
     assert ctx.weight_structure() == {"time": 2, "product": 1, "general": 0}[kind]
+    if C == 3:
+        # the row has no column for T_T: tfs_eval refuses until the caller states it (never a silent 2-channel statistic)
+        with pytest.raises(api.TfsError) as e:
+            api.eval_host(ctx, params, 1)
+        assert e.value.code == api.TFS_EINVAL and "tfs_set_third_channel_factor" in str(e.value)
+        ctx.set_third_channel_factor(0.0, 0.0)                         # channel T left out on purpose
     for N_seg in (1, 9):
         gpu = api.eval_host(ctx, params, N_seg)
         ora = _oracle(params, coeff, weight, gap, w, N_seg)            # three channels: T_T = 0
         r = assert_parity(gpu, ora, N_seg, label=f"C={C} {kind} N_seg={N_seg}")
         assert r["n_active"] >= 30
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("kind", ["time", "product", "general"])
+def test_third_channel_constant_factor(api, kind):
+    """A, E, T with constant factors (Eq. 3): T_A, T_E from the row, T_T from tfs_set_third_channel_factor,
+    against the oracle's evaluate_tf with one-knot tables holding the same three constants; tfs_eval_tseg takes the
+    same constant; a table passed to tfs_eval_tf overrides it."""
+    w, coeff, weight, gap, params = _data(3, kind=kind, seed=77)
+    n = len(params)
+    t3 = 0.4 - 0.7j
+    tables = np.empty((n, 3, 1, 2))
+    tables[:, 0, 0, 0], tables[:, 0, 0, 1] = params[:, 3], params[:, 4]
+    tables[:, 1, 0, 0], tables[:, 1, 0, 1] = params[:, 5], params[:, 6]
+    tables[:, 2, 0, 0], tables[:, 2, 0, 1] = t3.real, t3.imag
+    ctx = api.Tfs(w.Nt, w.Nf, w.dt, 3)
+    ctx.upload_data(coeff, weight, gap)
+    ctx.set_third_channel_factor(t3.real, t3.imag)
+    two = _oracle(params, coeff, weight, gap, w, 1)["upsilon"]
+    for N_seg in (1, 6):
+        gpu = api.eval_host(ctx, params, N_seg)
+        ora = _oracle(params, coeff, weight, gap, w, N_seg, tables, 0.0, 1.0)
+        r = assert_parity(gpu, ora, N_seg, label=f"A,E,T constant {kind} N_seg={N_seg}")
+        assert r["n_active"] >= 30
+    assert np.max(np.abs(_oracle(params, coeff, weight, gap, w, 1, tables, 0.0, 1.0)["upsilon"] - two)) > 0.1   # T matters
+    # fixed-duration segments: Nt = 300, 50 tranches per segment == N_seg = 6 (the equal-index rule, P15)
+    ts = api.eval_tseg_host(ctx, params, 50)
+    assert_parity(ts, ora, 6, label=f"A,E,T constant {kind} tseg")
+    # a table overrides the constant
+    tab2 = np.random.default_rng(5).standard_normal((n, 3, 3, 2)).astype(np.float32)
+    gpu = api.eval_host(ctx, params, 6, transfer=tab2, f_knot0=4e-3, f_knot_step=0.03)
+    ora2 = _oracle(params, coeff, weight, gap, w, 6, tab2.astype(np.float64), 4e-3, 0.03)
+    assert_parity(gpu, ora2, 6, label=f"A,E,T table over constant {kind}")
+    with pytest.raises(api.TfsError):
+        api.Tfs(w.Nt, w.Nf, w.dt, 2).set_third_channel_factor(1.0, 0.0)
     ctx.destroy()
 
 

@@ -154,3 +154,31 @@ def test_non_finite_samples_drop_their_tranche(api):
     r2 = api.eval_host(ctx, synth.make_templates(w), 2)
     assert np.array_equal(r["upsilon"], r2["upsilon"]) and not np.array_equal(r["upsilon"], ref["upsilon"])
     ctx.destroy()
+
+
+def test_time_series_upload_with_paper_fresnel_mode(api):
+    """fresnel_mode = 1 always evaluates with the per-pixel-weight kernel, so tfs_upload_timeseries must materialise W
+    even with weight_mode = 0 and no weight_out (it once took the per-bin-table shortcut and left W unwritten).  A first
+    upload with different weights on the same context makes stale weights visible if the second upload skips W.
+    Tolerance 2e-3 as in test_paper_fresnel_mode (the printed approximants' branch discontinuity, reading C8)."""
+    w = synth.scaled(synth.WORKLOADS["cfg1"], Nt=64, Nf=512, n_templates=24)
+    x, mask, psd = synth.make_timeseries(w)
+    g = O.Grid(w.Nt, w.Nf, w.dt)
+    params = synth.make_templates(w)
+    ctx = api.Tfs(w.Nt, w.Nf, w.dt, fresnel_mode=1)
+    ctx.upload_timeseries(x, mask, np.ascontiguousarray(psd * 7.0), tukey_alpha=0.1)      # stale weights: 1/7 of the right ones
+    ctx.upload_timeseries(x, mask, psd, tukey_alpha=0.1)
+    Do, Wo, go = F.frontend(x, w.Nt, w.Nf, w.dt, sample_mask=mask, psd=psd, tukey_alpha=0.1)
+    for N_seg in (1, 4):
+        gpu = api.eval_host(ctx, params, N_seg)
+        ora = O.evaluate(params, Do, Wo, go, g, N_seg, O.Opts(fresnel_mode=1))
+        r = assert_parity(gpu, ora, N_seg, tol=2e-3, label=f"time series, fresnel_mode=1, N_seg={N_seg}")
+        assert r["n_active"] >= 12
+    ctx.destroy()
+    ctx = api.Tfs(w.Nt, w.Nf, w.dt, fresnel_mode=1)                                       # and without a PSD: W = 1
+    ctx.upload_timeseries(x, mask, None, tukey_alpha=0.0)
+    Do, Wo, go = F.frontend(x, w.Nt, w.Nf, w.dt, sample_mask=mask, psd=None, tukey_alpha=0.0)
+    gpu = api.eval_host(ctx, params, 2)
+    ora = O.evaluate(params, Do, Wo, go, g, 2, O.Opts(fresnel_mode=1))
+    assert_parity(gpu, ora, 2, tol=2e-3, label="time series, fresnel_mode=1, no PSD")
+    ctx.destroy()

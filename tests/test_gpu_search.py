@@ -84,3 +84,45 @@ def test_tile_search_recovers_an_injection_like_the_oracle(api):
     res = search.search_tiles(ctx, [tile, far], ROW, 6, 12, **kw)
     assert res[0].upsilon == gpu.upsilon and res[1].upsilon == quiet.upsilon           # deterministic
     ctx.destroy()
+
+
+def test_tile_search_with_a_shared_transfer_table_and_on_a_side_stream(api):
+    """search_tile(transfer=...) routes through tfs_eval_tf with one table for the whole tile: a one-knot table holding
+    ROW's own (T_A, T_E) must reproduce the plain search (factors applied in fp32 either way); on a 3-channel context it
+    is the way to T_T.  With stream= the search runs on that stream (allocations and read-backs ordered with it) and
+    returns the same numbers."""
+    import torch
+    from paper_2510_19047_b200 import search
+    g = O.Grid(48, 256, 40.0)
+    rng = np.random.default_rng(22)
+    coeff = rng.standard_normal((3, g.Nt, g.Nf, 2)).astype(np.float32)
+    Mc, fin = 27.3, 8.037e-3
+    inj = ROW.copy(); inj[0] = Mc; inj[1] = float(S.tau_of_f(Mc, fin))
+    sig = O.injection(inj, 25.0, np.ones((2, g.Nt, g.Nf)), None, g)
+    coeff[:2, ..., 0] += sig.real.astype(np.float32)
+    coeff[:2, ..., 1] += sig.imag.astype(np.float32)
+    tile = (25.0, 30.0, 8.0e-3, 8.1e-3)
+    kw = dict(stages=(4, 1), keep=6, r=3, max_extra=2, tol=1e-3)
+    ctx = api.Tfs(g.Nt, g.Nf, g.dt)
+    ctx.upload_data(np.ascontiguousarray(coeff[:2]), None, None)
+    plain = search.search_tile(ctx, tile, ROW, 6, 12, **kw)
+    tab2 = np.array([[[ROW[3], ROW[4]]], [[ROW[5], ROW[6]]]], dtype=np.float32)
+    with_tab = search.search_tile(ctx, tile, ROW, 6, 12, transfer=(tab2, 0.0, 1.0), **kw)
+    assert abs(with_tab.upsilon - plain.upsilon) <= 1e-5 * plain.upsilon and np.array_equal(with_tab.params, plain.params)
+    side = torch.cuda.Stream()
+    on_side = search.search_tile(ctx, tile, ROW, 6, 12, stream=side.cuda_stream, **kw)
+    side.synchronize()
+    assert on_side.upsilon == plain.upsilon and np.array_equal(on_side.params, plain.params)
+    ctx.destroy()
+    # three channels: the plain search is refused until T_T is stated; a table with T_T = 0 equals the 2-channel search
+    ctx3 = api.Tfs(g.Nt, g.Nf, g.dt, 3)
+    ctx3.upload_data(coeff, None, None)
+    with pytest.raises(api.TfsError):
+        search.search_tile(ctx3, tile, ROW, 6, 12, **kw)
+    tab3 = np.concatenate([tab2, np.zeros((1, 1, 2), dtype=np.float32)])
+    three = search.search_tile(ctx3, tile, ROW, 6, 12, transfer=(tab3, 0.0, 1.0), **kw)
+    assert abs(three.upsilon - plain.upsilon) <= 1e-5 * plain.upsilon
+    tab3[2, 0] = (0.8, 0.1)                                    # noise-only third channel with weight: the statistic moves
+    moved = search.search_tile(ctx3, tile, ROW, 6, 12, transfer=(tab3, 0.0, 1.0), **kw)
+    assert moved.upsilon != three.upsilon and moved.upsilon > 0.5 * plain.upsilon
+    ctx3.destroy()
