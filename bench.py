@@ -114,6 +114,28 @@ def _oracle_one(i):
     return float(r["upsilon"][0]), int((r["seg_hh"][0] > 0).sum())
 
 
+def _sparse_eval(p, g, o, seg, coeff, weight, gap, N_seg):
+    """Upsilon of one template from its window pixels only, with the oracle's track, kernel and combine routines."""
+    from oracle import tfs_oracle as O
+    tr = O.track(p[0], p[1], p[2], p[7], g, o, gap)
+    ms = np.nonzero(tr["active"])[0]
+    z = np.zeros(N_seg, dtype=np.complex128)
+    hh = np.zeros(N_seg)
+    if ms.size:
+        lo, hi = tr["k_lo"][ms], tr["k_hi"][ms]
+        mm = np.repeat(ms, hi - lo + 1)
+        kk = np.concatenate([np.arange(a, b + 1) for a, b in zip(lo, hi)])
+        H = O.kernel_pixels(tr["x"][mm], tr["c"][mm], tr["phi"][mm], tr["A"][mm], kk)
+        T = (p[3] + 1j * p[4], p[5] + 1j * p[6])
+        for a in range(2):
+            D = coeff[a, mm, kk, 0].astype(np.float64) + 1j * coeff[a, mm, kk, 1]
+            Wp = weight[a, mm, kk].astype(np.float64)
+            z += T[a] * (np.bincount(seg[mm], weights=(Wp * np.conj(D) * H).real, minlength=N_seg) +
+                         1j * np.bincount(seg[mm], weights=(Wp * np.conj(D) * H).imag, minlength=N_seg))
+            hh += abs(T[a]) ** 2 * np.bincount(seg[mm], weights=Wp * np.abs(H) ** 2, minlength=N_seg)
+    return float(O.combine(z, hh)[1])
+
+
 def sparse_cpu_rate(w, coeff, weight, gap, params, N_seg, budget_s=6.0):
     """The analogue of the paper's single-core CPU curve (Fig. 1): the same statistic evaluated
     on the track's window pixels only, one template at a time on ONE core, with the oracle's own track,
@@ -126,27 +148,36 @@ def sparse_cpu_rate(w, coeff, weight, gap, params, N_seg, budget_s=6.0):
     t0 = time.perf_counter()
     done = 0
     for p in params:
-        tr = O.track(p[0], p[1], p[2], p[7], g, o, gap)
-        ms = np.nonzero(tr["active"])[0]
-        z = np.zeros(N_seg, dtype=np.complex128)
-        hh = np.zeros(N_seg)
-        if ms.size:
-            lo, hi = tr["k_lo"][ms], tr["k_hi"][ms]
-            mm = np.repeat(ms, hi - lo + 1)
-            kk = np.concatenate([np.arange(a, b + 1) for a, b in zip(lo, hi)])
-            H = O.kernel_pixels(tr["x"][mm], tr["c"][mm], tr["phi"][mm], tr["A"][mm], kk)
-            T = (p[3] + 1j * p[4], p[5] + 1j * p[6])
-            for a in range(2):
-                D = coeff[a, mm, kk, 0].astype(np.float64) + 1j * coeff[a, mm, kk, 1]
-                Wp = weight[a, mm, kk].astype(np.float64)
-                z += T[a] * (np.bincount(seg[mm], weights=(Wp * np.conj(D) * H).real, minlength=N_seg) +
-                             1j * np.bincount(seg[mm], weights=(Wp * np.conj(D) * H).imag, minlength=N_seg))
-                hh += abs(T[a]) ** 2 * np.bincount(seg[mm], weights=Wp * np.abs(H) ** 2, minlength=N_seg)
-        O.combine(z, hh)
+        _sparse_eval(p, g, o, seg, coeff, weight, gap, N_seg)
         done += 1
         if time.perf_counter() - t0 > budget_s:
             break
     return done / (time.perf_counter() - t0), done
+
+
+def _sparse_one(i):
+    d = _ORA
+    return _sparse_eval(d["params"][i], d["grid"], d["opts"], d["seg"], d["coeff"], d["weight"], d["gap"], d["N_seg"])
+
+
+def sparse_cpu_rate_mp(w, coeff, weight, gap, params, N_seg, procs):
+    """The window-sparse CPU evaluation on `procs` processes (fork; call BEFORE CUDA init): the fairest CPU line this
+    bench prints -- what a multi-core CPU implementation that, like the GPU path, touches the window pixels only would
+    reach with numpy.  Returns (templates/s, seconds, [Upsilon])."""
+    import multiprocessing as mp
+    from oracle import tfs_oracle as O
+    _ORA.update(params=params, coeff=coeff, weight=weight, gap=gap, grid=O.Grid(w.Nt, w.Nf, w.dt), opts=O.Opts(),
+                seg=O.segment_of_bin(np.arange(w.Nt), w.Nt, N_seg), N_seg=N_seg)
+    idx = list(range(len(params)))
+    t0 = time.perf_counter()
+    if procs > 1:
+        with mp.get_context("fork").Pool(procs) as pool:
+            ups = pool.map(_sparse_one, idx, chunksize=max(1, len(idx) // (8 * procs)))
+    else:
+        ups = [_sparse_one(i) for i in idx]
+    dt = time.perf_counter() - t0
+    _ORA.clear()
+    return len(idx) / dt, dt, ups
 
 
 def oracle_throughput(w, coeff, weight, gap, params, N_seg, n_sample, procs):
@@ -326,7 +357,7 @@ def main_wdm(args, info, w, n, N_seg, k_top, cfg):
     kern_ms = (prof["slab_kernel_ms"] + prof["list_kernel_ms"]) / n_launch
     bytes_per_launch = 8.0 * 2 * pixels / (n_launch / args.steps)
     achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
-    line = {"metric": "templates/sec", "value": world * n / (leg["ms_step"] * 1e-3), "unit": "templates/s", "n_gpus": world,
+    line = {"metric": "templates/sec", "value": replicas.aggregate_rate(n, leg["ms_step"] * 1e-3, info), "unit": "templates/s", "n_gpus": world,
             "steps": args.steps, "warmup": warm, "ms_per_step": leg["ms_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
             "pixel_evals_per_sec": world * 2 * pixels / (leg["ms_step"] * 1e-3), "pixel_evals_per_template": 2 * pixels / n,
@@ -338,7 +369,7 @@ def main_wdm(args, info, w, n, N_seg, k_top, cfg):
                          "note": "a first kernel for this basis: four table look-ups and two fp64 phase reductions per pixel; "
                                  "it is instruction-bound, far from the byte roof"},
             "cpu_baseline": cpu_baseline, "parity": parity,
-            "e2e": {"value": world * n / (ms_e2e * 1e-3), "unit": "templates/s", "h2d_bytes_per_step": int(params.nbytes),
+            "e2e": {"value": replicas.aggregate_rate(n, ms_e2e * 1e-3, info), "unit": "templates/s", "h2d_bytes_per_step": int(params.nbytes),
                     "d2h_bytes_per_step": int(4 * n + 12 * k_top), "ms_per_step": ms_e2e},
             "gpu_launches": int(prof["kernel_launches"]), "clocks": leg["clocks"]}
     print(json.dumps(line))
@@ -428,13 +459,23 @@ def main():
         ns = args.cpu_sample or 64 * procs      # ~60 s of CPU work at cfg3 on 16 cores (why not 4096)
         r, dt, ora = oracle_throughput(w, coeff, weight, gap, params[:ns], N_seg, ns, procs)   # before CUDA init
         sp_rate, sp_n = sparse_cpu_rate(w, coeff, weight, gap, params[:ns], N_seg)
+        mp_rate, mp_dt, mp_ups = sparse_cpu_rate_mp(w, coeff, weight, gap, params[:ns], N_seg, procs)
+        dense_ups = np.array([u for u, _ in ora])
+        mp_err = float(np.max(np.abs(np.array(mp_ups) - dense_ups) / np.maximum(dense_ups, 2.0 * N_seg)))
         cpu_baseline = {"value": r, "unit": "templates/s", "cores": procs, "kind": "oracle",
                         "sample": f"first {ns} templates of the bank, {dt:.1f} s wall (dense fp64 oracle, {procs} "
                                   f"processes of {cores} cores)",
                         "sparse_single_core": {"value": sp_rate, "unit": "templates/s", "cores": 1, "templates": sp_n,
                                                "what": "window pixels only, one template at a time with the oracle's "
                                                        "track/kernel routines (analogue of the paper's Fig. 1 CPU "
-                                                       "curve, P:243); not the oracle"}}
+                                                       "curve, P:243); not the oracle"},
+                        "sparse_multi_core": {"value": mp_rate, "unit": "templates/s", "cores": procs, "templates": ns,
+                                              "seconds": mp_dt, "max_err_vs_dense_oracle": mp_err,
+                                              "what": "the same window-sparse evaluation on all the processes the dense "
+                                                      "oracle used, checked against the dense oracle's Upsilon on every "
+                                                      "template of the sample: the CPU figure to compare the GPU arm "
+                                                      "with (the dense oracle above sums over every pixel of the grid "
+                                                      "and is slow by construction)"}}
 
     import torch
     from paper_2510_19047_b200 import api, build
@@ -531,7 +572,7 @@ def main():
     prof = leg["prof"]
     n_launch = max(prof["eval_launches"], 1)
     line = {
-        "metric": "templates/sec", "value": world * n / (ms_step * 1e-3), "unit": "templates/s",
+        "metric": "templates/sec", "value": replicas.aggregate_rate(n, ms_step * 1e-3, info), "unit": "templates/s",
         "n_gpus": world, "steps": args.steps, "warmup": warm, "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "config": cfg,
@@ -551,7 +592,7 @@ def main():
                      "terms": terms},
         "cpu_baseline": cpu_baseline,
         "parity": parity,
-        "e2e": {"value": world * n / (ms_e2e * 1e-3), "unit": "templates/s",
+        "e2e": {"value": replicas.aggregate_rate(n, ms_e2e * 1e-3, info), "unit": "templates/s",
                 "h2d_bytes_per_step": int(params.nbytes + h_ups.numpy().nbytes),
                 "d2h_bytes_per_step": int(h_ups.numpy().nbytes + h_idx.numpy().nbytes + h_val.numpy().nbytes),
                 "ms_per_step": ms_e2e, "matches_device_path": same},

@@ -29,14 +29,6 @@ def bank_seed(base_seed: int, rank: int) -> int:
     return base_seed + 7919 * rank
 
 
-def shard_bounds(n_total: int, rank: int, world: int):
-    """[lo, hi) of rank's share when a fixed bank of n_total templates is split (strong scaling
-    helper; the bench uses weak scaling, one full bank per rank)."""
-    base, rem = divmod(n_total, world)
-    lo = rank * base + min(rank, rem)
-    return lo, lo + base + (1 if rank < rem else 0)
-
-
 def init(info: RankInfo, backend: str, device=None):
     """Join the process group (no-op for world == 1).  Rendezvous comes from MASTER_ADDR/PORT."""
     if info.world == 1:

@@ -55,12 +55,3 @@ def test_single_rank_is_a_noop():
     replicas.barrier(info)
     assert replicas.max_over_ranks(3.25, info) == 3.25
     assert replicas.bank_seed(5, 0) == 5
-
-
-def test_shard_bounds_cover_exactly():
-    for n, world in [(10, 3), (7, 8), (1 << 20, 8), (0, 2)]:
-        b = [replicas.shard_bounds(n, r, world) for r in range(world)]
-        assert b[0][0] == 0 and b[-1][1] == n
-        assert all(b[i][1] == b[i + 1][0] for i in range(world - 1))
-        sizes = np.array([hi - lo for lo, hi in b])
-        assert sizes.max() - sizes.min() <= 1
