@@ -174,3 +174,50 @@ def test_w_time_domain_chirp_is_recovered():
     rho2 = float(np.sum(D[:, act, 1:] ** 2))                                 # time-domain SNR^2 over the pixels the template uses
     r = Wd.evaluate(q[None], D, ones, None, g, 1)
     assert math.sqrt(r["upsilon"][0] / rho2) > 0.98
+
+
+def _K_steepest_descent(x, kappa):
+    """K(x, kappa) = e^{i pi/4}/sqrt(kappa) int_{-1}^{1} cos(pi y/2) exp(-i pi (y + x)^2/kappa) dy (W4's definition)
+    by numerical steepest descent in mpmath: with w = y + x the integrand is entire, so the real segment is deformed
+    into the paths of constant phase leaving each end point (w^2 = w_a^2 - i p, p >= 0, on which the exponential is
+    exp(-i pi w_a^2/kappa) exp(-pi p/kappa)) plus, when the stationary point w = 0 lies between the end points, the
+    straight line w = sqrt(kappa) e^{-i pi/4} s through it.  Every piece is a smooth decaying integral whatever kappa
+    is; no Fresnel function and no completed square appear, so it shares nothing with the closed form it checks."""
+    import mpmath as mp
+    mp.mp.dps = 30
+    x, kap = mp.mpf(x), mp.mpf(kappa)
+
+    def endpoint(a):
+        wa = a + x
+        sg = 1 if wa > 0 else -1
+
+        def f(q):                                                   # p = kappa q
+            w = sg * mp.sqrt(wa * wa - 1j * kap * q)
+            return mp.cos(mp.pi * (w - x) / 2) * mp.exp(-mp.pi * q) * (-1j * kap) / (2 * w)
+        return mp.exp(-1j * mp.pi * wa * wa / kap) * mp.quad(f, [0, 1, 4, 16, mp.inf]), sg
+
+    (Ilo, slo), (Ihi, shi) = endpoint(mp.mpf(-1)), endpoint(mp.mpf(1))
+    tot = Ilo - Ihi
+    if slo != shi:
+        c = mp.sqrt(kap) * mp.exp(-0.25j * mp.pi)
+        tot += mp.quad(lambda s: mp.cos(mp.pi * (c * s - x) / 2) * mp.exp(-mp.pi * s * s) * c, [-mp.inf, -2, 0, 2, mp.inf])
+    return complex(tot * mp.exp(0.25j * mp.pi) / mp.sqrt(kap))
+
+
+def test_w_response_closed_form_for_slow_chirps_by_steepest_descent():
+    """Below kappa = 0.02 the oracle returns chirp_response_closed, the same Fresnel closed form the CUDA path
+    evaluates, and the plain quadrature of the definition is only affordable down to kappa ~ 1e-3.  Slow chirps
+    (c = 1e-4 ... 1e-3 give kappa = 4e-4 ... 4e-3, and the bank reaches 1e-6) are pinned here against an evaluation of
+    the SAME defining integral that works at any kappa and uses neither Fresnel integrals nor the completed square.
+    First the pin is itself checked against the Gauss-Legendre quadrature where that is cheap."""
+    xs = [-2.3, -1.2, -0.999, -0.4, 0.013, 0.77, 1.0001, 1.9]          # inside, outside and at the edges of the window
+    quad = Wd.chirp_response(np.array(xs), 0.5)
+    assert np.abs(np.array([_K_steepest_descent(x, 0.5) for x in xs]) - quad).max() < 1e-12
+    for kap in (4e-3, 1e-4, 1e-5, 1e-6):
+        ref = np.array([_K_steepest_descent(x, kap) for x in xs])
+        assert np.abs(Wd.chirp_response_closed(np.array(xs), kap) - ref).max() < 2e-12, kap
+        assert np.array_equal(Wd.chirp_response(np.array(xs), kap), Wd.chirp_response_closed(np.array(xs), kap))
+    # and the tone limit the oracle switches to below 1e-9 is what the integral tends to
+    lim = Wd.chirp_response(np.array(xs), 1e-10)
+    # (next to the window's edges |x| = 1 the end-point term is O(sqrt(kappa)) times the window's slope: 3e-6 at 1e-8)
+    assert np.abs(np.array([_K_steepest_descent(x, 1e-8) for x in xs]) - lim).max() < 1e-5
