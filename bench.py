@@ -35,6 +35,11 @@ ALG_BYTES_PER_PIXEL_EVAL = {0: 12.0, 1: 8.0, 2: 8.0}
 # 10 packed for the two auxiliary-function polynomials (20), h' = Godd(v0) - E Godd(v1) (4 scalar FMA),
 # z_A, z_E (4 packed: 8), |h'|^2 and q (1 packed: 2), u + c and u - 1 (2)  ->  36; + 2 MUFU.RCP (own pipe).
 ALG_LANE_OPS_PER_PIXEL = 36.0
+# The kernels evaluate a window offset in one of three tiers, chosen per warp (tfs_kernels.cuh); counted by the same rule:
+#   FAR  36 (above);  FAR2 24 (leading asymptotic term: 4 packed instead of 10 for f, g);
+#   NEAR 28 (table: v0, v1 (2), two look-ups = 1 + |v|, index FMA, packed interpolation (8), sign/scale of Godd (4),
+#            h' (4), z_A, z_E (8), q (2); the branch for pixels inside the swept band and the slow-chirp series are extra)
+TIER_LANE_OPS = {"far2": 24.0, "far": 36.0, "near": 28.0}
 SM_LANES = 128                       # lane-instructions issued per SM per clock (4 schedulers x 32 lanes)
 SMEM_BYTES_PER_CLK = 128             # shared-memory bandwidth per SM per clock (B300_MICROARCH.md: 128/N B/clk/SM)
 
@@ -244,7 +249,22 @@ def time_leg(api, torch, ctx, w, d_params, n, N_seg, k_top, steps, warmup, info,
     return dict(ms_step=ms_total / steps, ms_total=ms_total, prof=prof, clocks=clocks, d_ups=d_ups, d_idx=d_idx, d_val=d_val)
 
 
-def roofline_terms(leg, steps, pixels, wstruct, l2_gbs, peaks, peak_src, sm_count, sm_mhz):
+def tier_census(ctx, step):
+    """One untimed step with the library's tier counters on: pixel slots evaluated per tier (tfs_tier_census)."""
+    import torch
+    ctx.tier_census(True)
+    step()
+    torch.cuda.synchronize()
+    c = ctx.tier_census(False)
+    slots = {"far2": c[0], "far": c[1] + c[3], "near": c[2] + c[4]}
+    total = max(sum(slots.values()), 1)
+    mean_ops = sum(TIER_LANE_OPS[k] * v for k, v in slots.items()) / total
+    return {"pixel_slots": slots, "slab_kernel": {"far2": c[0], "far": c[1], "near": c[2]},
+            "list_kernel": {"far": c[3], "near": c[4]}, "lane_ops_per_tier": TIER_LANE_OPS,
+            "mean_lane_ops_per_slot": mean_ops, "pixel_slots_total": total}
+
+
+def roofline_terms(leg, steps, pixels, wstruct, l2_gbs, peaks, peak_src, sm_count, sm_mhz, census=None, issue=None):
     """The roofline terms of the evaluation kernels (eval_list_kernel + eval_slab_kernel, one pair per step)."""
     n_launch = max(leg["prof"]["eval_launches"], 1)
     kern_ms = (leg["prof"]["slab_kernel_ms"] + leg["prof"]["list_kernel_ms"]) / n_launch
@@ -253,7 +273,11 @@ def roofline_terms(leg, steps, pixels, wstruct, l2_gbs, peaks, peak_src, sm_coun
     achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
     smem_peak = sm_count * SMEM_BYTES_PER_CLK * sm_mhz * 1e6 / 1e9
     alu_peak = sm_count * SM_LANES * sm_mhz * 1e6 / 1e12           # T lane-instructions / s
-    alu_ach = ALG_LANE_OPS_PER_PIXEL * pixels / per_step / (kern_ms * 1e-3) / 1e12
+    # arithmetic actually needed: the tiers the kernels executed (census), on the window pixels only (the padding slots
+    # of inactive lanes and masked tails are waste, not work); without a census the flat far-tier figure
+    ops = census["mean_lane_ops_per_slot"] if census else ALG_LANE_OPS_PER_PIXEL
+    alu_ach = ops * pixels / per_step / (kern_ms * 1e-3) / 1e12
+    alu_flat = ALG_LANE_OPS_PER_PIXEL * pixels / per_step / (kern_ms * 1e-3) / 1e12
     terms = {
         "l2": {"achieved": achieved, "peak": l2_gbs, "unit": "GB/s", "frac": achieved / l2_gbs,
                "peak_source": "tfs_probe_l2_bandwidth, 32 MiB buffer, this run (the SM's L1 -> register return path)"},
@@ -263,8 +287,21 @@ def roofline_terms(leg, steps, pixels, wstruct, l2_gbs, peaks, peak_src, sm_coun
         "hbm_if_every_gather_missed_l2": {"achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                           "frac": achieved / peaks["hbm_gbs"], "peak_source": peak_src},
         "alu": {"achieved": alu_ach, "peak": alu_peak, "unit": "T lane-instr/s", "frac": alu_ach / alu_peak,
-                "peak_source": f"{sm_count} SMs x {SM_LANES} lanes x {sm_mhz:.0f} MHz (sampled)"},
+                "peak_source": f"{sm_count} SMs x {SM_LANES} lanes x {sm_mhz:.0f} MHz (sampled)",
+                "lane_ops_per_pixel": ops,
+                "lane_ops_source": "tier census of this run (tfs_tier_census)" if census else "flat far-tier count",
+                "frac_flat_36_ops": alu_flat / alu_peak},
     }
+    if census:
+        terms["alu"]["tier_census"] = census
+        terms["alu"]["padding_slots_frac"] = 1.0 - pixels / census["pixel_slots_total"]      # the census covers one whole step
+    if issue:
+        lanes = max(32.0 * issue[0], 64.0 * issue[1])
+        meas_peak = sm_count * lanes * sm_mhz * 1e6 / 1e12
+        terms["alu"].update({"peak_measured": meas_peak, "frac_of_measured_peak": alu_ach / meas_peak,
+                             "peak_measured_source": f"tfs_probe_fp32_issue, this run: {issue[0]:.2f} scalar FFMA / "
+                                                     f"{issue[1]:.2f} packed FFMA2 warp-instr/clk/SM = {lanes:.1f} "
+                                                     "FMA lane-slots/clk/SM"})
     return terms, kern_ms, bytes_per_launch
 
 
@@ -377,8 +414,127 @@ def main_wdm(args, info, w, n, N_seg, k_top, cfg):
     return 0
 
 
+# ---------------------------------------------------------------------------------------------
+# secondary legs of the default run: the configurations next to the headline one, each timed on the device for a
+# few steps and compared with the oracle on SEC_ROWS rows of its own bank (so that they are driver-witnessed numbers)
+# ---------------------------------------------------------------------------------------------
+SEC_ROWS = 64
+SEC_KNOTS, SEC_F0, SEC_STEP = 16, 1e-3, 6.6e-3          # transfer tables: 16 knots over 1-100 mHz
+
+
+def _sec_one(job):
+    leg, i = job
+    d = _ORA[leg]
+    from oracle import tfs_oracle as O
+    p = d["params"][i:i + 1]
+    if leg == "aet_tables":
+        r = O.evaluate_tf(p, d["tables"][i:i + 1], SEC_F0, SEC_STEP, d["D"], d["W"], d["gap"], d["grid"], d["N_seg"])
+    elif leg == "wdm":
+        from oracle import tfs_wdm as Wd
+        r = Wd.evaluate(p, d["D"], d["W"], d["gap"], d["grid"], d["N_seg"])
+        return float(r["upsilon"][0]), int((r["seg_gram"][0, :, 0] > 0).sum())
+    else:
+        r = O.evaluate(p, d["D"], d["W"], d["gap"], d["grid"], d["N_seg"], d["opts"])
+    return float(r["upsilon"][0]), int((r["seg_hh"][0] > 0).sum())
+
+
+def secondary_inputs(w, coeff, weight, gap):
+    """Seeded inputs of the four secondary legs (host arrays; no method arithmetic)."""
+    rng = np.random.default_rng(33)
+    n_aet, n_tuk, n_wdm = 200_000, 100_000, 500_000
+    w4 = synth.WORKLOADS["cfg4"]
+    c4, wt4, g4 = synth.make_data(w4)
+    return {
+        "aet_tables": dict(what="A, E, T (third channel = a copy of A's data) with a 16-knot complex transfer table per template "
+                                "and channel interpolated per tranche (tfs_eval_tf), cfg3 grid and bank",
+                           coeff=np.ascontiguousarray(np.concatenate([coeff, coeff[:1]])),
+                           weight=np.ascontiguousarray(np.concatenate([weight, weight[:1]])), gap=gap, w=w, N_seg=w.N_seg,
+                           params=synth.make_templates(w, n_aet),
+                           tables=rng.standard_normal((n_aet, 3, SEC_KNOTS, 2)).astype(np.float32)),
+        "tukey_0.1": dict(what="window-aware template, tukey_alpha = 0.1 (P:271), cfg3 grid and bank", coeff=coeff, weight=weight,
+                          gap=gap, w=w, N_seg=w.N_seg, params=synth.make_templates(w, n_tuk)),
+        "cfg4": dict(what="BASELINE.json configs[3]: one batch of 2^20 templates (20 % merging inside the grid), N_seg = 32",
+                     coeff=c4, weight=wt4, gap=g4, w=w4, N_seg=w4.N_seg, params=synth.make_templates(w4, w4.n_templates)),
+        "wdm": dict(what="real WDM wavelet pixels (tfs_opts.basis = 1) on the cfg3-shaped grid, general per-pixel weights",
+                    coeff=np.ascontiguousarray(coeff[..., 0]), weight=weight, gap=gap, w=w, N_seg=w.N_seg,
+                    params=synth.make_templates(w, n_wdm)),
+    }
+
+
+def secondary_oracle(sec, procs):
+    """Oracle Upsilon of the first SEC_ROWS rows of every secondary leg (fork pool: call BEFORE CUDA init)."""
+    import multiprocessing as mp
+    from oracle import tfs_oracle as O
+    from oracle import tfs_wdm as Wd
+    for leg, d in sec.items():
+        w = d["w"]
+        if leg == "wdm":
+            _ORA[leg] = dict(params=d["params"], D=d["coeff"].astype(np.float64), W=d["weight"].astype(np.float64), gap=d["gap"],
+                             grid=Wd.WdmGrid(w.Nt, w.Nf, w.dt), N_seg=d["N_seg"])
+            continue
+        c = d["coeff"].astype(np.float64)
+        _ORA[leg] = dict(params=d["params"], D=c[..., 0] + 1j * c[..., 1], W=d["weight"].astype(np.float64), gap=d["gap"],
+                         grid=O.Grid(w.Nt, w.Nf, w.dt), N_seg=d["N_seg"],
+                         opts=O.Opts(tukey_alpha=0.1) if leg == "tukey_0.1" else O.Opts())
+        if leg == "aet_tables":
+            t = d["tables"][:SEC_ROWS].astype(np.float64)
+            _ORA[leg]["tables"] = t[..., 0] + 1j * t[..., 1]
+    jobs = [(leg, i) for leg in sec for i in range(SEC_ROWS)]
+    t0 = time.perf_counter()
+    with mp.get_context("fork").Pool(procs) as pool:
+        out = pool.map(_sec_one, jobs, chunksize=1)
+    dt = time.perf_counter() - t0
+    _ORA.clear()
+    res = {leg: out[j * SEC_ROWS:(j + 1) * SEC_ROWS] for j, leg in enumerate(sec)}
+    return res, dt
+
+
+def secondary_legs(api, torch, dev, sec, ora, steps=3):
+    """Device-timed secondary legs (CUDA events around `steps` calls after two warm-up calls) + parity with `ora`."""
+    out = {}
+    for leg, d in sec.items():
+        w, N_seg = d["w"], d["N_seg"]
+        kw = {"aet_tables": dict(n_channels=3), "tukey_0.1": dict(tukey_alpha=0.1), "wdm": dict(basis=1)}.get(leg, {})
+        ctx = api.Tfs(w.Nt, w.Nf, w.dt, **kw)
+        ctx.upload_data(d["coeff"], d["weight"], d["gap"])
+        dp = torch.from_numpy(d["params"]).to(dev)
+        n = dp.shape[0]
+        ups = torch.empty(n, dtype=torch.float32, device=dev)
+        counts = torch.empty(n, dtype=torch.int64, device=dev)
+        ctx.count_pixels(dp, counts)
+        if leg == "aet_tables":
+            tab = torch.from_numpy(d["tables"]).to(dev)
+            call = lambda: ctx.eval_tf(dp, N_seg, tab, SEC_KNOTS, SEC_F0, SEC_STEP, ups)
+        else:
+            call = lambda: ctx.eval(dp, N_seg, ups)
+        for _ in range(2):
+            call()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            call()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        n_ch = 3 if leg == "aet_tables" else 2
+        r = {"what": d["what"], "templates": int(n), "N_seg": int(N_seg), "ms_per_call": ms, "value": n / (ms * 1e-3),
+             "unit": "templates/s", "pixel_evals_per_sec": n_ch * int(counts.sum().item()) / (ms * 1e-3), "steps": steps}
+        if ora is not None:
+            uo = np.array([u for u, _ in ora[leg]]); neff = np.maximum(np.array([e for _, e in ora[leg]]), 1)
+            err = np.abs(ups[:len(uo)].cpu().numpy().astype(np.float64) - uo) / np.maximum(uo, 2.0 * neff)
+            r["parity"] = {"n": int(len(uo)), "max_norm_err": float(err.max()), "tolerance": 1e-4, "ok": bool(err.max() <= 1e-4),
+                           "n_active": int((uo > 0).sum())}
+        out[leg] = r
+        ctx.destroy()
+        del dp, ups, counts
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--no-secondary", action="store_true",
+                    help="skip the secondary legs (A,E,T + tables, window-aware template, cfg4, WDM basis)")
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
@@ -477,6 +633,15 @@ def main():
                                                       "with (the dense oracle above sums over every pixel of the grid "
                                                       "and is slow by construction)"}}
 
+    sec, sec_ora, sec_dt, sec_err = None, None, None, None
+    if rank == 0 and world == 1 and not args.no_secondary and w.name == "cfg3":
+        try:        # the secondary legs must never take the headline measurement down with them
+            sec = secondary_inputs(w, coeff, weight, gap)
+            if not args.no_cpu_baseline:
+                sec_ora, sec_dt = secondary_oracle(sec, max(1, min(host_cores(), 16)))      # before CUDA init (fork)
+        except Exception as exc:
+            sec, sec_ora, sec_err = None, None, f"{type(exc).__name__}: {exc}"
+
     import torch
     from paper_2510_19047_b200 import api, build
     if not torch.cuda.is_available():
@@ -545,6 +710,8 @@ def main():
     ms_e2e = max(e2.elapsed_time(e3), 1e3 * wall_e2e) / args.steps
     ms_e2e = replicas.max_over_ranks(ms_e2e, info, dev)
     same = bool(np.array_equal(h_ups.numpy(), d_ups.cpu().numpy()))
+    census = tier_census(ctx, lambda: ctx.eval(d_params, N_seg, d_ups)) if rank == 0 else None
+    issue = ctx.probe_fp32_issue(1 << 16) if rank == 0 else None
     wstruct = ctx.weight_structure()
     launches_total = int(leg["prof"]["kernel_launches"])
     ctx.destroy()
@@ -563,9 +730,20 @@ def main():
         replicas.finish(info)
         return 0
 
+    secondary = {"error": sec_err} if sec_err else None
+    if sec is not None:
+        try:
+            secondary = secondary_legs(api, torch, dev, sec, sec_ora)
+        except Exception as exc:
+            secondary = {"error": f"{type(exc).__name__}: {exc}"}
+        secondary["oracle_seconds"] = sec_dt
+        secondary["note"] = (f"each leg: 3 device-timed calls after 2 warm-up calls; parity = timed output vs oracle/ on the first "
+                             f"{SEC_ROWS} rows of the leg's bank, criterion as in `parity`")
+
     peaks, peak_src = measured_peaks()
     sm_mhz = (clocks or {}).get("sm_mhz") or peaks.get("sm_max_mhz", 1965.0)
-    terms, kern_ms, bytes_per_launch = roofline_terms(leg, args.steps, pixels, wstruct, l2_gbs, peaks, peak_src, sm_count, sm_mhz)
+    terms, kern_ms, bytes_per_launch = roofline_terms(leg, args.steps, pixels, wstruct, l2_gbs, peaks, peak_src, sm_count, sm_mhz,
+                                                      census, issue)
     # the larger of the byte term -- against the level that serves the gathers: shared memory for the slab
     # kernel -- and the arithmetic term (BASELINE.json north_star); the L1/L2 and HBM figures are context
     bound = "smem" if terms["smem"]["frac"] >= terms["alu"]["frac"] else "alu"
@@ -585,13 +763,14 @@ def main():
                      "unit": terms[bound]["unit"], "frac": terms[bound]["frac"], "traffic": None,
                      "algorithmic_bytes_per_launch": bytes_per_launch,
                      "algorithmic_bytes_per_pixel_eval": ALG_BYTES_PER_PIXEL_EVAL[wstruct],
-                     "algorithmic_lane_ops_per_pixel": ALG_LANE_OPS_PER_PIXEL,
+                     "algorithmic_lane_ops_per_pixel": terms["alu"]["lane_ops_per_pixel"],
                      "weight_structure": wstruct, "kernel_ms_per_launch": kern_ms,
                      "slab_kernel_ms": prof["slab_kernel_ms"] / n_launch, "list_kernel_ms": prof["list_kernel_ms"] / n_launch,
                      "kernel_share_of_step": (prof["slab_kernel_ms"] + prof["list_kernel_ms"]) / leg["ms_total"],
                      "terms": terms},
         "cpu_baseline": cpu_baseline,
         "parity": parity,
+        "secondary": secondary,
         "e2e": {"value": replicas.aggregate_rate(n, ms_e2e * 1e-3, info), "unit": "templates/s",
                 "h2d_bytes_per_step": int(params.nbytes + h_ups.numpy().nbytes),
                 "d2h_bytes_per_step": int(h_ups.numpy().nbytes + h_idx.numpy().nbytes + h_val.numpy().nbytes),

@@ -295,11 +295,31 @@ TFS_API int tfs_get_profile(tfs_ctx* ctx, double* main_kernel_ms, long long* mai
 TFS_API int tfs_get_profile_kernels(tfs_ctx* ctx, double* slab_kernel_ms, double* list_kernel_ms,
                                     long long* eval_launches, long long* kernel_launches);
 
+/* Measurement hook (bench.py's per-tier operation count).  The evaluation kernels pick, warp by warp, one of three ways
+ * to evaluate the Fresnel auxiliary functions of a window offset (tfs_kernels.cuh: FAR2 = leading asymptotic term, FAR =
+ * fitted polynomials, NEAR = table) and also evaluate the padding slots of lanes whose tranche is inactive or whose
+ * window is shorter than the warp's longest.  While the census is on, every evaluation call on the context adds the
+ * number of pixel slots (lane x window offset, both channels of the pair together) it evaluated per tier to five
+ * device counters:  counts[0..2] = slab kernel FAR2, FAR, NEAR;  counts[3..4] = list kernel FAR, NEAR.
+ * tfs_tier_census synchronises the device, returns the counters accumulated since its previous call (counts may be NULL),
+ * zeroes them and switches the census on or off.  Off by default; while on, a counting build of the two kernels runs
+ * (a few atomics per work item; the default build carries no counting code), so switch it off before timing.  Counted
+ * for basis 0, fresnel_mode 0, tukey_alpha 0 only (other modes leave the counters untouched). */
+TFS_API int tfs_tier_census(tfs_ctx* ctx, int on, long long* counts);
+
 /* Measurement aid for the roofline (bench.py): allocate a zero-filled scratch buffer of `bytes`
  * (choose it well inside the L2, e.g. 32 MiB), read it `iters` times with coalesced 16-byte loads from
  * one 1024-thread CTA per SM, and return the sustained read bandwidth in GB/s (CUDA events around the
  * launch; one warm-up launch first).  Synchronises `stream`.  The buffer is freed before returning. */
 TFS_API int tfs_probe_l2_bandwidth(tfs_ctx* ctx, long long bytes, int iters, double* gb_per_s, void* stream);
+
+/* Measurement aid for the roofline's arithmetic term (bench.py): how many FP32 fused multiply-add WARP instructions one
+ * SM issues per clock when nothing else is in the way -- 32 resident warps per SM, 8 independent dependent chains per
+ * thread, `iters` steps per chain -- for scalar FFMA (*scalar_ipc) and for the packed fma.rn.f32x2 the pixel loops use
+ * (*packed_ipc; one such instruction is two fused multiply-adds per lane).  Cycles come from the SM's clock64 (median
+ * over the SMs), so the figures do not depend on the clock the GPU happens to run at.  FMA-pipe lane-slots per clock per
+ * SM = max(32 * scalar_ipc, 64 * packed_ipc).  Allocates and frees two small buffers; synchronises `stream`. */
+TFS_API int tfs_probe_fp32_issue(tfs_ctx* ctx, int iters, double* scalar_ipc, double* packed_ipc, void* stream);
 
 TFS_API void tfs_destroy(tfs_ctx* ctx);
 

@@ -82,6 +82,10 @@ def load_library():
     lib.tfs_get_profile.restype = ip
     lib.tfs_get_profile_kernels.argtypes = [vp, C.POINTER(dp), C.POINTER(dp), C.POINTER(ll), C.POINTER(ll)]
     lib.tfs_get_profile_kernels.restype = ip
+    lib.tfs_probe_fp32_issue.argtypes = [vp, ip, C.POINTER(dp), C.POINTER(dp), vp]
+    lib.tfs_probe_fp32_issue.restype = ip
+    lib.tfs_tier_census.argtypes = [vp, ip, C.POINTER(ll)]
+    lib.tfs_tier_census.restype = ip
     lib.tfs_probe_l2_bandwidth.argtypes = [vp, ll, ip, C.POINTER(dp), vp]
     lib.tfs_probe_l2_bandwidth.restype = ip
     lib.tfs_destroy.argtypes = [vp]
@@ -187,6 +191,18 @@ class Tfs:
                                           _ptr(upsilon, np.float32, n), _ptr(seg_power, np.float32, n * N_seg),
                                           _ptr(seg_dh, np.float32, 2 * n * N_seg),
                                           _ptr(seg_hh, np.float32, n * N_seg), _stream(stream)))
+
+    def probe_fp32_issue(self, iters=1 << 16, stream=None):
+        """tfs_probe_fp32_issue: (scalar FFMA, packed FFMA2) warp instructions per clock per SM."""
+        a, b = C.c_double(), C.c_double()
+        self._check(self._lib.tfs_probe_fp32_issue(self._h, int(iters), C.byref(a), C.byref(b), _stream(stream)))
+        return a.value, b.value
+
+    def tier_census(self, on):
+        """tfs_tier_census: returns the five tier counters accumulated since the previous call, then switches the census on/off."""
+        out = (C.c_longlong * 5)()
+        self._check(self._lib.tfs_tier_census(self._h, int(bool(on)), out))
+        return [int(v) for v in out]
 
     def set_third_channel_factor(self, re, im=0.0):
         self._check(self._lib.tfs_set_third_channel_factor(self._h, float(re), float(im)))

@@ -24,6 +24,45 @@ constexpr size_t kScratchBytes = 2ull << 30;  // cap for the piece-partials buff
 
 }  // namespace
 
+// FP32 issue probe (tfs_probe_fp32_issue): one 1024-thread CTA per SM, every thread runs kProbeChains independent
+// chains of dependent fused multiply-adds -- scalar FFMA, or packed FFMA2 (fma.rn.f32x2, the instruction the pixel loops
+// are made of) -- and the CTA's duration is read from the SM's own cycle counter.
+constexpr int kProbeChains = 8;
+__global__ void __launch_bounds__(1024, 1) fp32_issue_probe_kernel(int iters, int packed, float* sink, unsigned long long* cycles) {
+  const float x = 1.0f + 1e-7f * (float)threadIdx.x, y = 1e-9f * (float)(blockIdx.x + 1);
+  float acc = 0.f;
+  __syncthreads();
+  const long long t0 = clock64();
+  if (packed) {
+    f2_t v[kProbeChains];
+#pragma unroll
+    for (int c = 0; c < kProbeChains; ++c) v[c] = pk((float)c, (float)c + 0.5f);
+    const f2_t m = pk(x, x), b = pk(y, y);
+#pragma unroll 4
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+      for (int c = 0; c < kProbeChains; ++c) v[c] = ffma2(v[c], m, b);
+    }
+#pragma unroll
+    for (int c = 0; c < kProbeChains; ++c) { float lo, hi; upk(v[c], lo, hi); acc += lo + hi; }
+  } else {
+    float v[kProbeChains];
+#pragma unroll
+    for (int c = 0; c < kProbeChains; ++c) v[c] = (float)c;
+#pragma unroll 4
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+      for (int c = 0; c < kProbeChains; ++c) v[c] = fmaf(v[c], x, y);
+    }
+#pragma unroll
+    for (int c = 0; c < kProbeChains; ++c) acc += v[c];
+  }
+  __syncthreads();
+  const long long t1 = clock64();
+  if (threadIdx.x == 0) cycles[blockIdx.x] = (unsigned long long)(t1 - t0);
+  if (acc == 123.456f) *sink = acc;      // keeps the chains alive
+}
+
 struct tfs_ctx {
   int Nt = 0, Nf = 0, C = 0;
   double dt = 0, DT = 0, df = 0;
@@ -59,6 +98,8 @@ struct tfs_ctx {
   FarCoef far{};
   unsigned long long* bad = nullptr;       // device counter
   unsigned long long* work = nullptr;      // [2] device unit counters of the slab and the list kernel
+  unsigned long long* census = nullptr;    // [5] device tier counters (tfs_tier_census); handed to the kernels only while census_on
+  bool census_on = false;
   long long bad_host = 0;
 
   // growable device scratch
@@ -324,6 +365,7 @@ EvalArgs base_args(const tfs_ctx* ctx, int pr = 0) {
   a.vprefix = ctx->vprefix; a.valid_m = ctx->valid_m;
   a.bad_count = ctx->bad;
   a.work_counter = ctx->work;
+  a.census = ctx->census_on ? ctx->census : nullptr;
   a.Nt = ctx->Nt; a.Nf = ctx->Nf; a.ncol = ctx->ncol;
   a.H = ctx->opts.half_width; a.adaptive = ctx->opts.adaptive_width;
   a.DT = ctx->DT;
@@ -495,6 +537,8 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
   if ((e = cudaMalloc((void**)&ctx->lut, (kLutN + 1) * sizeof(float4))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc lut", e);
   if ((e = cudaMalloc((void**)&ctx->bad, sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
   if ((e = cudaMalloc((void**)&ctx->work, 2 * sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
+  if ((e = cudaMalloc((void**)&ctx->census, 5 * sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc counter", e);
+  if ((e = cudaMemset(ctx->census, 0, 5 * sizeof(unsigned long long))) != cudaSuccess) return bail(TFS_ECUDA, "cudaMemset counter", e);
   if ((e = cudaFuncSetAttribute(eval_list_kernel<0, kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_list_kernel<0, kWSeparable>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_list_kernel<0, kWTimeOnly>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
@@ -505,7 +549,14 @@ int tfs_create(tfs_ctx** out, int Nt, int Nf, double dt, int n_channels, const t
       (e = cudaFuncSetAttribute(eval_wdm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_slab_kernel<kWGeneral>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWGeneral))) != cudaSuccess ||
       (e = cudaFuncSetAttribute(eval_slab_kernel<kWSeparable>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWSeparable))) != cudaSuccess ||
-      (e = cudaFuncSetAttribute(eval_slab_kernel<kWTimeOnly>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWTimeOnly))) != cudaSuccess)
+      (e = cudaFuncSetAttribute(eval_slab_kernel<kWTimeOnly>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWTimeOnly))) != cudaSuccess ||
+      // the counting builds of tfs_tier_census
+      (e = cudaFuncSetAttribute(eval_list_kernel<0, kWGeneral, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_list_kernel<0, kWSeparable, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_list_kernel<0, kWTimeOnly, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLutListBytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_slab_kernel<kWGeneral, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWGeneral))) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_slab_kernel<kWSeparable, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWSeparable))) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(eval_slab_kernel<kWTimeOnly, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, slab_smem_bytes(kWTimeOnly))) != cudaSuccess)
     return bail(TFS_ECUDA, "cudaFuncSetAttribute(max dynamic shared memory)", e);
   if ((e = cudaMalloc((void**)&ctx->sel, sizeof(SelectState))) != cudaSuccess) return bail(TFS_ENOMEM, "cudaMalloc select state", e);
   std::vector<float4> lut;
@@ -522,6 +573,21 @@ int tfs_set_profiling(tfs_ctx* ctx, int on) {
   ctx->profiling = (on != 0);
   ctx->ev_used = 0;
   ctx->launches = 0;
+  return TFS_OK;
+}
+
+int tfs_tier_census(tfs_ctx* ctx, int on, long long* counts) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_tier_census: ctx is NULL");
+  int rc = check_device(ctx, "tfs_tier_census");
+  if (rc) return rc;
+  TFS_CUDA(ctx, cudaDeviceSynchronize());
+  if (counts) {
+    unsigned long long h[5];
+    TFS_CUDA(ctx, cudaMemcpy(h, ctx->census, sizeof(h), cudaMemcpyDeviceToHost));
+    for (int i = 0; i < 5; ++i) counts[i] = (long long)h[i];
+  }
+  TFS_CUDA(ctx, cudaMemset(ctx->census, 0, 5 * sizeof(unsigned long long)));
+  ctx->census_on = (on != 0);
   return TFS_OK;
 }
 
@@ -558,7 +624,7 @@ void tfs_destroy(tfs_ctx* ctx) {
   for (auto& ev : ctx->ev_pool) cudaEventDestroy(ev);
   void* bufs[] = {ctx->pair[0].grid, ctx->pair[0].wgt, ctx->pair[0].wa, ctx->pair[0].wb, ctx->pair[1].grid, ctx->pair[1].wgt,
                   ctx->pair[1].wa, ctx->pair[1].wb, ctx->colmax, ctx->wcounts, ctx->gap, ctx->vprefix, ctx->valid_m, ctx->lut,
-                  ctx->bad, ctx->work, ctx->sel, ctx->buf_params, ctx->buf_partials, ctx->buf_prep, ctx->buf_ttab,
+                  ctx->bad, ctx->work, ctx->census, ctx->sel, ctx->buf_params, ctx->buf_partials, ctx->buf_prep, ctx->buf_ttab,
                   ctx->buf_out[0], ctx->buf_out[1], ctx->buf_out[2], ctx->buf_out[3], ctx->buf_out[4], ctx->buf_keys,
                   ctx->buf_tk_in, ctx->buf_tk_idx, ctx->buf_tk_val, ctx->buf_counts, ctx->buf_children, ctx->buf_fe};
   for (void* b : bufs) if (b) cudaFree(b);
@@ -788,7 +854,15 @@ namespace {
 
 template <int WMODE>
 void launch_slab(const EvalArgs& a, const tfs_ctx::Pair& P, unsigned blocks, cudaStream_t st) {
-  eval_slab_kernel<WMODE><<<blocks, kSlabWarps * 32, slab_smem_bytes(WMODE), st>>>(a, P.map_y, P.map_w);
+  if (a.census) eval_slab_kernel<WMODE, true><<<blocks, kSlabWarps * 32, slab_smem_bytes(WMODE), st>>>(a, P.map_y, P.map_w);
+  else eval_slab_kernel<WMODE><<<blocks, kSlabWarps * 32, slab_smem_bytes(WMODE), st>>>(a, P.map_y, P.map_w);
+}
+
+// the list kernel of the default template (MODE 0): the counting build while a tier census is on
+template <int WMODE>
+void launch_list0(const EvalArgs& a, unsigned blocks, cudaStream_t st) {
+  if (a.census) eval_list_kernel<0, WMODE, true><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
+  else eval_list_kernel<0, WMODE><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
 }
 
 // the evaluation proper (rows a1-a8) for one batch; `transfer` = per-template table [n][C][n_knots] complex or NULL
@@ -968,9 +1042,9 @@ int eval_impl(tfs_ctx* ctx, const double* params, long long n, int N_seg, const 
       else if (windowed && wm == kWTimeOnly) eval_list_kernel<2, kWTimeOnly><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
       else if (windowed && wm == kWSeparable) eval_list_kernel<2, kWSeparable><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
       else if (windowed) eval_list_kernel<2, kWGeneral><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
-      else if (wm == kWTimeOnly) eval_list_kernel<0, kWTimeOnly><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
-      else if (wm == kWSeparable) eval_list_kernel<0, kWSeparable><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
-      else eval_list_kernel<0, kWGeneral><<<blocks, kWarpsPerCta * 32, kLutListBytes, st>>>(a);
+      else if (wm == kWTimeOnly) launch_list0<kWTimeOnly>(a, blocks, st);
+      else if (wm == kWSeparable) launch_list0<kWSeparable>(a, blocks, st);
+      else launch_list0<kWGeneral>(a, blocks, st);
       TFS_CUDA(ctx, cudaGetLastError());
       if (ev[1]) TFS_CUDA(ctx, cudaEventRecord(ev[1], st));
       ctx->launches += 1;
@@ -1232,6 +1306,42 @@ int tfs_set_third_channel_factor(tfs_ctx* ctx, double re, double im) {
   if (!std::isfinite(re) || !std::isfinite(im)) return fail(ctx, TFS_EINVAL, "tfs_set_third_channel_factor: the factor must be finite");
   ctx->t3[0] = re; ctx->t3[1] = im; ctx->t3_set = true;
   return TFS_OK;
+}
+
+int tfs_probe_fp32_issue(tfs_ctx* ctx, int iters, double* scalar_ipc, double* packed_ipc, void* stream) {
+  if (!ctx) return fail(nullptr, TFS_EINVAL, "tfs_probe_fp32_issue: ctx is NULL");
+  if (iters < 1 || iters > (1 << 24)) return fail(ctx, TFS_EINVAL, "tfs_probe_fp32_issue: need 1 <= iters <= 2^24");
+  int rc = check_device(ctx, "tfs_probe_fp32_issue");
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int nb = ctx->sm_count;
+  unsigned long long* d_cyc = nullptr;
+  float* d_sink = nullptr;
+  cudaError_t e;
+  auto done = [&](int code, const char* what, cudaError_t err) {
+    if (d_cyc) cudaFree(d_cyc);
+    if (d_sink) cudaFree(d_sink);
+    return code == TFS_OK ? TFS_OK : fail(ctx, code, "tfs_probe_fp32_issue: %s failed: %s", what, cudaGetErrorString(err));
+  };
+  if ((e = cudaMalloc((void**)&d_cyc, (size_t)nb * sizeof(unsigned long long))) != cudaSuccess) return done(TFS_ENOMEM, "cudaMalloc", e);
+  if ((e = cudaMalloc((void**)&d_sink, sizeof(float))) != cudaSuccess) return done(TFS_ENOMEM, "cudaMalloc", e);
+  std::vector<unsigned long long> h((size_t)nb);
+  double out[2] = {0.0, 0.0};
+  for (int packed = 0; packed < 2; ++packed) {
+    fp32_issue_probe_kernel<<<nb, 1024, 0, st>>>(iters / 8 + 1, packed, d_sink, d_cyc);      // warm-up
+    fp32_issue_probe_kernel<<<nb, 1024, 0, st>>>(iters, packed, d_sink, d_cyc);
+    ctx->launches += 2;
+    if ((e = cudaGetLastError()) != cudaSuccess) return done(TFS_ECUDA, "fp32_issue_probe_kernel", e);
+    if ((e = cudaMemcpyAsync(h.data(), d_cyc, (size_t)nb * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(st)) != cudaSuccess)
+      return done(TFS_ECUDA, "fp32_issue_probe_kernel", e);
+    std::sort(h.begin(), h.end());
+    const double cyc = (double)h[h.size() / 2];                       // median SM
+    out[packed] = 32.0 * kProbeChains * (double)iters / cyc;           // warp instructions per clock per SM
+  }
+  if (scalar_ipc) *scalar_ipc = out[0];
+  if (packed_ipc) *packed_ipc = out[1];
+  return done(TFS_OK, "", cudaSuccess);
 }
 
 int tfs_topk(tfs_ctx* ctx, const float* upsilon, long long n, int k, long long* idx, float* val, void* stream) {

@@ -104,6 +104,7 @@ struct EvalArgs {
   int* __restrict__ n_units;           // [2] {slab, list}
   float4* __restrict__ partials;       // [n_pieces][n] {z.re, z.im, hh, 0}
   unsigned long long* bad_count;       // templates rejected
+  unsigned long long* census;          // NULL (default), or [5] pixel slots evaluated per tier: slab FAR2, FAR, NEAR; list FAR, NEAR (tfs_tier_census)
   unsigned long long* work_counter;    // [2] next unclaimed unit of {slab kernel, list kernel} (zeroed before each launch)
   // optional per-template transfer table (Eq. 29, "computed once per tranche"): T_alpha(f) at n_knots
   // knots f_knot0 + j f_knot_step, linear in between, clamped outside; [n][tt_C][tt_K] complex
@@ -672,7 +673,7 @@ constexpr int kLutCopiesSlab = TFS_LUT_COPIES_SLAB;
 // This is the item evaluator of eval_list_kernel (pixels gathered from global memory); eval_slab_kernel uses
 // eval_item_pair below.
 // ------------------------------------------------------------------------------------------
-template <int MODE, int WMODE>
+template <int MODE, int WMODE, bool CENSUS>
 __device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it, const int tile, const int lane,
                                           const unsigned lut_lane) {
   const TplConst T = a.tconst[it];
@@ -755,6 +756,10 @@ __device__ __forceinline__ void eval_item(const EvalArgs& a, const long long it,
       int JB = min(__reduce_max_sync(0xffffffffu, jb), Wmax);
       if (MODE == 1) { JA = 0; JB = Wmax; }          // the paper's approximants are used for every pixel
       JA = min(JA, JB);
+      if (CENSUS && lane == 0) {        // measurement only: 32 pixel slots per offset, NEAR in [JA, JB)
+        atomicAdd(a.census + 3, 32ull * (unsigned)(Wmax - (JB - JA)));
+        atomicAdd(a.census + 4, 32ull * (unsigned)(JB - JA));
+      }
 
       // ---------------- pixel loop (a3-a5): lane walks its own window ----------------
       LaneSums s;
@@ -967,7 +972,7 @@ __device__ __forceinline__ void pair_zone(const SlabPair<WMODE>& sl, const PairT
   }
 }
 
-template <int WMODE>
+template <int WMODE, bool CENSUS>
 __device__ __forceinline__ void eval_item_pair(const EvalArgs& a, const long long it, const int tile, const int lane,
                                                const unsigned lut_lane, const unsigned slab_y, const unsigned slab_w,
                                                const int row0) {
@@ -1042,6 +1047,12 @@ __device__ __forceinline__ void eval_item_pair(const EvalArgs& a, const long lon
       int JA = min(__reduce_min_sync(0xffffffffu, ja), JB);
       const int J2A = min(__reduce_min_sync(0xffffffffu, j2a), JA);
       const int J2B = max(min(__reduce_max_sync(0xffffffffu, j2b), Wmax), JB);
+      if (CENSUS && lane == 0) {
+        // measurement only: [0, Wmax) splits into FAR2 | FAR | NEAR | FAR | FAR2 at J2A <= JA <= JB <= J2B; 64 pixel slots per offset
+        atomicAdd(a.census + 0, 64ull * (unsigned)(J2A + Wmax - J2B));
+        atomicAdd(a.census + 1, 64ull * (unsigned)((JA - J2A) + (J2B - JB)));
+        atomicAdd(a.census + 2, 64ull * (unsigned)(JB - JA));
+      }
 
       // ---------------- pixel loop (a3-a5) ----------------
       PairTrack L;
@@ -1235,7 +1246,7 @@ static_assert(sizeof(SlabCtl) <= kSlabCtlBytes, "SlabCtl");
 // left it.  Units come in tile-major, band-major order, so consecutive units mostly reload the same slab
 // from the L2.
 // ------------------------------------------------------------------------------------------
-template <int WMODE>
+template <int WMODE, bool CENSUS = false>      // CENSUS: the measurement build of tfs_tier_census (the default build carries no counting code)
 __global__ void __launch_bounds__(kSlabWarps * 32, 1)
 eval_slab_kernel(const EvalArgs a, const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_w) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -1291,7 +1302,7 @@ eval_slab_kernel(const EvalArgs a, const __grid_constant__ CUtensorMap map_y, co
       k = __shfl_sync(0xffffffffu, k, 0);
       if (k >= d.cnt) break;
       const long long it = (long long)a.list[d.off + (unsigned)k];
-      eval_item_pair<WMODE>(a, it, d.tile, lane, lut_lane, slab_y, slab_w, d.row0);
+      eval_item_pair<WMODE, CENSUS>(a, it, d.tile, lane, lut_lane, slab_y, slab_w, d.row0);
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(bar_empty + 8u * stage);
@@ -1314,7 +1325,7 @@ eval_slab_kernel(const EvalArgs a, const __grid_constant__ CUtensorMap map_y, co
 // ------------------------------------------------------------------------------------------
 constexpr int kLutListBytes = (kLutN + 1) * kLutCopiesList * (int)sizeof(float4);
 
-template <int MODE, int WMODE>
+template <int MODE, int WMODE, bool CENSUS = false>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, 1)
 eval_list_kernel(const EvalArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -1335,7 +1346,7 @@ eval_list_kernel(const EvalArgs a) {
     const Unit d = a.units_list[uid];
     for (int k = 0; k < d.cnt; ++k) {
       const long long it = (long long)a.list[d.off + (unsigned)k];
-      eval_item<MODE, WMODE>(a, it, d.tile, lane, lut_lane);
+      eval_item<MODE, WMODE, CENSUS>(a, it, d.tile, lane, lut_lane);
     }
   }
 }
